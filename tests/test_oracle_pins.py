@@ -1,0 +1,439 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU).
+
+Each test checks oracle/tbsma_oracle.c against something other than itself: closed forms
+derived by hand (dimer, FCC shell sums), the paper's printed lattice parameter (Table 1,
+P:67) as the zero-pressure point, finite differences of the oracle's own energy (forces,
+virial), conservation laws, rigid-motion invariance, time reversibility of velocity Verlet,
+the Ornstein-Uhlenbeck closed form, brute force vs linked cells, and NVIDIA's cuRAND host
+Philox4x32-10 generator (a library routine).  P:NN = /root/reference/PAPER.md line NN.
+"""
+import ctypes
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1311_3890_b200 import workloads as W
+
+A, XI, P_, Q_, R0 = 0.2061, 1.790, 10.229, 4.036, 2.884
+KB, ACC, MASS = 8.617333262e-5, 9.648533212e-3, 196.96657
+# FCC shells: distance a*sqrt(k/2), multiplicity (textbook): k = 1..7
+FCC_SHELLS = [(1, 12), (2, 6), (3, 24), (4, 12), (5, 24), (6, 8), (7, 48)]
+
+
+def test_golden_table1_matches_oracle_params(golden_dir):
+    vals = {}
+    for line in open(os.path.join(golden_dir, "table1_au.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()[:2]
+        vals[k] = float(v)
+    p = oracle.au_params()
+    assert (p.A, p.xi, p.p, p.q) == (vals["A"], vals["xi"], vals["p"], vals["q"])
+    assert p.r0 == vals["r0_exponent"]
+    assert abs(vals["table1_r0_column"] / math.sqrt(2) - p.r0) < 5e-4   # reading A1
+
+
+# ---------------------------------------------------------------- P7: dimer closed form
+def dimer_energy(r):
+    x = r / R0 - 1
+    return 2 * A * math.exp(-P_ * x) - 2 * XI * math.exp(-Q_ * x)
+
+
+def dimer_force_mag(r):      # -dE/dr
+    x = r / R0 - 1
+    return (2 * A * P_ / R0) * math.exp(-P_ * x) - (2 * Q_ * XI / R0) * math.exp(-Q_ * x)
+
+
+@pytest.mark.parametrize("r", [2.2, 2.5, 2.884, 3.5, 5.0, 6.9])
+def test_dimer_closed_form(r):
+    # Eq.1-3 for two atoms: rho = xi^2 e^{-2qx}, E_B^i = -xi e^{-qx}, E_R^i = A e^{-px}
+    x = np.array([[0.1, -0.2, 0.3], [0.1 + r, -0.2, 0.3]])
+    o = oracle.compute(x, 7.0, fp32_pred=False)
+    assert o["e_rep"][0] == pytest.approx(dimer_energy(r), rel=1e-13)
+    assert o["e_atom"][0] == pytest.approx(0.5 * dimer_energy(r), rel=1e-13)
+    # force on atom 1 along +x is -dE/dr; atom 0 gets the opposite
+    assert o["f"][1, 0] == pytest.approx(dimer_force_mag(r), rel=1e-12, abs=1e-15)
+    assert o["f"][0, 0] == pytest.approx(-dimer_force_mag(r), rel=1e-12, abs=1e-15)
+    assert np.all(o["f"][:, 1:] == 0)
+    # virial: W_xx = 1/2 * 2 * d_x f_x = r * F(r); other components 0
+    assert o["w_rep"][0, 0] == pytest.approx(r * dimer_force_mag(r), rel=1e-12)
+    assert np.allclose(o["w_rep"][0, 1:], 0)
+
+
+def test_dimer_hand_values():
+    # E(r0) = 2A - 2 xi exactly (x = 0)
+    assert dimer_energy(R0) == pytest.approx(2 * 0.2061 - 2 * 1.790, abs=1e-15)
+    x = np.array([[0, 0, 0], [0, R0, 0.0]])
+    assert oracle.compute(x, 7.0, fp32_pred=False)["e_rep"][0] == pytest.approx(-3.1678, abs=1e-12)
+    # equilibrium separation r_eq = r0 [1 + ln(A p / (xi q)) / (p - q)]: force vanishes there
+    req = R0 * (1 + math.log(A * P_ / (XI * Q_)) / (P_ - Q_))
+    xe = np.array([[0, 0, 0], [0, 0, req]])
+    assert abs(oracle.compute(xe, 7.0, fp32_pred=False)["f"][1, 2]) < 1e-12
+
+
+def test_isolated_atom_and_beyond_cutoff():      # reading A5
+    o = oracle.compute(np.zeros((1, 3)), 7.0)
+    assert o["e_rep"][0] == 0 and np.all(o["f"] == 0) and o["rho"][0] == 0
+    o = oracle.compute(np.array([[0, 0, 0], [7.5, 0, 0.0]]), 7.0)
+    assert o["e_rep"][0] == 0 and np.all(o["f"] == 0)
+    # strict inequality at the cutoff (reading A4): r == r_cut is excluded
+    o = oracle.compute(np.array([[0, 0, 0], [7.0, 0, 0.0]]), 7.0)
+    assert o["e_rep"][0] == 0
+    o = oracle.compute(np.array([[0, 0, 0], [np.float32(6.9999995), 0, 0.0]]), 7.0)
+    assert o["e_rep"][0] != 0
+
+
+# ---------------------------------------------------------------- P4/P5/P6: FCC lattice sums
+def lattice_energy(a, nshell):
+    rep = sum(m * A * math.exp(-P_ * (a * math.sqrt(k / 2) / R0 - 1)) for k, m in FCC_SHELLS[:nshell])
+    rho = sum(m * XI ** 2 * math.exp(-2 * Q_ * (a * math.sqrt(k / 2) / R0 - 1)) for k, m in FCC_SHELLS[:nshell])
+    return rep - math.sqrt(rho), rho
+
+
+def bulk(a, ncell=4):
+    x = W.fcc_bulk(ncell, a)
+    L = ncell * a
+    return x, L
+
+
+@pytest.mark.parametrize("a,rcut,nshell", [(4.08, 7.0, 5), (4.079, 5.8, 4), (4.079, 7.0, 5)])
+def test_perfect_fcc_lattice_sum(a, rcut, nshell):
+    x, L = bulk(a, 4)
+    o = oracle.compute(x, rcut, lo=0.0, hi=np.float32(L), periodic=1, fp32_pred=False)
+    Lf = float(np.float32(L))           # the oracle's box length is the fp32 value
+    e_ref, rho_ref = lattice_energy(a, nshell)
+    # every site identical (P4) and equal to the hand-written shell sum (P5)
+    assert np.ptp(o["e_atom"]) < 1e-6 and np.ptp(o["rho"]) < 1e-4   # fp32-rounded L
+    assert abs(Lf - L) < 1e-6
+    assert o["e_atom"].mean() == pytest.approx(e_ref, abs=2e-6)
+    assert o["rho"].mean() == pytest.approx(rho_ref, rel=1e-6)
+    assert np.abs(o["f"]).max() < 1e-6      # fp32-rounded box breaks symmetry only at 1e-7 level
+
+
+def test_perfect_fcc_exact_box_every_site_identical():
+    # a box length exactly representable in fp32 (a = 4.0): spread at rounding level only
+    x, L = bulk(4.0, 4)
+    o = oracle.compute(x, 7.0, lo=0.0, hi=L, periodic=1, fp32_pred=False)
+    assert np.ptp(o["e_atom"]) < 1e-12
+    assert np.abs(o["f"]).max() < 1e-11
+    e_ref, _ = lattice_energy(4.0, 6)        # a*sqrt(3) = 6.93 < 7.0: six shells
+    assert o["e_atom"][0] == pytest.approx(e_ref, abs=1e-12)
+
+
+def test_cohesive_energy_and_printed_lattice_parameter():
+    """parameters were 'obtained from fits to the Au experimental cohesive energy, lattice
+    parameter'; Table 1 prints 4.079 A.  With the paper's r_cut = 5.8 A (4 shells) the
+    oracle's zero-pressure lattice constant must be that number, and the energy there the Au
+    cohesive energy 3.78 eV/atom.  (With r0 = 4.079 in the exponent it would be +30 eV: A1.)"""
+    def trw(a):
+        x, L = bulk(a, 3)
+        o = oracle.compute(x, 1.45 * a, lo=0.0, hi=np.float32(L), periodic=1, fp32_pred=False)
+        return o["w_rep"][0, :3].sum(), o["e_rep"][0] / len(x)
+    lo_a, hi_a = 4.05, 4.11                  # 1.45 a keeps exactly 4 shells (sqrt2 a < 1.45a < sqrt2.5 a)
+    assert trw(lo_a)[0] > 0 > trw(hi_a)[0]   # compressed: positive virial (repulsion); stretched: negative
+    for _ in range(40):
+        mid = 0.5 * (lo_a + hi_a)
+        if trw(mid)[0] > 0:
+            lo_a = mid
+        else:
+            hi_a = mid
+    a_eq = 0.5 * (lo_a + hi_a)
+    assert a_eq == pytest.approx(4.079, abs=1.0e-3)
+    assert trw(a_eq)[1] == pytest.approx(-3.779, abs=2e-3)
+
+
+def test_perfect_lattice_neighbour_counts():      # P11, reading A4
+    x, L = bulk(4.079, 5)
+    p4 = W.pack_pos4(x)
+    for radius, expect in [(5.8, 54), (7.0, 78), (7.3, 86)]:
+        c, lst = oracle.neighbors(p4, radius, lo=0.0, hi=np.float32(L), periodic=1, max_nb=100)
+        assert np.all(c == expect)
+        # symmetry j in L(i) <=> i in L(j)
+        pairs = {(i, j) for i in range(0, len(x), 37) for j in lst[i, :c[i]]}
+        for i, j in pairs:
+            assert i in lst[j, :c[j]]
+
+
+# ---------------------------------------------------------------- P1/P2/P3/P12 on a wire
+def small_wire(seed=7, sigma=0.05):
+    return W.displace(W.fcc_wire(14.0, 20.0), sigma, seed)
+
+
+def total_energy(x, **kw):
+    return oracle.compute(x, 7.0, fp32_pred=False, **kw)["e_rep"].sum()
+
+
+def test_force_is_minus_gradient_central_differences():        # P1
+    x = small_wire()
+    o = oracle.compute(x, 7.0, fp32_pred=False)
+    rng = np.random.default_rng(0)
+    h = 1e-5
+    worst = 0.0
+    for i in rng.choice(len(x), 12, replace=False):
+        for a in range(3):
+            xp, xm = x.copy(), x.copy()
+            xp[i, a] += h
+            xm[i, a] -= h
+            fd = -(total_energy(xp) - total_energy(xm)) / (2 * h)
+            worst = max(worst, abs(fd - o["f"][i, a]) / max(np.linalg.norm(o["f"][i]), 1e-3))
+    assert worst < 1e-6
+
+
+def test_momentum_and_torque_conservation():                   # P2
+    x = small_wire()
+    f = oracle.compute(x, 7.0, fp32_pred=False)["f"]
+    assert np.abs(f.sum(0)).max() < 1e-10
+    assert np.abs(np.cross(x, f).sum(0)).max() < 1e-10
+    assert np.abs(f).max() > 0.1
+
+
+def test_rigid_motion_invariance():                            # P3
+    x = small_wire()
+    e0 = total_energy(x)
+    rng = np.random.default_rng(1)
+    qm, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    if np.linalg.det(qm) < 0:
+        qm[:, 0] *= -1
+    xr = x @ qm.T + np.array([3.3, -1.7, 12.9])
+    o0 = oracle.compute(x, 7.0, fp32_pred=False)
+    o1 = oracle.compute(xr, 7.0, fp32_pred=False)
+    assert o1["e_rep"][0] == pytest.approx(e0, rel=1e-12)
+    assert np.allclose(o1["f"], o0["f"] @ qm.T, atol=1e-11)   # forces rotate with the frame
+    assert np.allclose(o1["e_atom"], o0["e_atom"], atol=1e-12)
+
+
+def test_virial_identities():                                  # P12
+    x = small_wire()
+    o = oracle.compute(x, 7.0, fp32_pred=False)
+    w = o["w_rep"][0]
+    f = o["f"]
+    # non-periodic: W_ab = sum_i r_i,a F_i,b (pair form == atom form)
+    full = x.T @ f
+    assert np.allclose([full[0, 0], full[1, 1], full[2, 2], full[0, 1], full[0, 2], full[1, 2]], w, atol=1e-9)
+    assert np.allclose(full, full.T, atol=1e-9)
+    # W_ab = -dE/d eps_ab under a homogeneous strain (finite difference)
+    h = 1e-6
+    for comp, (a, b) in enumerate([(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]):
+        def strained(eps):
+            y = x.copy()
+            y[:, a] += eps * x[:, b]
+            return y
+        de = (total_energy(strained(h)) - total_energy(strained(-h))) / (2 * h)
+        assert -de == pytest.approx(w[comp], rel=2e-6, abs=1e-6)
+
+
+def test_virial_periodic_strain():
+    a, nc = 4.0, 4
+    x = W.displace(W.fcc_bulk(nc, a), 0.05, 3)
+    L = nc * a
+
+    def e_of(scale_z):
+        y = x.copy()
+        y[:, 2] *= scale_z
+        hi = np.array([L, L, L * scale_z], dtype=np.float32)
+        assert float(hi[2]) == L * scale_z          # chosen exactly representable
+        return oracle.compute(y, 6.5, lo=0.0, hi=hi, periodic=1, fp32_pred=False)
+    h = 2.0 ** -16
+    o = e_of(1.0)
+    de = (e_of(1 + h)["e_rep"][0] - e_of(1 - h)["e_rep"][0]) / (2 * h)
+    assert -de == pytest.approx(o["w_rep"][0, 2], rel=1e-5)
+    assert np.abs(o["f"].sum(0)).max() < 1e-10
+
+
+def test_energy_per_atom_sums_and_replica_batching():
+    w = W.config4(3, seed=11)
+    o = oracle.compute(w.x64(), 7.0, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, periodic=w.periodic)
+    for r in range(3):
+        s = slice(w.offsets[r], w.offsets[r + 1])
+        single = oracle.compute(w.x64()[s], 7.0)
+        assert o["e_rep"][r] == pytest.approx(single["e_rep"][0], rel=1e-13)
+        assert o["e_rep"][r] == pytest.approx(o["e_atom"][s].sum(), rel=1e-13)
+        assert np.allclose(o["f"][s], single["f"], atol=1e-13)       # replicas never interact
+
+
+# ---------------------------------------------------------------- cell list vs brute force
+@pytest.mark.parametrize("periodic", [0, 1])
+def test_celllist_equals_bruteforce(periodic):
+    if periodic:
+        x = W.displace(W.fcc_bulk(6, 4.08), 0.05, 5)
+        L = np.float32(6 * 4.08)
+        x = np.mod(x, float(L)).astype(np.float32).astype(np.float64)
+        kw = dict(lo=0.0, hi=L, periodic=1)
+    else:
+        w = W.config1()
+        x = w.x64()
+        kw = dict(lo=w.box_lo, hi=w.box_hi, periodic=0)
+    a = oracle.compute(x, 7.0, **kw)
+    b = oracle.compute(x, 7.0, cells=True, **kw)
+    assert np.array_equal(a["rho"] > 0, b["rho"] > 0)
+    assert np.allclose(a["f"], b["f"], atol=1e-12) and np.allclose(a["e_atom"], b["e_atom"], atol=1e-12)
+    assert np.allclose(a["w_rep"], b["w_rep"], rtol=1e-11, atol=1e-9)
+    cnt, _ = oracle.neighbors(W.pack_pos4(x), 7.0, **kw)
+    assert b["n_pairs_directed"] == cnt.sum()
+
+
+def test_sampled_compute_equals_full():
+    w = W.config4(2, seed=5)
+    full = oracle.compute(w.x64(), 7.0, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, periodic=w.periodic)
+    idx = np.array([0, 17, 2000, w.offsets[1], w.n_atoms - 1])
+    s = oracle.compute_sample(w.x64(), 7.0, idx, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, periodic=w.periodic)
+    assert np.allclose(s["f"], full["f"][idx], atol=1e-13)
+    assert np.allclose(s["e_atom"], full["e_atom"][idx], atol=1e-13)
+
+
+def test_neighbor_statistics_of_config1():
+    # DESIGN.md quotes n_L = 68.1 (7.3 A) and n_C = 63.4 (7.0 A) for config 1; 2655 atoms
+    w = W.config1()
+    assert w.n_atoms == 2655
+    cl, _ = oracle.neighbors(w.pos4, 7.3)
+    cc, _ = oracle.neighbors(w.pos4, 7.0)
+    assert cl.mean() == pytest.approx(68.1, abs=0.1) and cl.max() <= 96
+    assert cc.mean() == pytest.approx(63.4, abs=0.1)
+
+
+def test_wire_generator_matches_table2_increment():
+    # Table 2: N = 8823 + 8850 k; a D0 = 3.1 nm, L0 = 20.4 nm wire has 8850 atoms
+    assert len(W.fcc_wire(31.0, 204.0, a=4.08)) == 8850
+    assert [len(W.fcc_wire(30.0, L)) for L in (60.0, 120.0, 240.0)] == [2655, 5133, 10443]
+
+
+# ---------------------------------------------------------------- P10: Philox vs cuRAND host
+def _curand_host():
+    for name in ("libcurand.so", "libcurand.so.10", "/usr/local/cuda/lib64/libcurand.so"):
+        try:
+            return ctypes.CDLL(name)
+        except OSError:
+            continue
+    return None
+
+
+def test_philox_against_curand_host_generator():
+    """cuRAND's host generator CURAND_RNG_PSEUDO_PHILOX4_32_10 (=161) emits, as its n-th block of
+    four words, Philox4x32-10 of counter (n div 65536 [64 bit: c0,c1], n mod 65536 [c2], 0)
+    under key = seed.  Compare blocks with oracle.philox4x32_10 word for word."""
+    cr = _curand_host()
+    if cr is None:
+        pytest.skip("libcurand not found")
+    for seed in (0x0123456789ABCDEF, 1, 0xFFFFFFFF00000000):
+        g = ctypes.c_void_p()
+        assert cr.curandCreateGeneratorHost(ctypes.byref(g), 161) == 0
+        assert cr.curandSetPseudoRandomGeneratorSeed(g, ctypes.c_ulonglong(seed)) == 0
+        key = [seed & 0xFFFFFFFF, seed >> 32]
+        for block0 in (0, 65536 * 5 + 123, 65536 * ((7 << 32) + 0xDEADBEEF) + 40000):
+            assert cr.curandSetGeneratorOffset(g, ctypes.c_ulonglong(4 * block0)) == 0
+            out = np.zeros(4 * 64, dtype=np.uint32)
+            assert cr.curandGenerate(g, out.ctypes.data_as(ctypes.c_void_p), ctypes.c_size_t(out.size)) == 0
+            for k in range(64):
+                n = block0 + k
+                hi, c2 = divmod(n, 65536)
+                ctr = [hi & 0xFFFFFFFF, hi >> 32, c2, 0]
+                assert np.array_equal(oracle.philox4x32_10(ctr, key), out[4 * k:4 * k + 4]), (seed, n)
+        cr.curandDestroyGenerator(g)
+
+
+def test_gauss3_counter_layout_and_moments():      # reading A9
+    g, raw = oracle.gauss3(0x1122334455667788, 12345, (3 << 32) + 99)
+    assert np.array_equal(raw, oracle.philox4x32_10([12345, 99, 3, 0], [0x55667788, 0x11223344]))
+    u = ((raw >> 8).astype(np.float64) + 0.5) / 2 ** 24
+    ra, rb = math.sqrt(-2 * math.log(u[0])), math.sqrt(-2 * math.log(u[2]))
+    assert np.allclose(g, [ra * math.cos(2 * math.pi * u[1]), ra * math.sin(2 * math.pi * u[1]),
+                           rb * math.cos(2 * math.pi * u[3])], rtol=1e-14)
+    gs = np.array([oracle.gauss3(42, t, s)[0] for t in range(200) for s in range(100)])
+    assert abs(gs.mean()) < 0.02 and gs.var(axis=0) == pytest.approx(1.0, abs=0.03)
+    assert abs(np.corrcoef(gs.T)[0, 1]) < 0.02 and abs(np.corrcoef(gs.T)[0, 2]) < 0.02
+    # different tag / step / seed -> different stream
+    assert not np.array_equal(oracle.gauss3(42, 1, 0)[1], oracle.gauss3(42, 0, 1)[1])
+    assert not np.array_equal(oracle.gauss3(42, 1, 0)[1], oracle.gauss3(43, 1, 0)[1])
+
+
+# ---------------------------------------------------------------- P8/P9 and the integrator
+def test_gamma_zero_is_velocity_verlet_and_time_reversible():
+    x = small_wire(sigma=0.08)
+    n = len(x)
+    v = W.maxwell_velocities(n, 300.0, 5)
+    md = oracle.MD(x, v, np.zeros(n, np.int32), 7.0)
+    # one step against textbook velocity Verlet written with the oracle's force call
+    f0 = oracle.compute(x, 7.0, fp32_pred=False)["f"]
+    k = 0.5 * 2.0 * ACC / MASS
+    vh = v + k * f0
+    x1 = x + 2.0 * vh
+    f1 = oracle.compute(x1, 7.0, fp32_pred=False)["f"]
+    v1 = vh + k * f1
+    md.step(2.0, 0.0, 0.0, 1, 0)
+    assert np.allclose(md.x, x1, atol=1e-13) and np.allclose(md.v, v1, atol=1e-15)
+    # reversibility: 20 steps forward, flip v, 20 steps -> back at the start
+    for s in range(1, 20):
+        md.step(2.0, 0.0, 0.0, 1, s)
+    md.v *= -1
+    for s in range(20):
+        md.step(2.0, 0.0, 0.0, 1, s)
+    assert np.abs(md.x - x).max() < 1e-9
+    assert np.abs(md.v + v).max() < 1e-11
+
+
+def test_nve_energy_conservation_1000_steps():                 # P8 (config 1, fp64)
+    w = W.config1()
+    md = oracle.MD(w.x64(), w.v64(), w.flags, 7.0, lo=w.box_lo, hi=w.box_hi, cells=True)
+    n = w.n_atoms
+    e = [(md.e_rep[0] + md.ekin_rep[0]) / n]
+    for s in range(1000):
+        md.step(2.0, 0.0, 0.0, 1, s)
+        e.append((md.e_rep[0] + md.ekin_rep[0]) / n)
+    e = np.array(e)
+    assert np.abs(e - e[0]).max() < 3e-5            # eV/atom: bounded fluctuation (cutoff jumps, A4)
+    assert abs(e[-200:].mean() - e[:200].mean()) < 5e-6
+    t_kin = 2 * md.ekin_rep[0] / (3 * n * KB)
+    assert 80 < t_kin < 200                          # sigma = 0.05 A start equilibrates near 130 K
+
+
+def test_langevin_ou_closed_form_free_particles():             # P9
+    # atoms 10 A apart never interact (r_cut 7): the O step alone acts on v
+    g = np.arange(12) * 10.0
+    x = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    n = len(x)
+    T, gamma, dt = 298.0, 0.02, 2.0
+    v0 = np.full((n, 3), 3e-3)
+    md = oracle.MD(x, v0, np.zeros(n, np.int32), 7.0, cells=True, lo=-5.0, hi=120.0)
+    c1 = math.exp(-gamma * dt)
+    md.step(dt, T, gamma, 9, 0)
+    assert np.abs(md.f).max() == 0
+    # after one step the mean decays by c1 exactly (noise has zero mean): <v> = c1 v0 +- sigma/sqrt(3n)
+    sig = math.sqrt(KB * T * ACC / MASS)
+    assert md.v.mean() == pytest.approx(c1 * 3e-3, abs=4 * sig * math.sqrt(1 - c1 ** 2) / math.sqrt(3 * n))
+    # positions moved by dt/2 (v0 + v1)
+    assert np.allclose(md.x - x, 0.5 * dt * (v0 + md.v), atol=1e-12)
+    for s in range(1, 400):
+        md.step(dt, T, gamma, 9, s)
+    va = md.v.copy()
+    assert (va ** 2).mean() == pytest.approx(sig ** 2, rel=0.06)       # equipartition
+    lag = 25
+    for s in range(400, 400 + lag):
+        md.step(dt, T, gamma, 9, s)
+    corr = (va * md.v).mean() / sig ** 2
+    assert corr == pytest.approx(math.exp(-gamma * dt * lag), abs=0.05)  # <v(0)v(t)> = e^{-gamma t}<v^2>
+    # reproducible: same (seed, tag, step) -> same noise
+    md2 = oracle.MD(x, v0, np.zeros(n, np.int32), 7.0, cells=True, lo=-5.0, hi=120.0)
+    md2.step(dt, T, gamma, 9, 0)
+    md3 = oracle.MD(x, v0, np.zeros(n, np.int32), 7.0, cells=True, lo=-5.0, hi=120.0)
+    md3.step(dt, T, gamma, 9, 0)
+    assert np.array_equal(md2.v, md3.v)
+
+
+def test_grips_are_rigid_and_placed():                         # readings A10, A12
+    w = W.config2(length=40.0)
+    md = oracle.MD(w.x64(), w.v64(), w.flags, 7.0, lo=w.box_lo, hi=w.box_hi, cells=True)
+    x0 = md.x.copy()
+    fixed, pulled, dyn = w.flags == 1, w.flags == 2, w.flags == 0
+    assert fixed.sum() > 0 and pulled.sum() == fixed.sum()
+    for s in range(5):
+        md.step(2.0, 298.0, 1e-3, 77, s, slab_disp=0.01 * (s + 1))
+    assert np.array_equal(md.x[fixed], x0[fixed])
+    assert np.array_equal(md.x[pulled][:, :2], x0[pulled][:, :2])
+    assert np.allclose(md.x[pulled][:, 2], x0[pulled][:, 2] + 0.05, atol=1e-14)
+    assert np.all(md.v[~dyn] == 0) and np.abs(md.x[dyn] - x0[dyn]).max() > 1e-3
+    # kinetic energy counts dynamic atoms only
+    ek = 0.5 * MASS / ACC * (md.v[dyn] ** 2).sum()
+    assert md.ekin_rep[0] == pytest.approx(ek, rel=1e-13)
