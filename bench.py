@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched TB-SMA MD step on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl tbsma|reference]
+
+A "step" is one MD step of EVERY replica of the workload: integrate (B A O A + grips), per-replica
+neighbour rebuild when due, density pass, force pass (+ closing half kick).  Default workload =
+BASELINE.json configs[2] ("config3": 256 replicas x 3 nm x 24 nm Au wire, 2 673 408 atoms, 10 K and
+298 K halves, Langevin + pulling) -- the headline batched configuration; configs 1-2 are latency
+cases and parity tests, configs 4, 5a, 5b can be selected with --config.
+metric = atom-timesteps/s (whole job).  N > 1 (torchrun): every rank runs its own batch of replicas
+(weak scaling, replicas only, no collective on the data path).
+--impl reference times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1311_3890_b200 import workloads as W  # noqa: E402
+
+METRIC = "atom_timesteps_per_s"
+UNIT = "atom-steps/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def make_workload(cfg, rank=0, replicas=None):
+    seed_shift = 1000 * rank
+    if cfg == "1":
+        return W.config1(1 + seed_shift)
+    if cfg == "2":
+        return W.config2(2 + seed_shift)
+    if cfg == "3":
+        return W.config3(replicas or 256, 3 + seed_shift)
+    if cfg == "4":
+        return W.config4(replicas or 2048, 4 + seed_shift)
+    if cfg == "5a":
+        return W.config5a(64, 5 + seed_shift)
+    if cfg == "5b":
+        return W.config5b(6 + seed_shift)
+    raise SystemExit(f"unknown --config {cfg}")
+
+
+class ClockSampler(threading.Thread):
+    """SM clock / throttle reasons sampled with NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.stop_flag, self.ok = [], False, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                reasons = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                self.samples.append((time.perf_counter(), mhz, int(reasons)))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self, t0, t1):
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable"]}
+        nv = self.nv
+        sel = [s for s in self.samples if t0 <= s[0] <= t1] or self.samples[-3:]
+        names = {
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        seen = set()
+        for _, _, r in sel:
+            for bit, nm in names.items():
+                if r & bit:
+                    seen.add(nm)
+        mhz = sorted(s[1] for s in sel)
+        return {"sm_mhz": mhz[len(mhz) // 2] if mhz else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(seen), "samples": len(sel)}
+
+
+def cpu_oracle_rate(w, n_rep, n_steps):
+    """The oracle as it stands (brute force O(N^2) per replica, fp64, OpenMP), timed on a bounded
+    sample: the first n_rep replicas for n_steps MD steps.  Returns (atom-steps/s, cores, text)."""
+    import oracle
+    sub = w.take(0, min(n_rep, w.n_replicas))
+    md = oracle.MD(sub.x64(), sub.v64(), sub.flags, sub.r_cut, offsets=sub.offsets, lo=sub.box_lo, hi=sub.box_hi,
+                   periodic=sub.periodic, fp32_pred=False, cells=False, zref=sub.vel4[:, 3].astype(np.float64))
+    t0 = time.perf_counter()
+    for s in range(n_steps):
+        md.step(sub.dt, sub.T.astype(np.float64), sub.gamma, sub.seed, s, slab_disp=sub.slab_rate * (s + 1))
+    dt = time.perf_counter() - t0
+    return sub.n_atoms * n_steps / dt, oracle.num_threads(), \
+        f"first {sub.n_replicas} replica(s) of {w.name} ({sub.n_atoms} atoms) x {n_steps} steps, brute-force O(N^2) oracle"
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle on the box's host cores, same metric / config."""
+    if rank != 0:
+        return
+    w = make_workload(args.config, 0, replicas=2 if args.config in ("3", "4") else None)
+    if args.config == "5a":
+        w = W.config5a(8, 5)     # 2 048-atom periodic block: the O(N^2) oracle cannot do 10^6 atoms per step
+    sub = w.take(0, 1)
+    import oracle
+    md = oracle.MD(sub.x64(), sub.v64(), sub.flags, sub.r_cut, offsets=sub.offsets, lo=sub.box_lo, hi=sub.box_hi,
+                   periodic=sub.periodic, fp32_pred=False, cells=False, zref=sub.vel4[:, 3].astype(np.float64))
+    s = 0
+    for _ in range(args.warmup):
+        md.step(sub.dt, sub.T.astype(np.float64), sub.gamma, sub.seed, s, slab_disp=sub.slab_rate * (s + 1))
+        s += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        md.step(sub.dt, sub.T.astype(np.float64), sub.gamma, sub.seed, s, slab_disp=sub.slab_rate * (s + 1))
+        s += 1
+    dt = time.perf_counter() - t0
+    value = sub.n_atoms * args.steps / dt
+    sample = f"each step = 1 replica of {w.name} ({sub.n_atoms} atoms), brute-force O(N^2) fp64 oracle, OpenMP"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=60)
+    ap.add_argument("--config", default="3", choices=["1", "2", "3", "4", "5a", "5b"])
+    ap.add_argument("--replicas", type=int, default=None, help="override the replica count of config 3/4")
+    ap.add_argument("--impl", default="tbsma", choices=["tbsma", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--kernel-steps", type=int, default=60, help="steps of the per-kernel CUDA-event timing pass")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if args.gpus != world:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("for --gpus N > 1 launch with: python -m torch.distributed.run --nnodes=1 "
+                             "--nproc-per-node N --master-addr 127.0.0.1 --master-port P bench.py --gpus N ...")
+    import torch
+    import torch.distributed as dist
+    from paper_1311_3890_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world > 1:
+            t = torch.tensor([x], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+        return float(x)
+
+    def sum_over_ranks(x):
+        if world > 1:
+            t = torch.tensor([x], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+            return float(t.item())
+        return float(x)
+
+    w = make_workload(args.config, rank, args.replicas)
+    ctx = B.make_context(w)
+    st = B.DeviceState(w, dev)
+    stream = torch.cuda.Stream(device=dev)
+    K, Wm = args.steps, args.warmup
+    with torch.cuda.stream(stream):
+        ctx.build_cells(st.pos, st.vel, st.tag)
+        ctx.build_neighbors(st.pos)
+        ctx.compute(st.pos, st.force, st.e_rep, None)
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, Wm, None, st.slab_rate,
+                   w.rebuild_every, st.e_rep, None, st.ekin)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    stats0 = ctx.get_stats()
+    launches0 = ctx.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_host0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, Wm, K, None, st.slab_rate,
+                   w.rebuild_every, st.e_rep, None, st.ekin)
+        ev1.record(stream)
+    barrier()
+    t_host1 = time.perf_counter()
+    sampler.stop_flag = True
+    ms = max_over_ranks(ev0.elapsed_time(ev1))
+    launches = ctx.launch_count() - launches0
+    stats1 = ctx.get_stats()
+    status = ctx.status()
+    n_total = sum_over_ranks(w.n_atoms)
+    value = n_total * K / (ms * 1e-3)
+    entries, pairs = ctx.count_pairs(st.pos, stream)
+    n_l = entries / w.n_atoms
+    builds = stats1["n_replica_builds"] - stats0["n_replica_builds"]
+    k_eff = K * w.n_replicas / max(builds, 1)          # mean steps between rebuilds of a replica
+    pair_rate = sum_over_ranks(0.5 * pairs) * K / (ms * 1e-3)
+
+    # per-kernel pass: CUDA events on the launching stream around every kernel class
+    ctx.set_timing(True)
+    ks = min(args.kernel_steps, 512)
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, Wm + K, ks, None, st.slab_rate,
+                   w.rebuild_every, st.e_rep, None, st.ekin)
+    tms, tsteps = ctx.get_timing()
+    ctx.set_timing(False)
+    peak, peak_src = load_peaks()
+    per_kernel_ms = {k: v / max(tsteps, 1) for k, v in tms.items()}
+    # algorithmic bytes per launch: force pass 4 n_L + 40 B/atom,
+    # density pass 4 n_L + 24 B/atom, whole step 8 n_L + 160 + (4 n_L + 120)/K_eff B/atom
+    force_bytes = (4.0 * n_l + 40.0) * w.n_atoms
+    dens_bytes = (4.0 * n_l + 24.0) * w.n_atoms
+    step_bytes = (8.0 * n_l + 160.0 + (4.0 * n_l + 120.0) / k_eff) * w.n_atoms
+    ach_force = force_bytes / (per_kernel_ms["force"] * 1e-3) / 1e9 if per_kernel_ms["force"] > 0 else 0.0
+    ach_dens = dens_bytes / (per_kernel_ms["density"] * 1e-3) / 1e9 if per_kernel_ms["density"] > 0 else 0.0
+    ach_step = step_bytes / (ms / K * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_force (force/energy pass + closing half kick)",
+                "achieved": ach_force, "peak": peak, "unit": "GB/s", "frac": ach_force / peak, "traffic": None,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": force_bytes,
+                "avg_launch_ms": per_kernel_ms["force"],
+                "density_pass": {"achieved": ach_dens, "frac": ach_dens / peak, "avg_launch_ms": per_kernel_ms["density"]},
+                "whole_step": {"achieved": ach_step, "frac": ach_step / peak, "bytes_per_atom_step": step_bytes / w.n_atoms},
+                "per_kernel_ms": per_kernel_ms, "timed_steps": tsteps}
+    traffic_file = os.path.join(ROOT, "profiles", "force_kernel_dram_bytes.json")
+    if os.path.exists(traffic_file):
+        try:
+            tf = json.load(open(traffic_file))
+            if tf.get("workload") == w.name:
+                roofline["traffic"] = tf.get("dram_bytes_per_launch")
+        except Exception:
+            pass
+
+    # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        ctx2 = B.make_context(w)
+        hp = torch.from_numpy(w.pos4.copy()).pin_memory()
+        hv = torch.from_numpy(w.vel4.copy()).pin_memory()
+        hf = torch.zeros_like(hp).pin_memory()
+        ht = torch.arange(w.n_atoms, dtype=torch.int32).pin_memory()
+        he, hk = np.zeros(w.n_replicas), np.zeros(w.n_replicas)
+        k2 = max(10, K // 3)
+        # warm-up call (allocates the staging buffers, instantiates the graph)
+        ctx2.md_run_host(hp.numpy(), hv.numpy(), hf.numpy(), ht.numpy(), w.dt, w.T, w.gamma, w.seed, 0, 8, None,
+                         w.slab_rate, w.rebuild_every, he, None, hk)
+        hp.copy_(torch.from_numpy(w.pos4)); hv.copy_(torch.from_numpy(w.vel4))
+        ht.copy_(torch.arange(w.n_atoms, dtype=torch.int32))
+        barrier()
+        t0 = time.perf_counter()
+        ctx2.md_run_host(hp.numpy(), hv.numpy(), hf.numpy(), ht.numpy(), w.dt, w.T, w.gamma, w.seed, 0, k2, None,
+                         w.slab_rate, w.rebuild_every, he, None, hk)
+        dt_e2e = max_over_ranks(time.perf_counter() - t0)
+        h2d = w.n_atoms * 36 + w.n_replicas * 28
+        d2h = w.n_atoms * 52 + w.n_replicas * 16
+        e2e = {"value": n_total * k2 / dt_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d / k2,
+               "d2h_bytes_per_step": d2h / k2, "steps": k2,
+               "call": "tbsma_md_run_host (H2D pos/vel/tag, cell+list build, initial forces, steps, D2H pos/vel/force/tag)"}
+        ctx2.destroy()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nrep, nst = (4, 8) if args.config in ("3",) else (8, 10) if args.config == "4" else (1, 10)
+        if args.config in ("5a", "5b"):
+            wc = W.config5a(8, 5) if args.config == "5a" else W.config2()
+            rate, cores, sample = cpu_oracle_rate(wc, 1, 10)
+        else:
+            rate, cores, sample = cpu_oracle_rate(w, nrep, nst)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "atoms_per_gpu": w.n_atoms, "replicas_per_gpu": w.n_replicas,
+                       "r_cut": w.r_cut, "skin": w.skin, "dt_fs": w.dt, "gamma_per_fs": w.gamma,
+                       "rebuild": "displacement > skin/2 per replica" if not w.rebuild_every else f"every {w.rebuild_every} steps",
+                       "mean_list_length": n_l, "mean_steps_between_rebuilds": k_eff,
+                       "l2": "inputs larger than L2 (index list %.0f MB per pass)" % (entries * 4 / 1e6),
+                       "parallelism": "replicas only" if world > 1 else "1 gpu"},
+            "pair_interactions_per_s": pair_rate,
+            "clocks": sampler.summary(t_host0, t_host1),
+            "e2e": e2e, "gpu_launches": int(launches), "status_flags": status,
+            "roofline": roofline, "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,184 @@
+/*
+ * tbsma.h -- C ABI of libtbsma: batched TB-SMA (Au) force evaluation + MD step on one B200.
+ *
+ * The method is the second-moment tight-binding potential of arXiv:1311.3890, section 2.1
+ * ("P:NN" = line NN of /root/reference/PAPER.md; "D:Ak" = reading Ak in DESIGN.md):
+ *     rho_i = sum_j xi^2 exp(-2q (r_ij/r0 - 1))                       P:47 Eq.1
+ *     E_i   = sum_j A exp(-p (r_ij/r0 - 1)) - sqrt(rho_i)              P:47-55 Eq.1-3
+ *     F_i   = -dE_C/dr_i, which needs rho_i and rho_j
+ * evaluated "in two stages (two CUDA kernels), each stage looping over atom i's neighbors"
+ * over a cutoff neighbour list with a buffer radius, inside a velocity-Verlet
+ * step of 2 fs with rigid gripping layers.  Many independent nanowire replicas are
+ * processed by every launch (the paper's science is > 2000 independent runs).
+ *
+ * Conventions
+ *   - Units: Angstrom, eV, fs, amu, K.  1 eV/(A amu) = 9.648533212e-3 A/fs^2,
+ *     kB = 8.617333262e-5 eV/K.
+ *   - "d_" pointers are DEVICE memory owned by the caller; "h_" pointers are HOST memory.
+ *     The context owns only its scratch (cells, lists, positions at build time, 1/sqrt(rho)).
+ *   - pos / vel / force_energy are arrays of n_atoms x 4 floats (float4, 16-byte aligned):
+ *       pos   = (x, y, z, flag)   flag = int32 bit pattern: 0 dynamic, 1 fixed grip, 2 pulled grip
+ *       vel   = (vx, vy, vz, zref) zref = reference z of a grip atom; a pulled atom is PLACED at
+ *                                  zref + D_r every step (D:A10, fp64 displacement, never
+ *                                  incremented in fp32); ignored for dynamic atoms
+ *       force_energy = (Fx, Fy, Fz, E_i)
+ *   - Atoms of replica r occupy the index range [off[r], off[r+1]) at all times.  Inside that
+ *     range tbsma_build_cells permutes atoms into cell order IN PLACE and records the original
+ *     index of every slot in d_tag; everything the caller compares is compared in tag space.
+ *   - Every call is asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default
+ *     stream) and never synchronises, except tbsma_status, tbsma_count_pairs, tbsma_get_stats
+ *     and the *_host entry point.  Calls are safe to capture into a CUDA graph.
+ *   - Errors: every function returns TBSMA_OK (0) or a negative code; nothing throws or aborts.
+ *     Asynchronous faults (list overflow, skin violated, ...) are reported by tbsma_status.
+ *   - There is no CPU fallback: without a CUDA device every call returns TBSMA_ECUDA.
+ */
+#ifndef TBSMA_H
+#define TBSMA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tbsma_ctx tbsma_ctx; /* opaque */
+
+/* Table 1 of the paper; r0 is the first-neighbour distance a/sqrt(2) (D:A1). */
+typedef struct {
+    double A, xi, p, q, r0, mass_amu;
+} tbsma_params;
+
+enum {
+    TBSMA_OK = 0,
+    TBSMA_EINVAL = -1, /* bad argument (NULL, negative size, box shorter than 2 (r_cut+skin) on a periodic axis) */
+    TBSMA_ENOMEM = -2, /* device or host allocation failed */
+    TBSMA_ECUDA = -3,  /* a CUDA runtime call failed (or no device) */
+    TBSMA_ESTATE = -4  /* call order violated (e.g. compute before build_neighbors) */
+};
+
+/* bits of the status word returned by tbsma_status */
+enum {
+    TBSMA_FLAG_NLIST_OVERFLOW = 1u, /* an atom had more than max_neighbors partners: list truncated, results invalid */
+    TBSMA_FLAG_OUT_OF_BOX = 2u,     /* an atom left its replica's (non-periodic) box: still correct, edge cells grow */
+    TBSMA_FLAG_NONFINITE = 4u,      /* a non-finite force was produced */
+    TBSMA_FLAG_SKIN_VIOLATED = 8u   /* with a fixed rebuild cadence an atom moved more than skin/2 between rebuilds */
+};
+
+typedef struct {
+    uint64_t n_steps;          /* md steps taken since tbsma_set_system */
+    uint64_t n_replica_builds; /* neighbour-list builds, counted per replica */
+    uint64_t n_build_passes;   /* steps (or explicit calls) in which at least one replica was rebuilt */
+    int32_t max_neighbors_seen;
+    int32_t reserved;
+} tbsma_stats;
+
+/* Create a context for one parameter set.  r_cut: interaction cutoff, plain truncation, strict
+ * r < r_cut (D:A4).  skin: neighbour-list buffer radius r_buff. */
+int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ctx **out);
+int tbsma_destroy(tbsma_ctx *ctx);
+
+/* Describe the batch: n_replicas independent systems, atoms of replica r are
+ * [h_replica_offsets[r], h_replica_offsets[r+1]).  h_box_lo / h_box_hi: n_replicas x 3 floats;
+ * h_periodic: n_replicas x 3 bytes (wires: 0,0,0; bulk: 1,1,1; D:A7).  On a periodic axis the box
+ * length is the fp32 difference hi - lo and must be >= 2 (r_cut + skin); positions must lie in
+ * [lo, hi).  On a non-periodic axis the box only sizes the cell grid (size it for the longest
+ * elongation expected; atoms outside are binned into the edge cells and flagged OUT_OF_BOX).
+ * max_neighbors: list capacity per atom (rounded up to a multiple of 4; 96 suits r_cut+skin=7.3 A).
+ * All arguments are HOST pointers; (re)allocates the context's device scratch. */
+int tbsma_set_system(tbsma_ctx *ctx, int64_t n_atoms, int32_t n_replicas,
+                     const int32_t *h_replica_offsets, const float *h_box_lo,
+                     const float *h_box_hi, const uint8_t *h_periodic, int32_t max_neighbors);
+
+/* Cell binning (counting sort over replica x cell keys, stable by tag inside a cell) and in-place
+ * reorder of d_pos, d_vel (nullable) and d_tag into cell order; positions on periodic axes are
+ * wrapped into [lo, hi).  d_tag must hold the current tag of every slot (0..n-1 before the
+ * first call).  Rebuilds every replica. */
+int tbsma_build_cells(tbsma_ctx *ctx, float *d_pos, float *d_vel, int32_t *d_tag, void *stream);
+
+/* Neighbour list of every atom: all j != i of the same replica with |r_i - r_j| < r_cut + skin,
+ * membership decided by the fp32 predicate of D:A6.  Needs tbsma_build_cells on the same d_pos. */
+int tbsma_build_neighbors(tbsma_ctx *ctx, const float *d_pos, void *stream);
+
+/* One force evaluation (stage 1 densities, stage 2 forces) over the current list.
+ * d_force_energy: out, n x 4 (F_i, E_i).  d_replica_energy: out, n_replicas doubles, E_C of each
+ * replica (Eq.3).  d_replica_virial: out or NULL, n_replicas x 6 doubles, W_ab = 1/2 sum_i sum_j
+ * d_ij,a f_ij,b in the order xx yy zz xy xz yz (potential part of Eq.5; D:A11). */
+int tbsma_compute(tbsma_ctx *ctx, const float *d_pos, float *d_force_energy,
+                  double *d_replica_energy, double *d_replica_virial, void *stream);
+
+/* One MD step of every replica (thermostat D:A8 = BAOAB Langevin, gamma = 0 is exactly
+ * velocity Verlet):  B A O A, neighbour rebuild of the replicas whose atoms moved more than
+ * skin/2 since their last build (D:A14), forces, B.  On entry d_force_energy must hold the
+ * forces of d_pos (from tbsma_compute or the previous step); on exit pos, vel, force are those
+ * of the next step.  d_T: n_replicas floats (K); gamma_per_fs: friction; d_seed: n_replicas
+ * uint64 Philox keys; step: the counter that, with the atom's tag inside its replica, selects
+ * the noise (D:A9); d_slab_disp: n_replicas doubles, TOTAL displacement D_r of the pulled slab
+ * (NULL = 0).  Outputs d_replica_energy / d_replica_virial / d_replica_ekin (eV, dynamic atoms,
+ * after the final B) may each be NULL.  d_vel and d_tag are permuted with d_pos on rebuilds. */
+int tbsma_md_step(tbsma_ctx *ctx, float *d_pos, float *d_vel, float *d_force_energy,
+                  int32_t *d_tag, double dt_fs, const float *d_T, double gamma_per_fs,
+                  const uint64_t *d_seed, uint64_t step, const double *d_slab_disp,
+                  double *d_replica_energy, double *d_replica_virial, double *d_replica_ekin,
+                  void *stream);
+
+/* n_steps MD steps, steps step0 .. step0+n_steps-1, the pulled slab of replica r at
+ * D_r(s) = d_slab_disp0[r] + d_slab_rate[r] * (s + 1 - step0) during step s (both nullable = 0).
+ * rebuild_every > 0 additionally rebuilds every replica whenever s % rebuild_every == 0 and
+ * raises SKIN_VIOLATED if an atom nevertheless moved more than skin/2 (BASELINE config 5).
+ * The per-replica outputs are those of the last step.  One launch set per step for all replicas;
+ * no host synchronisation. */
+int tbsma_md_run(tbsma_ctx *ctx, float *d_pos, float *d_vel, float *d_force_energy,
+                 int32_t *d_tag, double dt_fs, const float *d_T, double gamma_per_fs,
+                 const uint64_t *d_seed, uint64_t step0, int64_t n_steps,
+                 const double *d_slab_disp0, const double *d_slab_rate, int32_t rebuild_every,
+                 double *d_replica_energy, double *d_replica_virial, double *d_replica_ekin,
+                 void *stream);
+
+/* Same as tbsma_md_run but with HOST buffers: copies pos, vel, tag, T, seed, slab arrays to
+ * the device, builds cells + lists, evaluates the initial forces, runs n_steps, and copies pos,
+ * vel, force_energy, tag and the per-replica outputs back.  Synchronises.  h_tag in/out. */
+int tbsma_md_run_host(tbsma_ctx *ctx, float *h_pos, float *h_vel, float *h_force_energy,
+                      int32_t *h_tag, double dt_fs, const float *h_T, double gamma_per_fs,
+                      const uint64_t *h_seed, uint64_t step0, int64_t n_steps,
+                      const double *h_slab_disp0, const double *h_slab_rate, int32_t rebuild_every,
+                      double *h_replica_energy, double *h_replica_virial, double *h_replica_ekin);
+
+/* Neighbour lists in TAG space for parity checks: d_counts[t] and d_list[t*max_neighbors + k]
+ * (k < count, unsorted) for the atom whose tag is t.  d_tag as left by tbsma_build_cells. */
+int tbsma_get_neighbors(tbsma_ctx *ctx, const int32_t *d_tag, int32_t *d_counts, int32_t *d_list,
+                        void *stream);
+
+/* Number of directed (i,j) list entries and of directed in-cutoff pairs for d_pos (synchronises). */
+int tbsma_count_pairs(tbsma_ctx *ctx, const float *d_pos, int64_t *h_list_entries,
+                      int64_t *h_cutoff_pairs, void *stream);
+
+int tbsma_status(tbsma_ctx *ctx, uint32_t *h_flags); /* synchronises the device; clears nothing */
+int tbsma_clear_status(tbsma_ctx *ctx);
+int tbsma_get_stats(tbsma_ctx *ctx, tbsma_stats *h_out); /* synchronises */
+
+/* Selects the neighbour-gather kernel variant: 0 = auto, 1 = thread-per-atom over a k-major
+ * int32 list with L1-cached global gathers.  Other values are reserved. */
+int tbsma_set_variant(tbsma_ctx *ctx, int32_t variant);
+
+/* md_run replays one captured step as a CUDA graph when enabled (default 1) and the stream is
+ * not the legacy default stream. */
+int tbsma_set_graph(tbsma_ctx *ctx, int32_t enable);
+
+/* Per-kernel-class timing of tbsma_md_step / tbsma_md_run with CUDA events recorded on the
+ * launching stream (graph replay is off while enabled; at most 512 steps are recorded).
+ * tbsma_get_timing synchronises on the last event, returns the summed milliseconds of the classes
+ * {0 integrate, 1 rebuild chain, 2 density pass, 3 force pass, 4 step bookkeeping} and the number
+ * of steps they cover, and resets the record. */
+int tbsma_set_timing(tbsma_ctx *ctx, int32_t enable);
+int tbsma_get_timing(tbsma_ctx *ctx, double *h_ms_sum5, int64_t *h_steps);
+
+/* Number of this library's kernels launched through ctx since tbsma_set_system (host counter). */
+int64_t tbsma_launch_count(const tbsma_ctx *ctx);
+
+const char *tbsma_strerror(int code);
+const char *tbsma_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TBSMA_H */

@@ -1,0 +1,523 @@
+// tbsma_api.cu -- the C ABI declared in include/tbsma.h: argument checking, host-side geometry,
+// scratch ownership and the launch sequences.  No arithmetic of the method lives here.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "tbsma_internal.cuh"
+
+#define CK(call)                                   \
+    do {                                           \
+        cudaError_t e_ = (call);                   \
+        if (e_ != cudaSuccess) return map_cuda(e_); \
+    } while (0)
+
+namespace {
+
+int map_cuda(cudaError_t e)
+{
+    if (e == cudaErrorMemoryAllocation) return TBSMA_ENOMEM;
+    return TBSMA_ECUDA;
+}
+
+template <class T>
+cudaError_t dalloc(T **p, size_t count)
+{
+    *p = nullptr;
+    if (count == 0) count = 1;
+    return cudaMalloc((void **)p, count * sizeof(T));
+}
+
+void free_system(tbsma_ctx *c)
+{
+    cudaFree(c->d_geom); cudaFree(c->d_atom_rep); cudaFree(c->d_cell_count); cudaFree(c->d_cell_start);
+    cudaFree(c->d_cell_of); cudaFree(c->d_slot); cudaFree(c->d_order); cudaFree(c->d_pos_build);
+    cudaFree(c->d_tmp4); cudaFree(c->d_tmp_tag); cudaFree(c->d_nlist); cudaFree(c->d_nn); cudaFree(c->d_xs);
+    cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters);
+    c->d_geom = nullptr; c->d_atom_rep = nullptr; c->d_cell_count = nullptr; c->d_cell_start = nullptr;
+    c->d_cell_of = nullptr; c->d_slot = nullptr; c->d_order = nullptr; c->d_pos_build = nullptr;
+    c->d_tmp4 = nullptr; c->d_tmp_tag = nullptr; c->d_nlist = nullptr; c->d_nn = nullptr; c->d_xs = nullptr;
+    c->d_dirty = nullptr; c->d_ctrl = nullptr; c->d_counters = nullptr;
+    free(c->h_off); free(c->h_geom);
+    c->h_off = nullptr; c->h_geom = nullptr;
+    c->cells_built = c->list_built = 0;
+}
+
+void free_staging(tbsma_ctx *c)
+{
+    cudaFree(c->s_pos); cudaFree(c->s_vel); cudaFree(c->s_force); cudaFree(c->s_tag); cudaFree(c->s_T);
+    cudaFree(c->s_seed); cudaFree(c->s_disp0); cudaFree(c->s_rate); cudaFree(c->s_e); cudaFree(c->s_w); cudaFree(c->s_k);
+    c->s_pos = c->s_vel = c->s_force = nullptr; c->s_tag = nullptr; c->s_T = nullptr; c->s_seed = nullptr;
+    c->s_disp0 = c->s_rate = c->s_e = c->s_w = c->s_k = nullptr;
+    c->s_n = 0; c->s_R = 0;
+}
+
+// Fold the pair-function constants in double, round once to fp32.
+void fold_constants(tbsma_ctx *c)
+{
+    const tbsma_params &P = c->prm;
+    PairConst &k = c->pc;
+    const float rc = (float)c->r_cut, rl = (float)(c->r_cut + c->skin);
+    k.rc2 = rc * rc;   // fp32 product, as D:A6 prescribes
+    k.rl2 = rl * rl;
+    k.r0f = (float)P.r0;
+    const double log2e = 1.4426950408889634074;
+    const double aq = -2.0 * P.q / P.r0 * log2e, ap = -P.p / P.r0 * log2e;
+    const double dr0 = (double)k.r0f - P.r0;     // t = r - r0f  =>  r - r0 = t + dr0
+    k.aq = (float)aq;
+    k.ap = (float)ap;
+    k.b_rho = (float)(log2(P.xi * P.xi) + aq * dr0);
+    k.b_rep = (float)(log2(2.0 * P.A * P.p / P.r0) + ap * dr0);
+    k.b_band = (float)(log2(P.q * P.xi * P.xi / P.r0) + aq * dr0);
+    k.e_rep_scale = (float)(P.r0 / (2.0 * P.p));
+}
+
+int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *tag, double dt, const float *T,
+              double gamma, const unsigned long long *seed, unsigned long long step0, int64_t n_steps,
+              const double *disp0, const double *rate, int rebuild_every, double *e_rep, double *w_rep,
+              double *ekin, bool advance, cudaStream_t st)
+{
+    StepArgs a;
+    a.half_dt = (float)(0.5 * dt);
+    a.kick = (float)(0.5 * dt * TBSMA_ACC / c->prm.mass_amu);
+    const double c1 = exp(-gamma * dt);
+    a.c1 = (float)c1;
+    a.c2 = (float)sqrt(1.0 - c1 * c1);
+    a.sigma_scale = (float)sqrt(TBSMA_KB * TBSMA_ACC / c->prm.mass_amu);
+    a.skin_half2 = (float)(0.25 * c->skin * c->skin);
+    a.thermostat = gamma > 0.0;
+    a.rebuild_every = rebuild_every;
+    a.step_base = step0;
+    a.T = T; a.seed = seed; a.disp0 = disp0; a.rate = rate;
+    a.e_rep = e_rep; a.w_rep = w_rep; a.ekin = ekin;
+    KickArgs kk;
+    kk.vel = vel; kk.kick = a.kick; kk.ke_scale = (float)(0.5 * c->prm.mass_amu / TBSMA_ACC); kk.ekin = ekin;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        cudaEvent_t *ev = nullptr;
+        if (c->timing && c->tev && c->tev_steps < TBSMA_TIMING_MAX_STEPS) ev = c->tev + 6 * (c->tev_steps++);
+        if (ev) CK(cudaEventRecord(ev[0], st));
+        CK(tbsma_launch_integrate_pre(c, pos, vel, force, tag, a, st));
+        if (ev) CK(cudaEventRecord(ev[1], st));
+        CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
+        if (ev) CK(cudaEventRecord(ev[2], st));
+        CK(tbsma_launch_density(c, pos, st));
+        if (ev) CK(cudaEventRecord(ev[3], st));
+        CK(tbsma_launch_force(c, force, e_rep, w_rep, kk, st));
+        if (ev) CK(cudaEventRecord(ev[4], st));
+        CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
+        if (ev) CK(cudaEventRecord(ev[5], st));
+    }
+    return TBSMA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *tbsma_version(void) { return "tbsma-b200 0.1 (sm_100a)"; }
+
+const char *tbsma_strerror(int code)
+{
+    switch (code) {
+        case TBSMA_OK: return "ok";
+        case TBSMA_EINVAL: return "invalid argument";
+        case TBSMA_ENOMEM: return "out of memory";
+        case TBSMA_ECUDA: return "CUDA runtime error (or no CUDA device)";
+        case TBSMA_ESTATE: return "call order violated";
+        default: return "unknown error";
+    }
+}
+
+int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ctx **out)
+{
+    if (!params || !out || !(r_cut > 0.0) || !(skin >= 0.0) || !(params->r0 > 0.0) || !(params->mass_amu > 0.0) ||
+        !(params->xi > 0.0) || !(params->A > 0.0))
+        return TBSMA_EINVAL;
+    *out = nullptr;
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return TBSMA_ECUDA;   // no CPU fallback
+    CK(cudaGetDevice(&dev));
+    tbsma_ctx *c = (tbsma_ctx *)calloc(1, sizeof(tbsma_ctx));
+    if (!c) return TBSMA_ENOMEM;
+    c->prm = *params;
+    c->r_cut = r_cut;
+    c->skin = skin;
+    c->device = dev;
+    c->variant = 1;
+    c->use_graph = 1;
+    int sm = 0;
+    if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sm < 1) sm = 148;
+    c->n_sm = sm;
+    fold_constants(c);
+    *out = c;
+    return TBSMA_OK;
+}
+
+int tbsma_destroy(tbsma_ctx *c)
+{
+    if (!c) return TBSMA_EINVAL;
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    free_system(c);
+    free_staging(c);
+    if (c->own_stream) cudaStreamDestroy(c->own_stream);
+    if (c->tev) {
+        for (int i = 0; i < 6 * TBSMA_TIMING_MAX_STEPS; ++i) if (c->tev[i]) cudaEventDestroy(c->tev[i]);
+        free(c->tev);
+    }
+    free(c);
+    return TBSMA_OK;
+}
+
+int tbsma_set_variant(tbsma_ctx *c, int32_t variant)
+{
+    if (!c || variant < 0 || variant > 1) return TBSMA_EINVAL;
+    c->variant = variant == 0 ? 1 : variant;
+    return TBSMA_OK;
+}
+
+int tbsma_set_graph(tbsma_ctx *c, int32_t enable)
+{
+    if (!c) return TBSMA_EINVAL;
+    c->use_graph = enable != 0;
+    return TBSMA_OK;
+}
+
+int tbsma_set_timing(tbsma_ctx *c, int32_t enable)
+{
+    if (!c) return TBSMA_EINVAL;
+    if (enable && !c->tev) {
+        c->tev = (cudaEvent_t *)calloc(6 * TBSMA_TIMING_MAX_STEPS, sizeof(cudaEvent_t));
+        if (!c->tev) return TBSMA_ENOMEM;
+        for (int i = 0; i < 6 * TBSMA_TIMING_MAX_STEPS; ++i) CK(cudaEventCreate(&c->tev[i]));
+    }
+    c->timing = enable != 0;
+    c->tev_steps = 0;
+    return TBSMA_OK;
+}
+
+int tbsma_get_timing(tbsma_ctx *c, double *h_ms_sum5, int64_t *h_steps)
+{
+    if (!c || !h_ms_sum5 || !h_steps) return TBSMA_EINVAL;
+    for (int k = 0; k < 5; ++k) h_ms_sum5[k] = 0.0;
+    *h_steps = 0;
+    if (!c->tev || c->tev_steps == 0) return TBSMA_OK;
+    CK(cudaEventSynchronize(c->tev[6 * (c->tev_steps - 1) + 5]));
+    for (int s = 0; s < c->tev_steps; ++s)
+        for (int k = 0; k < 5; ++k) {
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, c->tev[6 * s + k], c->tev[6 * s + k + 1]));
+            h_ms_sum5[k] += (double)ms;
+        }
+    *h_steps = c->tev_steps;
+    c->tev_steps = 0;
+    return TBSMA_OK;
+}
+
+int64_t tbsma_launch_count(const tbsma_ctx *c) { return c ? c->launches : 0; }
+
+int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const int32_t *h_off,
+                     const float *h_lo, const float *h_hi, const uint8_t *h_per, int32_t max_neighbors)
+{
+    if (!c || n_atoms < 0 || n_atoms > 0x7ffffff0ll || n_replicas < 1 || !h_off || !h_lo || !h_hi || !h_per ||
+        max_neighbors < 1 || max_neighbors > 4096)
+        return TBSMA_EINVAL;
+    if (h_off[0] != 0 || h_off[n_replicas] != n_atoms) return TBSMA_EINVAL;
+    for (int r = 0; r < n_replicas; ++r)
+        if (h_off[r + 1] < h_off[r]) return TBSMA_EINVAL;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    free_system(c);
+    const int R = n_replicas;
+    c->n = n_atoms;
+    c->R = R;
+    c->n_pad = (int)((n_atoms + 31) / 32 * 32);
+    if (c->n_pad < 32) c->n_pad = 32;
+    c->kmax = (max_neighbors + 3) / 4 * 4;
+    c->launches = 0;
+    c->h_off = (int32_t *)malloc(sizeof(int32_t) * (R + 1));
+    c->h_geom = (RepGeom *)calloc(R, sizeof(RepGeom));
+    if (!c->h_off || !c->h_geom) { free_system(c); return TBSMA_ENOMEM; }
+    memcpy(c->h_off, h_off, sizeof(int32_t) * (R + 1));
+    const double r_list = c->r_cut + c->skin;
+    const double w_min = r_list * (1.0 + 1e-5) + 1e-4;   // margin over fp32 rounding of cell coordinates
+    int64_t cells = 0;
+    c->any_periodic = 0;
+    for (int r = 0; r < R; ++r) {
+        RepGeom &g = c->h_geom[r];
+        g.periodic = 0;
+        int64_t nc_r = 1;
+        for (int a = 0; a < 3; ++a) {
+            const float lo = h_lo[3 * r + a], hi = h_hi[3 * r + a];
+            const float len = hi - lo;          // fp32 difference
+            if (!(len >= 0.0f) || !isfinite(len)) { free_system(c); return TBSMA_EINVAL; }
+            const bool per = h_per[3 * r + a] != 0;
+            if (per) {
+                if ((double)len < 2.0 * r_list) { free_system(c); return TBSMA_EINVAL; }
+                g.periodic |= 1 << a;
+                c->any_periodic = 1;
+            }
+            int nc = (int)floor((double)len / w_min);
+            if (nc < 1) nc = 1;
+            if (nc > 1024) nc = 1024;
+            g.lo[a] = lo;
+            g.len[a] = len;
+            g.nc[a] = nc;
+            g.inv_w[a] = len > 0.0f ? (float)((double)nc / (double)len) : 0.0f;
+            nc_r *= nc;
+        }
+        g.cell_base = (int)cells;
+        g.atom_begin = h_off[r];
+        g.atom_end = h_off[r + 1];
+        cells += nc_r;
+        if (cells > 0x7ffffff0ll) { free_system(c); return TBSMA_EINVAL; }
+    }
+    c->n_cells = cells;
+    const size_t n = (size_t)n_atoms;
+    cudaError_t e = cudaSuccess;
+#define DA(ptr, cnt) if (e == cudaSuccess) e = dalloc(&(ptr), (cnt))
+    DA(c->d_geom, (size_t)R); DA(c->d_atom_rep, n); DA(c->d_cell_count, (size_t)cells);
+    DA(c->d_cell_start, (size_t)cells + 1); DA(c->d_cell_of, n); DA(c->d_slot, n); DA(c->d_order, n);
+    DA(c->d_pos_build, n); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
+    DA(c->d_nlist, (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, n); DA(c->d_xs, n);
+    DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8);
+#undef DA
+    if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
+    int32_t *rep = (int32_t *)malloc(sizeof(int32_t) * (n ? n : 1));
+    if (!rep) { free_system(c); return TBSMA_ENOMEM; }
+    for (int r = 0; r < R; ++r)
+        for (int64_t i = h_off[r]; i < h_off[r + 1]; ++i) rep[i] = r;
+    e = cudaMemcpy(c->d_atom_rep, rep, sizeof(int32_t) * n, cudaMemcpyHostToDevice);
+    free(rep);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_geom, c->h_geom, sizeof(RepGeom) * R, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(c->d_cell_count, 0, sizeof(int32_t) * (size_t)cells);
+    if (e == cudaSuccess) e = cudaMemset(c->d_cell_start, 0, sizeof(int32_t) * ((size_t)cells + 1));
+    if (e == cudaSuccess) e = cudaMemset(c->d_dirty, 0, sizeof(int32_t) * R);
+    if (e == cudaSuccess) e = cudaMemset(c->d_ctrl, 0, sizeof(int32_t) * 8);
+    if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, sizeof(unsigned long long) * 8);
+    if (e == cudaSuccess) e = cudaMemset(c->d_nn, 0, sizeof(int32_t) * (n ? n : 1));
+    if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
+    return TBSMA_OK;
+}
+
+int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, void *stream)
+{
+    if (!c || !d_pos || !d_tag) return TBSMA_EINVAL;
+    if (!c->d_geom) return TBSMA_ESTATE;
+    if (c->n == 0) { c->cells_built = 1; return TBSMA_OK; }
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(tbsma_launch_mark_all_dirty(c, st));
+    CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, true, false, st));
+    c->cells_built = 1;
+    c->list_built = 0;
+    return TBSMA_OK;
+}
+
+int tbsma_build_neighbors(tbsma_ctx *c, const float *d_pos, void *stream)
+{
+    if (!c || !d_pos) return TBSMA_EINVAL;
+    if (!c->d_geom || !c->cells_built) return TBSMA_ESTATE;
+    if (c->n == 0) { c->list_built = 1; return TBSMA_OK; }
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(tbsma_launch_mark_all_dirty(c, st));
+    CK(tbsma_launch_rebuild(c, (float4 *)d_pos, nullptr, nullptr, false, true, st));
+    CK(tbsma_launch_finish_step(c, 0, st));
+    c->list_built = 1;
+    return TBSMA_OK;
+}
+
+int tbsma_compute(tbsma_ctx *c, const float *d_pos, float *d_force_energy, double *d_e, double *d_w, void *stream)
+{
+    if (!c || !d_pos || !d_force_energy) return TBSMA_EINVAL;
+    if (!c->d_geom || !c->list_built) return TBSMA_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (d_e) CK(cudaMemsetAsync(d_e, 0, sizeof(double) * c->R, st));
+    if (d_w) CK(cudaMemsetAsync(d_w, 0, sizeof(double) * 6 * c->R, st));
+    if (c->n == 0) return TBSMA_OK;
+    CK(tbsma_launch_density(c, (const float4 *)d_pos, st));
+    KickArgs kk = {nullptr, 0.f, 0.f, nullptr};
+    CK(tbsma_launch_force(c, (float4 *)d_force_energy, d_e, d_w, kk, st));
+    return TBSMA_OK;
+}
+
+int tbsma_md_step(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energy, int32_t *d_tag, double dt_fs,
+                  const float *d_T, double gamma_per_fs, const uint64_t *d_seed, uint64_t step,
+                  const double *d_slab_disp, double *d_e, double *d_w, double *d_k, void *stream)
+{
+    if (!c || !d_pos || !d_vel || !d_force_energy || !d_tag || !(dt_fs > 0.0) || !(gamma_per_fs >= 0.0)) return TBSMA_EINVAL;
+    if (gamma_per_fs > 0.0 && (!d_T || !d_seed)) return TBSMA_EINVAL;
+    if (!c->d_geom || !c->list_built) return TBSMA_ESTATE;
+    if (c->n == 0) return TBSMA_OK;
+    return run_steps(c, (float4 *)d_pos, (float4 *)d_vel, (float4 *)d_force_energy, d_tag, dt_fs, d_T, gamma_per_fs,
+                     (const unsigned long long *)d_seed, step, 1, d_slab_disp, nullptr, 0, d_e, d_w, d_k, false,
+                     (cudaStream_t)stream);
+}
+
+int tbsma_md_run(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energy, int32_t *d_tag, double dt_fs,
+                 const float *d_T, double gamma_per_fs, const uint64_t *d_seed, uint64_t step0, int64_t n_steps,
+                 const double *d_disp0, const double *d_rate, int32_t rebuild_every, double *d_e, double *d_w,
+                 double *d_k, void *stream)
+{
+    if (!c || !d_pos || !d_vel || !d_force_energy || !d_tag || !(dt_fs > 0.0) || !(gamma_per_fs >= 0.0) ||
+        n_steps < 0 || rebuild_every < 0)
+        return TBSMA_EINVAL;
+    if (gamma_per_fs > 0.0 && (!d_T || !d_seed)) return TBSMA_EINVAL;
+    if (!c->d_geom || !c->list_built) return TBSMA_ESTATE;
+    if (c->n == 0 || n_steps == 0) return TBSMA_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    float4 *pos = (float4 *)d_pos, *vel = (float4 *)d_vel, *force = (float4 *)d_force_energy;
+    const unsigned long long *seed = (const unsigned long long *)d_seed;
+    CK(cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned long long), st));   // in-run step offset = 0
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (st) cudaStreamIsCapturing(st, &cap);
+    const bool graph = c->use_graph && !c->timing && st != nullptr && cap == cudaStreamCaptureStatusNone && n_steps >= 8;
+    if (!graph) {
+        int rc = run_steps(c, pos, vel, force, d_tag, dt_fs, d_T, gamma_per_fs, seed, step0, n_steps, d_disp0, d_rate,
+                           rebuild_every, d_e, d_w, d_k, true, st);
+        if (rc) return rc;
+    } else {
+        // One step captured into a CUDA graph and replayed: the step counter lives on the device
+        // (d_counters[0]), so every replay integrates the next step.  Cached while the arguments repeat.
+        GraphKey key;
+        memset(&key, 0, sizeof(key));
+        key.p[0] = pos; key.p[1] = vel; key.p[2] = force; key.p[3] = d_tag; key.p[4] = d_T; key.p[5] = seed;
+        key.p[6] = d_disp0; key.p[7] = d_rate; key.p[8] = d_e; key.p[9] = d_w; key.p[10] = d_k;
+        key.dt = dt_fs; key.gamma = gamma_per_fs; key.step0 = step0; key.rebuild_every = rebuild_every;
+        if (!c->graph_exec || memcmp(&key, &c->graph_key, sizeof(key)) != 0) {
+            if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+            cudaGraph_t g = nullptr;
+            CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            const int64_t before = c->launches;
+            int rc = run_steps(c, pos, vel, force, d_tag, dt_fs, d_T, gamma_per_fs, seed, step0, 1, d_disp0, d_rate,
+                               rebuild_every, d_e, d_w, d_k, true, st);
+            cudaError_t e = cudaStreamEndCapture(st, &g);
+            c->graph_launches_per_step = c->launches - before;
+            c->launches = before;
+            if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+            if (e != cudaSuccess) return map_cuda(e);
+            e = cudaGraphInstantiate(&c->graph_exec, g, 0);
+            cudaGraphDestroy(g);
+            if (e != cudaSuccess) { c->graph_exec = nullptr; return map_cuda(e); }
+            c->graph_key = key;
+        }
+        for (int64_t s = 0; s < n_steps; ++s) CK(cudaGraphLaunch(c->graph_exec, st));
+        c->launches += c->graph_launches_per_step * n_steps;
+    }
+    CK(cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned long long), st));
+    return TBSMA_OK;
+}
+
+int tbsma_md_run_host(tbsma_ctx *c, float *h_pos, float *h_vel, float *h_force, int32_t *h_tag, double dt_fs,
+                      const float *h_T, double gamma_per_fs, const uint64_t *h_seed, uint64_t step0, int64_t n_steps,
+                      const double *h_disp0, const double *h_rate, int32_t rebuild_every, double *h_e, double *h_w,
+                      double *h_k)
+{
+    if (!c || !h_pos || !h_vel || !h_force || !h_tag || !h_T || !h_seed) return TBSMA_EINVAL;
+    if (!c->d_geom) return TBSMA_ESTATE;
+    const size_t n = (size_t)c->n;
+    const int R = c->R;
+    if (!c->own_stream) CK(cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking));
+    cudaStream_t st = c->own_stream;
+    if (c->s_n != c->n || c->s_R != R) {
+        free_staging(c);
+        cudaError_t e = cudaSuccess;
+#define DA(ptr, cnt) if (e == cudaSuccess) e = dalloc(&(ptr), (cnt))
+        DA(c->s_pos, n); DA(c->s_vel, n); DA(c->s_force, n); DA(c->s_tag, n); DA(c->s_T, (size_t)R);
+        DA(c->s_seed, (size_t)R); DA(c->s_disp0, (size_t)R); DA(c->s_rate, (size_t)R); DA(c->s_e, (size_t)R);
+        DA(c->s_w, (size_t)6 * R); DA(c->s_k, (size_t)R);
+#undef DA
+        if (e != cudaSuccess) { free_staging(c); return map_cuda(e); }
+        c->s_n = c->n; c->s_R = R;
+    }
+    const cudaMemcpyKind H2D = cudaMemcpyHostToDevice, D2H = cudaMemcpyDeviceToHost;
+    CK(cudaMemcpyAsync(c->s_pos, h_pos, 16 * n, H2D, st));
+    CK(cudaMemcpyAsync(c->s_vel, h_vel, 16 * n, H2D, st));
+    CK(cudaMemcpyAsync(c->s_tag, h_tag, 4 * n, H2D, st));
+    CK(cudaMemcpyAsync(c->s_T, h_T, 4 * (size_t)R, H2D, st));
+    CK(cudaMemcpyAsync(c->s_seed, h_seed, 8 * (size_t)R, H2D, st));
+    if (h_disp0) CK(cudaMemcpyAsync(c->s_disp0, h_disp0, 8 * (size_t)R, H2D, st));
+    if (h_rate) CK(cudaMemcpyAsync(c->s_rate, h_rate, 8 * (size_t)R, H2D, st));
+    int rc = tbsma_build_cells(c, (float *)c->s_pos, (float *)c->s_vel, c->s_tag, st);
+    if (!rc) rc = tbsma_build_neighbors(c, (float *)c->s_pos, st);
+    if (!rc) rc = tbsma_compute(c, (float *)c->s_pos, (float *)c->s_force, c->s_e, h_w ? c->s_w : nullptr, st);
+    if (!rc) rc = tbsma_md_run(c, (float *)c->s_pos, (float *)c->s_vel, (float *)c->s_force, c->s_tag, dt_fs, c->s_T,
+                               gamma_per_fs, (const uint64_t *)c->s_seed, step0, n_steps, h_disp0 ? c->s_disp0 : nullptr,
+                               h_rate ? c->s_rate : nullptr, rebuild_every, c->s_e, h_w ? c->s_w : nullptr, c->s_k, st);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(h_pos, c->s_pos, 16 * n, D2H, st));
+    CK(cudaMemcpyAsync(h_vel, c->s_vel, 16 * n, D2H, st));
+    CK(cudaMemcpyAsync(h_force, c->s_force, 16 * n, D2H, st));
+    CK(cudaMemcpyAsync(h_tag, c->s_tag, 4 * n, D2H, st));
+    if (h_e) CK(cudaMemcpyAsync(h_e, c->s_e, 8 * (size_t)R, D2H, st));
+    if (h_w) CK(cudaMemcpyAsync(h_w, c->s_w, 48 * (size_t)R, D2H, st));
+    if (h_k) CK(cudaMemcpyAsync(h_k, c->s_k, 8 * (size_t)R, D2H, st));
+    CK(cudaStreamSynchronize(st));
+    return TBSMA_OK;
+}
+
+int tbsma_get_neighbors(tbsma_ctx *c, const int32_t *d_tag, int32_t *d_counts, int32_t *d_list, void *stream)
+{
+    if (!c || !d_tag || !d_counts || !d_list) return TBSMA_EINVAL;
+    if (!c->list_built) return TBSMA_ESTATE;
+    if (c->n == 0) return TBSMA_OK;
+    CK(tbsma_launch_get_neighbors(c, d_tag, d_counts, d_list, (cudaStream_t)stream));
+    return TBSMA_OK;
+}
+
+int tbsma_count_pairs(tbsma_ctx *c, const float *d_pos, int64_t *h_entries, int64_t *h_pairs, void *stream)
+{
+    if (!c || !d_pos) return TBSMA_EINVAL;
+    if (!c->list_built) return TBSMA_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long out[2] = {0, 0};
+    if (c->n > 0) {
+        CK(cudaMemsetAsync(c->d_counters + 4, 0, 2 * sizeof(unsigned long long), st));
+        CK(tbsma_launch_count_pairs(c, (const float4 *)d_pos, c->d_counters + 4, st));
+        CK(cudaMemcpyAsync(out, c->d_counters + 4, sizeof(out), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    if (h_entries) *h_entries = (int64_t)out[0];
+    if (h_pairs) *h_pairs = (int64_t)out[1];
+    return TBSMA_OK;
+}
+
+int tbsma_status(tbsma_ctx *c, uint32_t *h_flags)
+{
+    if (!c || !h_flags) return TBSMA_EINVAL;
+    *h_flags = 0;
+    if (!c->d_ctrl) return TBSMA_OK;
+    CK(cudaDeviceSynchronize());
+    int v = 0;
+    CK(cudaMemcpy(&v, c->d_ctrl + 1, sizeof(int), cudaMemcpyDeviceToHost));
+    *h_flags = (uint32_t)v;
+    return TBSMA_OK;
+}
+
+int tbsma_clear_status(tbsma_ctx *c)
+{
+    if (!c) return TBSMA_EINVAL;
+    if (!c->d_ctrl) return TBSMA_OK;
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemset(c->d_ctrl + 1, 0, sizeof(int)));
+    return TBSMA_OK;
+}
+
+int tbsma_get_stats(tbsma_ctx *c, tbsma_stats *out)
+{
+    if (!c || !out) return TBSMA_EINVAL;
+    memset(out, 0, sizeof(*out));
+    if (!c->d_ctrl) return TBSMA_OK;
+    CK(cudaDeviceSynchronize());
+    unsigned long long cnt[4];
+    int ctrl[4];
+    CK(cudaMemcpy(cnt, c->d_counters, sizeof(cnt), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(ctrl, c->d_ctrl, sizeof(ctrl), cudaMemcpyDeviceToHost));
+    out->n_steps = cnt[3];
+    out->n_replica_builds = cnt[1];
+    out->n_build_passes = cnt[2];
+    out->max_neighbors_seen = ctrl[2];
+    return TBSMA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,142 @@
+// tbsma_internal.cuh -- context layout and launcher declarations shared by the csrc/*.cu files.
+// Product code: shares nothing with oracle/.  P:NN = /root/reference/PAPER.md line NN.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "tbsma.h"
+
+#define TBSMA_KB 8.617333262e-5   // eV/K
+#define TBSMA_ACC 9.648533212e-3  // 1 eV/(A amu) in A/fs^2
+
+// fp32 constants of the pair functions, folded on the host in double.
+// With t = r - r0f (r0f = fl32(r0)):
+//   xi^2 exp(-2q x)          = exp2(aq * t + b_rho)
+//   (2Ap/r0) exp(-p x)       = exp2(ap * t + b_rep)
+//   (q xi^2/r0) exp(-2q x)   = exp2(aq * t + b_band)
+struct PairConst {
+    float rc2;        // fl32(r_cut)^2 (fp32 product) -- interaction predicate threshold, D:A6
+    float rl2;        // fl32(r_cut+skin)^2           -- list predicate threshold
+    float r0f;
+    float aq, ap;
+    float b_rho, b_rep, b_band;
+    float e_rep_scale;  // r0/(2p): sum of (2Ap/r0)e^{-px} -> sum of A e^{-px}
+};
+
+// Per-replica geometry (device arrays of R entries).
+struct RepGeom {
+    float lo[3];
+    float len[3];      // fl32(hi - lo): THE box length on periodic axes (D:A6)
+    float inv_w[3];    // 1 / cell width
+    int nc[3];         // cells per axis
+    int cell_base;     // first cell of this replica in the global cell arrays
+    int periodic;      // bit a set = axis a periodic
+    int atom_begin, atom_end;
+};
+
+struct GraphKey {          // arguments a cached one-step CUDA graph was captured with
+    const void *p[11];
+    double dt, gamma;
+    unsigned long long step0;
+    int rebuild_every;
+    int pad;
+};
+
+struct tbsma_ctx {
+    tbsma_params prm;
+    double r_cut, skin;
+    PairConst pc;
+    int device;
+    int n_sm;
+
+    int64_t n;        // atoms
+    int n_pad;        // n rounded up to a multiple of 32 (row pitch of the k-major list)
+    int R;            // replicas
+    int kmax;         // list capacity per atom, multiple of 4
+    int64_t n_cells;  // total cells over all replicas
+    int any_periodic;
+    int variant;
+
+    // host copies
+    int32_t *h_off;
+    RepGeom *h_geom;
+
+    // device: topology
+    RepGeom *d_geom;        // R
+    int32_t *d_atom_rep;    // n: replica of slot i (constant: atoms never change replica)
+    // device: cells
+    int32_t *d_cell_count;  // n_cells (zero between builds)
+    int32_t *d_cell_start;  // n_cells + 1 (global slot of the first atom of each cell)
+    int32_t *d_cell_of;     // n
+    int32_t *d_slot;        // n
+    int32_t *d_order;       // n: new slot -> old slot
+    float4 *d_pos_build;    // n: positions at the last build (sorted)
+    float4 *d_tmp4;         // n: scratch for the in-place permutation of vel
+    int32_t *d_tmp_tag;     // n
+    // device: lists
+    int32_t *d_nlist;       // kmax/4 x n_pad x int4, group-major: entry k of atom i at ((k>>2)*n_pad+i)*4+(k&3)
+    int32_t *d_nn;          // n: count | flag<<16
+    float4 *d_xs;           // n: (x, y, z, 1/sqrt(rho)) written by the density pass
+    // device: control
+    int32_t *d_dirty;       // R: replica needs a rebuild
+    int32_t *d_ctrl;        // [0] any_dirty, [1] status flags, [2] max neighbours seen
+    unsigned long long *d_counters; // [0] step offset inside md_run, [1] replica builds, [2] build passes, [3] steps
+    // host staging for *_host entry point
+    float4 *s_pos, *s_vel, *s_force;
+    int32_t *s_tag;
+    float *s_T;
+    unsigned long long *s_seed;
+    double *s_disp0, *s_rate, *s_e, *s_w, *s_k;
+    int64_t s_n;
+    int s_R;
+
+    int cells_built, list_built;
+    int64_t launches;
+    // md_run: one step captured as a CUDA graph and replayed
+    int use_graph;
+    cudaGraphExec_t graph_exec;
+    GraphKey graph_key;
+    int64_t graph_launches_per_step;
+    cudaStream_t own_stream;   // used by the *_host entry point
+    // optional per-kernel-class timing with CUDA events on the launching stream
+    int timing;
+    cudaEvent_t *tev;          // 6 events per timed step (class boundaries)
+    int tev_steps;             // steps recorded so far
+};
+#define TBSMA_TIMING_MAX_STEPS 512
+
+// ---- launchers (each returns cudaError_t of the launch) -------------------------------------
+// cells / lists (tbsma_cells.cu)
+cudaError_t tbsma_launch_rebuild(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, bool do_cells,
+                                 bool do_list, cudaStream_t st);
+cudaError_t tbsma_launch_mark_all_dirty(tbsma_ctx *c, cudaStream_t st);
+cudaError_t tbsma_launch_get_neighbors(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
+                                       cudaStream_t st);
+// forces (tbsma_force.cu)
+struct KickArgs {
+    float4 *vel;          // nullptr = no fused half kick
+    float kick;           // (dt/2) c/m
+    float ke_scale;       // m/(2c)
+    double *ekin;         // per replica, nullable
+};
+cudaError_t tbsma_launch_density(tbsma_ctx *c, const float4 *pos, cudaStream_t st);
+cudaError_t tbsma_launch_force(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kick,
+                               cudaStream_t st);
+cudaError_t tbsma_launch_count_pairs(tbsma_ctx *c, const float4 *pos, unsigned long long *d_out2,
+                                     cudaStream_t st);
+// integrator (tbsma_integrate.cu)
+struct StepArgs {
+    float half_dt, kick, c1, c2, sigma_scale;  // sigma_v = sigma_scale * sqrt(T)
+    float skin_half2;
+    int thermostat;          // gamma > 0
+    int rebuild_every;
+    unsigned long long step_base;
+    const float *T;
+    const unsigned long long *seed;
+    const double *disp0;     // nullable
+    const double *rate;      // nullable
+    double *e_rep, *w_rep, *ekin;  // zeroed here for the force pass; nullable
+};
+cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, const float4 *force,
+                                       const int32_t *tag, const StepArgs &a, cudaStream_t st);
+cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st);

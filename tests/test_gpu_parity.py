@@ -1,0 +1,378 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the fp64 oracle on
+the same seeded inputs.  Bars (BASELINE.json north_star): neighbour sets bit-exact; per-atom
+force |dF| <= 1e-4 eV/A + 1e-5 |F|; total energy relative error <= 1e-6; trajectories within
+1e-3 A RMS after 100 steps.  Everything is compared in tag (original index) space."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1311_3890_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+KB, ACC, MASS = 8.617333262e-5, 9.648533212e-3, 196.96657
+F_ABS, F_REL, E_REL, TRAJ_RMS = 1e-4, 1e-5, 1e-6, 1e-3
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1311_3890_b200 import binding
+    return binding
+
+
+def setup(B, w, max_nb=96):
+    ctx = B.make_context(w, max_nb)
+    st = B.DeviceState(w)
+    ctx.build_cells(st.pos, st.vel, st.tag)
+    ctx.build_neighbors(st.pos)
+    return ctx, st
+
+
+def gpu_neighbors(B, ctx, st):
+    counts = torch.zeros(ctx.n, dtype=torch.int32, device="cuda")
+    lst = torch.full((ctx.n, ctx.max_neighbors), -1, dtype=torch.int32, device="cuda")
+    ctx.get_neighbors(st.tag, counts, lst)
+    torch.cuda.synchronize()
+    return counts.cpu().numpy(), lst.cpu().numpy()
+
+
+def assert_same_sets(cg, lg, co, lo):
+    assert np.array_equal(cg, co)
+    for i in range(len(cg)):
+        assert np.array_equal(np.sort(lg[i, :cg[i]]), lo[i, :co[i]]), i
+
+
+def assert_forces(fg, fo):
+    err = np.linalg.norm(fg - fo, axis=1)
+    tol = F_ABS + F_REL * np.linalg.norm(fo, axis=1)
+    assert np.all(err <= tol), f"max force error {err.max():.3e}"
+    return err.max()
+
+
+def small_bulk(ncell=6, seed=5, a=4.08):
+    """periodic block, positions wrapped in fp32 like config 5a"""
+    w = W.config5a(ncell, seed)
+    return w
+
+
+WORKLOADS = {
+    "config1": lambda: W.config1(),
+    "config2": lambda: W.config2(),
+    "config4_ragged": lambda: W.config4(5, seed=9),
+    "config3_small": lambda: W.config3(2, seed=3, length=60.0),
+    "bulk_6": lambda: small_bulk(6),
+    "bulk_4_two_cells": lambda: small_bulk(4),       # 16.32 A box: only 2 cells per axis
+    "bulk_9": lambda: small_bulk(9),
+}
+
+
+@pytest.mark.parametrize("name", list(WORKLOADS))
+def test_neighbor_sets_bit_exact(B, name):
+    w = WORKLOADS[name]()
+    ctx, st = setup(B, w)
+    cg, lg = gpu_neighbors(B, ctx, st)
+    co, lo = oracle.neighbors(w.pos4, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+    assert ctx.status() & B.FLAG_NLIST_OVERFLOW == 0
+    assert_same_sets(cg, lg, co, lo)
+    # tags are a permutation that keeps every atom inside its replica
+    tag = st.tag.cpu().numpy()
+    assert np.array_equal(np.sort(tag), np.arange(w.n_atoms))
+    for r in range(w.n_replicas):
+        s = slice(w.offsets[r], w.offsets[r + 1])
+        assert tag[s].min() >= w.offsets[r] and tag[s].max() < w.offsets[r + 1]
+    entries, pairs = ctx.count_pairs(st.pos)
+    assert entries == co.sum()
+    cc, _ = oracle.neighbors(w.pos4, w.r_cut, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+    assert pairs == cc.sum()
+
+
+@pytest.mark.parametrize("name", list(WORKLOADS))
+def test_force_energy_virial_parity(B, name):
+    w = WORKLOADS[name]()
+    ctx, st = setup(B, w)
+    ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    o = oracle.compute(w.x64(), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, periodic=w.periodic)
+    fe = st.untag(st.force)
+    assert_forces(fe[:, :3].astype(np.float64), o["f"])
+    assert np.abs(fe[:, 3] - o["e_atom"]).max() <= 2e-6 * np.abs(o["e_atom"]).max() + 1e-6
+    e = st.e_rep.cpu().numpy()
+    assert np.all(np.abs(e - o["e_rep"]) <= E_REL * np.abs(o["e_rep"]))
+    wv = st.w_rep.cpu().numpy()
+    scale = np.abs(o["w_rep"][:, :3]).sum(1, keepdims=True) + w.n_atoms / w.n_replicas * 1e-3
+    assert np.all(np.abs(wv - o["w_rep"]) <= 2e-5 * scale)
+    # positions were only permuted (and wrapped), never changed, by the build
+    assert np.array_equal(st.untag(st.pos)[:, :3], w.pos4[:, :3])
+    # energy-only call (virial = NULL) gives the same forces bit for bit
+    f2 = torch.zeros_like(st.force)
+    ctx.compute(st.pos, f2, st.e_rep, None)
+    torch.cuda.synchronize()
+    assert torch.equal(f2, st.force)
+
+
+def test_paper_cutoff_5p8(B):
+    """the paper's own r_cut = 5.8 A, r_buff = 0.29 A"""
+    w = W.config1()
+    w.r_cut, w.skin = 5.8, 0.29
+    ctx, st = setup(B, w)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    o = oracle.compute(w.x64(), 5.8)
+    assert_forces(st.untag(st.force)[:, :3].astype(np.float64), o["f"])
+    assert abs(st.e_rep.item() - o["e_rep"][0]) <= E_REL * abs(o["e_rep"][0])
+    cg, lg = gpu_neighbors(B, ctx, st)
+    co, lo = oracle.neighbors(w.pos4, 5.8 + 0.29)
+    assert_same_sets(cg, lg, co, lo)
+
+
+def test_degenerate_systems(B):
+    # single atom, dimer inside / outside the cutoff, an empty replica in the middle (reading A5)
+    x = np.array([[0, 0, 0], [10, 0, 0], [12.5, 0, 0], [30, 0, 0], [38, 0, 0]], dtype=np.float64)
+    offs = np.array([0, 1, 3, 3, 5], dtype=np.int32)
+    lo = np.array([[-5, -5, -5], [5, -5, -5], [0, 0, 0], [25, -5, -5]], np.float32)
+    hi = np.array([[5, 5, 5], [20, 5, 5], [1, 1, 1], [45, 5, 5]], np.float32)
+    w = W.Workload("degenerate", W.pack_pos4(x), W.pack_vel4(np.zeros((5, 3)), W.pack_pos4(x)), offs, lo, hi,
+                   np.zeros((4, 3), np.uint8), np.zeros(4, np.float32), np.arange(4, dtype=np.uint64), np.zeros(4))
+    ctx, st = setup(B, w)
+    ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
+    torch.cuda.synchronize()
+    o = oracle.compute(x, 7.0, offsets=offs, lo=lo, hi=hi, periodic=0)
+    fe = st.untag(st.force)
+    assert np.all(fe[[0, 3, 4]] == 0) and np.all(np.isfinite(fe))
+    assert_forces(fe[:, :3].astype(np.float64), o["f"])
+    assert np.allclose(st.e_rep.cpu().numpy(), o["e_rep"], rtol=1e-6, atol=0)
+    assert st.e_rep[0].item() == 0 and st.e_rep[2].item() == 0 and st.e_rep[3].item() == 0
+    assert ctx.status() == 0
+
+
+def test_list_overflow_is_flagged(B):
+    w = W.config1()
+    ctx = B.make_context(w, 32)            # far too small for r = 7.3 A (up to 86 partners)
+    st = B.DeviceState(w)
+    ctx.build_cells(st.pos, st.vel, st.tag)
+    ctx.build_neighbors(st.pos)
+    assert ctx.status() & B.FLAG_NLIST_OVERFLOW
+    assert ctx.get_stats()["max_neighbors_seen"] == 86
+    ctx.clear_status()
+    assert ctx.status() == 0
+
+
+def test_call_order_and_arguments(B):
+    w = W.config1()
+    ctx = B.make_context(w)
+    st = B.DeviceState(w)
+    with pytest.raises(B.TbsmaError) as e:
+        ctx.compute(st.pos, st.force)
+    assert e.value.code == B.ESTATE
+    with pytest.raises(B.TbsmaError) as e:
+        ctx.build_neighbors(st.pos)
+    assert e.value.code == B.ESTATE
+    bad = B.Context()
+    with pytest.raises(B.TbsmaError) as e:        # periodic box shorter than 2 (r_cut + skin)
+        bad.set_system([0, 10], 0.0, 14.0, 1)
+    assert e.value.code == B.EINVAL
+
+
+def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False):
+    ctx, st = setup(B, w)
+    ctx.set_graph(graph)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        if use_run:
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None,
+                       st.slab_rate, w.rebuild_every, st.e_rep, st.w_rep if virial else None, st.ekin)
+        else:
+            for s in range(n_steps):
+                disp = torch.from_numpy(w.slab_rate * (s + 1)).cuda()
+                ctx.md_step(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, s, disp, st.e_rep,
+                            st.w_rep if virial else None, st.ekin)
+    torch.cuda.synchronize()
+    return ctx, st
+
+
+def run_oracle_md(w, n_steps, cells=True):
+    md = oracle.MD(w.x64(), w.v64(), w.flags, w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi,
+                   periodic=w.periodic, fp32_pred=False, cells=cells, zref=w.vel4[:, 3].astype(np.float64))
+    for s in range(n_steps):
+        md.step(w.dt, w.T.astype(np.float64), w.gamma, w.seed, s, slab_disp=w.slab_rate * (s + 1))
+    return md
+
+
+def traj_rms(xg, xo, box_len=None):
+    d = xg - xo
+    if box_len is not None:
+        d -= np.round(d / box_len) * box_len
+    return math.sqrt((d ** 2).sum(1).mean())
+
+
+def test_trajectory_config1_nve_100_steps(B):
+    w = W.config1()
+    ctx, st = run_gpu_md(B, w, 100)
+    md = run_oracle_md(w, 100)
+    assert traj_rms(st.untag(st.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+    assert abs(st.e_rep.item() - md.e_rep[0]) <= 5e-6 * abs(md.e_rep[0])
+    assert abs(st.ekin.item() - md.ekin_rep[0]) <= 1e-3 * md.ekin_rep[0]
+    # the forces left in the buffer are those of the final positions
+    assert_forces(st.untag(st.force)[:, :3].astype(np.float64),
+                  oracle.compute(st.untag(st.pos)[:, :3].astype(np.float64), 7.0)["f"])
+    assert ctx.status() == 0
+    assert ctx.get_stats()["n_steps"] == 100
+
+
+def test_trajectory_config2_langevin_grips_pull(B):
+    w = W.config2()
+    n_steps = 100
+    ctx, st = run_gpu_md(B, w, n_steps)
+    md = run_oracle_md(w, n_steps)
+    xg = st.untag(st.pos)[:, :3].astype(np.float64)
+    assert traj_rms(xg, md.x) <= TRAJ_RMS
+    vg = st.untag(st.vel)[:, :3].astype(np.float64)
+    assert np.abs(vg - md.v).max() < 2e-5
+    fl = w.flags
+    # grips: fixed atoms never move, pulled atoms sit at zref + D to 1 ulp (H5), v = 0
+    assert np.array_equal(xg[fl == 1], w.x64()[fl == 1])
+    zt = (w.vel4[fl == 2, 3].astype(np.float64) + w.slab_rate[0] * n_steps).astype(np.float32)
+    assert np.array_equal(st.untag(st.pos)[fl == 2, 2], zt)
+    assert np.all(vg[fl != 0] == 0)
+    stats = ctx.get_stats()
+    assert stats["n_replica_builds"] >= 1          # 298 K: atoms pass skin/2 within 100 steps
+    assert abs(st.ekin.item() - md.ekin_rep[0]) <= 2e-3 * md.ekin_rep[0]
+    assert ctx.status() == 0
+
+
+def test_md_step_equals_md_run_and_graph_bitwise(B):
+    w = W.config2(length=60.0)
+    _, a = run_gpu_md(B, w, 40, use_run=True, graph=True)
+    _, b = run_gpu_md(B, w, 40, use_run=True, graph=False)
+    _, c = run_gpu_md(B, w, 40, use_run=False)
+    for s in (b, c):
+        assert np.array_equal(a.untag(a.pos), s.untag(s.pos))
+        assert np.array_equal(a.untag(a.vel), s.untag(s.vel))
+        assert np.array_equal(a.untag(a.force), s.untag(s.force))
+
+
+def test_replicas_are_independent_and_ragged_batch_matches_single_runs(B):
+    w = W.config4(4, seed=21)
+    n_steps = 60
+    _, st = run_gpu_md(B, w, n_steps)
+    xb = st.untag(st.pos)
+    assert len(set(np.diff(w.offsets))) > 1        # really ragged
+    for r in range(w.n_replicas):
+        single = w.take(r, r + 1)
+        _, ss = run_gpu_md(B, single, n_steps)
+        s = slice(w.offsets[r], w.offsets[r + 1])
+        assert np.array_equal(xb[s], ss.untag(ss.pos))          # bit-identical: no cross-replica effect
+
+
+def test_philox_noise_matches_oracle(B):
+    """free particles (10 A apart, no forces): one step gives v1 = c1 v0 + c2 sigma g, so g is
+    recovered from the GPU velocities and compared with the oracle's Philox/Box-Muller."""
+    g = np.arange(6) * 10.0
+    x = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    n = len(x)
+    offs = np.array([0, 100, n], np.int32)
+    p4 = W.pack_pos4(x)
+    T = np.array([298.0, 10.0], np.float32)
+    seed = np.array([0x0123456789ABCDEF, 77], dtype=np.uint64)
+    w = W.Workload("free", p4, W.pack_vel4(np.zeros((n, 3)), p4), offs, np.full((2, 3), -5, np.float32),
+                   np.full((2, 3), 60, np.float32), np.zeros((2, 3), np.uint8), T, seed, np.zeros(2), gamma=0.05)
+    ctx, st = setup(B, w)
+    ctx.compute(st.pos, st.force)
+    step = (5 << 32) + 12345
+    ctx.md_step(st.pos, st.vel, st.force, st.tag, 2.0, st.T, w.gamma, st.seed, step)
+    torch.cuda.synchronize()
+    v = st.untag(st.vel)[:, :3].astype(np.float64)
+    c2 = math.sqrt(1 - math.exp(-2 * w.gamma * 2.0))
+    for i in range(n):
+        r = 0 if i < 100 else 1
+        sig = math.sqrt(KB * float(T[r]) * ACC / MASS)
+        gi, _ = oracle.gauss3(int(seed[r]), i - offs[r], step)
+        assert np.allclose(v[i] / (c2 * sig), gi, atol=2e-5), i
+
+
+def test_rebuild_every_cadence_bulk(B):
+    w = small_bulk(6)
+    ctx, st = run_gpu_md(B, w, 50)
+    md = run_oracle_md(w, 50)
+    L = float(w.box_hi[0, 0])
+    assert traj_rms(st.untag(st.pos)[:, :3].astype(np.float64), md.x, L) <= TRAJ_RMS
+    stats = ctx.get_stats()
+    # the initial explicit build + the cadence rebuilds at steps 0, 10, 20, 30, 40
+    assert stats["n_build_passes"] == 6 and stats["n_replica_builds"] == 6
+    assert ctx.status() & B.FLAG_SKIN_VIOLATED == 0
+    assert abs(st.e_rep.item() - md.e_rep[0]) <= 5e-6 * abs(md.e_rep[0])
+
+
+def test_nve_energy_conservation_gpu(B):
+    w = W.config1()
+    ctx, st = setup(B, w)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    e = []
+    with torch.cuda.stream(stream):
+        for blk in range(20):
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, 2.0, st.T, 0.0, st.seed, blk * 50, 50, None, None, 0,
+                       st.e_rep, None, st.ekin)
+            stream.synchronize()
+            e.append((st.e_rep.item() + st.ekin.item()) / w.n_atoms)
+    e = np.array(e)
+    assert np.abs(e - e[0]).max() < 3e-5 and abs(e[-4:].mean() - e[:4].mean()) < 5e-6
+
+
+def test_md_run_host_matches_device_path(B):
+    w = W.config2(length=60.0)
+    _, st = run_gpu_md(B, w, 30)
+    ctx = B.make_context(w)
+    pos, vel = w.pos4.copy(), w.vel4.copy()
+    force = np.zeros_like(pos)
+    tag = np.arange(w.n_atoms, dtype=np.int32)
+    e, k = np.zeros(1), np.zeros(1)
+    ctx.md_run_host(pos, vel, force, tag, w.dt, w.T, w.gamma, w.seed, 0, 30, None, w.slab_rate, 0, e, None, k)
+    out = np.empty_like(pos)
+    out[tag] = pos
+    assert np.array_equal(out, st.untag(st.pos))
+    assert e[0] == pytest.approx(st.e_rep.item(), rel=1e-12) and k[0] == pytest.approx(st.ekin.item(), rel=1e-12)
+
+
+@pytest.mark.parametrize("which", ["config3", "config5a"])
+def test_full_size_sampled_parity(B, which):
+    """BASELINE full sizes, in the configuration bench.py times: sampled atoms recomputed one by one
+    by the oracle from scratch (brute force over the whole replica)."""
+    w = W.config3() if which == "config3" else W.config5a()
+    ctx, st = setup(B, w)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    rng = np.random.default_rng(0)
+    m = 48 if which == "config3" else 24
+    idx = np.sort(rng.choice(w.n_atoms, m, replace=False))
+    s = oracle.compute_sample(w.x64(), w.r_cut, idx, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, periodic=w.periodic)
+    fe = st.untag(st.force)
+    assert_forces(fe[idx, :3].astype(np.float64), s["f"])
+    assert np.abs(fe[idx, 3] - s["e_atom"]).max() < 1e-5
+    # properties that hold at any size: momentum conservation per replica, list symmetry via counts
+    f = fe[:, :3].astype(np.float64)
+    for r in range(0, w.n_replicas, max(1, w.n_replicas // 8)):
+        sl = slice(w.offsets[r], w.offsets[r + 1])
+        assert np.abs(f[sl].sum(0)).max() < 2e-3
+    entries, pairs = ctx.count_pairs(st.pos)
+    assert entries % 2 == 0 and pairs % 2 == 0
+    # whole-replica energy against the linked-cell oracle for one replica / a 10^6-atom box
+    if which == "config3":
+        r = 200
+        sub = w.take(r, r + 1)
+        oc = oracle.compute(sub.x64(), w.r_cut, lo=sub.box_lo, hi=sub.box_hi, cells=True)
+        assert abs(st.e_rep[r].item() - oc["e_rep"][0]) <= E_REL * abs(oc["e_rep"][0])
+    else:
+        oc = oracle.compute(w.x64(), w.r_cut, lo=w.box_lo, hi=w.box_hi, periodic=1, cells=True)
+        assert abs(st.e_rep[0].item() - oc["e_rep"][0]) <= E_REL * abs(oc["e_rep"][0])
+        assert_forces(f, oc["f"])
+        assert pairs == oc["n_pairs_directed"]
