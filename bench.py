@@ -217,7 +217,7 @@ def main():
     K, Wm = args.steps, args.warmup
     with torch.cuda.stream(stream):
         ctx.build_cells(st.pos, st.vel, st.tag)
-        ctx.build_neighbors(st.pos)
+        ctx.build_neighbors(st.pos, st.vel, st.tag)
         ctx.compute(st.pos, st.force, st.e_rep, None)
         ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, Wm, None, st.slab_rate,
                    w.rebuild_every, st.e_rep, None, st.ekin)

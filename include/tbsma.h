@@ -61,7 +61,9 @@ enum {
     TBSMA_FLAG_NLIST_OVERFLOW = 1u, /* an atom had more than max_neighbors partners: list truncated, results invalid */
     TBSMA_FLAG_OUT_OF_BOX = 2u,     /* an atom left its replica's (non-periodic) box: still correct, edge cells grow */
     TBSMA_FLAG_NONFINITE = 4u,      /* a non-finite force was produced */
-    TBSMA_FLAG_SKIN_VIOLATED = 8u   /* with a fixed rebuild cadence an atom moved more than skin/2 between rebuilds */
+    TBSMA_FLAG_SKIN_VIOLATED = 8u,  /* with a fixed rebuild cadence an atom moved more than skin/2 between rebuilds */
+    TBSMA_FLAG_TILE_OVERFLOW = 16u  /* shared-memory variant: a tile's halo outgrew its shared-memory image (sized at
+                                       tbsma_build_cells with 25 % headroom); that tile was skipped, results invalid */
 };
 
 typedef struct {
@@ -96,8 +98,11 @@ int tbsma_set_system(tbsma_ctx *ctx, int64_t n_atoms, int32_t n_replicas,
 int tbsma_build_cells(tbsma_ctx *ctx, float *d_pos, float *d_vel, int32_t *d_tag, void *stream);
 
 /* Neighbour list of every atom: all j != i of the same replica with |r_i - r_j| < r_cut + skin,
- * membership decided by the fp32 predicate of D:A6.  Needs tbsma_build_cells on the same d_pos. */
-int tbsma_build_neighbors(tbsma_ctx *ctx, const float *d_pos, void *stream);
+ * membership decided by the fp32 predicate of D:A6.  Must directly follow tbsma_build_cells on the
+ * same d_pos / d_vel (nullable) / d_tag.  The shared-memory variant additionally reorders the atoms
+ * inside every z-layer of cells by neighbour count (longest lists first, ties by slot) and permutes
+ * d_pos, d_vel and d_tag accordingly; the global variant leaves them untouched. */
+int tbsma_build_neighbors(tbsma_ctx *ctx, float *d_pos, float *d_vel, int32_t *d_tag, void *stream);
 
 /* One force evaluation (stage 1 densities, stage 2 forces) over the current list.
  * d_force_energy: out, n x 4 (F_i, E_i).  d_replica_energy: out, n_replicas doubles, E_C of each
@@ -156,9 +161,22 @@ int tbsma_status(tbsma_ctx *ctx, uint32_t *h_flags); /* synchronises the device;
 int tbsma_clear_status(tbsma_ctx *ctx);
 int tbsma_get_stats(tbsma_ctx *ctx, tbsma_stats *h_out); /* synchronises */
 
-/* Selects the neighbour-gather kernel variant: 0 = auto, 1 = thread-per-atom over a k-major
- * int32 list with L1-cached global gathers.  Other values are reserved. */
+/* Selects the neighbour-gather kernel variant (takes effect at the next tbsma_build_cells):
+ *   1 = thread per atom over a k-major int32 list, neighbour records gathered from global memory
+ *       through L1 (any system, periodic or not);
+ *   2 = shared-memory tiles: one CTA per run of z-layers of cells of a NON-periodic replica stages
+ *       the positions of its atoms and their halo in shared memory; 16-bit list entries, atoms
+ *       ordered by list length inside a layer, lists ordered for conflict-free shared-memory gathers.
+ *       tbsma_build_cells returns TBSMA_EINVAL if a replica is periodic or its layers do not fit;
+ *   0 = auto (default): 2 when it fits, else 1.
+ * tbsma_get_variant returns the variant the current lists were built for. */
 int tbsma_set_variant(tbsma_ctx *ctx, int32_t variant);
+int tbsma_get_variant(const tbsma_ctx *ctx);
+
+/* Shape of the shared-memory tiles: own z-layers of cells per tile (1..8, default 2; a replica whose
+ * layers are too populated gets fewer) and threads per CTA of the two gather kernels (multiple of
+ * 32, <= 512, default 256).  Takes effect at the next tbsma_build_cells. */
+int tbsma_set_tile(tbsma_ctx *ctx, int32_t layers_per_tile, int32_t threads);
 
 /* md_run replays one captured step as a CUDA graph when enabled (default 1) and the stream is
  * not the legacy default stream. */

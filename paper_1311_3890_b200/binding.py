@@ -14,12 +14,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtbsma.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
-FLAG_NLIST_OVERFLOW, FLAG_OUT_OF_BOX, FLAG_NONFINITE, FLAG_SKIN_VIOLATED = 1, 2, 4, 8
+FLAG_NLIST_OVERFLOW, FLAG_OUT_OF_BOX, FLAG_NONFINITE, FLAG_SKIN_VIOLATED, FLAG_TILE_OVERFLOW = 1, 2, 4, 8, 16
 
 EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
+    "tbsma_get_variant", "tbsma_set_tile",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
 
@@ -61,7 +62,7 @@ def lib():
         L.tbsma_destroy.argtypes = [vp]
         L.tbsma_set_system.argtypes = [vp, i64, i32, vp, vp, vp, vp, i32]
         L.tbsma_build_cells.argtypes = [vp, vp, vp, vp, vp]
-        L.tbsma_build_neighbors.argtypes = [vp, vp, vp]
+        L.tbsma_build_neighbors.argtypes = [vp, vp, vp, vp, vp]
         L.tbsma_compute.argtypes = [vp, vp, vp, vp, vp, vp]
         L.tbsma_md_step.argtypes = [vp, vp, vp, vp, vp, dbl, vp, dbl, vp, C.c_uint64, vp, vp, vp, vp, vp]
         L.tbsma_md_run.argtypes = [vp, vp, vp, vp, vp, dbl, vp, dbl, vp, C.c_uint64, i64, vp, vp, i32, vp, vp, vp, vp]
@@ -72,6 +73,8 @@ def lib():
         L.tbsma_clear_status.argtypes = [vp]
         L.tbsma_get_stats.argtypes = [vp, C.POINTER(Stats)]
         L.tbsma_set_variant.argtypes = [vp, i32]
+        L.tbsma_get_variant.argtypes = [vp]
+        L.tbsma_set_tile.argtypes = [vp, i32, i32]
         L.tbsma_set_graph.argtypes = [vp, i32]
         L.tbsma_set_timing.argtypes = [vp, i32]
         L.tbsma_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
@@ -151,8 +154,9 @@ class Context:
     def build_cells(self, pos, vel, tag, stream=None):
         _check(lib().tbsma_build_cells(self._h, _dp(pos), _dp(vel), _dp(tag), _stream(stream)), "tbsma_build_cells")
 
-    def build_neighbors(self, pos, stream=None):
-        _check(lib().tbsma_build_neighbors(self._h, _dp(pos), _stream(stream)), "tbsma_build_neighbors")
+    def build_neighbors(self, pos, vel, tag, stream=None):
+        _check(lib().tbsma_build_neighbors(self._h, _dp(pos), _dp(vel), _dp(tag), _stream(stream)),
+               "tbsma_build_neighbors")
 
     def compute(self, pos, force_energy, replica_energy=None, replica_virial=None, stream=None):
         _check(lib().tbsma_compute(self._h, _dp(pos), _dp(force_energy), _dp(replica_energy), _dp(replica_virial),
@@ -206,6 +210,12 @@ class Context:
 
     def set_variant(self, variant):
         _check(lib().tbsma_set_variant(self._h, int(variant)), "tbsma_set_variant")
+
+    def get_variant(self):
+        return int(lib().tbsma_get_variant(self._h))
+
+    def set_tile(self, layers_per_tile, threads):
+        _check(lib().tbsma_set_tile(self._h, int(layers_per_tile), int(threads)), "tbsma_set_tile")
 
     def set_graph(self, enable):
         _check(lib().tbsma_set_graph(self._h, int(bool(enable))), "tbsma_set_graph")

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtbsma.so")
-SOURCES = ["tbsma_api.cu", "tbsma_cells.cu", "tbsma_force.cu", "tbsma_integrate.cu"]
+SOURCES = ["tbsma_api.cu", "tbsma_cells.cu", "tbsma_force.cu", "tbsma_integrate.cu", "tbsma_tile.cu"]
 
 
 def _stale():

@@ -37,6 +37,11 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_cell_of); cudaFree(c->d_slot); cudaFree(c->d_order); cudaFree(c->d_pos_build);
     cudaFree(c->d_tmp4); cudaFree(c->d_tmp_tag); cudaFree(c->d_nlist); cudaFree(c->d_nn); cudaFree(c->d_xs);
     cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters);
+    cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_newslot); cudaFree(c->d_oldof);
+    cudaFree(c->d_nn_tmp); cudaFree(c->d_tmp_pos);
+    c->d_tiles = nullptr; c->d_maxpop = nullptr; c->d_hbase = nullptr; c->d_newslot = nullptr; c->d_oldof = nullptr;
+    c->d_nn_tmp = nullptr; c->d_tmp_pos = nullptr;
+    c->n_tiles = 0; c->active_variant = 1;
     c->d_geom = nullptr; c->d_atom_rep = nullptr; c->d_cell_count = nullptr; c->d_cell_start = nullptr;
     c->d_cell_of = nullptr; c->d_slot = nullptr; c->d_order = nullptr; c->d_pos_build = nullptr;
     c->d_tmp4 = nullptr; c->d_tmp_tag = nullptr; c->d_nlist = nullptr; c->d_nn = nullptr; c->d_xs = nullptr;
@@ -103,9 +108,11 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         if (ev) CK(cudaEventRecord(ev[1], st));
         CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
         if (ev) CK(cudaEventRecord(ev[2], st));
-        CK(tbsma_launch_density(c, pos, st));
+        if (c->active_variant == 2) CK(tbsma_launch_density_tile(c, pos, st));
+        else CK(tbsma_launch_density(c, pos, st));
         if (ev) CK(cudaEventRecord(ev[3], st));
-        CK(tbsma_launch_force(c, force, e_rep, w_rep, kk, st));
+        if (c->active_variant == 2) CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, st));
+        else CK(tbsma_launch_force(c, force, e_rep, w_rep, kk, st));
         if (ev) CK(cudaEventRecord(ev[4], st));
         CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
         if (ev) CK(cudaEventRecord(ev[5], st));
@@ -146,7 +153,10 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->r_cut = r_cut;
     c->skin = skin;
     c->device = dev;
-    c->variant = 1;
+    c->variant = 0;
+    c->active_variant = 1;
+    c->tile_layers = 2;
+    c->tile_threads = 256;
     c->use_graph = 1;
     int sm = 0;
     if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sm < 1) sm = 148;
@@ -173,8 +183,22 @@ int tbsma_destroy(tbsma_ctx *c)
 
 int tbsma_set_variant(tbsma_ctx *c, int32_t variant)
 {
-    if (!c || variant < 0 || variant > 1) return TBSMA_EINVAL;
-    c->variant = variant == 0 ? 1 : variant;
+    if (!c || variant < 0 || variant > 2) return TBSMA_EINVAL;
+    c->variant = variant;
+    c->cells_built = c->list_built = 0;   // lists must be rebuilt for the new variant
+    return TBSMA_OK;
+}
+
+int tbsma_get_variant(const tbsma_ctx *c) { return c ? c->active_variant : TBSMA_EINVAL; }
+
+int tbsma_set_tile(tbsma_ctx *c, int32_t layers_per_tile, int32_t threads)
+{
+    if (!c || layers_per_tile < 1 || layers_per_tile > TBSMA_TILE_MAX_LAYERS || threads < 32 || threads > 512 ||
+        (threads & 31))
+        return TBSMA_EINVAL;
+    c->tile_layers = layers_per_tile;
+    c->tile_threads = threads;
+    c->cells_built = c->list_built = 0;
     return TBSMA_OK;
 }
 
@@ -282,6 +306,8 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     DA(c->d_pos_build, n); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
     DA(c->d_nlist, (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, n); DA(c->d_xs, n);
     DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8);
+    DA(c->d_maxpop, (size_t)R); DA(c->d_hbase, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
+    DA(c->d_tmp_pos, n);
 #undef DA
     if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
     int32_t *rep = (int32_t *)malloc(sizeof(int32_t) * (n ? n : 1));
@@ -307,21 +333,24 @@ int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, 
     if (!c->d_geom) return TBSMA_ESTATE;
     if (c->n == 0) { c->cells_built = 1; return TBSMA_OK; }
     cudaStream_t st = (cudaStream_t)stream;
+    c->list_built = 0;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // tiles may change
     CK(tbsma_launch_mark_all_dirty(c, st));
     CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, true, false, st));
+    const int rc = tbsma_tile_setup(c, st);   // picks the gather variant for these cells (synchronises)
+    if (rc) return rc;
     c->cells_built = 1;
-    c->list_built = 0;
     return TBSMA_OK;
 }
 
-int tbsma_build_neighbors(tbsma_ctx *c, const float *d_pos, void *stream)
+int tbsma_build_neighbors(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, void *stream)
 {
-    if (!c || !d_pos) return TBSMA_EINVAL;
+    if (!c || !d_pos || !d_tag) return TBSMA_EINVAL;
     if (!c->d_geom || !c->cells_built) return TBSMA_ESTATE;
     if (c->n == 0) { c->list_built = 1; return TBSMA_OK; }
     cudaStream_t st = (cudaStream_t)stream;
     CK(tbsma_launch_mark_all_dirty(c, st));
-    CK(tbsma_launch_rebuild(c, (float4 *)d_pos, nullptr, nullptr, false, true, st));
+    CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, false, true, st));
     CK(tbsma_launch_finish_step(c, 0, st));
     c->list_built = 1;
     return TBSMA_OK;
@@ -335,9 +364,14 @@ int tbsma_compute(tbsma_ctx *c, const float *d_pos, float *d_force_energy, doubl
     if (d_e) CK(cudaMemsetAsync(d_e, 0, sizeof(double) * c->R, st));
     if (d_w) CK(cudaMemsetAsync(d_w, 0, sizeof(double) * 6 * c->R, st));
     if (c->n == 0) return TBSMA_OK;
-    CK(tbsma_launch_density(c, (const float4 *)d_pos, st));
     KickArgs kk = {nullptr, 0.f, 0.f, nullptr};
-    CK(tbsma_launch_force(c, (float4 *)d_force_energy, d_e, d_w, kk, st));
+    if (c->active_variant == 2) {
+        CK(tbsma_launch_density_tile(c, (const float4 *)d_pos, st));
+        CK(tbsma_launch_force_tile(c, (float4 *)d_force_energy, d_e, d_w, kk, st));
+    } else {
+        CK(tbsma_launch_density(c, (const float4 *)d_pos, st));
+        CK(tbsma_launch_force(c, (float4 *)d_force_energy, d_e, d_w, kk, st));
+    }
     return TBSMA_OK;
 }
 
@@ -439,7 +473,7 @@ int tbsma_md_run_host(tbsma_ctx *c, float *h_pos, float *h_vel, float *h_force, 
     if (h_disp0) CK(cudaMemcpyAsync(c->s_disp0, h_disp0, 8 * (size_t)R, H2D, st));
     if (h_rate) CK(cudaMemcpyAsync(c->s_rate, h_rate, 8 * (size_t)R, H2D, st));
     int rc = tbsma_build_cells(c, (float *)c->s_pos, (float *)c->s_vel, c->s_tag, st);
-    if (!rc) rc = tbsma_build_neighbors(c, (float *)c->s_pos, st);
+    if (!rc) rc = tbsma_build_neighbors(c, (float *)c->s_pos, (float *)c->s_vel, c->s_tag, st);
     if (!rc) rc = tbsma_compute(c, (float *)c->s_pos, (float *)c->s_force, c->s_e, h_w ? c->s_w : nullptr, st);
     if (!rc) rc = tbsma_md_run(c, (float *)c->s_pos, (float *)c->s_vel, (float *)c->s_force, c->s_tag, dt_fs, c->s_T,
                                gamma_per_fs, (const uint64_t *)c->s_seed, step0, n_steps, h_disp0 ? c->s_disp0 : nullptr,
@@ -461,7 +495,8 @@ int tbsma_get_neighbors(tbsma_ctx *c, const int32_t *d_tag, int32_t *d_counts, i
     if (!c || !d_tag || !d_counts || !d_list) return TBSMA_EINVAL;
     if (!c->list_built) return TBSMA_ESTATE;
     if (c->n == 0) return TBSMA_OK;
-    CK(tbsma_launch_get_neighbors(c, d_tag, d_counts, d_list, (cudaStream_t)stream));
+    if (c->active_variant == 2) CK(tbsma_launch_get_neighbors_tile(c, d_tag, d_counts, d_list, (cudaStream_t)stream));
+    else CK(tbsma_launch_get_neighbors(c, d_tag, d_counts, d_list, (cudaStream_t)stream));
     return TBSMA_OK;
 }
 
@@ -473,7 +508,8 @@ int tbsma_count_pairs(tbsma_ctx *c, const float *d_pos, int64_t *h_entries, int6
     unsigned long long out[2] = {0, 0};
     if (c->n > 0) {
         CK(cudaMemsetAsync(c->d_counters + 4, 0, 2 * sizeof(unsigned long long), st));
-        CK(tbsma_launch_count_pairs(c, (const float4 *)d_pos, c->d_counters + 4, st));
+        if (c->active_variant == 2) CK(tbsma_launch_count_pairs_tile(c, (const float4 *)d_pos, c->d_counters + 4, st));
+        else CK(tbsma_launch_count_pairs(c, (const float4 *)d_pos, c->d_counters + 4, st));
         CK(cudaMemcpyAsync(out, c->d_counters + 4, sizeof(out), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
     }

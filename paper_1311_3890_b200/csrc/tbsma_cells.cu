@@ -165,13 +165,13 @@ __global__ void k_reorder_gather(const float4 *__restrict__ pos, const float4 *_
 
 __global__ void k_reorder_copyback(float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ tag,
                                    const int *__restrict__ atom_rep, const int *__restrict__ dirty,
-                                   const int *__restrict__ ctrl, const float4 *__restrict__ pos_build,
+                                   const int *__restrict__ ctrl, const float4 *__restrict__ tmp_pos,
                                    const float4 *__restrict__ tmp4, const int *__restrict__ tmp_tag, int n)
 {
     if (!ctrl[0]) return;
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
         if (!dirty[atom_rep[k]]) continue;
-        pos[k] = pos_build[k];
+        pos[k] = tmp_pos[k];
         if (vel) vel[k] = tmp4[k];
         tag[k] = tmp_tag[k];
     }
@@ -306,11 +306,23 @@ cudaError_t tbsma_launch_rebuild(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t
                                                                       (int)c->n_cells);
         // d_slot is free after the scatter: reuse it for the cell id of every sorted slot
         k_reorder_gather<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, c->d_geom, c->d_dirty,
-                                                  c->d_ctrl, c->d_order, c->d_cell_of, c->d_pos_build,
+                                                  c->d_ctrl, c->d_order, c->d_cell_of, c->d_tmp_pos,
                                                   c->d_tmp4, c->d_tmp_tag, c->d_slot, n);
-        k_reorder_copyback<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, c->d_dirty, c->d_ctrl,
-                                                    c->d_pos_build, c->d_tmp4, c->d_tmp_tag, n);
-        c->launches += 6;
+        c->launches += 5;
+        // the tile variant moves the atoms once more (count order inside each layer) while it builds
+        // the lists, so its copy-back is part of tbsma_launch_tile_lists
+        if (!(do_list && c->active_variant == 2)) {
+            k_reorder_copyback<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, c->d_dirty, c->d_ctrl,
+                                                        c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, n);
+            c->launches++;
+        }
+    }
+    if (do_list && c->active_variant == 2) {
+        if (!do_cells) {
+            cudaError_t e = tbsma_launch_stage_copy(c, pos, vel, tag, st);
+            if (e != cudaSuccess) return e;
+        }
+        return tbsma_launch_tile_lists(c, pos, vel, tag, st);
     }
     if (do_list) {
         const int gl = grid_for(c, n, 128, 16);

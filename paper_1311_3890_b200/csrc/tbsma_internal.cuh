@@ -34,6 +34,24 @@ struct RepGeom {
     int atom_begin, atom_end;
 };
 
+// One tile of the shared-memory ("wire") variant: a run of consecutive z-layers of cells of one
+// non-periodic replica.  Atoms are in cell order (z slowest), so the tile's own atoms and its halo
+// (one more layer on each side) are contiguous index ranges; both follow from cell_start at run time.
+struct TileDesc {
+    int rep;          // replica
+    int ch0;          // global cell index of the first cell of the first halo layer
+    int nlay_h;       // halo layers = own layers + (0..2)
+    int own_first;    // index, among the halo layers, of the first own layer (0 or 1)
+    int own_n;        // own layers
+    int layer_cells;  // nx * ny
+    int nx, ny, nz;
+    int z_h0;         // z index of the first halo layer
+    int cell_base;    // first cell of the replica
+    int pad;
+};
+#define TBSMA_TILE_MAX_LAYERS 8      // own layers per tile
+#define TBSMA_TILE_MAX_RECORDS 4095  // halo records per tile: (records + sentinel) * 16 B <= 64 KB, u16 byte offsets
+
 struct GraphKey {          // arguments a cached one-step CUDA graph was captured with
     const void *p[11];
     double dt, gamma;
@@ -55,7 +73,21 @@ struct tbsma_ctx {
     int kmax;         // list capacity per atom, multiple of 4
     int64_t n_cells;  // total cells over all replicas
     int any_periodic;
-    int variant;
+    int variant;        // requested: 0 auto, 1 global gather, 2 shared-memory tiles
+    int active_variant; // what the lists are currently built for (1 or 2)
+    // tile variant
+    int tile_layers;    // own layers per tile requested (<= TBSMA_TILE_MAX_LAYERS)
+    int tile_threads;   // CTA size of the tile kernels
+    int tile_cap;       // halo records a tile may hold in shared memory
+    int tile_cell_cap;  // halo cells (+1) a tile may hold in shared memory
+    int n_tiles;
+    TileDesc *d_tiles;
+    int32_t *d_maxpop;  // R: largest layer population of each replica (measured at build_cells)
+    int32_t *d_hbase;   // n: first halo slot of the tile that owns slot i
+    int32_t *d_newslot; // n: cell-order slot -> final slot
+    int32_t *d_oldof;   // n: final slot -> cell-order slot
+    int32_t *d_nn_tmp;  // n
+    float4 *d_tmp_pos;  // n: cell-ordered positions during a rebuild
 
     // host copies
     int32_t *h_off;
@@ -124,6 +156,18 @@ cudaError_t tbsma_launch_force(tbsma_ctx *c, float4 *force, double *e_rep, doubl
                                cudaStream_t st);
 cudaError_t tbsma_launch_count_pairs(tbsma_ctx *c, const float4 *pos, unsigned long long *d_out2,
                                      cudaStream_t st);
+// shared-memory tile variant (tbsma_tile.cu)
+int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st);   // host: sizes the tiles from the binned cells (synchronises)
+cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, cudaStream_t st);
+cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float4 *vel, const int32_t *tag,
+                                    cudaStream_t st);
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, cudaStream_t st);
+cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kick,
+                                    cudaStream_t st);
+cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
+                                            cudaStream_t st);
+cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsigned long long *d_out2,
+                                          cudaStream_t st);
 // integrator (tbsma_integrate.cu)
 struct StepArgs {
     float half_dt, kick, c1, c2, sigma_scale;  // sigma_v = sigma_scale * sqrt(T)

@@ -1,0 +1,681 @@
+// tbsma_tile.cu -- the shared-memory ("wire") variant of the neighbour machinery and of the two
+// neighbour-gather passes for NON-PERIODIC replicas.
+//
+// The paper's systems are thin [100] wires and its best performance came with the
+// atoms ordered along the wire axis.  With cells numbered z-slowest, a run of z-layers of
+// cells ("tile") and its one-layer halo are CONTIGUOUS index ranges, so one CTA can stage every
+// position its atoms will ever gather (a few thousand records) in shared memory with one coalesced
+// copy and serve all neighbour gathers from there.  That allows
+//   * 16-bit neighbour entries (byte offsets into the tile's shared-memory image): half the list
+//     bytes of the int32 list, which is the dominant HBM stream of both passes;
+//   * atoms ordered inside each layer by neighbour count (longest lists first), so the 32 lanes of
+//     a warp run the same number of iterations (surface atoms of a 3 nm wire have 42 partners,
+//     core atoms 86);
+//   * each atom's list ordered so that at step p lane l reads a record of bank group (l + p) mod 8:
+//     the eight lanes served by one shared-memory wavefront of a 128-bit load then hit eight
+//     different 16-byte bank groups (summation order is free, A15).
+// Membership is the fp32 predicate of D:A6, operation for operation, as in tbsma_cells.cu.
+#include "tbsma_internal.cuh"
+
+namespace {
+
+constexpr int kTileThreads = 256;   // build kernels; the gather kernels use c->tile_threads
+
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// index ranges of a tile, from the cell starts at its layer boundaries
+struct TileRange { int halo_lo, nh, lo, hi; };
+__device__ __forceinline__ TileRange tile_range(const TileDesc &t, const int *__restrict__ cell_start)
+{
+    TileRange r;
+    r.halo_lo = cell_start[t.ch0];
+    r.nh = cell_start[t.ch0 + t.nlay_h * t.layer_cells] - r.halo_lo;
+    r.lo = cell_start[t.ch0 + t.own_first * t.layer_cells];
+    r.hi = cell_start[t.ch0 + (t.own_first + t.own_n) * t.layer_cells];
+    return r;
+}
+
+// largest layer population of every replica (sizes the tiles; host reads it back at build_cells)
+__global__ void k_layer_maxpop(const RepGeom *__restrict__ geom, const int *__restrict__ cell_start,
+                               int *__restrict__ maxpop, int R)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    const RepGeom *g = geom + r;
+    const int lc = g->nc[0] * g->nc[1];
+    int m = 0;
+    for (int z = 0; z < g->nc[2]; ++z)
+        m = max(m, cell_start[g->cell_base + (z + 1) * lc] - cell_start[g->cell_base + z * lc]);
+    maxpop[r] = m;
+}
+
+// ---- K1: scan.  Cell-ordered positions of the tile + halo in shared memory; every own atom scans
+// its 3 x 3 runs of x-adjacent cells, writes its partners (halo-local cell-order indices, u16) to
+// the temporary list, and is ranked inside its layer by (count descending, slot ascending).
+__global__ void __launch_bounds__(kTileThreads)
+k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
+            const int *__restrict__ cell_sorted, const int *__restrict__ dirty, int *__restrict__ ctrl,
+            const float4 *__restrict__ pos_sorted, uint2 *__restrict__ nl_tmp, int *__restrict__ nn_tmp,
+            int *__restrict__ newslot, int *__restrict__ oldof, int n_pad, int kmax, float rl2,
+            int s_cap, int cell_cap)
+{
+    if (!ctrl[0]) return;
+    const TileDesc t = tiles[blockIdx.x];
+    if (!dirty[t.rep]) return;
+    extern __shared__ float4 smem_f4[];
+    float4 *sm = smem_f4;
+    int *cs = reinterpret_cast<int *>(sm + s_cap);
+    unsigned short *cnts = reinterpret_cast<unsigned short *>(cs + cell_cap);
+    __shared__ int lb[TBSMA_TILE_MAX_LAYERS + 4];
+    const int tid = threadIdx.x;
+    if (tid <= t.nlay_h) lb[tid] = cell_start[t.ch0 + tid * t.layer_cells];
+    __syncthreads();
+    const int halo_lo = lb[0], nh = lb[t.nlay_h] - halo_lo;
+    const int lo = lb[t.own_first], hi = lb[t.own_first + t.own_n];
+    if (hi <= lo) return;
+    if (nh > s_cap) {
+        if (tid == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
+        return;
+    }
+    const int ncell_h = t.nlay_h * t.layer_cells;
+    for (int k = tid; k <= ncell_h; k += kTileThreads) cs[k] = cell_start[t.ch0 + k] - halo_lo;
+    for (int k = tid; k < nh; k += kTileThreads) sm[k] = pos_sorted[halo_lo + k];
+    __syncthreads();
+    const int nx = t.nx, ny = t.ny, nz = t.nz;
+    for (int a = lo + tid; a < hi; a += kTileThreads) {
+        const int al = a - halo_lo;
+        const float4 pi = sm[al];
+        const int lc = cell_sorted[a] - t.cell_base;
+        const int cx = lc % nx, cy = (lc / nx) % ny, cz = lc / t.layer_cells;
+        const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
+        uint2 *row = nl_tmp + a;
+        unsigned w0 = 0u, w1 = 0u;
+        int cnt = 0;
+        for (int zz = max(cz - 1, 0); zz <= min(cz + 1, nz - 1); ++zz)
+            for (int yy = max(cy - 1, 0); yy <= min(cy + 1, ny - 1); ++yy) {
+                const int cb = ((zz - t.z_h0) * ny + yy) * nx;
+                const int s = cs[cb + x0], e = cs[cb + x1 + 1];
+                for (int j = s; j < e; ++j) {
+                    const float4 pj = sm[j];
+                    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
+                    if (d2 < rl2 && j != al) {
+                        if (cnt < kmax) {
+                            const unsigned v = (unsigned)j << ((cnt & 1) << 4);
+                            if (cnt & 2) w1 |= v; else w0 |= v;
+                            if ((cnt & 3) == 3) {
+                                row[(size_t)(cnt >> 2) * n_pad] = make_uint2(w0, w1);
+                                w0 = w1 = 0u;
+                            }
+                        }
+                        ++cnt;
+                    }
+                }
+            }
+        if (cnt > kmax) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
+        atomicMax(ctrl + 2, cnt);
+        cnt = min(cnt, kmax);
+        if (cnt & 3) row[(size_t)(cnt >> 2) * n_pad] = make_uint2(w0, w1);
+        cnts[a - lo] = (unsigned short)cnt;
+        nn_tmp[a] = cnt | ((__float_as_int(pi.w) & 3) << 16);
+    }
+    __syncthreads();
+    for (int a = lo + tid; a < hi; a += kTileThreads) {
+        int m = t.own_first;
+        while (a >= lb[m + 1]) ++m;
+        const int l0 = lb[m] - lo, l1 = lb[m + 1] - lo, me = a - lo;
+        const int my = cnts[me];
+        int rank = 0;
+        for (int b = l0; b < l1; ++b) {
+            const int cb = cnts[b];
+            rank += (cb > my) || (cb == my && b < me);
+        }
+        const int ns = lb[m] + rank;
+        newslot[a] = ns;
+        oldof[ns] = a;
+    }
+}
+
+__device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { return (unsigned)(v >> (c << 3)) & 0xffu; }
+
+// ---- K2: finish.  One thread per FINAL slot of the tile: reads the temporary row of the atom that
+// moves there, translates every partner to its final position (byte offset of its record in the
+// tile's shared-memory image, record k at (k + 1) * 16, the sentinel at 0), and writes the row in
+// bank-scheduled order: step p of lane l takes a partner of class (l + p) & 7 (class = bank group
+// of the record), falling back to the fullest class when that one is used up.
+__global__ void __launch_bounds__(kTileThreads)
+k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
+              const int *__restrict__ dirty, int *__restrict__ ctrl, const uint2 *__restrict__ nl_tmp,
+              const int *__restrict__ nn_tmp, const int *__restrict__ newslot, const int *__restrict__ oldof,
+              uint2 *__restrict__ nl, int *__restrict__ nn, int *__restrict__ hbase, int n_pad, int kmax,
+              int s_cap)
+{
+    if (!ctrl[0]) return;
+    const TileDesc t = tiles[blockIdx.x];
+    if (!dirty[t.rep]) return;
+    extern __shared__ float4 smem_f4[];
+    unsigned short *map = reinterpret_cast<unsigned short *>(smem_f4);   // s_cap entries
+    unsigned short *scr = map + ((s_cap + 7) & ~7);                      // kmax x kTileThreads
+    const TileRange r = tile_range(t, cell_start);
+    if (r.hi <= r.lo || r.nh > s_cap) return;
+    const int tid = threadIdx.x, lane = tid & 31;
+    for (int k = tid; k < r.nh; k += kTileThreads)
+        map[k] = (unsigned short)((newslot[r.halo_lo + k] - r.halo_lo + 1) << 4);
+    __syncthreads();
+    for (int ip = r.lo + tid; ip < r.hi; ip += kTileThreads) {
+        const int a = oldof[ip];
+        const int nnv = nn_tmp[a];
+        const int cnt = nnv & 0xffff;
+        const uint2 *src = nl_tmp + a;
+        const int ng = (cnt + 3) >> 2;
+        // pass A: population of the 8 classes (packed bytes; kmax <= 248)
+        unsigned long long pop = 0ull;
+        for (int g = 0; g < ng; ++g) {
+            const uint2 w = src[(size_t)g * n_pad];
+            const unsigned e[4] = {w.x & 0xffffu, w.x >> 16, w.y & 0xffffu, w.y >> 16};
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (4 * g + q < cnt) pop += 1ull << (((map[e[q]] >> 4) & 7) << 3);
+        }
+        unsigned long long off = 0ull;
+        {
+            unsigned run = 0;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) { off |= (unsigned long long)run << (c << 3); run += byte_of(pop, c); }
+        }
+        // pass B: class-sorted copy in shared memory (column tid: conflict-free for any row)
+        unsigned long long cur = 0ull;
+        for (int g = 0; g < ng; ++g) {
+            const uint2 w = src[(size_t)g * n_pad];
+            const unsigned e[4] = {w.x & 0xffffu, w.x >> 16, w.y & 0xffffu, w.y >> 16};
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (4 * g + q < cnt) {
+                    const unsigned m = map[e[q]];
+                    const int c = (m >> 4) & 7;
+                    const unsigned idx = byte_of(off, c) + byte_of(cur, c);
+                    cur += 1ull << (c << 3);
+                    scr[idx * kTileThreads + tid] = (unsigned short)m;
+                }
+        }
+        // emission in scheduled order
+        unsigned long long rem = pop;
+        cur = 0ull;
+        uint2 *dst = nl + ip;
+        unsigned w0 = 0u, w1 = 0u;
+        for (int p = 0; p < cnt; ++p) {
+            int c = (lane + p) & 7;
+            if (byte_of(rem, c) == 0u) {
+                unsigned best = 0u;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const int cc = (c + 4 + q) & 7;
+                    const unsigned v = byte_of(rem, cc);
+                    if (v > best) { best = v; c = cc; }
+                }
+            }
+            const unsigned idx = byte_of(off, c) + byte_of(cur, c);
+            cur += 1ull << (c << 3);
+            rem -= 1ull << (c << 3);
+            const unsigned v = (unsigned)scr[idx * kTileThreads + tid] << ((p & 1) << 4);
+            if (p & 2) w1 |= v; else w0 |= v;
+            if ((p & 3) == 3) {
+                dst[(size_t)(p >> 2) * n_pad] = make_uint2(w0, w1);
+                w0 = w1 = 0u;
+            }
+        }
+        if (cnt & 3) dst[(size_t)(cnt >> 2) * n_pad] = make_uint2(w0, w1);   // unused entries = 0 = the sentinel
+        nn[ip] = nnv;
+        hbase[ip] = r.halo_lo;
+    }
+}
+
+// ---- K3: move positions / velocities / tags from cell order to the final order (identity when
+// oldof is null) and record the positions of this build for the displacement check.
+__global__ void k_tile_permute(float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ tag,
+                               float4 *__restrict__ pos_build, const int *__restrict__ atom_rep,
+                               const int *__restrict__ dirty, const int *__restrict__ ctrl,
+                               const int *__restrict__ oldof, const float4 *__restrict__ tmp_pos,
+                               const float4 *__restrict__ tmp_vel, const int *__restrict__ tmp_tag, int n)
+{
+    if (!ctrl[0]) return;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
+        if (!dirty[atom_rep[k]]) continue;
+        const int a = oldof[k];
+        const float4 p = tmp_pos[a];
+        pos[k] = p;
+        pos_build[k] = p;
+        if (vel) vel[k] = tmp_vel[a];
+        tag[k] = tmp_tag[a];
+    }
+}
+
+// API path of tbsma_build_neighbors: stage the caller's arrays as the "cell-ordered" source of K3
+__global__ void k_stage_copy(const float4 *__restrict__ pos, const float4 *__restrict__ vel,
+                             const int *__restrict__ tag, float4 *__restrict__ tmp_pos,
+                             float4 *__restrict__ tmp_vel, int *__restrict__ tmp_tag, int n)
+{
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
+        tmp_pos[k] = pos[k];
+        if (vel) tmp_vel[k] = vel[k];
+        tmp_tag[k] = tag[k];
+    }
+}
+
+// ---- the two gather passes ---------------------------------------------------------------------
+// Shared-memory image of a tile: record 0 is a sentinel far from everything (list rows are padded
+// with offset 0 to a multiple of four entries: it fails the cutoff test like any distant atom, so
+// the loops need no self / padding test), record k + 1 is the atom at slot halo_lo + k.
+#define TBSMA_SENTINEL 1.0e9f
+
+__device__ __forceinline__ void fill_tile(float4 *sm, const float4 *__restrict__ src, int halo_lo, int nh)
+{
+    if (threadIdx.x == 0) sm[0] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
+    for (int k = threadIdx.x; k < nh; k += blockDim.x) sm[k + 1] = src[halo_lo + k];
+    __syncthreads();
+}
+
+__device__ __forceinline__ float4 lds_rec(const float4 *sm, unsigned byte_off)
+{
+    return *reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(sm) + byte_off);
+}
+
+__device__ __forceinline__ float rho_term_t(const float4 &pi, const float4 &pj, const PairConst &pc)
+{
+    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6 order
+    const float rinv = rsqrt_approx(d2);
+    const float t = __fmaf_rn(d2, rinv, -pc.r0f);                                // r - r0
+    const float e = ex2_approx(__fmaf_rn(pc.aq, t, pc.b_rho));                   // xi^2 e^{-2q x}
+    return d2 < pc.rc2 ? e : 0.f;
+}
+
+// stage 1 (Eq.1): rho_i over the list, s_i = rho_i^(-1/2) packed with the position
+__global__ void __launch_bounds__(512, 2)
+k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
+               const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
+               float4 *__restrict__ xs, int *__restrict__ ctrl, int n_pad, int s_cap, PairConst pc)
+{
+    const TileDesc t = tiles[blockIdx.x];
+    const TileRange r = tile_range(t, cell_start);
+    if (r.hi <= r.lo) return;
+    if (r.nh > s_cap) {
+        if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
+        return;
+    }
+    extern __shared__ float4 smem_f4[];
+    const float4 *sm = smem_f4;
+    fill_tile(smem_f4, pos, r.halo_lo, r.nh);
+    for (int i = r.lo + threadIdx.x; i < r.hi; i += blockDim.x) {
+        const float4 pi = sm[i - r.halo_lo + 1];
+        const int cnt = nn[i] & 0xffff;
+        const int ng = (cnt + 3) >> 2;
+        const uint2 *row = nl + i;
+        float rho0 = 0.f, rho1 = 0.f;
+        uint2 nxt = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
+        for (int g = 0; g < ng; ++g) {
+            const uint2 jj = nxt;
+            if (g + 1 < ng) nxt = __ldcs(row + (size_t)(g + 1) * n_pad);
+            const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
+            const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
+            rho0 += rho_term_t(pi, p0, pc);
+            rho1 += rho_term_t(pi, p1, pc);
+            rho0 += rho_term_t(pi, p2, pc);
+            rho1 += rho_term_t(pi, p3, pc);
+        }
+        const float rho = rho0 + rho1;
+        const float s = rho > 0.f ? 1.0f / sqrtf(rho) : 0.f;     // once per atom, IEEE (D:A5 for rho = 0)
+        xs[i] = make_float4(pi.x, pi.y, pi.z, s);
+    }
+}
+
+struct AccT {
+    float fx, fy, fz, er;
+    float wxx, wyy, wzz, wxy, wxz, wyz;
+};
+
+template <bool VIRIAL>
+__device__ __forceinline__ void force_term_t(const float4 &pi, const float4 &pj, const PairConst &pc, AccT &a)
+{
+    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+    const bool in = d2 < pc.rc2;
+    const float rinv = rsqrt_approx(d2);
+    const float t = __fmaf_rn(d2, rinv, -pc.r0f);
+    float er = ex2_approx(__fmaf_rn(pc.ap, t, pc.b_rep));          // (2Ap/r0) e^{-p x}
+    const float eb = ex2_approx(__fmaf_rn(pc.aq, t, pc.b_band));   // (q xi^2/r0) e^{-2q x}
+    float fp = (er - eb * (pi.w + pj.w)) * rinv;                   // -dE/dr / r
+    fp = in ? fp : 0.f;
+    er = in ? er : 0.f;
+    a.fx = __fmaf_rn(fp, dx, a.fx); a.fy = __fmaf_rn(fp, dy, a.fy); a.fz = __fmaf_rn(fp, dz, a.fz);
+    a.er += er;
+    if (VIRIAL) {
+        const float fx = __fmul_rn(fp, dx), fy = __fmul_rn(fp, dy), fz = __fmul_rn(fp, dz);
+        a.wxx = __fmaf_rn(dx, fx, a.wxx); a.wyy = __fmaf_rn(dy, fy, a.wyy); a.wzz = __fmaf_rn(dz, fz, a.wzz);
+        a.wxy = __fmaf_rn(dx, fy, a.wxy); a.wxz = __fmaf_rn(dx, fz, a.wxz); a.wyz = __fmaf_rn(dy, fz, a.wyz);
+    }
+}
+
+__device__ __forceinline__ double warp_sum_d(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// a6: CTA-wide fp64 sum -> one atomic per CTA (a tile belongs to exactly one replica)
+__device__ __forceinline__ void cta_add(double *dst, double v, double *red)
+{
+    v = warp_sum_d(v);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        double x = lane < nw ? red[lane] : 0.0;
+        x = warp_sum_d(x);
+        if (lane == 0) atomicAdd(dst, x);
+    }
+}
+
+// stage 2 (Eq.1-3, Eq.5): forces, per-atom energy, virial, closing half kick, E_kin
+template <bool VIRIAL, bool KICK>
+__global__ void __launch_bounds__(512, 2)
+k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
+             const float4 *__restrict__ xs, const uint2 *__restrict__ nl, const int *__restrict__ nn,
+             float4 *__restrict__ force, double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk,
+             int *__restrict__ ctrl, int n_pad, int s_cap, PairConst pc)
+{
+    const TileDesc t = tiles[blockIdx.x];
+    const TileRange r = tile_range(t, cell_start);
+    if (r.hi <= r.lo) return;
+    if (r.nh > s_cap) {
+        if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
+        return;
+    }
+    extern __shared__ float4 smem_f4[];
+    __shared__ double red[32];
+    const float4 *sm = smem_f4;
+    fill_tile(smem_f4, xs, r.halo_lo, r.nh);
+    double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    bool bad = false;
+    for (int i = r.lo + threadIdx.x; i < r.hi; i += blockDim.x) {
+        const float4 pi = sm[i - r.halo_lo + 1];
+        const int nni = nn[i];
+        const int ng = ((nni & 0xffff) + 3) >> 2;
+        const uint2 *row = nl + i;
+        AccT a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        uint2 nxt = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
+        for (int g = 0; g < ng; ++g) {
+            const uint2 jj = nxt;
+            if (g + 1 < ng) nxt = __ldcs(row + (size_t)(g + 1) * n_pad);
+            const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
+            const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
+            force_term_t<VIRIAL>(pi, p0, pc, a);
+            force_term_t<VIRIAL>(pi, p1, pc, a);
+            force_term_t<VIRIAL>(pi, p2, pc, a);
+            force_term_t<VIRIAL>(pi, p3, pc, a);
+        }
+        const float sqrt_rho = pi.w > 0.f ? 1.0f / pi.w : 0.f;
+        const float ei = __fmaf_rn(a.er, pc.e_rep_scale, -sqrt_rho);   // Eq.1-3: E_R^i + E_B^i
+        force[i] = make_float4(a.fx, a.fy, a.fz, ei);
+        bad = bad || !isfinite(a.fx + a.fy + a.fz + ei);
+        se += (double)ei;
+        if (KICK && (nni >> 16) == 0) {       // final B of the step, dynamic atoms only
+            float4 v = kk.vel[i];
+            v.x = __fmaf_rn(kk.kick, a.fx, v.x);
+            v.y = __fmaf_rn(kk.kick, a.fy, v.y);
+            v.z = __fmaf_rn(kk.kick, a.fz, v.z);
+            kk.vel[i] = v;
+            sk += (double)(kk.ke_scale * (v.x * v.x + v.y * v.y + v.z * v.z));
+        }
+        if (VIRIAL) {
+            sw[0] += 0.5 * (double)a.wxx; sw[1] += 0.5 * (double)a.wyy; sw[2] += 0.5 * (double)a.wzz;
+            sw[3] += 0.5 * (double)a.wxy; sw[4] += 0.5 * (double)a.wxz; sw[5] += 0.5 * (double)a.wyz;
+        }
+    }
+    if (bad) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NONFINITE);
+    if (e_rep) cta_add(e_rep + t.rep, se, red);
+    if (KICK && kk.ekin) cta_add(kk.ekin + t.rep, sk, red);
+    if (VIRIAL) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) cta_add(w_rep + 6 * (size_t)t.rep + k, sw[k], red);
+    }
+}
+
+// ---- inspection (parity tests, bench statistics) ----------------------------------------------
+__device__ __forceinline__ unsigned entry_of(const uint2 *__restrict__ nl, int n_pad, int i, int k)
+{
+    const uint2 w = nl[(size_t)(k >> 2) * n_pad + i];
+    const unsigned h = (k & 2) ? w.y : w.x;
+    return (k & 1) ? (h >> 16) : (h & 0xffffu);
+}
+
+__global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *__restrict__ nl,
+                                     const int *__restrict__ nn, const int *__restrict__ hbase,
+                                     int *__restrict__ counts, int *__restrict__ list, int n, int n_pad, int kmax)
+{
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int t = tag[i];
+        const int cnt = nn[i] & 0xffff;
+        counts[t] = cnt;
+        for (int k = 0; k < cnt; ++k)
+            list[(size_t)t * kmax + k] = tag[hbase[i] + (int)(entry_of(nl, n_pad, i, k) >> 4) - 1];
+    }
+}
+
+__global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *__restrict__ nl,
+                                   const int *__restrict__ nn, const int *__restrict__ hbase,
+                                   unsigned long long *__restrict__ out, int n, int n_pad, float rc2)
+{
+    unsigned long long entries = 0, inside = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float4 pi = pos[i];
+        const int cnt = nn[i] & 0xffff;
+        entries += cnt;
+        for (int k = 0; k < cnt; ++k) {
+            const float4 pj = pos[hbase[i] + (int)(entry_of(nl, n_pad, i, k) >> 4) - 1];
+            const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            inside += d2 < rc2;
+        }
+    }
+    atomicAdd(out, entries);
+    atomicAdd(out + 1, inside);
+}
+
+inline int grid_for(const tbsma_ctx *c, int64_t work, int threads, int per_sm)
+{
+    int64_t b = (work + threads - 1) / threads;
+    const int64_t cap = (int64_t)c->n_sm * per_sm;
+    if (b > cap) b = cap;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+size_t scan_smem(const tbsma_ctx *c)
+{
+    return (size_t)c->tile_cap * 16 + (size_t)c->tile_cell_cap * 4 + (size_t)c->tile_cap * 2;
+}
+size_t finish_smem(const tbsma_ctx *c)
+{
+    return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax * kTileThreads * 2;
+}
+size_t gather_smem(const tbsma_ctx *c) { return (size_t)(c->tile_cap + 1) * 16; }
+
+}  // namespace
+
+// Sizes the tiles of every replica from the cells just binned: replica r gets L_r own layers per
+// tile, the largest L <= tile_layers whose halo (L + 2 layers of the replica's most populated
+// layer, + 25 %) fits the shared-memory image.  L_r depends on replica r alone, so a replica is
+// tiled (and therefore summed) identically whatever batch it is part of.  Returns TBSMA_OK and
+// sets active_variant = 2, or leaves active_variant = 1 when a replica does not fit.
+int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
+{
+    c->active_variant = 1;
+    if (c->variant == 1 || c->n == 0) return TBSMA_OK;
+    if (c->any_periodic || c->kmax > 248) return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;
+    const int R = c->R;
+    k_layer_maxpop<<<(R + 127) / 128, 128, 0, st>>>(c->d_geom, c->d_cell_start, c->d_maxpop, R);
+    c->launches++;
+    int *maxpop = (int *)malloc(sizeof(int) * R);
+    if (!maxpop) return TBSMA_ENOMEM;
+    cudaError_t e = cudaMemcpyAsync(maxpop, c->d_maxpop, sizeof(int) * R, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { free(maxpop); return TBSMA_ECUDA; }
+    const int cap = TBSMA_TILE_MAX_RECORDS;
+    int lmax = c->tile_layers;
+    if (lmax < 1) lmax = 1;
+    if (lmax > TBSMA_TILE_MAX_LAYERS) lmax = TBSMA_TILE_MAX_LAYERS;
+    int64_t n_tiles = 0;
+    int cell_cap = 0, rec_cap = 0;
+    bool fits = true;
+    int *Lr = (int *)malloc(sizeof(int) * R);
+    if (!Lr) { free(maxpop); return TBSMA_ENOMEM; }
+    for (int r = 0; r < R && fits; ++r) {
+        const RepGeom &g = c->h_geom[r];
+        const int64_t pop = ((int64_t)maxpop[r] * 5 + 3) / 4 + 1;    // + 25 % for later rebuilds
+        int L = (int)(cap / pop) - 2;
+        if (L > lmax) L = lmax;
+        if (L < 1) { fits = false; break; }
+        const int lc = g.nc[0] * g.nc[1];
+        if ((int64_t)(L + 2) * lc + 1 > 8192) { fits = false; break; }
+        if ((L + 2) * lc + 1 > cell_cap) cell_cap = (L + 2) * lc + 1;
+        if ((int)((L + 2) * pop) > rec_cap) rec_cap = (int)((L + 2) * pop);
+        Lr[r] = L;
+        n_tiles += (g.nc[2] + L - 1) / L;
+    }
+    free(maxpop);
+    if (!fits || n_tiles > 0x7fffffff) {
+        free(Lr);
+        return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;   // forced tile variant that does not fit
+    }
+    TileDesc *h = (TileDesc *)malloc(sizeof(TileDesc) * (size_t)(n_tiles ? n_tiles : 1));
+    if (!h) { free(Lr); return TBSMA_ENOMEM; }
+    int64_t k = 0;
+    for (int r = 0; r < R; ++r) {
+        const RepGeom &g = c->h_geom[r];
+        const int lc = g.nc[0] * g.nc[1], nz = g.nc[2], L = Lr[r];
+        for (int z0 = 0; z0 < nz; z0 += L) {
+            const int z1 = z0 + L < nz ? z0 + L : nz;
+            const int zh0 = z0 > 0 ? z0 - 1 : 0, zh1 = z1 < nz ? z1 + 1 : nz;
+            TileDesc &t = h[k++];
+            t.rep = r;
+            t.ch0 = g.cell_base + zh0 * lc;
+            t.nlay_h = zh1 - zh0;
+            t.own_first = z0 - zh0;
+            t.own_n = z1 - z0;
+            t.layer_cells = lc;
+            t.nx = g.nc[0]; t.ny = g.nc[1]; t.nz = nz;
+            t.z_h0 = zh0;
+            t.cell_base = g.cell_base;
+            t.pad = 0;
+        }
+    }
+    free(Lr);
+    cudaFree(c->d_tiles);
+    c->d_tiles = nullptr;
+    e = cudaMalloc((void **)&c->d_tiles, sizeof(TileDesc) * (size_t)(n_tiles ? n_tiles : 1));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tiles, h, sizeof(TileDesc) * (size_t)n_tiles, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    free(h);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? TBSMA_ENOMEM : TBSMA_ECUDA;
+    c->n_tiles = (int)n_tiles;
+    c->tile_cap = rec_cap < cap ? rec_cap : cap;   // shared-memory image sized to the largest halo expected
+    c->tile_cell_cap = (cell_cap + 3) & ~3;
+    // opt in to > 48 KB of dynamic shared memory
+    const int sm_scan = (int)scan_smem(c), sm_fin = (int)finish_smem(c), sm_g = (int)gather_smem(c);
+    e = cudaFuncSetAttribute(k_tile_scan, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_scan);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tile_finish, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_fin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_density_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
+    if (e != cudaSuccess) return TBSMA_ECUDA;
+    c->active_variant = 2;
+    return TBSMA_OK;
+}
+
+// K1 -> K2 -> K3 for the dirty replicas; expects cell-ordered pos / vel / tag in the tmp buffers
+cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, cudaStream_t st)
+{
+    const int n = (int)c->n;
+    uint2 *nl = reinterpret_cast<uint2 *>(c->d_nlist);
+    uint2 *nl_tmp = nl + (size_t)(c->kmax / 4) * c->n_pad;    // second half of the int32-sized allocation
+    k_tile_scan<<<c->n_tiles, kTileThreads, scan_smem(c), st>>>(c->d_tiles, c->d_cell_start, c->d_slot, c->d_dirty,
+                                                               c->d_ctrl, c->d_tmp_pos, nl_tmp, c->d_nn_tmp,
+                                                               c->d_newslot, c->d_oldof, c->n_pad, c->kmax, c->pc.rl2,
+                                                               c->tile_cap, c->tile_cell_cap);
+    k_tile_finish<<<c->n_tiles, kTileThreads, finish_smem(c), st>>>(c->d_tiles, c->d_cell_start, c->d_dirty, c->d_ctrl,
+                                                                   nl_tmp, c->d_nn_tmp, c->d_newslot, c->d_oldof, nl,
+                                                                   c->d_nn, c->d_hbase, c->n_pad, c->kmax, c->tile_cap);
+    k_tile_permute<<<grid_for(c, n, 256, 8), 256, 0, st>>>(pos, vel, tag, c->d_pos_build, c->d_atom_rep, c->d_dirty,
+                                                          c->d_ctrl, c->d_oldof, c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, n);
+    c->launches += 3;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float4 *vel, const int32_t *tag,
+                                    cudaStream_t st)
+{
+    k_stage_copy<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(pos, vel, tag, c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, (int)c->n);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, cudaStream_t st)
+{
+    k_density_tile<<<c->n_tiles, c->tile_threads, gather_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos,
+                                                                       reinterpret_cast<const uint2 *>(c->d_nlist), c->d_nn,
+                                                                       c->d_xs, c->d_ctrl, c->n_pad, c->tile_cap, c->pc);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kk,
+                                    cudaStream_t st)
+{
+    const uint2 *nl = reinterpret_cast<const uint2 *>(c->d_nlist);
+    const size_t sm = gather_smem(c);
+    const int g = c->n_tiles, b = c->tile_threads;
+#define TBSMA_FT(V, K)                                                                                             \
+    k_force_tile<V, K><<<g, b, sm, st>>>(c->d_tiles, c->d_cell_start, c->d_xs, nl, c->d_nn, force, e_rep, w_rep, kk, \
+                                         c->d_ctrl, c->n_pad, c->tile_cap, c->pc)
+    if (w_rep) { if (kk.vel) TBSMA_FT(true, true); else TBSMA_FT(true, false); }
+    else       { if (kk.vel) TBSMA_FT(false, true); else TBSMA_FT(false, false); }
+#undef TBSMA_FT
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
+                                            cudaStream_t st)
+{
+    k_get_neighbors_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(tag, reinterpret_cast<const uint2 *>(c->d_nlist),
+                                                                   c->d_nn, c->d_hbase, counts, list, (int)c->n,
+                                                                   c->n_pad, c->kmax);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsigned long long *d_out2,
+                                          cudaStream_t st)
+{
+    k_count_pairs_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(pos, reinterpret_cast<const uint2 *>(c->d_nlist),
+                                                                 c->d_nn, c->d_hbase, d_out2, (int)c->n, c->n_pad,
+                                                                 c->pc.rc2);
+    c->launches++;
+    return cudaGetLastError();
+}

@@ -25,11 +25,21 @@ def B():
     return binding
 
 
-def setup(B, w, max_nb=96):
+VARIANTS = [1, 2]     # 1 = global-gather lists, 2 = shared-memory tiles (non-periodic replicas only)
+
+
+def setup(B, w, max_nb=96, variant=0, tile=None):
+    if variant == 2 and np.any(w.periodic):
+        pytest.skip("the shared-memory tile variant is for non-periodic replicas")
     ctx = B.make_context(w, max_nb)
+    ctx.set_variant(variant)
+    if tile:
+        ctx.set_tile(*tile)
     st = B.DeviceState(w)
     ctx.build_cells(st.pos, st.vel, st.tag)
-    ctx.build_neighbors(st.pos)
+    ctx.build_neighbors(st.pos, st.vel, st.tag)
+    if variant:
+        assert ctx.get_variant() == variant
     return ctx, st
 
 
@@ -71,10 +81,11 @@ WORKLOADS = {
 }
 
 
+@pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("name", list(WORKLOADS))
-def test_neighbor_sets_bit_exact(B, name):
+def test_neighbor_sets_bit_exact(B, name, variant):
     w = WORKLOADS[name]()
-    ctx, st = setup(B, w)
+    ctx, st = setup(B, w, variant=variant)
     cg, lg = gpu_neighbors(B, ctx, st)
     co, lo = oracle.neighbors(w.pos4, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
     assert ctx.status() & B.FLAG_NLIST_OVERFLOW == 0
@@ -91,10 +102,11 @@ def test_neighbor_sets_bit_exact(B, name):
     assert pairs == cc.sum()
 
 
+@pytest.mark.parametrize("variant", VARIANTS)
 @pytest.mark.parametrize("name", list(WORKLOADS))
-def test_force_energy_virial_parity(B, name):
+def test_force_energy_virial_parity(B, name, variant):
     w = WORKLOADS[name]()
-    ctx, st = setup(B, w)
+    ctx, st = setup(B, w, variant=variant)
     ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
     torch.cuda.synchronize()
     assert ctx.status() == 0
@@ -116,11 +128,12 @@ def test_force_energy_virial_parity(B, name):
     assert torch.equal(f2, st.force)
 
 
-def test_paper_cutoff_5p8(B):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_paper_cutoff_5p8(B, variant):
     """the paper's own r_cut = 5.8 A, r_buff = 0.29 A"""
     w = W.config1()
     w.r_cut, w.skin = 5.8, 0.29
-    ctx, st = setup(B, w)
+    ctx, st = setup(B, w, variant=variant)
     ctx.compute(st.pos, st.force, st.e_rep, None)
     o = oracle.compute(w.x64(), 5.8)
     assert_forces(st.untag(st.force)[:, :3].astype(np.float64), o["f"])
@@ -130,7 +143,8 @@ def test_paper_cutoff_5p8(B):
     assert_same_sets(cg, lg, co, lo)
 
 
-def test_degenerate_systems(B):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_degenerate_systems(B, variant):
     # single atom, dimer inside / outside the cutoff, an empty replica in the middle (reading A5)
     x = np.array([[0, 0, 0], [10, 0, 0], [12.5, 0, 0], [30, 0, 0], [38, 0, 0]], dtype=np.float64)
     offs = np.array([0, 1, 3, 3, 5], dtype=np.int32)
@@ -138,7 +152,7 @@ def test_degenerate_systems(B):
     hi = np.array([[5, 5, 5], [20, 5, 5], [1, 1, 1], [45, 5, 5]], np.float32)
     w = W.Workload("degenerate", W.pack_pos4(x), W.pack_vel4(np.zeros((5, 3)), W.pack_pos4(x)), offs, lo, hi,
                    np.zeros((4, 3), np.uint8), np.zeros(4, np.float32), np.arange(4, dtype=np.uint64), np.zeros(4))
-    ctx, st = setup(B, w)
+    ctx, st = setup(B, w, variant=variant)
     ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
     torch.cuda.synchronize()
     o = oracle.compute(x, 7.0, offsets=offs, lo=lo, hi=hi, periodic=0)
@@ -150,12 +164,14 @@ def test_degenerate_systems(B):
     assert ctx.status() == 0
 
 
-def test_list_overflow_is_flagged(B):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_list_overflow_is_flagged(B, variant):
     w = W.config1()
     ctx = B.make_context(w, 32)            # far too small for r = 7.3 A (up to 86 partners)
+    ctx.set_variant(variant)
     st = B.DeviceState(w)
     ctx.build_cells(st.pos, st.vel, st.tag)
-    ctx.build_neighbors(st.pos)
+    ctx.build_neighbors(st.pos, st.vel, st.tag)
     assert ctx.status() & B.FLAG_NLIST_OVERFLOW
     assert ctx.get_stats()["max_neighbors_seen"] == 86
     ctx.clear_status()
@@ -170,7 +186,7 @@ def test_call_order_and_arguments(B):
         ctx.compute(st.pos, st.force)
     assert e.value.code == B.ESTATE
     with pytest.raises(B.TbsmaError) as e:
-        ctx.build_neighbors(st.pos)
+        ctx.build_neighbors(st.pos, st.vel, st.tag)
     assert e.value.code == B.ESTATE
     bad = B.Context()
     with pytest.raises(B.TbsmaError) as e:        # periodic box shorter than 2 (r_cut + skin)
@@ -178,8 +194,8 @@ def test_call_order_and_arguments(B):
     assert e.value.code == B.EINVAL
 
 
-def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False):
-    ctx, st = setup(B, w)
+def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None):
+    ctx, st = setup(B, w, variant=variant, tile=tile)
     ctx.set_graph(graph)
     ctx.compute(st.pos, st.force, st.e_rep, None)
     stream = torch.cuda.Stream()
@@ -212,9 +228,10 @@ def traj_rms(xg, xo, box_len=None):
     return math.sqrt((d ** 2).sum(1).mean())
 
 
-def test_trajectory_config1_nve_100_steps(B):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_trajectory_config1_nve_100_steps(B, variant):
     w = W.config1()
-    ctx, st = run_gpu_md(B, w, 100)
+    ctx, st = run_gpu_md(B, w, 100, variant=variant)
     md = run_oracle_md(w, 100)
     assert traj_rms(st.untag(st.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
     assert abs(st.e_rep.item() - md.e_rep[0]) <= 5e-6 * abs(md.e_rep[0])
@@ -226,10 +243,11 @@ def test_trajectory_config1_nve_100_steps(B):
     assert ctx.get_stats()["n_steps"] == 100
 
 
-def test_trajectory_config2_langevin_grips_pull(B):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_trajectory_config2_langevin_grips_pull(B, variant):
     w = W.config2()
     n_steps = 100
-    ctx, st = run_gpu_md(B, w, n_steps)
+    ctx, st = run_gpu_md(B, w, n_steps, variant=variant)
     md = run_oracle_md(w, n_steps)
     xg = st.untag(st.pos)[:, :3].astype(np.float64)
     assert traj_rms(xg, md.x) <= TRAJ_RMS
@@ -247,28 +265,57 @@ def test_trajectory_config2_langevin_grips_pull(B):
     assert ctx.status() == 0
 
 
-def test_md_step_equals_md_run_and_graph_bitwise(B):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_md_step_equals_md_run_and_graph_bitwise(B, variant):
     w = W.config2(length=60.0)
-    _, a = run_gpu_md(B, w, 40, use_run=True, graph=True)
-    _, b = run_gpu_md(B, w, 40, use_run=True, graph=False)
-    _, c = run_gpu_md(B, w, 40, use_run=False)
+    _, a = run_gpu_md(B, w, 40, use_run=True, graph=True, variant=variant)
+    _, b = run_gpu_md(B, w, 40, use_run=True, graph=False, variant=variant)
+    _, c = run_gpu_md(B, w, 40, use_run=False, variant=variant)
     for s in (b, c):
         assert np.array_equal(a.untag(a.pos), s.untag(s.pos))
         assert np.array_equal(a.untag(a.vel), s.untag(s.vel))
         assert np.array_equal(a.untag(a.force), s.untag(s.force))
 
 
-def test_replicas_are_independent_and_ragged_batch_matches_single_runs(B):
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_replicas_are_independent_and_ragged_batch_matches_single_runs(B, variant):
     w = W.config4(4, seed=21)
     n_steps = 60
-    _, st = run_gpu_md(B, w, n_steps)
+    _, st = run_gpu_md(B, w, n_steps, variant=variant)
     xb = st.untag(st.pos)
     assert len(set(np.diff(w.offsets))) > 1        # really ragged
     for r in range(w.n_replicas):
         single = w.take(r, r + 1)
-        _, ss = run_gpu_md(B, single, n_steps)
+        _, ss = run_gpu_md(B, single, n_steps, variant=variant)
         s = slice(w.offsets[r], w.offsets[r + 1])
         assert np.array_equal(xb[s], ss.untag(ss.pos))          # bit-identical: no cross-replica effect
+
+
+def test_auto_variant_and_tile_shapes(B):
+    """auto picks the shared-memory tiles for wires and the global lists for periodic systems; every
+    tile shape gives the same neighbour sets and forces within the bars"""
+    _, _ = setup(B, small_bulk(4))
+    ctx, st = setup(B, small_bulk(4))
+    assert ctx.get_variant() == 1
+    w = W.config4(3, seed=5)
+    co, lo = oracle.neighbors(w.pos4, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+    o = oracle.compute(w.x64(), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, periodic=w.periodic)
+    for tile in [None, (1, 128), (2, 64), (3, 512), (8, 256)]:
+        ctx, st = setup(B, w, tile=tile)
+        assert ctx.get_variant() == 2
+        cg, lg = gpu_neighbors(B, ctx, st)
+        assert_same_sets(cg, lg, co, lo)
+        ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
+        torch.cuda.synchronize()
+        assert ctx.status() == 0
+        assert_forces(st.untag(st.force)[:, :3].astype(np.float64), o["f"])
+        assert np.all(np.abs(st.e_rep.cpu().numpy() - o["e_rep"]) <= E_REL * np.abs(o["e_rep"]))
+    bad = B.make_context(small_bulk(4))
+    bad.set_variant(2)
+    stb = B.DeviceState(small_bulk(4))
+    with pytest.raises(B.TbsmaError) as e:       # periodic replicas cannot use the tile variant
+        bad.build_cells(stb.pos, stb.vel, stb.tag)
+    assert e.value.code == B.EINVAL
 
 
 def test_philox_noise_matches_oracle(B):
