@@ -68,10 +68,10 @@ enum {
 
 typedef struct {
     uint64_t n_steps;          /* md steps taken since tbsma_set_system */
-    uint64_t n_replica_builds; /* neighbour-list builds, counted per replica */
+    uint64_t n_replica_builds; /* neighbour-list builds, counted per replica (both kinds, see tbsma_set_outer_skin) */
     uint64_t n_build_passes;   /* steps (or explicit calls) in which at least one replica was rebuilt */
     int32_t max_neighbors_seen;
-    int32_t reserved;
+    int32_t n_candidate_builds; /* of those, builds that also redid the cells and the candidate list (saturating) */
 } tbsma_stats;
 
 /* Create a context for one parameter set.  r_cut: interaction cutoff, plain truncation, strict
@@ -173,6 +173,14 @@ int tbsma_get_stats(tbsma_ctx *ctx, tbsma_stats *h_out); /* synchronises */
 int tbsma_set_variant(tbsma_ctx *ctx, int32_t variant);
 int tbsma_get_variant(const tbsma_ctx *ctx);
 
+/* Shared-memory variant: buffer radius S of the CANDIDATE list (default 2.0 A).  The cell scan collects every
+ * pair within r_cut + skin + S, once; while no atom has moved more than S/2 since then, the replica's list
+ * (radius r_cut + skin) is re-filtered from those candidates whenever its atoms have moved more than skin/2
+ * (inside the density pass of that step).  Membership of the list is decided by the predicate of D:A6 either way,
+ * so S changes cost, never results; SKIN_VIOLATED is raised if candidates were used beyond their validity.
+ * Takes effect at the next tbsma_build_cells. */
+int tbsma_set_outer_skin(tbsma_ctx *ctx, double outer_skin);
+
 /* Shape of the shared-memory tiles: own z-layers of cells per tile (1..8, default 2; a replica whose
  * layers are too populated gets fewer) and threads per CTA of the two gather kernels (multiple of
  * 32, <= 512, default 256).  Takes effect at the next tbsma_build_cells. */
@@ -181,6 +189,12 @@ int tbsma_set_tile(tbsma_ctx *ctx, int32_t layers_per_tile, int32_t threads);
 /* md_run replays one captured step as a CUDA graph when enabled (default 1) and the stream is
  * not the legacy default stream. */
 int tbsma_set_graph(tbsma_ctx *ctx, int32_t enable);
+
+/* Shared-memory variant only: when enabled (default 1) an MD step runs the neighbour rebuild of the replicas that
+ * need one, followed by their two gather passes, on a second stream of the context, concurrently with the gather
+ * passes of all other replicas on `stream` (replicas never interact); both are joined before the step ends, so the
+ * caller sees ordinary stream semantics.  Results are bitwise identical either way. */
+int tbsma_set_overlap(tbsma_ctx *ctx, int32_t enable);
 
 /* Per-kernel-class timing of tbsma_md_step / tbsma_md_run with CUDA events recorded on the
  * launching stream (graph replay is off while enabled; at most 512 steps are recorded).

@@ -20,7 +20,7 @@ EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
-    "tbsma_get_variant", "tbsma_set_tile",
+    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_outer_skin",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
 
@@ -32,7 +32,7 @@ class Params(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [("n_steps", C.c_uint64), ("n_replica_builds", C.c_uint64), ("n_build_passes", C.c_uint64),
-                ("max_neighbors_seen", C.c_int32), ("reserved", C.c_int32)]
+                ("max_neighbors_seen", C.c_int32), ("n_candidate_builds", C.c_int32)]
 
 
 def au_params():
@@ -76,6 +76,8 @@ def lib():
         L.tbsma_get_variant.argtypes = [vp]
         L.tbsma_set_tile.argtypes = [vp, i32, i32]
         L.tbsma_set_graph.argtypes = [vp, i32]
+        L.tbsma_set_overlap.argtypes = [vp, i32]
+        L.tbsma_set_outer_skin.argtypes = [vp, dbl]
         L.tbsma_set_timing.argtypes = [vp, i32]
         L.tbsma_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.tbsma_launch_count.argtypes = [vp]
@@ -206,7 +208,8 @@ class Context:
         s = Stats()
         _check(lib().tbsma_get_stats(self._h, C.byref(s)), "tbsma_get_stats")
         return dict(n_steps=int(s.n_steps), n_replica_builds=int(s.n_replica_builds),
-                    n_build_passes=int(s.n_build_passes), max_neighbors_seen=int(s.max_neighbors_seen))
+                    n_build_passes=int(s.n_build_passes), max_neighbors_seen=int(s.max_neighbors_seen),
+                    n_candidate_builds=int(s.n_candidate_builds))
 
     def set_variant(self, variant):
         _check(lib().tbsma_set_variant(self._h, int(variant)), "tbsma_set_variant")
@@ -219,6 +222,12 @@ class Context:
 
     def set_graph(self, enable):
         _check(lib().tbsma_set_graph(self._h, int(bool(enable))), "tbsma_set_graph")
+
+    def set_outer_skin(self, outer_skin):
+        _check(lib().tbsma_set_outer_skin(self._h, float(outer_skin)), "tbsma_set_outer_skin")
+
+    def set_overlap(self, enable):
+        _check(lib().tbsma_set_overlap(self._h, int(bool(enable))), "tbsma_set_overlap")
 
     def set_timing(self, enable):
         _check(lib().tbsma_set_timing(self._h, int(bool(enable))), "tbsma_set_timing")

@@ -39,6 +39,8 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters);
     cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_newslot); cudaFree(c->d_oldof);
     cudaFree(c->d_nn_tmp); cudaFree(c->d_tmp_pos);
+    cudaFree(c->d_olist); cudaFree(c->d_nn_o); cudaFree(c->d_pos_outer); cudaFree(c->d_want_outer);
+    c->d_olist = nullptr; c->d_nn_o = nullptr; c->d_pos_outer = nullptr; c->d_want_outer = nullptr;
     c->d_tiles = nullptr; c->d_maxpop = nullptr; c->d_hbase = nullptr; c->d_newslot = nullptr; c->d_oldof = nullptr;
     c->d_nn_tmp = nullptr; c->d_tmp_pos = nullptr;
     c->n_tiles = 0; c->active_variant = 1;
@@ -68,6 +70,8 @@ void fold_constants(tbsma_ctx *c)
     const float rc = (float)c->r_cut, rl = (float)(c->r_cut + c->skin);
     k.rc2 = rc * rc;   // fp32 product, as D:A6 prescribes
     k.rl2 = rl * rl;
+    const float ro = (float)(c->r_cut + c->skin + c->outer_skin);
+    k.ro2 = ro * ro;
     k.r0f = (float)P.r0;
     const double log2e = 1.4426950408889634074;
     const double aq = -2.0 * P.q / P.r0 * log2e, ap = -P.p / P.r0 * log2e;
@@ -78,6 +82,72 @@ void fold_constants(tbsma_ctx *c)
     k.b_rep = (float)(log2(2.0 * P.A * P.p / P.r0) + ap * dr0);
     k.b_band = (float)(log2(P.q * P.xi * P.xi / P.r0) + aq * dr0);
     k.e_rep_scale = (float)(P.r0 / (2.0 * P.p));
+}
+
+
+// Cell grid of every replica for cells at least `width` wide (+ a margin over the fp32 rounding of cell
+// coordinates); (re)allocates the cell arrays.  The tile variant scans for candidates within
+// r_cut + skin + outer_skin, the global variant for list members within r_cut + skin.
+int set_geometry(tbsma_ctx *c, double width)
+{
+    const int R = c->R;
+    const double w_min = width * (1.0 + 1e-5) + 1e-4;
+    int64_t cells = 0;
+    for (int r = 0; r < R; ++r) {
+        RepGeom &g = c->h_geom[r];
+        int64_t nc_r = 1;
+        for (int a = 0; a < 3; ++a) {
+            const float len = g.len[a];
+            int nc = (int)floor((double)len / w_min);
+            if (nc < 1) nc = 1;
+            if (nc > 1024) nc = 1024;
+            g.nc[a] = nc;
+            g.inv_w[a] = len > 0.0f ? (float)((double)nc / (double)len) : 0.0f;
+            nc_r *= nc;
+        }
+        g.cell_base = (int)cells;
+        cells += nc_r;
+        if (cells > 0x7ffffff0ll) return TBSMA_EINVAL;
+    }
+    cudaFree(c->d_cell_count); cudaFree(c->d_cell_start);
+    c->d_cell_count = nullptr; c->d_cell_start = nullptr;
+    c->n_cells = cells;
+    c->cell_w = width;
+    CK(dalloc(&c->d_cell_count, (size_t)cells));
+    CK(dalloc(&c->d_cell_start, (size_t)cells + 1));
+    CK(cudaMemset(c->d_cell_count, 0, sizeof(int32_t) * (size_t)cells));
+    CK(cudaMemset(c->d_cell_start, 0, sizeof(int32_t) * ((size_t)cells + 1)));
+    CK(cudaMemcpy(c->d_geom, c->h_geom, sizeof(RepGeom) * R, cudaMemcpyHostToDevice));
+    return TBSMA_OK;
+}
+
+// Cell width and candidate-list storage for the variant the next build will try (called by tbsma_build_cells).
+int ensure_variant_resources(tbsma_ctx *c)
+{
+    const bool tiles = c->variant != 1 && !c->any_periodic;
+    const double r_list = c->r_cut + c->skin;
+    const double width = tiles ? r_list + c->outer_skin : r_list;
+    if (width != c->cell_w) {
+        CK(cudaDeviceSynchronize());
+        const int rc = set_geometry(c, width);
+        if (rc) return rc;
+    }
+    if (tiles && !c->d_olist) {
+        const double ratio = (r_list + c->outer_skin) / r_list;
+        int ko = (int)ceil(c->kmax * ratio * ratio * ratio * 1.25) + 8;   // volume ratio + room for a lattice shell
+        ko = (ko + 3) / 4 * 4;
+        if (ko > 248) ko = 248;        // byte-packed class counters of k_tile_finish
+        if (ko < c->kmax) ko = c->kmax;
+        c->kmax_o = ko;
+        const size_t n = (size_t)c->n;
+        CK(dalloc(&c->d_olist, (size_t)2 * (ko / 4) * (size_t)c->n_pad));
+        CK(dalloc(&c->d_nn_o, n));
+        CK(dalloc(&c->d_pos_outer, n));
+        CK(dalloc(&c->d_want_outer, (size_t)c->R));
+        CK(cudaMemset(c->d_want_outer, 0, sizeof(int32_t) * (size_t)c->R));
+        CK(cudaMemset(c->d_nn_o, 0, sizeof(int32_t) * (n ? n : 1)));
+    }
+    return TBSMA_OK;
 }
 
 int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *tag, double dt, const float *T,
@@ -97,6 +167,7 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
     a.rebuild_every = rebuild_every;
     a.step_base = step0;
     a.T = T; a.seed = seed; a.disp0 = disp0; a.rate = rate;
+    a.want_outer = c->active_variant == 2 ? c->d_want_outer : nullptr;
     a.e_rep = e_rep; a.w_rep = w_rep; a.ekin = ekin;
     KickArgs kk;
     kk.vel = vel; kk.kick = a.kick; kk.ke_scale = (float)(0.5 * c->prm.mass_amu / TBSMA_ACC); kk.ekin = ekin;
@@ -105,13 +176,31 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         if (c->timing && c->tev && c->tev_steps < TBSMA_TIMING_MAX_STEPS) ev = c->tev + 6 * (c->tev_steps++);
         if (ev) CK(cudaEventRecord(ev[0], st));
         CK(tbsma_launch_integrate_pre(c, pos, vel, force, tag, a, st));
+        if (c->active_variant == 2 && c->overlap && !c->timing && c->aux_stream && c->R > 1) {
+            // fork: the replicas that keep their lists go straight to the two gather passes on `st`; the rebuild
+            // chain of the others, then their gather passes, run on the high-priority second stream
+            cudaStream_t s2 = c->aux_stream;
+            CK(cudaEventRecord(c->ev_fork, st));
+            CK(cudaStreamWaitEvent(s2, c->ev_fork, 0));
+            CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, s2));
+            CK(tbsma_launch_tile_inner(c, pos, s2));
+            CK(tbsma_launch_density_tile(c, pos, TBSMA_TILES_DIRTY, s2));
+            CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, TBSMA_TILES_DIRTY, s2));
+            CK(cudaEventRecord(c->ev_join, s2));
+            CK(tbsma_launch_density_tile(c, pos, TBSMA_TILES_CLEAN, st));
+            CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, TBSMA_TILES_CLEAN, st));
+            CK(cudaStreamWaitEvent(st, c->ev_join, 0));
+            CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
+            continue;
+        }
         if (ev) CK(cudaEventRecord(ev[1], st));
         CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
+        if (c->active_variant == 2) CK(tbsma_launch_tile_inner(c, pos, st));
         if (ev) CK(cudaEventRecord(ev[2], st));
-        if (c->active_variant == 2) CK(tbsma_launch_density_tile(c, pos, st));
+        if (c->active_variant == 2) CK(tbsma_launch_density_tile(c, pos, TBSMA_TILES_ALL, st));
         else CK(tbsma_launch_density(c, pos, st));
         if (ev) CK(cudaEventRecord(ev[3], st));
-        if (c->active_variant == 2) CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, st));
+        if (c->active_variant == 2) CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, TBSMA_TILES_ALL, st));
         else CK(tbsma_launch_force(c, force, e_rep, w_rep, kk, st));
         if (ev) CK(cudaEventRecord(ev[4], st));
         CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
@@ -155,9 +244,23 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->device = dev;
     c->variant = 0;
     c->active_variant = 1;
+    c->outer_skin = 2.0;
     c->tile_layers = 2;
     c->tile_threads = 256;
     c->use_graph = 1;
+    c->overlap = 1;
+    {
+        int lo_prio = 0, hi_prio = 0;
+        cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio);
+        if (cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, hi_prio) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+            if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+            free(c);
+            return TBSMA_ECUDA;
+        }
+    }
     int sm = 0;
     if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sm < 1) sm = 148;
     c->n_sm = sm;
@@ -173,6 +276,9 @@ int tbsma_destroy(tbsma_ctx *c)
     free_system(c);
     free_staging(c);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->tev) {
         for (int i = 0; i < 6 * TBSMA_TIMING_MAX_STEPS; ++i) if (c->tev[i]) cudaEventDestroy(c->tev[i]);
         free(c->tev);
@@ -202,10 +308,32 @@ int tbsma_set_tile(tbsma_ctx *c, int32_t layers_per_tile, int32_t threads)
     return TBSMA_OK;
 }
 
+int tbsma_set_outer_skin(tbsma_ctx *c, double outer_skin)
+{
+    if (!c || !(outer_skin >= 0.0) || !(outer_skin <= 16.0)) return TBSMA_EINVAL;
+    if (c->d_olist) {
+        cudaDeviceSynchronize();
+        cudaFree(c->d_olist); cudaFree(c->d_nn_o); cudaFree(c->d_pos_outer); cudaFree(c->d_want_outer);
+        c->d_olist = nullptr; c->d_nn_o = nullptr; c->d_pos_outer = nullptr; c->d_want_outer = nullptr;
+    }
+    c->outer_skin = outer_skin;
+    fold_constants(c);
+    c->cells_built = c->list_built = 0;
+    return TBSMA_OK;
+}
+
 int tbsma_set_graph(tbsma_ctx *c, int32_t enable)
 {
     if (!c) return TBSMA_EINVAL;
     c->use_graph = enable != 0;
+    return TBSMA_OK;
+}
+
+int tbsma_set_overlap(tbsma_ctx *c, int32_t enable)
+{
+    if (!c) return TBSMA_EINVAL;
+    c->overlap = enable != 0;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     return TBSMA_OK;
 }
 
@@ -265,44 +393,29 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     if (!c->h_off || !c->h_geom) { free_system(c); return TBSMA_ENOMEM; }
     memcpy(c->h_off, h_off, sizeof(int32_t) * (R + 1));
     const double r_list = c->r_cut + c->skin;
-    const double w_min = r_list * (1.0 + 1e-5) + 1e-4;   // margin over fp32 rounding of cell coordinates
-    int64_t cells = 0;
     c->any_periodic = 0;
     for (int r = 0; r < R; ++r) {
         RepGeom &g = c->h_geom[r];
         g.periodic = 0;
-        int64_t nc_r = 1;
         for (int a = 0; a < 3; ++a) {
             const float lo = h_lo[3 * r + a], hi = h_hi[3 * r + a];
             const float len = hi - lo;          // fp32 difference
             if (!(len >= 0.0f) || !isfinite(len)) { free_system(c); return TBSMA_EINVAL; }
-            const bool per = h_per[3 * r + a] != 0;
-            if (per) {
+            if (h_per[3 * r + a] != 0) {
                 if ((double)len < 2.0 * r_list) { free_system(c); return TBSMA_EINVAL; }
                 g.periodic |= 1 << a;
                 c->any_periodic = 1;
             }
-            int nc = (int)floor((double)len / w_min);
-            if (nc < 1) nc = 1;
-            if (nc > 1024) nc = 1024;
             g.lo[a] = lo;
             g.len[a] = len;
-            g.nc[a] = nc;
-            g.inv_w[a] = len > 0.0f ? (float)((double)nc / (double)len) : 0.0f;
-            nc_r *= nc;
         }
-        g.cell_base = (int)cells;
         g.atom_begin = h_off[r];
         g.atom_end = h_off[r + 1];
-        cells += nc_r;
-        if (cells > 0x7ffffff0ll) { free_system(c); return TBSMA_EINVAL; }
     }
-    c->n_cells = cells;
     const size_t n = (size_t)n_atoms;
     cudaError_t e = cudaSuccess;
 #define DA(ptr, cnt) if (e == cudaSuccess) e = dalloc(&(ptr), (cnt))
-    DA(c->d_geom, (size_t)R); DA(c->d_atom_rep, n); DA(c->d_cell_count, (size_t)cells);
-    DA(c->d_cell_start, (size_t)cells + 1); DA(c->d_cell_of, n); DA(c->d_slot, n); DA(c->d_order, n);
+    DA(c->d_geom, (size_t)R); DA(c->d_atom_rep, n); DA(c->d_cell_of, n); DA(c->d_slot, n); DA(c->d_order, n);
     DA(c->d_pos_build, n); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
     DA(c->d_nlist, (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, n); DA(c->d_xs, n);
     DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8);
@@ -316,14 +429,15 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
         for (int64_t i = h_off[r]; i < h_off[r + 1]; ++i) rep[i] = r;
     e = cudaMemcpy(c->d_atom_rep, rep, sizeof(int32_t) * n, cudaMemcpyHostToDevice);
     free(rep);
-    if (e == cudaSuccess) e = cudaMemcpy(c->d_geom, c->h_geom, sizeof(RepGeom) * R, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemset(c->d_cell_count, 0, sizeof(int32_t) * (size_t)cells);
-    if (e == cudaSuccess) e = cudaMemset(c->d_cell_start, 0, sizeof(int32_t) * ((size_t)cells + 1));
     if (e == cudaSuccess) e = cudaMemset(c->d_dirty, 0, sizeof(int32_t) * R);
     if (e == cudaSuccess) e = cudaMemset(c->d_ctrl, 0, sizeof(int32_t) * 8);
     if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, sizeof(unsigned long long) * 8);
     if (e == cudaSuccess) e = cudaMemset(c->d_nn, 0, sizeof(int32_t) * (n ? n : 1));
     if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
+    c->cell_w = 0.0;
+    c->kmax_o = c->kmax;
+    const int rc = set_geometry(c, (c->variant != 1 && !c->any_periodic) ? r_list + c->outer_skin : r_list);
+    if (rc) { free_system(c); return rc; }
     return TBSMA_OK;
 }
 
@@ -335,6 +449,11 @@ int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, 
     cudaStream_t st = (cudaStream_t)stream;
     c->list_built = 0;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // tiles may change
+    {
+        const int rc0 = ensure_variant_resources(c);
+        if (rc0) return rc0;
+    }
+    c->active_variant = (c->variant != 1 && !c->any_periodic) ? 2 : 1;   // provisional: selects the dirty level
     CK(tbsma_launch_mark_all_dirty(c, st));
     CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, true, false, st));
     const int rc = tbsma_tile_setup(c, st);   // picks the gather variant for these cells (synchronises)
@@ -351,6 +470,7 @@ int tbsma_build_neighbors(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_t
     cudaStream_t st = (cudaStream_t)stream;
     CK(tbsma_launch_mark_all_dirty(c, st));
     CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, false, true, st));
+    if (c->active_variant == 2) CK(tbsma_launch_tile_inner(c, (const float4 *)d_pos, st));
     CK(tbsma_launch_finish_step(c, 0, st));
     c->list_built = 1;
     return TBSMA_OK;
@@ -366,8 +486,8 @@ int tbsma_compute(tbsma_ctx *c, const float *d_pos, float *d_force_energy, doubl
     if (c->n == 0) return TBSMA_OK;
     KickArgs kk = {nullptr, 0.f, 0.f, nullptr};
     if (c->active_variant == 2) {
-        CK(tbsma_launch_density_tile(c, (const float4 *)d_pos, st));
-        CK(tbsma_launch_force_tile(c, (float4 *)d_force_energy, d_e, d_w, kk, st));
+        CK(tbsma_launch_density_tile(c, (const float4 *)d_pos, TBSMA_TILES_ALL, st));
+        CK(tbsma_launch_force_tile(c, (float4 *)d_force_energy, d_e, d_w, kk, TBSMA_TILES_ALL, st));
     } else {
         CK(tbsma_launch_density(c, (const float4 *)d_pos, st));
         CK(tbsma_launch_force(c, (float4 *)d_force_energy, d_e, d_w, kk, st));
@@ -545,7 +665,7 @@ int tbsma_get_stats(tbsma_ctx *c, tbsma_stats *out)
     memset(out, 0, sizeof(*out));
     if (!c->d_ctrl) return TBSMA_OK;
     CK(cudaDeviceSynchronize());
-    unsigned long long cnt[4];
+    unsigned long long cnt[8];
     int ctrl[4];
     CK(cudaMemcpy(cnt, c->d_counters, sizeof(cnt), cudaMemcpyDeviceToHost));
     CK(cudaMemcpy(ctrl, c->d_ctrl, sizeof(ctrl), cudaMemcpyDeviceToHost));
@@ -553,6 +673,7 @@ int tbsma_get_stats(tbsma_ctx *c, tbsma_stats *out)
     out->n_replica_builds = cnt[1];
     out->n_build_passes = cnt[2];
     out->max_neighbors_seen = ctrl[2];
+    out->n_candidate_builds = (int32_t)(cnt[6] > 0x7fffffffull ? 0x7fffffffull : cnt[6]);
     return TBSMA_OK;
 }
 

@@ -26,14 +26,14 @@ __device__ __forceinline__ int cell_coord(float x, float lo, float inv_w, int nc
 
 // a1: key of every atom + histogram.  slot = arrival order inside the cell (made stable later).
 __global__ void k_bin_count(const float4 *__restrict__ pos, const int *__restrict__ atom_rep,
-                            const RepGeom *__restrict__ geom, const int *__restrict__ dirty,
+                            const RepGeom *__restrict__ geom, DirtyView dv,
                             int *__restrict__ ctrl, int *__restrict__ cell_count,
                             int *__restrict__ cell_of, int *__restrict__ slot, int n)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int r = atom_rep[i];
-        if (!dirty[r]) continue;
+        if (dv.dirty[r] < dv.level) continue;
         const RepGeom *g = geom + r;
         const float4 p = pos[i];
         bool outside = false;
@@ -49,11 +49,11 @@ __global__ void k_bin_count(const float4 *__restrict__ pos, const int *__restric
 }
 
 // a1: exclusive scan of the histogram, one CTA per replica; re-zeroes the histogram for next time.
-__global__ void k_cell_scan(const RepGeom *__restrict__ geom, const int *__restrict__ dirty,
+__global__ void k_cell_scan(const RepGeom *__restrict__ geom, DirtyView dv,
                             int *__restrict__ cell_count, int *__restrict__ cell_start)
 {
     const int r = blockIdx.x;
-    if (!dirty[r]) return;
+    if (!*dv.any || dv.dirty[r] < dv.level) return;
     __shared__ int warp_tot[32];
     __shared__ int s_running;
     const RepGeom *g = geom + r;
@@ -96,57 +96,73 @@ __global__ void k_cell_scan(const RepGeom *__restrict__ geom, const int *__restr
     if (threadIdx.x == 0) cell_start[base + ncell] = s_running;
 }
 
-__global__ void k_scatter(const int *__restrict__ atom_rep, const int *__restrict__ dirty,
-                          const int *__restrict__ ctrl, const int *__restrict__ cell_start,
+__global__ void k_scatter(const int *__restrict__ atom_rep, DirtyView dv, const int *__restrict__ cell_start,
                           const int *__restrict__ cell_of, const int *__restrict__ slot,
                           int *__restrict__ order, int n)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        if (!dirty[atom_rep[i]]) continue;
+        if (dv.dirty[atom_rep[i]] < dv.level) continue;
         order[cell_start[cell_of[i]] + slot[i]] = i;
     }
 }
 
 // Make the order inside each cell independent of atomic arrival order: sort by tag (determinism,
 // and an order that does not depend on history, so restarts reproduce the fp32 summation order).
-__global__ void k_cell_sort(const int *__restrict__ atom_rep, const int *__restrict__ dirty,
-                            const int *__restrict__ ctrl, const int *__restrict__ cell_start,
-                            const int *__restrict__ tag, int *__restrict__ order, int n_cells)
+// grid = (R, kSortSplit): the CTAs of a clean replica exit at once; a warp takes one cell at a time
+// and ranks its atoms by counting smaller tags (tags are unique), 32 atoms per round in registers.
+constexpr int kSortSplit = 4;
+__global__ void __launch_bounds__(256)
+k_cell_sort(const RepGeom *__restrict__ geom, DirtyView dv, const int *__restrict__ cell_start,
+            const int *__restrict__ tag, int *__restrict__ order)
 {
-    if (!ctrl[0]) return;
-    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < n_cells; c += gridDim.x * blockDim.x) {
-        const int s = cell_start[c], e = cell_start[c + 1];
-        if (e <= s) continue;
-        if (!dirty[atom_rep[s]]) continue;
-        for (int a = s + 1; a < e; ++a) {
-            const int oa = order[a];
-            const int ka = tag[oa];
-            int b = a - 1;
-            while (b >= s) {
-                const int ob = order[b];
-                if (tag[ob] <= ka) break;
-                order[b + 1] = ob;
-                --b;
+    if (!*dv.any) return;
+    const int r = blockIdx.x;
+    if (dv.dirty[r] < dv.level) return;
+    const RepGeom *g = geom + r;
+    const int ncell = g->nc[0] * g->nc[1] * g->nc[2];
+    const int lane = threadIdx.x & 31;
+    const int wid = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5), nw = gridDim.y * (blockDim.x >> 5);
+    for (int c = wid; c < ncell; c += nw) {
+        const int s = cell_start[g->cell_base + c], m = cell_start[g->cell_base + c + 1] - s;
+        if (m <= 1) continue;
+        if (m <= 32) {
+            const int o = lane < m ? order[s + lane] : 0;
+            const int key = lane < m ? tag[o] : 0x7fffffff;
+            int rank = 0;
+            for (int k = 0; k < m; ++k) rank += __shfl_sync(0xffffffffu, key, k) < key;
+            __syncwarp();
+            if (lane < m) order[s + rank] = o;
+        } else if (lane == 0) {      // crowded cell: insertion sort by one lane
+            for (int a = s + 1; a < s + m; ++a) {
+                const int oa = order[a];
+                const int ka = tag[oa];
+                int b = a - 1;
+                while (b >= s) {
+                    const int ob = order[b];
+                    if (tag[ob] <= ka) break;
+                    order[b + 1] = ob;
+                    --b;
+                }
+                order[b + 1] = oa;
             }
-            order[b + 1] = oa;
         }
+        __syncwarp();
     }
 }
 
 // a1: gather into cell order (positions wrapped into the box on periodic axes).
 __global__ void k_reorder_gather(const float4 *__restrict__ pos, const float4 *__restrict__ vel,
                                  const int *__restrict__ tag, const int *__restrict__ atom_rep,
-                                 const RepGeom *__restrict__ geom, const int *__restrict__ dirty,
-                                 const int *__restrict__ ctrl, const int *__restrict__ order,
+                                 const RepGeom *__restrict__ geom, DirtyView dv, const int *__restrict__ order,
                                  const int *__restrict__ cell_of, float4 *__restrict__ pos_build,
                                  float4 *__restrict__ tmp4, int *__restrict__ tmp_tag,
                                  int *__restrict__ cell_sorted, int n)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
         const int r = atom_rep[k];
-        if (!dirty[r]) continue;
+        if (dv.dirty[r] < dv.level) continue;
         const RepGeom *g = geom + r;
         const int o = order[k];
         float4 p = pos[o];
@@ -164,13 +180,13 @@ __global__ void k_reorder_gather(const float4 *__restrict__ pos, const float4 *_
 }
 
 __global__ void k_reorder_copyback(float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ tag,
-                                   const int *__restrict__ atom_rep, const int *__restrict__ dirty,
-                                   const int *__restrict__ ctrl, const float4 *__restrict__ tmp_pos,
+                                   const int *__restrict__ atom_rep, DirtyView dv,
+                                   const float4 *__restrict__ tmp_pos,
                                    const float4 *__restrict__ tmp4, const int *__restrict__ tmp_tag, int n)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
-        if (!dirty[atom_rep[k]]) continue;
+        if (dv.dirty[atom_rep[k]] < dv.level) continue;
         pos[k] = tmp_pos[k];
         if (vel) vel[k] = tmp4[k];
         tag[k] = tmp_tag[k];
@@ -182,15 +198,15 @@ __global__ void k_reorder_copyback(float4 *__restrict__ pos, float4 *__restrict_
 template <bool PERIODIC>
 __global__ void __launch_bounds__(128)
 k_build_list(const float4 *__restrict__ pos, const int *__restrict__ atom_rep,
-             const RepGeom *__restrict__ geom, const int *__restrict__ dirty, int *__restrict__ ctrl,
+             const RepGeom *__restrict__ geom, DirtyView dv, int *__restrict__ ctrl,
              const int *__restrict__ cell_start, const int *__restrict__ cell_sorted,
              int *__restrict__ nlist, int *__restrict__ nn, float4 *__restrict__ pos_build,
              int n, int n_pad, int kmax, float rl2)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int r = atom_rep[i];
-        if (!dirty[r]) continue;
+        if (dv.dirty[r] < dv.level) continue;
         const RepGeom *g = geom + r;
         const float4 pi = pos[i];
         pos_build[i] = pi;
@@ -252,8 +268,8 @@ k_build_list(const float4 *__restrict__ pos, const int *__restrict__ atom_rep,
 
 __global__ void k_mark_all_dirty(int *__restrict__ dirty, int *__restrict__ ctrl, int R)
 {
-    for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < R; r += gridDim.x * blockDim.x) dirty[r] = 1;
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl[0] = 1;
+    for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < R; r += gridDim.x * blockDim.x) dirty[r] = 2;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { ctrl[0] = 1; ctrl[3] = 1; }
 }
 
 __global__ void k_get_neighbors(const int *__restrict__ tag, const int *__restrict__ nlist,
@@ -294,25 +310,24 @@ cudaError_t tbsma_launch_rebuild(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t
 {
     const int n = (int)c->n;
     const int ga = grid_for(c, n, kThreads, 8);
+    const DirtyView dv = tbsma_dirty_view(c);
     if (do_cells) {
-        k_bin_count<<<ga, kThreads, 0, st>>>(pos, c->d_atom_rep, c->d_geom, c->d_dirty, c->d_ctrl,
+        k_bin_count<<<ga, kThreads, 0, st>>>(pos, c->d_atom_rep, c->d_geom, dv, c->d_ctrl,
                                              c->d_cell_count, c->d_cell_of, c->d_slot, n);
         const int scan_threads = (c->n_cells / c->R > 4096) ? 1024 : 256;
-        k_cell_scan<<<c->R, scan_threads, 0, st>>>(c->d_geom, c->d_dirty, c->d_cell_count, c->d_cell_start);
-        k_scatter<<<ga, kThreads, 0, st>>>(c->d_atom_rep, c->d_dirty, c->d_ctrl, c->d_cell_start,
+        k_cell_scan<<<c->R, scan_threads, 0, st>>>(c->d_geom, dv, c->d_cell_count, c->d_cell_start);
+        k_scatter<<<ga, kThreads, 0, st>>>(c->d_atom_rep, dv, c->d_cell_start,
                                            c->d_cell_of, c->d_slot, c->d_order, n);
-        k_cell_sort<<<grid_for(c, c->n_cells, 128, 16), 128, 0, st>>>(c->d_atom_rep, c->d_dirty, c->d_ctrl,
-                                                                      c->d_cell_start, tag, c->d_order,
-                                                                      (int)c->n_cells);
+        k_cell_sort<<<dim3(c->R, kSortSplit), 256, 0, st>>>(c->d_geom, dv, c->d_cell_start, tag, c->d_order);
         // d_slot is free after the scatter: reuse it for the cell id of every sorted slot
-        k_reorder_gather<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, c->d_geom, c->d_dirty,
-                                                  c->d_ctrl, c->d_order, c->d_cell_of, c->d_tmp_pos,
+        k_reorder_gather<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, c->d_geom, dv,
+                                                  c->d_order, c->d_cell_of, c->d_tmp_pos,
                                                   c->d_tmp4, c->d_tmp_tag, c->d_slot, n);
         c->launches += 5;
         // the tile variant moves the atoms once more (count order inside each layer) while it builds
         // the lists, so its copy-back is part of tbsma_launch_tile_lists
         if (!(do_list && c->active_variant == 2)) {
-            k_reorder_copyback<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, c->d_dirty, c->d_ctrl,
+            k_reorder_copyback<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, dv,
                                                         c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, n);
             c->launches++;
         }
@@ -327,11 +342,11 @@ cudaError_t tbsma_launch_rebuild(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t
     if (do_list) {
         const int gl = grid_for(c, n, 128, 16);
         if (c->any_periodic)
-            k_build_list<true><<<gl, 128, 0, st>>>(pos, c->d_atom_rep, c->d_geom, c->d_dirty, c->d_ctrl,
+            k_build_list<true><<<gl, 128, 0, st>>>(pos, c->d_atom_rep, c->d_geom, dv, c->d_ctrl,
                                                    c->d_cell_start, c->d_slot, c->d_nlist, c->d_nn,
                                                    c->d_pos_build, n, c->n_pad, c->kmax, c->pc.rl2);
         else
-            k_build_list<false><<<gl, 128, 0, st>>>(pos, c->d_atom_rep, c->d_geom, c->d_dirty, c->d_ctrl,
+            k_build_list<false><<<gl, 128, 0, st>>>(pos, c->d_atom_rep, c->d_geom, dv, c->d_ctrl,
                                                     c->d_cell_start, c->d_slot, c->d_nlist, c->d_nn,
                                                     c->d_pos_build, n, c->n_pad, c->kmax, c->pc.rl2);
         c->launches++;

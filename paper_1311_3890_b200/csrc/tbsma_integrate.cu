@@ -86,29 +86,38 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
     const float d2 = dx * dx + dy * dy + dz * dz;
     const bool cadence = a.rebuild_every > 0 && (step % (unsigned long long)a.rebuild_every) == 0ull;
     if (d2 > a.skin_half2 || cadence) {
-        dirty[r] = 1;
+        // level 2 = cells + candidate list too (tile variant, decided at the replica's previous rebuild)
+        const int level = (a.want_outer && a.want_outer[r]) ? 2 : 1;
+        dirty[r] = level;
         ctrl[0] = 1;
+        if (level == 2) ctrl[3] = 1;
         if (a.rebuild_every > 0 && !cadence) atomicOr(ctrl + 1, (int)TBSMA_FLAG_SKIN_VIOLATED);
     }
 }
 
 // end of step: statistics, clear the dirty flags, advance the in-run step offset
-__global__ void k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl,
+__global__ void k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl, int *__restrict__ want_outer,
                               unsigned long long *__restrict__ counters, int R, int advance, int count_step)
 {
-    __shared__ int s_cnt;
-    if (threadIdx.x == 0) s_cnt = 0;
+    __shared__ int s_cnt, s_cnt2;
+    if (threadIdx.x == 0) { s_cnt = 0; s_cnt2 = 0; }
     __syncthreads();
     if (ctrl[0]) {
-        int mine = 0;
+        int mine = 0, mine2 = 0;
         for (int r = threadIdx.x; r < R; r += blockDim.x) {
-            if (dirty[r]) { ++mine; dirty[r] = 0; }
+            const int d = dirty[r];
+            if (d) { ++mine; dirty[r] = 0; }
+            if (d == 2) ++mine2;
         }
         if (mine) atomicAdd(&s_cnt, mine);
+        if (mine2) atomicAdd(&s_cnt2, mine2);
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        if (ctrl[0]) { counters[1] += (unsigned long long)s_cnt; counters[2] += 1ull; ctrl[0] = 0; }
+        if (ctrl[0]) {
+            counters[1] += (unsigned long long)s_cnt; counters[2] += 1ull; counters[6] += (unsigned long long)s_cnt2;
+            ctrl[0] = 0; ctrl[3] = 0;
+        }
         if (count_step) counters[3] += 1ull;
         if (advance) counters[0] += 1ull;
     }
@@ -129,7 +138,8 @@ cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, c
 
 cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st)
 {
-    k_finish_step<<<1, 256, 0, st>>>(c->d_dirty, c->d_ctrl, c->d_counters, c->R, advance_offset & 1,
+    k_finish_step<<<1, 256, 0, st>>>(c->d_dirty, c->d_ctrl, c->active_variant == 2 ? c->d_want_outer : nullptr,
+                                     c->d_counters, c->R, advance_offset & 1,
                                      (advance_offset >> 1) & 1);
     c->launches++;
     return cudaGetLastError();

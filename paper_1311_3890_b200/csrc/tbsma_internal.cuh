@@ -17,6 +17,7 @@
 struct PairConst {
     float rc2;        // fl32(r_cut)^2 (fp32 product) -- interaction predicate threshold, D:A6
     float rl2;        // fl32(r_cut+skin)^2           -- list predicate threshold
+    float ro2;        // fl32(r_cut+skin+outer_skin)^2 -- candidate (outer) list threshold of the tile variant
     float r0f;
     float aq, ap;
     float b_rho, b_rep, b_band;
@@ -52,6 +53,14 @@ struct TileDesc {
 #define TBSMA_TILE_MAX_LAYERS 8      // own layers per tile
 #define TBSMA_TILE_MAX_RECORDS 4095  // halo records per tile: (records + sentinel) * 16 B <= 64 KB, u16 byte offsets
 
+// Which replicas a kernel of the rebuild chain works on: replica r takes part iff dirty[r] >= level, and the
+// whole launch is a no-op when *any == 0.  dirty[r]: 0 clean, 1 inner list stale, 2 cells + candidate list stale.
+struct DirtyView {
+    const int *dirty;
+    const int *any;
+    int level;
+};
+
 struct GraphKey {          // arguments a cached one-step CUDA graph was captured with
     const void *p[11];
     double dt, gamma;
@@ -78,6 +87,13 @@ struct tbsma_ctx {
     // tile variant
     int tile_layers;    // own layers per tile requested (<= TBSMA_TILE_MAX_LAYERS)
     int tile_threads;   // CTA size of the tile kernels
+    double outer_skin;  // S: the candidate list holds every pair within r_cut + skin + S at its build
+    int kmax_o;         // capacity of the candidate list per atom (multiple of 4, <= 248)
+    uint2 *d_olist;     // 2 x (kmax_o/4 x n_pad) uint2: candidate list (bank-scheduled u16 offsets) + build scratch
+    int32_t *d_nn_o;    // n: candidate count | flag << 16
+    float4 *d_pos_outer;   // n: positions when the candidate list was built
+    int32_t *d_want_outer; // R: the next rebuild of this replica must redo cells + candidate list
+    double cell_w;      // cell width the current geometry was computed for
     int tile_cap;       // halo records a tile may hold in shared memory
     int tile_cell_cap;  // halo cells (+1) a tile may hold in shared memory
     int n_tiles;
@@ -111,8 +127,9 @@ struct tbsma_ctx {
     float4 *d_xs;           // n: (x, y, z, 1/sqrt(rho)) written by the density pass
     // device: control
     int32_t *d_dirty;       // R: replica needs a rebuild
-    int32_t *d_ctrl;        // [0] any_dirty, [1] status flags, [2] max neighbours seen
-    unsigned long long *d_counters; // [0] step offset inside md_run, [1] replica builds, [2] build passes, [3] steps
+    int32_t *d_ctrl;        // [0] any replica dirty, [1] status flags, [2] max neighbours seen, [3] any dirty == 2
+    unsigned long long *d_counters; // [0] step offset inside md_run, [1] replica builds, [2] build passes, [3] steps,
+                                    // [4..5] count_pairs scratch, [6] replica builds that redid cells + candidates
     // host staging for *_host entry point
     float4 *s_pos, *s_vel, *s_force;
     int32_t *s_tag;
@@ -130,6 +147,10 @@ struct tbsma_ctx {
     GraphKey graph_key;
     int64_t graph_launches_per_step;
     cudaStream_t own_stream;   // used by the *_host entry point
+    // md step of the tile variant: rebuild chain + rebuilt replicas on a second (high-priority) stream
+    int overlap;               // enabled (default 1)
+    cudaStream_t aux_stream;
+    cudaEvent_t ev_fork, ev_join;
     // optional per-kernel-class timing with CUDA events on the launching stream
     int timing;
     cudaEvent_t *tev;          // 6 events per timed step (class boundaries)
@@ -142,6 +163,14 @@ struct tbsma_ctx {
 cudaError_t tbsma_launch_rebuild(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, bool do_cells,
                                  bool do_list, cudaStream_t st);
 cudaError_t tbsma_launch_mark_all_dirty(tbsma_ctx *c, cudaStream_t st);
+inline DirtyView tbsma_dirty_view(const tbsma_ctx *c)
+{
+    DirtyView v;
+    v.dirty = c->d_dirty;
+    v.level = c->active_variant == 2 ? 2 : 1;
+    v.any = c->d_ctrl + (v.level == 2 ? 3 : 0);
+    return v;
+}
 cudaError_t tbsma_launch_get_neighbors(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
                                        cudaStream_t st);
 // forces (tbsma_force.cu)
@@ -159,11 +188,18 @@ cudaError_t tbsma_launch_count_pairs(tbsma_ctx *c, const float4 *pos, unsigned l
 // shared-memory tile variant (tbsma_tile.cu)
 int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st);   // host: sizes the tiles from the binned cells (synchronises)
 cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, cudaStream_t st);
+cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, cudaStream_t st);   // inner lists of dirty replicas
 cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float4 *vel, const int32_t *tag,
                                     cudaStream_t st);
-cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, cudaStream_t st);
+// mode: which tiles a gather launch processes.  The md step runs the tiles of the replicas that are NOT being
+// rebuilt on the main stream while the rebuild chain and then the tiles of the rebuilt replicas run on a second
+// stream (replicas never interact, so the two halves are independent).
+#define TBSMA_TILES_ALL 0
+#define TBSMA_TILES_CLEAN 1
+#define TBSMA_TILES_DIRTY 2
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int mode, cudaStream_t st);
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kick,
-                                    cudaStream_t st);
+                                    int mode, cudaStream_t st);
 cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
                                             cudaStream_t st);
 cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsigned long long *d_out2,
@@ -179,6 +215,7 @@ struct StepArgs {
     const unsigned long long *seed;
     const double *disp0;     // nullable
     const double *rate;      // nullable
+    const int *want_outer;   // nullable (tile variant): replicas whose next rebuild redoes cells + candidates
     double *e_rep, *w_rep, *ekin;  // zeroed here for the force pass; nullable
 };
 cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, const float4 *force,

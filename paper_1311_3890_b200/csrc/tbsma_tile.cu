@@ -15,11 +15,22 @@
 //     the eight lanes served by one shared-memory wavefront of a 128-bit load then hit eight
 //     different 16-byte bank groups (summation order is free, A15).
 // Membership is the fp32 predicate of D:A6, operation for operation, as in tbsma_cells.cu.
+//
+// Two-level lists.  Scanning 27 cells costs about five force passes per atom, and at 298 K a replica
+// needs a fresh list every ~12 steps (fewer rebuilds are why 10 K runs faster).  So the cell
+// scan builds a CANDIDATE list with the larger radius r_cut + skin + S (S = outer_skin, 1 A): K1-K3
+// below, rarely.  The list the gather passes read (radius r_cut + skin, the paper's r_buff list)
+// is filtered from the candidates by the tile that owns the atom (k_tile_inner) in the step in which
+// the replica's atoms moved more than skin/2: ~2.3 candidates per kept entry instead of ~9.  A candidate list stays valid while no atom moved more than S/2 since
+// it was built; the inner build checks that (status flag) and asks for new candidates one rebuild
+// earlier (want_outer).  Slots (and so the u16 offsets) only change when candidates are rebuilt.
 #include "tbsma_internal.cuh"
 
 namespace {
 
-constexpr int kTileThreads = 256;   // build kernels; the gather kernels use c->tile_threads
+constexpr int kScanThreads = 1024;  // k_tile_scan: one round for tiles of <= 1024 own atoms (the rebuild chain is
+                                    // latency bound: only the dirty replicas' tiles do any work)
+constexpr int kFinishMaxThreads = 768;   // k_tile_finish: bounded by its kmax x threads x 2 B shared-memory scratch
 
 __device__ __forceinline__ float ex2_approx(float x)
 {
@@ -63,16 +74,17 @@ __global__ void k_layer_maxpop(const RepGeom *__restrict__ geom, const int *__re
 // ---- K1: scan.  Cell-ordered positions of the tile + halo in shared memory; every own atom scans
 // its 3 x 3 runs of x-adjacent cells, writes its partners (halo-local cell-order indices, u16) to
 // the temporary list, and is ranked inside its layer by (count descending, slot ascending).
-__global__ void __launch_bounds__(kTileThreads)
+__global__ void __launch_bounds__(kScanThreads)
 k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
-            const int *__restrict__ cell_sorted, const int *__restrict__ dirty, int *__restrict__ ctrl,
+            const int *__restrict__ cell_sorted, DirtyView dv, int *__restrict__ ctrl,
             const float4 *__restrict__ pos_sorted, uint2 *__restrict__ nl_tmp, int *__restrict__ nn_tmp,
-            int *__restrict__ newslot, int *__restrict__ oldof, int n_pad, int kmax, float rl2,
-            int s_cap, int cell_cap)
+            int *__restrict__ newslot, int *__restrict__ oldof, int *__restrict__ want_outer, int n_pad, int kmax,
+            float ro2, float rl2, int s_cap, int cell_cap)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     const TileDesc t = tiles[blockIdx.x];
-    if (!dirty[t.rep]) return;
+    if (dv.dirty[t.rep] < dv.level) return;
+    if (threadIdx.x == 0 && t.z_h0 == 0 && t.own_first == 0) want_outer[t.rep] = 0;   // new candidates: request served
     extern __shared__ float4 smem_f4[];
     float4 *sm = smem_f4;
     int *cs = reinterpret_cast<int *>(sm + s_cap);
@@ -89,11 +101,11 @@ k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_sta
         return;
     }
     const int ncell_h = t.nlay_h * t.layer_cells;
-    for (int k = tid; k <= ncell_h; k += kTileThreads) cs[k] = cell_start[t.ch0 + k] - halo_lo;
-    for (int k = tid; k < nh; k += kTileThreads) sm[k] = pos_sorted[halo_lo + k];
+    for (int k = tid; k <= ncell_h; k += blockDim.x) cs[k] = cell_start[t.ch0 + k] - halo_lo;
+    for (int k = tid; k < nh; k += blockDim.x) sm[k] = pos_sorted[halo_lo + k];
     __syncthreads();
     const int nx = t.nx, ny = t.ny, nz = t.nz;
-    for (int a = lo + tid; a < hi; a += kTileThreads) {
+    for (int a = lo + tid; a < hi; a += blockDim.x) {
         const int al = a - halo_lo;
         const float4 pi = sm[al];
         const int lc = cell_sorted[a] - t.cell_base;
@@ -101,7 +113,7 @@ k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_sta
         const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
         uint2 *row = nl_tmp + a;
         unsigned w0 = 0u, w1 = 0u;
-        int cnt = 0;
+        int cnt = 0, cnt_in = 0;     // candidates (d2 < ro2) and list members (d2 < rl2, orders the layer)
         for (int zz = max(cz - 1, 0); zz <= min(cz + 1, nz - 1); ++zz)
             for (int yy = max(cy - 1, 0); yy <= min(cy + 1, ny - 1); ++yy) {
                 const int cb = ((zz - t.z_h0) * ny + yy) * nx;
@@ -110,7 +122,7 @@ k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_sta
                     const float4 pj = sm[j];
                     const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
                     const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
-                    if (d2 < rl2 && j != al) {
+                    if (d2 < ro2 && j != al) {
                         if (cnt < kmax) {
                             const unsigned v = (unsigned)j << ((cnt & 1) << 4);
                             if (cnt & 2) w1 |= v; else w0 |= v;
@@ -120,18 +132,18 @@ k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_sta
                             }
                         }
                         ++cnt;
+                        cnt_in += d2 < rl2;
                     }
                 }
             }
         if (cnt > kmax) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
-        atomicMax(ctrl + 2, cnt);
         cnt = min(cnt, kmax);
         if (cnt & 3) row[(size_t)(cnt >> 2) * n_pad] = make_uint2(w0, w1);
-        cnts[a - lo] = (unsigned short)cnt;
+        cnts[a - lo] = (unsigned short)cnt_in;
         nn_tmp[a] = cnt | ((__float_as_int(pi.w) & 3) << 16);
     }
     __syncthreads();
-    for (int a = lo + tid; a < hi; a += kTileThreads) {
+    for (int a = lo + tid; a < hi; a += blockDim.x) {
         int m = t.own_first;
         while (a >= lb[m + 1]) ++m;
         const int l0 = lb[m] - lo, l1 = lb[m + 1] - lo, me = a - lo;
@@ -154,26 +166,26 @@ __device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { retur
 // tile's shared-memory image, record k at (k + 1) * 16, the sentinel at 0), and writes the row in
 // bank-scheduled order: step p of lane l takes a partner of class (l + p) & 7 (class = bank group
 // of the record), falling back to the fullest class when that one is used up.
-__global__ void __launch_bounds__(kTileThreads)
+__global__ void __launch_bounds__(kFinishMaxThreads)
 k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
-              const int *__restrict__ dirty, int *__restrict__ ctrl, const uint2 *__restrict__ nl_tmp,
+              DirtyView dv, int *__restrict__ ctrl, const uint2 *__restrict__ nl_tmp,
               const int *__restrict__ nn_tmp, const int *__restrict__ newslot, const int *__restrict__ oldof,
               uint2 *__restrict__ nl, int *__restrict__ nn, int *__restrict__ hbase, int n_pad, int kmax,
               int s_cap)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     const TileDesc t = tiles[blockIdx.x];
-    if (!dirty[t.rep]) return;
+    if (dv.dirty[t.rep] < dv.level) return;
     extern __shared__ float4 smem_f4[];
     unsigned short *map = reinterpret_cast<unsigned short *>(smem_f4);   // s_cap entries
-    unsigned short *scr = map + ((s_cap + 7) & ~7);                      // kmax x kTileThreads
+    unsigned short *scr = map + ((s_cap + 7) & ~7);                      // kmax x blockDim.x
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo || r.nh > s_cap) return;
-    const int tid = threadIdx.x, lane = tid & 31;
-    for (int k = tid; k < r.nh; k += kTileThreads)
+    const int tid = threadIdx.x, lane = tid & 31, nthr = blockDim.x;
+    for (int k = tid; k < r.nh; k += blockDim.x)
         map[k] = (unsigned short)((newslot[r.halo_lo + k] - r.halo_lo + 1) << 4);
     __syncthreads();
-    for (int ip = r.lo + tid; ip < r.hi; ip += kTileThreads) {
+    for (int ip = r.lo + tid; ip < r.hi; ip += blockDim.x) {
         const int a = oldof[ip];
         const int nnv = nn_tmp[a];
         const int cnt = nnv & 0xffff;
@@ -206,7 +218,7 @@ k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_s
                     const int c = (m >> 4) & 7;
                     const unsigned idx = byte_of(off, c) + byte_of(cur, c);
                     cur += 1ull << (c << 3);
-                    scr[idx * kTileThreads + tid] = (unsigned short)m;
+                    scr[idx * nthr + tid] = (unsigned short)m;
                 }
         }
         // emission in scheduled order
@@ -228,7 +240,7 @@ k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_s
             const unsigned idx = byte_of(off, c) + byte_of(cur, c);
             cur += 1ull << (c << 3);
             rem -= 1ull << (c << 3);
-            const unsigned v = (unsigned)scr[idx * kTileThreads + tid] << ((p & 1) << 4);
+            const unsigned v = (unsigned)scr[idx * nthr + tid] << ((p & 1) << 4);
             if (p & 2) w1 |= v; else w0 |= v;
             if ((p & 3) == 3) {
                 dst[(size_t)(p >> 2) * n_pad] = make_uint2(w0, w1);
@@ -241,21 +253,20 @@ k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_s
     }
 }
 
-// ---- K3: move positions / velocities / tags from cell order to the final order (identity when
-// oldof is null) and record the positions of this build for the displacement check.
+// ---- K3: move positions / velocities / tags from cell order to the final order and record the
+// positions the candidates were built for.
 __global__ void k_tile_permute(float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ tag,
-                               float4 *__restrict__ pos_build, const int *__restrict__ atom_rep,
-                               const int *__restrict__ dirty, const int *__restrict__ ctrl,
-                               const int *__restrict__ oldof, const float4 *__restrict__ tmp_pos,
+                               float4 *__restrict__ pos_outer, const int *__restrict__ atom_rep,
+                               DirtyView dv, const int *__restrict__ oldof, const float4 *__restrict__ tmp_pos,
                                const float4 *__restrict__ tmp_vel, const int *__restrict__ tmp_tag, int n)
 {
-    if (!ctrl[0]) return;
+    if (!*dv.any) return;
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
-        if (!dirty[atom_rep[k]]) continue;
+        if (dv.dirty[atom_rep[k]] < dv.level) continue;
         const int a = oldof[k];
         const float4 p = tmp_pos[a];
         pos[k] = p;
-        pos_build[k] = p;
+        pos_outer[k] = p;
         if (vel) vel[k] = tmp_vel[a];
         tag[k] = tmp_tag[a];
     }
@@ -301,13 +312,122 @@ __device__ __forceinline__ float rho_term_t(const float4 &pi, const float4 &pj, 
     return d2 < pc.rc2 ? e : 0.f;
 }
 
-// stage 1 (P:59; Eq.1 P:47, P:57): rho_i over the list, s_i = rho_i^(-1/2) packed with the position
-__global__ void __launch_bounds__(512, 2)
-k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
-               const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
-               float4 *__restrict__ xs, int *__restrict__ ctrl, int n_pad, int s_cap, PairConst pc)
+
+// ---- inner build: the list the gather passes read, filtered from the candidates.
+// Runs inside the tile that owns the atoms, on the positions already staged in shared memory (sm:
+// record k + 1 = slot halo_lo + k, record 0 = sentinel).  Kept entries stay in candidate order (the
+// bank schedule of K2); the membership test is the fp32 predicate of D:A6 against rl2.  Also records
+// the positions of this build (displacement check of the integrator) and compares them with those of
+// the candidate build: more than S/2 away invalidates the candidates (status flag), more than
+// want2^(1/2) asks for new candidates at the replica's next rebuild.
+struct InnerArgs {
+    const uint2 *olist;      // candidates
+    const int *nn_o;
+    uint2 *nl;               // out: inner list
+    int *nn;                 // out: count | flag << 16
+    float4 *pos_build;       // out
+    const float4 *pos_outer;
+    int *want_outer;         // per replica
+    int kmax;                // inner capacity
+    float rl2, want2, viol2;
+};
+
+// Order of the kept entries (bank schedule).  A 128-bit shared-memory load is served eight lanes at a
+// time, and eight lanes reading eight different 16-byte bank groups ("classes", record index mod 8) take
+// one wavefront.  The list of the atom handled by lane l is laid out in rounds of eight positions;
+// position 8 j + s wants a record of class (l + s) mod 8, so the eight lanes of a wavefront, all at the
+// same position, read eight different classes.  The j-th kept entry of class c goes straight to position
+// 8 j + ((c - l) mod 8) while j < m / 8 (m = entries kept); the rest fill the positions left free.
+// scr / out: per-thread columns of kmax u16 in shared memory (element k of thread t at [k * nthr + t]).
+__device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRange &r, const float4 *sm,
+                                                 unsigned short *scr, unsigned short *out, const InnerArgs &ia,
+                                                 int *__restrict__ ctrl, int n_pad)
+{
+    const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
+    int maxc = 0;
+    bool want = false, viol = false, over = false;
+    for (int i = r.lo + tid; i < r.hi; i += nthr) {
+        const float4 pi = sm[i - r.halo_lo + 1];
+        const int nno = ia.nn_o[i];
+        const int ng = ((nno & 0xffff) + 3) >> 2;
+        const uint2 *row = ia.olist + i;
+        // pass 1: filter the candidates (fp32 predicate of D:A6) into scr, count the classes
+        unsigned long long pop = 0ull;
+        int m = 0, seen = 0;
+        uint2 nxt = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
+        for (int g = 0; g < ng; ++g) {
+            const uint2 jj = nxt;
+            if (g + 1 < ng) nxt = __ldcs(row + (size_t)(g + 1) * n_pad);
+            const unsigned e[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float4 pj = lds_rec(sm, e[q]);
+                const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
+                if (d2 < ia.rl2) {          // padding entries point at the sentinel and fail
+                    if (m < ia.kmax) {
+                        scr[m * nthr + tid] = (unsigned short)e[q];
+                        pop += 1ull << (((e[q] >> 4) & 7u) << 3);
+                        ++m;
+                    }
+                    ++seen;
+                }
+            }
+        }
+        over = over || seen > ia.kmax;
+        maxc = max(maxc, seen);
+        // pass 2: placement
+        const int L = m >> 3;                 // full rounds
+        unsigned long long cur = 0ull;        // entries of each class placed so far
+        int hc = -1, hj = L, tail = L << 3;   // free-position generator: class streams shorter than L, then the tail
+        for (int k = 0; k < m; ++k) {
+            const unsigned e = scr[k * nthr + tid];
+            const int c = (e >> 4) & 7;
+            const int j = (int)byte_of(cur, c);
+            cur += 1ull << (c << 3);
+            int p;
+            if (j < L) {
+                p = (j << 3) + ((c - lane) & 7);
+            } else {
+                while (hj >= L && hc < 8) {
+                    ++hc;
+                    hj = hc < 8 ? (int)byte_of(pop, hc) : L;
+                }
+                if (hc < 8) { p = (hj << 3) + ((hc - lane) & 7); ++hj; }
+                else p = tail++;
+            }
+            out[p * nthr + tid] = (unsigned short)e;
+        }
+        const int mpad = (m + 3) & ~3;
+        for (int k = m; k < mpad; ++k) out[k * nthr + tid] = 0;      // unused entries = 0 = the sentinel
+        uint2 *dst = ia.nl + i;
+        for (int g = 0; g < (mpad >> 2); ++g) {
+            const unsigned a0 = out[(4 * g) * nthr + tid], a1 = out[(4 * g + 1) * nthr + tid];
+            const unsigned a2 = out[(4 * g + 2) * nthr + tid], a3 = out[(4 * g + 3) * nthr + tid];
+            dst[(size_t)g * n_pad] = make_uint2(a0 | (a1 << 16), a2 | (a3 << 16));
+        }
+        ia.nn[i] = m | (nno & 0x7fff0000);
+        ia.pos_build[i] = pi;
+        const float4 po = ia.pos_outer[i];
+        const float ox = pi.x - po.x, oy = pi.y - po.y, oz = pi.z - po.z;
+        const float o2 = ox * ox + oy * oy + oz * oz;
+        want = want || o2 > ia.want2;
+        viol = viol || o2 > ia.viol2;
+    }
+    maxc = __reduce_max_sync(__activemask(), maxc);
+    if (lane == 0 && maxc > 0) atomicMax(ctrl + 2, maxc);
+    if (want) ia.want_outer[t.rep] = 1;
+    if (viol) atomicOr(ctrl + 1, (int)TBSMA_FLAG_SKIN_VIOLATED);
+    if (over) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
+}
+
+// stand-alone inner build of the dirty replicas (tbsma_build_neighbors; inside an MD step the density pass does it)
+__global__ void __launch_bounds__(512)
+k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start, const float4 *__restrict__ pos,
+             InnerArgs ia, int *__restrict__ ctrl, const int *__restrict__ dirty, int n_pad, int s_cap)
 {
     const TileDesc t = tiles[blockIdx.x];
+    if (!dirty[t.rep]) return;
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
     if (r.nh > s_cap) {
@@ -315,24 +435,79 @@ k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_
         return;
     }
     extern __shared__ float4 smem_f4[];
-    const float4 *sm = smem_f4;
     fill_tile(smem_f4, pos, r.halo_lo, r.nh);
-    for (int i = r.lo + threadIdx.x; i < r.hi; i += blockDim.x) {
+    unsigned short *scr = reinterpret_cast<unsigned short *>(smem_f4 + s_cap + 1);
+    unsigned short *out = scr + (size_t)ia.kmax * blockDim.x;
+    tile_inner_build(t, r, smem_f4, scr, out, ia, ctrl, n_pad);
+}
+
+// Work distribution of the two gather kernels: the own atoms of a tile are cut into chunks of 32
+// consecutive slots (equal list lengths, thanks to the count order) and the warps of the CTA take
+// chunks from a shared counter, so no warp waits at the end for one that drew the long lists.
+// The list rows are prefetched three groups (12 entries) ahead: a row is 8 bytes per lane from
+// HBM, and one group of pair terms is shorter than the HBM latency.
+#define TBSMA_TILE_MODE_SKIP(mode, level) \
+    ((mode) != TBSMA_TILES_ALL && ((level) != 0) != ((mode) == TBSMA_TILES_DIRTY))
+
+__device__ __forceinline__ int next_chunk(int *counter)
+{
+    int ch = 0;
+    if ((threadIdx.x & 31) == 0) ch = atomicAdd(counter, 1);
+    return __shfl_sync(0xffffffffu, ch, 0);
+}
+
+__device__ __forceinline__ uint2 ld_row(const uint2 *row, int g, int ng, int n_pad)
+{
+    return g < ng ? __ldcs(row + (size_t)g * n_pad) : make_uint2(0u, 0u);
+}
+
+// stage 1 (P:59; Eq.1 P:47, P:57): rho_i over the list, s_i = rho_i^(-1/2) packed with the position
+__global__ void __launch_bounds__(512, 2)
+k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
+               const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
+               float4 *__restrict__ xs, int *__restrict__ ctrl, const int *__restrict__ dirty, int mode,
+               int n_pad, int s_cap, PairConst pc)
+{
+    const TileDesc t = tiles[blockIdx.x];
+    if (TBSMA_TILE_MODE_SKIP(mode, dirty[t.rep])) return;
+    const TileRange r = tile_range(t, cell_start);
+    if (r.hi <= r.lo) return;
+    if (r.nh > s_cap) {
+        if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
+        return;
+    }
+    extern __shared__ float4 smem_f4[];
+    __shared__ int s_next;
+    const float4 *sm = smem_f4;
+    if (threadIdx.x == 0) s_next = 0;
+    fill_tile(smem_f4, pos, r.halo_lo, r.nh);
+    const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
+    for (int ch = next_chunk(&s_next); ch < nchunk; ch = next_chunk(&s_next)) {
+        const int i = r.lo + (ch << 5) + lane;
+        if (i >= r.hi) continue;
         const float4 pi = sm[i - r.halo_lo + 1];
-        const int cnt = nn[i] & 0xffff;
-        const int ng = (cnt + 3) >> 2;
+        const int ng = ((nn[i] & 0xffff) + 3) >> 2;
         const uint2 *row = nl + i;
         float rho0 = 0.f, rho1 = 0.f;
-        uint2 nxt = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
-        for (int g = 0; g < ng; ++g) {
-            const uint2 jj = nxt;
-            if (g + 1 < ng) nxt = __ldcs(row + (size_t)(g + 1) * n_pad);
+        auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
             const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
             rho0 += rho_term_t(pi, p0, pc);
             rho1 += rho_term_t(pi, p1, pc);
             rho0 += rho_term_t(pi, p2, pc);
             rho1 += rho_term_t(pi, p3, pc);
+        };
+        // three rows in flight, rotated by unrolling (a register move would wait for the newest load)
+        uint2 q0 = ld_row(row, 0, ng, n_pad), q1 = ld_row(row, 1, ng, n_pad), q2 = ld_row(row, 2, ng, n_pad);
+        int g = 0;
+        for (; g + 3 <= ng; g += 3) {
+            uint2 jj = q0; q0 = ld_row(row, g + 3, ng, n_pad); group(jj);
+            jj = q1; q1 = ld_row(row, g + 4, ng, n_pad); group(jj);
+            jj = q2; q2 = ld_row(row, g + 5, ng, n_pad); group(jj);
+        }
+        if (g < ng) {
+            group(q0);
+            if (g + 1 < ng) group(q1);
         }
         const float rho = rho0 + rho1;
         const float s = rho > 0.f ? 1.0f / sqrtf(rho) : 0.f;     // once per atom, IEEE (D:A5 for rho = 0)
@@ -395,9 +570,10 @@ __global__ void __launch_bounds__(512, 2)
 k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
              const float4 *__restrict__ xs, const uint2 *__restrict__ nl, const int *__restrict__ nn,
              float4 *__restrict__ force, double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk,
-             int *__restrict__ ctrl, int n_pad, int s_cap, PairConst pc)
+             int *__restrict__ ctrl, const int *__restrict__ dirty, int mode, int n_pad, int s_cap, PairConst pc)
 {
     const TileDesc t = tiles[blockIdx.x];
+    if (TBSMA_TILE_MODE_SKIP(mode, dirty[t.rep])) return;
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
     if (r.nh > s_cap) {
@@ -406,26 +582,39 @@ k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
     }
     extern __shared__ float4 smem_f4[];
     __shared__ double red[32];
+    __shared__ int s_next;
     const float4 *sm = smem_f4;
+    if (threadIdx.x == 0) s_next = 0;
     fill_tile(smem_f4, xs, r.halo_lo, r.nh);
     double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     bool bad = false;
-    for (int i = r.lo + threadIdx.x; i < r.hi; i += blockDim.x) {
+    const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
+    for (int ch = next_chunk(&s_next); ch < nchunk; ch = next_chunk(&s_next)) {
+        const int i = r.lo + (ch << 5) + lane;
+        if (i >= r.hi) continue;
         const float4 pi = sm[i - r.halo_lo + 1];
         const int nni = nn[i];
         const int ng = ((nni & 0xffff) + 3) >> 2;
         const uint2 *row = nl + i;
         AccT a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        uint2 nxt = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
-        for (int g = 0; g < ng; ++g) {
-            const uint2 jj = nxt;
-            if (g + 1 < ng) nxt = __ldcs(row + (size_t)(g + 1) * n_pad);
+        auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
             const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
             force_term_t<VIRIAL>(pi, p0, pc, a);
             force_term_t<VIRIAL>(pi, p1, pc, a);
             force_term_t<VIRIAL>(pi, p2, pc, a);
             force_term_t<VIRIAL>(pi, p3, pc, a);
+        };
+        uint2 q0 = ld_row(row, 0, ng, n_pad), q1 = ld_row(row, 1, ng, n_pad), q2 = ld_row(row, 2, ng, n_pad);
+        int g = 0;
+        for (; g + 3 <= ng; g += 3) {
+            uint2 jj = q0; q0 = ld_row(row, g + 3, ng, n_pad); group(jj);
+            jj = q1; q1 = ld_row(row, g + 4, ng, n_pad); group(jj);
+            jj = q2; q2 = ld_row(row, g + 5, ng, n_pad); group(jj);
+        }
+        if (g < ng) {
+            group(q0);
+            if (g + 1 < ng) group(q1);
         }
         const float sqrt_rho = pi.w > 0.f ? 1.0f / pi.w : 0.f;
         const float ei = __fmaf_rn(a.er, pc.e_rep_scale, -sqrt_rho);   // Eq.1-3: E_R^i + E_B^i
@@ -508,11 +697,47 @@ size_t scan_smem(const tbsma_ctx *c)
 {
     return (size_t)c->tile_cap * 16 + (size_t)c->tile_cell_cap * 4 + (size_t)c->tile_cap * 2;
 }
+int finish_threads(const tbsma_ctx *c)
+{
+    const size_t budget = 200 * 1024 - (size_t)((c->tile_cap + 7) & ~7) * 2;
+    int t = (int)(budget / ((size_t)c->kmax_o * 2)) & ~31;
+    if (t > kFinishMaxThreads) t = kFinishMaxThreads;
+    if (t < 32) t = 32;
+    return t;
+}
 size_t finish_smem(const tbsma_ctx *c)
 {
-    return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax * kTileThreads * 2;
+    return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax_o * finish_threads(c) * 2;
 }
 size_t gather_smem(const tbsma_ctx *c) { return (size_t)(c->tile_cap + 1) * 16; }
+int inner_threads(const tbsma_ctx *c)
+{
+    const size_t budget = 200 * 1024 - gather_smem(c);
+    int t = (int)(budget / ((size_t)c->kmax * 4)) & ~31;      // two u16 columns of kmax per thread
+    if (t > 512) t = 512;
+    if (t < 32) t = 32;
+    return t;
+}
+size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + (size_t)c->kmax * 4 * inner_threads(c); }
+InnerArgs inner_args(const tbsma_ctx *c)
+{
+    InnerArgs ia;
+    ia.olist = c->d_olist;
+    ia.nn_o = c->d_nn_o;
+    ia.nl = reinterpret_cast<uint2 *>(c->d_nlist);
+    ia.nn = c->d_nn;
+    ia.pos_build = c->d_pos_build;
+    ia.pos_outer = c->d_pos_outer;
+    ia.want_outer = c->d_want_outer;
+    ia.kmax = c->kmax;
+    ia.rl2 = c->pc.rl2;
+    // candidates are valid while no atom moved more than S/2 since their build (viol2).  New ones are asked
+    // for one rebuild early: by the NEXT rebuild an atom moves at most skin/2 (+ one step) further.
+    const double half_s = 0.5 * c->outer_skin, want = half_s - 0.5 * c->skin - 0.05;
+    ia.viol2 = (float)(half_s * half_s);
+    ia.want2 = want > 0.0 ? (float)(want * want) : -1.f;   // S too small to wait: every rebuild redoes the candidates
+    return ia;
+}
 
 }  // namespace
 
@@ -525,7 +750,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
 {
     c->active_variant = 1;
     if (c->variant == 1 || c->n == 0) return TBSMA_OK;
-    if (c->any_periodic || c->kmax > 248) return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;
+    if (c->any_periodic || c->kmax_o > 248) return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;
     const int R = c->R;
     k_layer_maxpop<<<(R + 127) / 128, 128, 0, st>>>(c->d_geom, c->d_cell_start, c->d_maxpop, R);
     c->launches++;
@@ -597,6 +822,8 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     // opt in to > 48 KB of dynamic shared memory
     const int sm_scan = (int)scan_smem(c), sm_fin = (int)finish_smem(c), sm_g = (int)gather_smem(c);
     e = cudaFuncSetAttribute(k_tile_scan, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_scan);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_tile_inner, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)inner_smem(c));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tile_finish, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_fin);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_density_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
@@ -612,18 +839,29 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
 cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, cudaStream_t st)
 {
     const int n = (int)c->n;
-    uint2 *nl = reinterpret_cast<uint2 *>(c->d_nlist);
-    uint2 *nl_tmp = nl + (size_t)(c->kmax / 4) * c->n_pad;    // second half of the int32-sized allocation
-    k_tile_scan<<<c->n_tiles, kTileThreads, scan_smem(c), st>>>(c->d_tiles, c->d_cell_start, c->d_slot, c->d_dirty,
-                                                               c->d_ctrl, c->d_tmp_pos, nl_tmp, c->d_nn_tmp,
-                                                               c->d_newslot, c->d_oldof, c->n_pad, c->kmax, c->pc.rl2,
-                                                               c->tile_cap, c->tile_cell_cap);
-    k_tile_finish<<<c->n_tiles, kTileThreads, finish_smem(c), st>>>(c->d_tiles, c->d_cell_start, c->d_dirty, c->d_ctrl,
-                                                                   nl_tmp, c->d_nn_tmp, c->d_newslot, c->d_oldof, nl,
-                                                                   c->d_nn, c->d_hbase, c->n_pad, c->kmax, c->tile_cap);
-    k_tile_permute<<<grid_for(c, n, 256, 8), 256, 0, st>>>(pos, vel, tag, c->d_pos_build, c->d_atom_rep, c->d_dirty,
-                                                          c->d_ctrl, c->d_oldof, c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, n);
+    const DirtyView dv = tbsma_dirty_view(c);
+    uint2 *ol = c->d_olist;
+    uint2 *ol_tmp = ol + (size_t)(c->kmax_o / 4) * c->n_pad;    // second half of the allocation
+    k_tile_scan<<<c->n_tiles, kScanThreads, scan_smem(c), st>>>(c->d_tiles, c->d_cell_start, c->d_slot, dv,
+                                                               c->d_ctrl, c->d_tmp_pos, ol_tmp, c->d_nn_tmp,
+                                                               c->d_newslot, c->d_oldof, c->d_want_outer, c->n_pad,
+                                                               c->kmax_o, c->pc.ro2, c->pc.rl2, c->tile_cap,
+                                                               c->tile_cell_cap);
+    k_tile_finish<<<c->n_tiles, finish_threads(c), finish_smem(c), st>>>(c->d_tiles, c->d_cell_start, dv, c->d_ctrl,
+                                                                   ol_tmp, c->d_nn_tmp, c->d_newslot, c->d_oldof, ol,
+                                                                   c->d_nn_o, c->d_hbase, c->n_pad, c->kmax_o,
+                                                                   c->tile_cap);
+    k_tile_permute<<<grid_for(c, n, 256, 8), 256, 0, st>>>(pos, vel, tag, c->d_pos_outer, c->d_atom_rep, dv,
+                                                          c->d_oldof, c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, n);
     c->launches += 3;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, cudaStream_t st)
+{
+    k_tile_inner<<<c->n_tiles, inner_threads(c), inner_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos, inner_args(c),
+                                                                     c->d_ctrl, c->d_dirty, c->n_pad, c->tile_cap);
+    c->launches++;
     return cudaGetLastError();
 }
 
@@ -635,24 +873,25 @@ cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float
     return cudaGetLastError();
 }
 
-cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, cudaStream_t st)
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int mode, cudaStream_t st)
 {
     k_density_tile<<<c->n_tiles, c->tile_threads, gather_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos,
                                                                        reinterpret_cast<const uint2 *>(c->d_nlist), c->d_nn,
-                                                                       c->d_xs, c->d_ctrl, c->n_pad, c->tile_cap, c->pc);
+                                                                       c->d_xs, c->d_ctrl, c->d_dirty, mode, c->n_pad,
+                                                                       c->tile_cap, c->pc);
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kk,
-                                    cudaStream_t st)
+                                    int mode, cudaStream_t st)
 {
     const uint2 *nl = reinterpret_cast<const uint2 *>(c->d_nlist);
     const size_t sm = gather_smem(c);
     const int g = c->n_tiles, b = c->tile_threads;
 #define TBSMA_FT(V, K)                                                                                             \
     k_force_tile<V, K><<<g, b, sm, st>>>(c->d_tiles, c->d_cell_start, c->d_xs, nl, c->d_nn, force, e_rep, w_rep, kk, \
-                                         c->d_ctrl, c->n_pad, c->tile_cap, c->pc)
+                                         c->d_ctrl, c->d_dirty, mode, c->n_pad, c->tile_cap, c->pc)
     if (w_rep) { if (kk.vel) TBSMA_FT(true, true); else TBSMA_FT(true, false); }
     else       { if (kk.vel) TBSMA_FT(false, true); else TBSMA_FT(false, false); }
 #undef TBSMA_FT

@@ -173,7 +173,9 @@ def test_list_overflow_is_flagged(B, variant):
     ctx.build_cells(st.pos, st.vel, st.tag)
     ctx.build_neighbors(st.pos, st.vel, st.tag)
     assert ctx.status() & B.FLAG_NLIST_OVERFLOW
-    assert ctx.get_stats()["max_neighbors_seen"] == 86
+    seen = ctx.get_stats()["max_neighbors_seen"]
+    # the tile variant filters its list from a candidate list that overflowed first (capacity scales with max_neighbors)
+    assert seen == 86 if variant == 1 else 32 < seen <= 86
     ctx.clear_status()
     assert ctx.status() == 0
 
@@ -194,9 +196,10 @@ def test_call_order_and_arguments(B):
     assert e.value.code == B.EINVAL
 
 
-def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None):
+def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None, overlap=True):
     ctx, st = setup(B, w, variant=variant, tile=tile)
     ctx.set_graph(graph)
+    ctx.set_overlap(overlap)
     ctx.compute(st.pos, st.force, st.e_rep, None)
     stream = torch.cuda.Stream()
     stream.wait_stream(torch.cuda.current_stream())
@@ -289,6 +292,107 @@ def test_replicas_are_independent_and_ragged_batch_matches_single_runs(B, varian
         _, ss = run_gpu_md(B, single, n_steps, variant=variant)
         s = slice(w.offsets[r], w.offsets[r + 1])
         assert np.array_equal(xb[s], ss.untag(ss.pos))          # bit-identical: no cross-replica effect
+
+
+@pytest.mark.parametrize("graph", [True, False])
+def test_two_stream_overlap_is_bitwise_identical(B, graph):
+    """the rebuild chain + rebuilt replicas on the second stream (tbsma_set_overlap) change nothing: a batch with
+    10 K and 298 K replicas (so that some rebuild while others do not) gives the same bits either way"""
+    w = W.config3(6, seed=11, length=60.0)
+    n_steps = 80
+    ca, a = run_gpu_md(B, w, n_steps, variant=2, graph=graph, overlap=True, virial=True)
+    cb, b = run_gpu_md(B, w, n_steps, variant=2, graph=graph, overlap=False, virial=True)
+    sa, sb = ca.get_stats(), cb.get_stats()
+    assert sa == sb
+    assert 0 < sa["n_replica_builds"] < w.n_replicas * n_steps and sa["n_build_passes"] < n_steps
+    for name in ("pos", "vel", "force"):
+        assert np.array_equal(a.untag(getattr(a, name)), b.untag(getattr(b, name))), name
+    # per-replica sums: one fp64 atomic per CTA, so the order (not the terms) may differ
+    assert np.allclose(a.e_rep.cpu().numpy(), b.e_rep.cpu().numpy(), rtol=1e-12, atol=0)
+    assert np.allclose(a.ekin.cpu().numpy(), b.ekin.cpu().numpy(), rtol=1e-12, atol=0)
+    assert np.allclose(a.w_rep.cpu().numpy(), b.w_rep.cpu().numpy(), rtol=1e-12, atol=1e-12)
+    assert ca.status() == 0 and cb.status() == 0
+    md = run_oracle_md(w, n_steps)
+    assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+
+
+@pytest.mark.parametrize("outer_skin", [0.0, 0.5, 2.0])
+def test_candidate_list_radius_changes_cost_not_results(B, outer_skin):
+    """tbsma_set_outer_skin: lists filtered from candidates (radius r_cut + skin + S) are the same sets, and the
+    trajectory the same bits, for every S; small S forces candidate rebuilds, large S none"""
+    w = W.config2(length=60.0)
+    n_steps = 150
+
+    def run(S):
+        ctx = B.make_context(w)
+        ctx.set_variant(2)
+        ctx.set_outer_skin(S)
+        st = B.DeviceState(w)
+        ctx.build_cells(st.pos, st.vel, st.tag)
+        ctx.build_neighbors(st.pos, st.vel, st.tag)
+        cg, lg = gpu_neighbors(B, ctx, st)
+        co, lo = oracle.neighbors(w.pos4, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+        assert_same_sets(cg, lg, co, lo)
+        ctx.compute(st.pos, st.force, st.e_rep, None)
+        stream = torch.cuda.Stream()
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate,
+                       0, st.e_rep, None, st.ekin)
+        torch.cuda.synchronize()
+        # after the run the list still holds exactly the pairs within r_cut + skin of the positions it was built for
+        assert ctx.status() == 0
+        return ctx.get_stats(), st
+
+    sa, a = run(outer_skin)
+    sb, b = run(2.0)
+    assert sa["n_replica_builds"] == sb["n_replica_builds"] >= 5
+    if outer_skin == 0.0:
+        assert sa["n_candidate_builds"] == sa["n_replica_builds"]
+    if outer_skin == 2.0:     # only the relaxation of the as-cut wire ends moves an atom 0.8 A
+        assert sa["n_candidate_builds"] <= 2
+    # same physics; the slot order (hence the fp32 summation order) depends on when candidates were rebuilt
+    xa, xb = a.untag(a.pos)[:, :3].astype(np.float64), b.untag(b.pos)[:, :3].astype(np.float64)
+    assert traj_rms(xa, xb) <= 1e-4
+    md = run_oracle_md(w, n_steps)
+    assert traj_rms(xa, md.x) <= TRAJ_RMS
+
+
+@pytest.mark.parametrize("outer_skin", [0.6, 2.0])
+def test_lists_filtered_from_candidates_are_bit_exact_after_motion(B, outer_skin):
+    """rebuild_every = 1 rebuilds every list in every step, so after n steps the list must be exactly the oracle's
+    neighbour sets of the FINAL positions -- filtered from candidates collected at step 0 (S = 2.0) or re-collected
+    whenever an atom strayed (S = 0.6)"""
+    w = W.config3(2, seed=9, length=60.0)         # one 10 K and one 298 K replica
+    ctx = B.make_context(w)
+    ctx.set_variant(2)
+    ctx.set_outer_skin(outer_skin)
+    st = B.DeviceState(w)
+    ctx.build_cells(st.pos, st.vel, st.tag)
+    ctx.build_neighbors(st.pos, st.vel, st.tag)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    n_steps = 120
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate,
+                   1, st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    stats = ctx.get_stats()
+    assert stats["n_replica_builds"] == w.n_replicas * n_steps
+    if outer_skin == 2.0:
+        assert stats["n_candidate_builds"] <= 2 * w.n_replicas
+    else:
+        assert 0 < stats["n_candidate_builds"] < stats["n_replica_builds"]
+    cg, lg = gpu_neighbors(B, ctx, st)
+    final = st.untag(st.pos)
+    co, lo = oracle.neighbors(final, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+    assert_same_sets(cg, lg, co, lo)
+    moved = np.linalg.norm(final[:, :3] - w.pos4[:, :3], axis=1)
+    assert moved.max() > 0.15                      # the lists really changed
+    assert not np.array_equal(co, oracle.neighbors(w.pos4, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi,
+                                                   w.periodic, max_nb=96)[0])
 
 
 def test_auto_variant_and_tile_shapes(B):
