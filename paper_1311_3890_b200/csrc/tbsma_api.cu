@@ -39,6 +39,8 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters);
     cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_newslot); cudaFree(c->d_oldof);
     cudaFree(c->d_nn_tmp); cudaFree(c->d_tmp_pos);
+    cudaFree(c->d_tile_first); cudaFree(c->d_work);
+    c->d_tile_first = nullptr; c->d_work = nullptr;
     cudaFree(c->d_olist); cudaFree(c->d_nn_o); cudaFree(c->d_pos_outer); cudaFree(c->d_want_outer);
     c->d_olist = nullptr; c->d_nn_o = nullptr; c->d_pos_outer = nullptr; c->d_want_outer = nullptr;
     c->d_tiles = nullptr; c->d_maxpop = nullptr; c->d_hbase = nullptr; c->d_newslot = nullptr; c->d_oldof = nullptr;
@@ -182,6 +184,7 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
             cudaStream_t s2 = c->aux_stream;
             CK(cudaEventRecord(c->ev_fork, st));
             CK(cudaStreamWaitEvent(s2, c->ev_fork, 0));
+            CK(tbsma_launch_tile_worklist(c, s2));
             CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, s2));
             CK(tbsma_launch_tile_inner(c, pos, s2));
             CK(tbsma_launch_density_tile(c, pos, TBSMA_TILES_DIRTY, s2));
@@ -194,6 +197,7 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
             continue;
         }
         if (ev) CK(cudaEventRecord(ev[1], st));
+        if (c->active_variant == 2) CK(tbsma_launch_tile_worklist(c, st));
         CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
         if (c->active_variant == 2) CK(tbsma_launch_tile_inner(c, pos, st));
         if (ev) CK(cudaEventRecord(ev[2], st));
@@ -313,7 +317,9 @@ int tbsma_set_outer_skin(tbsma_ctx *c, double outer_skin)
     if (!c || !(outer_skin >= 0.0) || !(outer_skin <= 16.0)) return TBSMA_EINVAL;
     if (c->d_olist) {
         cudaDeviceSynchronize();
-        cudaFree(c->d_olist); cudaFree(c->d_nn_o); cudaFree(c->d_pos_outer); cudaFree(c->d_want_outer);
+        cudaFree(c->d_tile_first); cudaFree(c->d_work);
+    c->d_tile_first = nullptr; c->d_work = nullptr;
+    cudaFree(c->d_olist); cudaFree(c->d_nn_o); cudaFree(c->d_pos_outer); cudaFree(c->d_want_outer);
         c->d_olist = nullptr; c->d_nn_o = nullptr; c->d_pos_outer = nullptr; c->d_want_outer = nullptr;
     }
     c->outer_skin = outer_skin;
@@ -469,6 +475,7 @@ int tbsma_build_neighbors(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_t
     if (c->n == 0) { c->list_built = 1; return TBSMA_OK; }
     cudaStream_t st = (cudaStream_t)stream;
     CK(tbsma_launch_mark_all_dirty(c, st));
+    if (c->active_variant == 2) CK(tbsma_launch_tile_worklist(c, st));
     CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, false, true, st));
     if (c->active_variant == 2) CK(tbsma_launch_tile_inner(c, (const float4 *)d_pos, st));
     CK(tbsma_launch_finish_step(c, 0, st));

@@ -98,6 +98,10 @@ struct tbsma_ctx {
     int tile_cell_cap;  // halo cells (+1) a tile may hold in shared memory
     int n_tiles;
     TileDesc *d_tiles;
+    int32_t *d_tile_first; // R + 1: the tiles of replica r are [first[r], first[r+1])
+    int32_t *d_work;       // [0] tiles of replicas with dirty >= 1, [1] with dirty == 2, then the two tile lists
+                           // (n_tiles entries each), rebuilt every step by k_tile_worklist
+    int own_cap;           // own atoms a tile may hold (sizes the split of the inner build)
     int32_t *d_maxpop;  // R: largest layer population of each replica (measured at build_cells)
     int32_t *d_hbase;   // n: first halo slot of the tile that owns slot i
     int32_t *d_newslot; // n: cell-order slot -> final slot
@@ -188,6 +192,7 @@ cudaError_t tbsma_launch_count_pairs(tbsma_ctx *c, const float4 *pos, unsigned l
 // shared-memory tile variant (tbsma_tile.cu)
 int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st);   // host: sizes the tiles from the binned cells (synchronises)
 cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, cudaStream_t st);
+cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st);   // tiles of the dirty replicas, from the flags
 cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, cudaStream_t st);   // inner lists of dirty replicas
 cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float4 *vel, const int32_t *tag,
                                     cudaStream_t st);

@@ -71,19 +71,77 @@ __global__ void k_layer_maxpop(const RepGeom *__restrict__ geom, const int *__re
     maxpop[r] = m;
 }
 
+// ---- worklists.  Only a few per cent of the replicas rebuild in a given step, so the kernels that
+// work on them loop over a list of their tiles instead of launching one (mostly idle) CTA per tile.
+// work[0] = tiles of replicas with dirty >= 1, work[1] = with dirty == 2, then the two tile lists.
+__global__ void __launch_bounds__(256)
+k_tile_worklist(const int *__restrict__ dirty, const int *__restrict__ tile_first, int *__restrict__ work, int R,
+                int n_tiles)
+{
+    __shared__ int s_base[2], s_warp[2][8];
+    if (threadIdx.x < 2) s_base[threadIdx.x] = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int r0 = 0; r0 < R; r0 += 256) {
+        const int r = r0 + threadIdx.x;
+        const int d = r < R ? dirty[r] : 0;
+        const int f = r < R ? tile_first[r] : 0, nt = r < R ? tile_first[r + 1] - f : 0;
+        int v[2] = {d >= 1 ? nt : 0, d == 2 ? nt : 0}, incl[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            int x = v[k];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, x, o);
+                if (lane >= o) x += y;
+            }
+            incl[k] = x;
+            if (lane == 31) s_warp[k][wid] = x;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            int off = s_base[k];
+            for (int w = 0; w < wid; ++w) off += s_warp[k][w];
+            int *dst = work + 2 + k * n_tiles + off + incl[k] - v[k];
+            for (int q = 0; q < v[k]; ++q) dst[q] = f + q;
+        }
+        __syncthreads();
+        if (threadIdx.x < 2) {
+            int tot = 0;
+            for (int w = 0; w < 8; ++w) tot += s_warp[threadIdx.x][w];
+            s_base[threadIdx.x] += tot;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x < 2) work[threadIdx.x] = s_base[threadIdx.x];
+}
+
 // ---- K1: scan.  Cell-ordered positions of the tile + halo in shared memory; every own atom scans
 // its 3 x 3 runs of x-adjacent cells, writes its partners (halo-local cell-order indices, u16) to
 // the temporary list, and is ranked inside its layer by (count descending, slot ascending).
-__global__ void __launch_bounds__(kScanThreads)
-k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
-            const int *__restrict__ cell_sorted, DirtyView dv, int *__restrict__ ctrl,
-            const float4 *__restrict__ pos_sorted, uint2 *__restrict__ nl_tmp, int *__restrict__ nn_tmp,
-            int *__restrict__ newslot, int *__restrict__ oldof, int *__restrict__ want_outer, int n_pad, int kmax,
-            float ro2, float rl2, int s_cap, int cell_cap)
+struct ScanArgs {
+    const int *cell_start, *cell_sorted;
+    int *ctrl;
+    const float4 *pos_sorted;
+    uint2 *nl_tmp;
+    int *nn_tmp, *newslot, *oldof, *want_outer;
+    int n_pad, kmax;
+    float ro2, rl2;
+    int s_cap, cell_cap;
+};
+
+__device__ __forceinline__ void scan_tile(const TileDesc &t, const ScanArgs &A)
 {
-    if (!*dv.any) return;
-    const TileDesc t = tiles[blockIdx.x];
-    if (dv.dirty[t.rep] < dv.level) return;
+    const int *__restrict__ cell_start = A.cell_start;
+    const int *__restrict__ cell_sorted = A.cell_sorted;
+    int *__restrict__ ctrl = A.ctrl;
+    const float4 *__restrict__ pos_sorted = A.pos_sorted;
+    uint2 *__restrict__ nl_tmp = A.nl_tmp;
+    int *__restrict__ nn_tmp = A.nn_tmp, *__restrict__ newslot = A.newslot, *__restrict__ oldof = A.oldof;
+    int *__restrict__ want_outer = A.want_outer;
+    const int n_pad = A.n_pad, kmax = A.kmax, s_cap = A.s_cap, cell_cap = A.cell_cap;
+    const float ro2 = A.ro2, rl2 = A.rl2;
     if (threadIdx.x == 0 && t.z_h0 == 0 && t.own_first == 0) want_outer[t.rep] = 0;   // new candidates: request served
     extern __shared__ float4 smem_f4[];
     float4 *sm = smem_f4;
@@ -159,6 +217,17 @@ k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_sta
     }
 }
 
+// K1 over the tiles of the replicas whose candidates are rebuilt (work list 1)
+__global__ void __launch_bounds__(kScanThreads)
+k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ work, int n_tiles, ScanArgs A)
+{
+    const int nw = work[1];
+    for (int w = blockIdx.x; w < nw; w += gridDim.x) {
+        __syncthreads();       // the previous tile's shared-memory image is no longer read
+        scan_tile(tiles[work[2 + n_tiles + w]], A);
+    }
+}
+
 __device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { return (unsigned)(v >> (c << 3)) & 0xffu; }
 
 // ---- K2: finish.  One thread per FINAL slot of the tile: reads the temporary row of the atom that
@@ -166,16 +235,23 @@ __device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { retur
 // tile's shared-memory image, record k at (k + 1) * 16, the sentinel at 0), and writes the row in
 // bank-scheduled order: step p of lane l takes a partner of class (l + p) & 7 (class = bank group
 // of the record), falling back to the fullest class when that one is used up.
-__global__ void __launch_bounds__(kFinishMaxThreads)
-k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
-              DirtyView dv, int *__restrict__ ctrl, const uint2 *__restrict__ nl_tmp,
-              const int *__restrict__ nn_tmp, const int *__restrict__ newslot, const int *__restrict__ oldof,
-              uint2 *__restrict__ nl, int *__restrict__ nn, int *__restrict__ hbase, int n_pad, int kmax,
-              int s_cap)
+struct FinishArgs {
+    const int *cell_start;
+    const uint2 *nl_tmp;
+    const int *nn_tmp, *newslot, *oldof;
+    uint2 *nl;
+    int *nn, *hbase;
+    int n_pad, s_cap;
+};
+
+__device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs &A)
 {
-    if (!*dv.any) return;
-    const TileDesc t = tiles[blockIdx.x];
-    if (dv.dirty[t.rep] < dv.level) return;
+    const int *__restrict__ cell_start = A.cell_start;
+    const uint2 *__restrict__ nl_tmp = A.nl_tmp;
+    const int *__restrict__ nn_tmp = A.nn_tmp, *__restrict__ newslot = A.newslot, *__restrict__ oldof = A.oldof;
+    uint2 *__restrict__ nl = A.nl;
+    int *__restrict__ nn = A.nn, *__restrict__ hbase = A.hbase;
+    const int n_pad = A.n_pad, s_cap = A.s_cap;
     extern __shared__ float4 smem_f4[];
     unsigned short *map = reinterpret_cast<unsigned short *>(smem_f4);   // s_cap entries
     unsigned short *scr = map + ((s_cap + 7) & ~7);                      // kmax x blockDim.x
@@ -253,6 +329,16 @@ k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_s
     }
 }
 
+__global__ void __launch_bounds__(kFinishMaxThreads)
+k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ work, int n_tiles, FinishArgs A)
+{
+    const int nw = work[1];
+    for (int w = blockIdx.x; w < nw; w += gridDim.x) {
+        __syncthreads();
+        finish_tile(tiles[work[2 + n_tiles + w]], A);
+    }
+}
+
 // ---- K3: move positions / velocities / tags from cell order to the final order and record the
 // positions the candidates were built for.
 __global__ void k_tile_permute(float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ tag,
@@ -290,11 +376,48 @@ __global__ void k_stage_copy(const float4 *__restrict__ pos, const float4 *__res
 // the loops need no self / padding test), record k + 1 is the atom at slot halo_lo + k.
 #define TBSMA_SENTINEL 1.0e9f
 
-__device__ __forceinline__ void fill_tile(float4 *sm, const float4 *__restrict__ src, int halo_lo, int nh)
+// The image is one contiguous run of records, so a single bulk copy (cp.async.bulk, the 1-D form of
+// TMA) issued by one thread moves it; everybody waits on the mbarrier the copy completes on.  The
+// caller has made sure (__syncthreads) that nobody still reads a previous image.  `phase` is the
+// parity of the barrier, flipped by every fill.
+struct TileFill {
+    unsigned long long *bar;
+    unsigned phase;
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ TileFill tile_fill_init(unsigned long long *bar)
 {
-    if (threadIdx.x == 0) sm[0] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
-    for (int k = threadIdx.x; k < nh; k += blockDim.x) sm[k + 1] = src[halo_lo + k];
+    if (threadIdx.x == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     __syncthreads();
+    TileFill f;
+    f.bar = bar;
+    f.phase = 0u;
+    return f;
+}
+
+__device__ __forceinline__ void fill_tile(float4 *sm, const float4 *__restrict__ src, int halo_lo, int nh, TileFill &f)
+{
+    const unsigned bar = smem_u32(f.bar);
+    if (threadIdx.x == 0) {
+        sm[0] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
+        const unsigned bytes = (unsigned)nh * 16u;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the image vs. this write
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(smem_u32(sm + 1)), "l"(src + halo_lo), "r"(bytes), "r"(bar) : "memory");
+    }
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(f.phase) : "memory");
+    } while (!done);
+    f.phase ^= 1u;
 }
 
 __device__ __forceinline__ float4 lds_rec(const float4 *sm, unsigned byte_off)
@@ -338,65 +461,88 @@ struct InnerArgs {
 // position 8 j + s wants a record of class (l + s) mod 8, so the eight lanes of a wavefront, all at the
 // same position, read eight different classes.  The j-th kept entry of class c goes straight to position
 // 8 j + ((c - l) mod 8) while j < m / 8 (m = entries kept); the rest fill the positions left free.
-// scr / out: per-thread columns of kmax u16 in shared memory (element k of thread t at [k * nthr + t]).
-__device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRange &r, const float4 *sm,
-                                                 unsigned short *scr, unsigned short *out, const InnerArgs &ia,
-                                                 int *__restrict__ ctrl, int n_pad)
+// Per-thread scratch in shared memory (element k of thread t at [k * nthr + t]): `out`, kmax u16, the list
+// being laid out; `msk`, one bit per candidate (a 32-bit word per eight groups) set by the first pass.
+__device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRange &r, int i_begin, int i_end,
+                                                 const float4 *sm, unsigned *msk, unsigned short *out,
+                                                 const InnerArgs &ia, int *__restrict__ ctrl, int n_pad)
 {
+    // i_begin - r.lo is a multiple of 32, so tid & 31 is the lane the gather kernels give the atom
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     int maxc = 0;
     bool want = false, viol = false, over = false;
-    for (int i = r.lo + tid; i < r.hi; i += nthr) {
+    for (int i = i_begin + tid; i < i_end; i += nthr) {
         const float4 pi = sm[i - r.halo_lo + 1];
         const int nno = ia.nn_o[i];
         const int ng = ((nno & 0xffff) + 3) >> 2;
         const uint2 *row = ia.olist + i;
-        // pass 1: filter the candidates (fp32 predicate of D:A6) into scr, count the classes
+        // pass 1: membership of every candidate (fp32 predicate of D:A6), class populations
         unsigned long long pop = 0ull;
         int m = 0, seen = 0;
-        uint2 nxt = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
-        for (int g = 0; g < ng; ++g) {
-            const uint2 jj = nxt;
-            if (g + 1 < ng) nxt = __ldcs(row + (size_t)(g + 1) * n_pad);
-            const unsigned e[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
+        {
+            uint2 q0 = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
+            uint2 q1 = ng > 1 ? __ldcs(row + (size_t)n_pad) : make_uint2(0u, 0u);
+            unsigned word = 0u;
+            for (int g = 0; g < ng; ++g) {
+                const uint2 jj = (g & 1) ? q1 : q0;
+                const uint2 nx = g + 2 < ng ? __ldcs(row + (size_t)(g + 2) * n_pad) : make_uint2(0u, 0u);
+                if (g & 1) q1 = nx; else q0 = nx;
+                const unsigned e[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
+                float d2[4];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const float4 pj = lds_rec(sm, e[q]);
-                const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
-                if (d2 < ia.rl2) {          // padding entries point at the sentinel and fail
-                    if (m < ia.kmax) {
-                        scr[m * nthr + tid] = (unsigned short)e[q];
-                        pop += 1ull << (((e[q] >> 4) & 7u) << 3);
-                        ++m;
+                for (int q = 0; q < 4; ++q) {
+                    const float4 pj = lds_rec(sm, e[q]);
+                    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                    d2[q] = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (d2[q] < ia.rl2) {          // padding entries point at the sentinel and fail
+                        if (m < ia.kmax) {
+                            word |= 1u << (((g & 7) << 2) + q);
+                            pop += 1ull << (((e[q] >> 4) & 7u) << 3);
+                            ++m;
+                        }
+                        ++seen;
                     }
-                    ++seen;
+                }
+                if ((g & 7) == 7 || g == ng - 1) {
+                    msk[(g >> 3) * nthr + tid] = word;
+                    word = 0u;
                 }
             }
         }
         over = over || seen > ia.kmax;
         maxc = max(maxc, seen);
-        // pass 2: placement
+        // pass 2: placement of the members
         const int L = m >> 3;                 // full rounds
-        unsigned long long cur = 0ull;        // entries of each class placed so far
+        unsigned long long cur = 0ull;        // members of each class placed so far
         int hc = -1, hj = L, tail = L << 3;   // free-position generator: class streams shorter than L, then the tail
-        for (int k = 0; k < m; ++k) {
-            const unsigned e = scr[k * nthr + tid];
-            const int c = (e >> 4) & 7;
-            const int j = (int)byte_of(cur, c);
-            cur += 1ull << (c << 3);
-            int p;
-            if (j < L) {
-                p = (j << 3) + ((c - lane) & 7);
-            } else {
-                while (hj >= L && hc < 8) {
-                    ++hc;
-                    hj = hc < 8 ? (int)byte_of(pop, hc) : L;
+        for (int g = 0; g < ng; ++g) {
+            const unsigned bits = (msk[(g >> 3) * nthr + tid] >> ((g & 7) << 2)) & 15u;
+            if (!bits) continue;
+            const uint2 jj = row[(size_t)g * n_pad];          // again, from L2
+            const unsigned e4[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (!((bits >> q) & 1u)) continue;
+                const unsigned e = e4[q];
+                const int c = (e >> 4) & 7;
+                const int j = (int)byte_of(cur, c);
+                cur += 1ull << (c << 3);
+                int p;
+                if (j < L) {
+                    p = (j << 3) + ((c - lane) & 7);
+                } else {
+                    while (hj >= L && hc < 8) {
+                        ++hc;
+                        hj = hc < 8 ? (int)byte_of(pop, hc) : L;
+                    }
+                    if (hc < 8) { p = (hj << 3) + ((hc - lane) & 7); ++hj; }
+                    else p = tail++;
                 }
-                if (hc < 8) { p = (hj << 3) + ((hc - lane) & 7); ++hj; }
-                else p = tail++;
+                out[p * nthr + tid] = (unsigned short)e;
             }
-            out[p * nthr + tid] = (unsigned short)e;
         }
         const int mpad = (m + 3) & ~3;
         for (int k = m; k < mpad; ++k) out[k * nthr + tid] = 0;      // unused entries = 0 = the sentinel
@@ -421,24 +567,34 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
     if (over) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
 }
 
-// stand-alone inner build of the dirty replicas (tbsma_build_neighbors; inside an MD step the density pass does it)
+// inner build of the dirty replicas: work list 0, every tile cut into pieces of blockDim.x own atoms
 __global__ void __launch_bounds__(512)
-k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start, const float4 *__restrict__ pos,
-             InnerArgs ia, int *__restrict__ ctrl, const int *__restrict__ dirty, int n_pad, int s_cap)
+k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, const int *__restrict__ cell_start,
+             const float4 *__restrict__ pos, InnerArgs ia, int *__restrict__ ctrl, int n_pad, int s_cap, int nsplit,
+             int mask_words)
 {
-    const TileDesc t = tiles[blockIdx.x];
-    if (!dirty[t.rep]) return;
-    const TileRange r = tile_range(t, cell_start);
-    if (r.hi <= r.lo) return;
-    if (r.nh > s_cap) {
-        if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
-        return;
-    }
     extern __shared__ float4 smem_f4[];
-    fill_tile(smem_f4, pos, r.halo_lo, r.nh);
-    unsigned short *scr = reinterpret_cast<unsigned short *>(smem_f4 + s_cap + 1);
-    unsigned short *out = scr + (size_t)ia.kmax * blockDim.x;
-    tile_inner_build(t, r, smem_f4, scr, out, ia, ctrl, n_pad);
+    __shared__ unsigned long long s_bar;
+    const int nu = work[0] * nsplit;
+    if ((int)blockIdx.x >= nu) return;
+    unsigned *msk = reinterpret_cast<unsigned *>(smem_f4 + s_cap + 1);
+    unsigned short *out = reinterpret_cast<unsigned short *>(msk + (size_t)mask_words * blockDim.x);
+    TileFill tf = tile_fill_init(&s_bar);
+    for (int u = blockIdx.x; u < nu; u += gridDim.x) {
+        const TileDesc t = tiles[work[2 + u / nsplit]];
+        const TileRange r = tile_range(t, cell_start);
+        const int i_begin = r.lo + (u % nsplit) * blockDim.x;
+        if (i_begin >= r.hi) continue;
+        if (r.nh > s_cap) {
+            if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
+            continue;
+        }
+        __syncthreads();
+        fill_tile(smem_f4, pos, r.halo_lo, r.nh, tf);
+        // the last piece also takes whatever a tile holds beyond the headroom it was sized with
+        const int i_end = (u % nsplit) == nsplit - 1 ? r.hi : min(i_begin + (int)blockDim.x, r.hi);
+        tile_inner_build(t, r, i_begin, i_end, smem_f4, msk, out, ia, ctrl, n_pad);
+    }
 }
 
 // Work distribution of the two gather kernels: the own atoms of a tile are cut into chunks of 32
@@ -446,9 +602,6 @@ k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
 // chunks from a shared counter, so no warp waits at the end for one that drew the long lists.
 // The list rows are prefetched three groups (12 entries) ahead: a row is 8 bytes per lane from
 // HBM, and one group of pair terms is shorter than the HBM latency.
-#define TBSMA_TILE_MODE_SKIP(mode, level) \
-    ((mode) != TBSMA_TILES_ALL && ((level) != 0) != ((mode) == TBSMA_TILES_DIRTY))
-
 __device__ __forceinline__ int next_chunk(int *counter)
 {
     int ch = 0;
@@ -462,14 +615,12 @@ __device__ __forceinline__ uint2 ld_row(const uint2 *row, int g, int ng, int n_p
 }
 
 // stage 1 (Eq.1): rho_i over the list, s_i = rho_i^(-1/2) packed with the position
-__global__ void __launch_bounds__(512, 2)
-k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
-               const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
-               float4 *__restrict__ xs, int *__restrict__ ctrl, const int *__restrict__ dirty, int mode,
-               int n_pad, int s_cap, PairConst pc)
+__device__ __forceinline__ void density_tile(const TileDesc &t, const int *__restrict__ cell_start,
+                                             const float4 *__restrict__ pos, const uint2 *__restrict__ nl,
+                                             const int *__restrict__ nn, float4 *__restrict__ xs,
+                                             int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
+                                             TileFill &tf)
 {
-    const TileDesc t = tiles[blockIdx.x];
-    if (TBSMA_TILE_MODE_SKIP(mode, dirty[t.rep])) return;
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
     if (r.nh > s_cap) {
@@ -480,7 +631,7 @@ k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_
     __shared__ int s_next;
     const float4 *sm = smem_f4;
     if (threadIdx.x == 0) s_next = 0;
-    fill_tile(smem_f4, pos, r.halo_lo, r.nh);
+    fill_tile(smem_f4, pos, r.halo_lo, r.nh, tf);
     const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
     for (int ch = next_chunk(&s_next); ch < nchunk; ch = next_chunk(&s_next)) {
         const int i = r.lo + (ch << 5) + lane;
@@ -513,6 +664,31 @@ k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_
         const float s = rho > 0.f ? 1.0f / sqrtf(rho) : 0.f;     // once per atom, IEEE (D:A5 for rho = 0)
         xs[i] = make_float4(pi.x, pi.y, pi.z, s);
     }
+}
+
+// mode ALL / CLEAN: one CTA per tile (CLEAN skips the replicas being rebuilt); mode DIRTY: the CTAs loop over
+// work list 0.  nn and nl are read-only here: they were written by an earlier kernel.
+__global__ void __launch_bounds__(512, 2)
+k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
+               const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
+               float4 *__restrict__ xs, int *__restrict__ ctrl, const int *__restrict__ dirty,
+               const int *__restrict__ work, int mode, int n_pad, int s_cap, PairConst pc)
+{
+    __shared__ unsigned long long s_bar;
+    if (mode == TBSMA_TILES_DIRTY) {
+        const int nw = work[0];
+        if ((int)blockIdx.x >= nw) return;
+        TileFill tf = tile_fill_init(&s_bar);
+        for (int w = blockIdx.x; w < nw; w += gridDim.x) {
+            __syncthreads();
+            density_tile(tiles[work[2 + w]], cell_start, pos, nl, nn, xs, ctrl, n_pad, s_cap, pc, tf);
+        }
+        return;
+    }
+    const TileDesc t = tiles[blockIdx.x];
+    if (mode == TBSMA_TILES_CLEAN && dirty[t.rep]) return;
+    TileFill tf = tile_fill_init(&s_bar);
+    density_tile(t, cell_start, pos, nl, nn, xs, ctrl, n_pad, s_cap, pc, tf);
 }
 
 struct AccT {
@@ -566,14 +742,13 @@ __device__ __forceinline__ void cta_add(double *dst, double v, double *red)
 
 // stage 2 (Eq.1-3, Eq.5): forces, per-atom energy, virial, closing half kick, E_kin
 template <bool VIRIAL, bool KICK>
-__global__ void __launch_bounds__(512, 2)
-k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
-             const float4 *__restrict__ xs, const uint2 *__restrict__ nl, const int *__restrict__ nn,
-             float4 *__restrict__ force, double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk,
-             int *__restrict__ ctrl, const int *__restrict__ dirty, int mode, int n_pad, int s_cap, PairConst pc)
+__device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restrict__ cell_start,
+                                           const float4 *__restrict__ xs, const uint2 *__restrict__ nl,
+                                           const int *__restrict__ nn, float4 *__restrict__ force,
+                                           double *__restrict__ e_rep, double *__restrict__ w_rep, const KickArgs &kk,
+                                           int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
+                                           TileFill &tf)
 {
-    const TileDesc t = tiles[blockIdx.x];
-    if (TBSMA_TILE_MODE_SKIP(mode, dirty[t.rep])) return;
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
     if (r.nh > s_cap) {
@@ -585,7 +760,7 @@ k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
     __shared__ int s_next;
     const float4 *sm = smem_f4;
     if (threadIdx.x == 0) s_next = 0;
-    fill_tile(smem_f4, xs, r.halo_lo, r.nh);
+    fill_tile(smem_f4, xs, r.halo_lo, r.nh, tf);
     double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     bool bad = false;
     const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
@@ -641,6 +816,32 @@ k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
 #pragma unroll
         for (int k = 0; k < 6; ++k) cta_add(w_rep + 6 * (size_t)t.rep + k, sw[k], red);
     }
+}
+
+template <bool VIRIAL, bool KICK>
+__global__ void __launch_bounds__(512, 2)
+k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
+             const float4 *__restrict__ xs, const uint2 *__restrict__ nl, const int *__restrict__ nn,
+             float4 *__restrict__ force, double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk,
+             int *__restrict__ ctrl, const int *__restrict__ dirty, const int *__restrict__ work, int mode,
+             int n_pad, int s_cap, PairConst pc)
+{
+    __shared__ unsigned long long s_bar;
+    if (mode == TBSMA_TILES_DIRTY) {
+        const int nw = work[0];
+        if ((int)blockIdx.x >= nw) return;
+        TileFill tf = tile_fill_init(&s_bar);
+        for (int w = blockIdx.x; w < nw; w += gridDim.x) {
+            __syncthreads();
+            force_tile<VIRIAL, KICK>(tiles[work[2 + w]], cell_start, xs, nl, nn, force, e_rep, w_rep, kk, ctrl, n_pad,
+                                     s_cap, pc, tf);
+        }
+        return;
+    }
+    const TileDesc t = tiles[blockIdx.x];
+    if (mode == TBSMA_TILES_CLEAN && dirty[t.rep]) return;
+    TileFill tf = tile_fill_init(&s_bar);
+    force_tile<VIRIAL, KICK>(t, cell_start, xs, nl, nn, force, e_rep, w_rep, kk, ctrl, n_pad, s_cap, pc, tf);
 }
 
 // ---- inspection (parity tests, bench statistics) ----------------------------------------------
@@ -710,15 +911,22 @@ size_t finish_smem(const tbsma_ctx *c)
     return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax_o * finish_threads(c) * 2;
 }
 size_t gather_smem(const tbsma_ctx *c) { return (size_t)(c->tile_cap + 1) * 16; }
+// grid of a gather launch: one CTA per tile, or (mode DIRTY) enough CTAs to loop over the work list
+int gather_grid(const tbsma_ctx *c, int mode)
+{
+    if (mode != TBSMA_TILES_DIRTY) return c->n_tiles;
+    return c->n_tiles < 4 * c->n_sm ? c->n_tiles : 4 * c->n_sm;
+}
+int inner_mask_words(const tbsma_ctx *c) { return (c->kmax_o / 4 + 7) / 8; }
+size_t inner_bytes_per_thread(const tbsma_ctx *c) { return (size_t)c->kmax * 2 + (size_t)inner_mask_words(c) * 4; }
 int inner_threads(const tbsma_ctx *c)
 {
-    const size_t budget = 200 * 1024 - gather_smem(c);
-    int t = (int)(budget / ((size_t)c->kmax * 4)) & ~31;      // two u16 columns of kmax per thread
+    int t = (int)((200 * 1024 - gather_smem(c)) / inner_bytes_per_thread(c)) & ~31;
     if (t > 512) t = 512;
     if (t < 32) t = 32;
     return t;
 }
-size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + (size_t)c->kmax * 4 * inner_threads(c); }
+size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + inner_bytes_per_thread(c) * inner_threads(c); }
 InnerArgs inner_args(const tbsma_ctx *c)
 {
     InnerArgs ia;
@@ -764,7 +972,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     if (lmax < 1) lmax = 1;
     if (lmax > TBSMA_TILE_MAX_LAYERS) lmax = TBSMA_TILE_MAX_LAYERS;
     int64_t n_tiles = 0;
-    int cell_cap = 0, rec_cap = 0;
+    int cell_cap = 0, rec_cap = 0, own_cap = 0;
     bool fits = true;
     int *Lr = (int *)malloc(sizeof(int) * R);
     if (!Lr) { free(maxpop); return TBSMA_ENOMEM; }
@@ -778,6 +986,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         if ((int64_t)(L + 2) * lc + 1 > 8192) { fits = false; break; }
         if ((L + 2) * lc + 1 > cell_cap) cell_cap = (L + 2) * lc + 1;
         if ((int)((L + 2) * pop) > rec_cap) rec_cap = (int)((L + 2) * pop);
+        if ((int)(L * pop) > own_cap) own_cap = (int)(L * pop);
         Lr[r] = L;
         n_tiles += (g.nc[2] + L - 1) / L;
     }
@@ -787,9 +996,11 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;   // forced tile variant that does not fit
     }
     TileDesc *h = (TileDesc *)malloc(sizeof(TileDesc) * (size_t)(n_tiles ? n_tiles : 1));
-    if (!h) { free(Lr); return TBSMA_ENOMEM; }
+    int *first = (int *)malloc(sizeof(int) * (size_t)(R + 1));
+    if (!h || !first) { free(Lr); free(h); free(first); return TBSMA_ENOMEM; }
     int64_t k = 0;
     for (int r = 0; r < R; ++r) {
+        first[r] = (int)k;
         const RepGeom &g = c->h_geom[r];
         const int lc = g.nc[0] * g.nc[1], nz = g.nc[2], L = Lr[r];
         for (int z0 = 0; z0 < nz; z0 += L) {
@@ -808,17 +1019,24 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
             t.pad = 0;
         }
     }
+    first[R] = (int)k;
     free(Lr);
-    cudaFree(c->d_tiles);
-    c->d_tiles = nullptr;
+    cudaFree(c->d_tiles); cudaFree(c->d_tile_first); cudaFree(c->d_work);
+    c->d_tiles = nullptr; c->d_tile_first = nullptr; c->d_work = nullptr;
     e = cudaMalloc((void **)&c->d_tiles, sizeof(TileDesc) * (size_t)(n_tiles ? n_tiles : 1));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_tile_first, sizeof(int) * (size_t)(R + 1));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_work, sizeof(int) * (size_t)(2 + 2 * n_tiles));
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->d_work, 0, sizeof(int) * (size_t)(2 + 2 * n_tiles), st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tiles, h, sizeof(TileDesc) * (size_t)n_tiles, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tile_first, first, sizeof(int) * (size_t)(R + 1), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     free(h);
+    free(first);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? TBSMA_ENOMEM : TBSMA_ECUDA;
     c->n_tiles = (int)n_tiles;
     c->tile_cap = rec_cap < cap ? rec_cap : cap;   // shared-memory image sized to the largest halo expected
     c->tile_cell_cap = (cell_cap + 3) & ~3;
+    c->own_cap = own_cap;
     // opt in to > 48 KB of dynamic shared memory
     const int sm_scan = (int)scan_smem(c), sm_fin = (int)finish_smem(c), sm_g = (int)gather_smem(c);
     e = cudaFuncSetAttribute(k_tile_scan, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_scan);
@@ -842,25 +1060,40 @@ cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int3
     const DirtyView dv = tbsma_dirty_view(c);
     uint2 *ol = c->d_olist;
     uint2 *ol_tmp = ol + (size_t)(c->kmax_o / 4) * c->n_pad;    // second half of the allocation
-    k_tile_scan<<<c->n_tiles, kScanThreads, scan_smem(c), st>>>(c->d_tiles, c->d_cell_start, c->d_slot, dv,
-                                                               c->d_ctrl, c->d_tmp_pos, ol_tmp, c->d_nn_tmp,
-                                                               c->d_newslot, c->d_oldof, c->d_want_outer, c->n_pad,
-                                                               c->kmax_o, c->pc.ro2, c->pc.rl2, c->tile_cap,
-                                                               c->tile_cell_cap);
-    k_tile_finish<<<c->n_tiles, finish_threads(c), finish_smem(c), st>>>(c->d_tiles, c->d_cell_start, dv, c->d_ctrl,
-                                                                   ol_tmp, c->d_nn_tmp, c->d_newslot, c->d_oldof, ol,
-                                                                   c->d_nn_o, c->d_hbase, c->n_pad, c->kmax_o,
-                                                                   c->tile_cap);
+    ScanArgs sa;
+    sa.cell_start = c->d_cell_start; sa.cell_sorted = c->d_slot; sa.ctrl = c->d_ctrl; sa.pos_sorted = c->d_tmp_pos;
+    sa.nl_tmp = ol_tmp; sa.nn_tmp = c->d_nn_tmp; sa.newslot = c->d_newslot; sa.oldof = c->d_oldof;
+    sa.want_outer = c->d_want_outer; sa.n_pad = c->n_pad; sa.kmax = c->kmax_o; sa.ro2 = c->pc.ro2; sa.rl2 = c->pc.rl2;
+    sa.s_cap = c->tile_cap; sa.cell_cap = c->tile_cell_cap;
+    FinishArgs fa;
+    fa.cell_start = c->d_cell_start; fa.nl_tmp = ol_tmp; fa.nn_tmp = c->d_nn_tmp; fa.newslot = c->d_newslot;
+    fa.oldof = c->d_oldof; fa.nl = ol; fa.nn = c->d_nn_o; fa.hbase = c->d_hbase; fa.n_pad = c->n_pad;
+    fa.s_cap = c->tile_cap;
+    const int gw = c->n_tiles < 2 * c->n_sm ? c->n_tiles : 2 * c->n_sm;
+    k_tile_scan<<<gw, kScanThreads, scan_smem(c), st>>>(c->d_tiles, c->d_work, c->n_tiles, sa);
+    k_tile_finish<<<gw, finish_threads(c), finish_smem(c), st>>>(c->d_tiles, c->d_work, c->n_tiles, fa);
     k_tile_permute<<<grid_for(c, n, 256, 8), 256, 0, st>>>(pos, vel, tag, c->d_pos_outer, c->d_atom_rep, dv,
                                                           c->d_oldof, c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, n);
     c->launches += 3;
     return cudaGetLastError();
 }
 
+cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st)
+{
+    k_tile_worklist<<<1, 256, 0, st>>>(c->d_dirty, c->d_tile_first, c->d_work, c->R, c->n_tiles);
+    c->launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, cudaStream_t st)
 {
-    k_tile_inner<<<c->n_tiles, inner_threads(c), inner_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos, inner_args(c),
-                                                                     c->d_ctrl, c->d_dirty, c->n_pad, c->tile_cap);
+    const int nt = inner_threads(c);
+    int nsplit = (c->own_cap + nt - 1) / nt;
+    if (nsplit < 1) nsplit = 1;
+    const int64_t units = (int64_t)c->n_tiles * nsplit;
+    const int grid = (int)(units < 2 * (int64_t)c->n_sm ? units : 2 * (int64_t)c->n_sm);
+    k_tile_inner<<<grid, nt, inner_smem(c), st>>>(c->d_tiles, c->d_work, c->d_cell_start, pos, inner_args(c), c->d_ctrl,
+                                                  c->n_pad, c->tile_cap, nsplit, inner_mask_words(c));
     c->launches++;
     return cudaGetLastError();
 }
@@ -875,10 +1108,11 @@ cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float
 
 cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int mode, cudaStream_t st)
 {
-    k_density_tile<<<c->n_tiles, c->tile_threads, gather_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos,
-                                                                       reinterpret_cast<const uint2 *>(c->d_nlist), c->d_nn,
-                                                                       c->d_xs, c->d_ctrl, c->d_dirty, mode, c->n_pad,
-                                                                       c->tile_cap, c->pc);
+    const int g = gather_grid(c, mode);
+    k_density_tile<<<g, c->tile_threads, gather_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos,
+                                                              reinterpret_cast<const uint2 *>(c->d_nlist), c->d_nn,
+                                                              c->d_xs, c->d_ctrl, c->d_dirty, c->d_work, mode, c->n_pad,
+                                                              c->tile_cap, c->pc);
     c->launches++;
     return cudaGetLastError();
 }
@@ -888,10 +1122,10 @@ cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, 
 {
     const uint2 *nl = reinterpret_cast<const uint2 *>(c->d_nlist);
     const size_t sm = gather_smem(c);
-    const int g = c->n_tiles, b = c->tile_threads;
+    const int g = gather_grid(c, mode), b = c->tile_threads;
 #define TBSMA_FT(V, K)                                                                                             \
     k_force_tile<V, K><<<g, b, sm, st>>>(c->d_tiles, c->d_cell_start, c->d_xs, nl, c->d_nn, force, e_rep, w_rep, kk, \
-                                         c->d_ctrl, c->d_dirty, mode, c->n_pad, c->tile_cap, c->pc)
+                                         c->d_ctrl, c->d_dirty, c->d_work, mode, c->n_pad, c->tile_cap, c->pc)
     if (w_rep) { if (kk.vel) TBSMA_FT(true, true); else TBSMA_FT(true, false); }
     else       { if (kk.vel) TBSMA_FT(false, true); else TBSMA_FT(false, false); }
 #undef TBSMA_FT
