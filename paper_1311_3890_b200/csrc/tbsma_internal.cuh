@@ -89,7 +89,7 @@ struct tbsma_ctx {
     int tile_threads;   // CTA size of the tile kernels
     double outer_skin;  // S: the candidate list holds every pair within r_cut + skin + S at its build
     int kmax_o;         // capacity of the candidate list per atom (multiple of 4, <= 248)
-    uint2 *d_olist;     // 2 x (kmax_o/4 x n_pad) uint2: candidate list (bank-scheduled u16 offsets) + build scratch
+    uint2 *d_olist;     // 2 x (kmax_o/4 x n_pad) uint2: candidate list (atom-major rows of kmax_o u16 offsets) + build scratch
     int32_t *d_nn_o;    // n: candidate count | flag << 16
     float4 *d_pos_outer;   // n: positions when the candidate list was built
     int32_t *d_want_outer; // R: the next rebuild of this replica must redo cells + candidate list

@@ -232,9 +232,9 @@ __device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { retur
 
 // ---- K2: finish.  One thread per FINAL slot of the tile: reads the temporary row of the atom that
 // moves there, translates every partner to its final position (byte offset of its record in the
-// tile's shared-memory image, record k at (k + 1) * 16, the sentinel at 0), and writes the row in
-// bank-scheduled order: step p of lane l takes a partner of class (l + p) & 7 (class = bank group
-// of the record), falling back to the fullest class when that one is used up.
+// tile's shared-memory image, record k at (k + 1) * 16, the sentinel at 0), and writes the row sorted
+// by CLASS (bank group of the record = record index mod 8; stable inside a class): the inner build
+// keeps this order when it filters, so its kept entries come out grouped by class as well.
 struct FinishArgs {
     const int *cell_start;
     const uint2 *nl_tmp;
@@ -257,7 +257,7 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs 
     unsigned short *scr = map + ((s_cap + 7) & ~7);                      // kmax x blockDim.x
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo || r.nh > s_cap) return;
-    const int tid = threadIdx.x, lane = tid & 31, nthr = blockDim.x;
+    const int tid = threadIdx.x, nthr = blockDim.x;
     for (int k = tid; k < r.nh; k += blockDim.x)
         map[k] = (unsigned short)((newslot[r.halo_lo + k] - r.halo_lo + 1) << 4);
     __syncthreads();
@@ -297,33 +297,14 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs 
                     scr[idx * nthr + tid] = (unsigned short)m;
                 }
         }
-        // emission in scheduled order
-        unsigned long long rem = pop;
-        cur = 0ull;
+        // rows of four entries, unused entries = 0 = the sentinel
         uint2 *dst = nl + ip;
-        unsigned w0 = 0u, w1 = 0u;
-        for (int p = 0; p < cnt; ++p) {
-            int c = (lane + p) & 7;
-            if (byte_of(rem, c) == 0u) {
-                unsigned best = 0u;
+        for (int g = 0; g < ng; ++g) {
+            unsigned e[4];
 #pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    const int cc = (c + 4 + q) & 7;
-                    const unsigned v = byte_of(rem, cc);
-                    if (v > best) { best = v; c = cc; }
-                }
-            }
-            const unsigned idx = byte_of(off, c) + byte_of(cur, c);
-            cur += 1ull << (c << 3);
-            rem -= 1ull << (c << 3);
-            const unsigned v = (unsigned)scr[idx * nthr + tid] << ((p & 1) << 4);
-            if (p & 2) w1 |= v; else w0 |= v;
-            if ((p & 3) == 3) {
-                dst[(size_t)(p >> 2) * n_pad] = make_uint2(w0, w1);
-                w0 = w1 = 0u;
-            }
+            for (int q = 0; q < 4; ++q) e[q] = 4 * g + q < cnt ? (unsigned)scr[(4 * g + q) * nthr + tid] : 0u;
+            dst[(size_t)g * n_pad] = make_uint2(e[0] | (e[1] << 16), e[2] | (e[3] << 16));
         }
-        if (cnt & 3) dst[(size_t)(cnt >> 2) * n_pad] = make_uint2(w0, w1);   // unused entries = 0 = the sentinel
         nn[ip] = nnv;
         hbase[ip] = r.halo_lo;
     }
@@ -437,14 +418,22 @@ __device__ __forceinline__ float rho_term_t(const float4 &pi, const float4 &pj, 
 
 
 // ---- inner build: the list the gather passes read, filtered from the candidates.
-// Runs inside the tile that owns the atoms, on the positions already staged in shared memory (sm:
-// record k + 1 = slot halo_lo + k, record 0 = sentinel).  Kept entries stay in candidate order (the
-// bank schedule of K2); the membership test is the fp32 predicate of D:A6 against rl2.  Also records
-// the positions of this build (displacement check of the integrator) and compares them with those of
-// the candidate build: more than S/2 away invalidates the candidates (status flag), more than
-// want2^(1/2) asks for new candidates at the replica's next rebuild.
+// Runs on the tile that owns the atoms, on the positions staged in shared memory (sm: record k + 1 =
+// slot halo_lo + k, record 0 = sentinel).  The membership test is the fp32 predicate of D:A6 against
+// rl2.  Also records the positions of this build (displacement check of the integrator) and compares
+// them with those of the candidate build: more than S/2 away invalidates the candidates (status
+// flag), more than want2^(1/2) asks for new candidates at the replica's next rebuild.
+//
+// Order of the kept entries (bank schedule).  A 128-bit shared-memory load is served eight lanes at a
+// time, and eight lanes reading eight different 16-byte bank groups ("classes", record index mod 8) take
+// one wavefront.  In the gather passes the atom is handled by lane l = (slot - first own slot) & 31 and
+// all lanes are at the same list position p, so position p of lane l should hold a record of class
+// (l + p) mod 8.  The candidates arrive sorted by class (K2), so the kept entries are eight runs, one per
+// class; the list is written round by round, round j taking the j-th entry of the classes l, l + 1, ...,
+// l + 7 (mod 8) that still have one.  While every class has a j-th entry that IS the schedule; when
+// classes run out the later entries close up.
 struct InnerArgs {
-    const uint2 *olist;      // candidates
+    const uint2 *olist;      // candidates (class-sorted rows)
     const int *nn_o;
     uint2 *nl;               // out: inner list
     int *nn;                 // out: count | flag << 16
@@ -455,17 +444,20 @@ struct InnerArgs {
     float rl2, want2, viol2;
 };
 
-// Order of the kept entries (bank schedule).  A 128-bit shared-memory load is served eight lanes at a
-// time, and eight lanes reading eight different 16-byte bank groups ("classes", record index mod 8) take
-// one wavefront.  The list of the atom handled by lane l is laid out in rounds of eight positions;
-// position 8 j + s wants a record of class (l + s) mod 8, so the eight lanes of a wavefront, all at the
-// same position, read eight different classes.  The j-th kept entry of class c goes straight to position
-// 8 j + ((c - l) mod 8) while j < m / 8 (m = entries kept); the rest fill the positions left free.
-// Per-thread scratch in shared memory (element k of thread t at [k * nthr + t]): `out`, kmax u16, the list
-// being laid out; `msk`, one bit per candidate (a 32-bit word per eight groups) set by the first pass.
+constexpr int kInnerThreads = 256;   // one atom per thread, kmax u16 of shared-memory scratch each
+
+__device__ __forceinline__ unsigned long long rotr64_bytes(unsigned long long v, int nbytes)
+{
+    const int s = (nbytes & 7) << 3;
+    return s ? (v >> s) | (v << (64 - s)) : v;
+}
+
+// tmp: element k of thread t at [((k >> 1) * nthr + t) * 2 + (k & 1)]: a thread's entries stay in one bank,
+// so the lanes of a warp never conflict, whatever k each of them is at
+#define TMP_AT(k) ((((k) >> 1) * nthr + tid) * 2 + ((k) & 1))
 __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRange &r, int i_begin, int i_end,
-                                                 const float4 *sm, unsigned *msk, unsigned short *out,
-                                                 const InnerArgs &ia, int *__restrict__ ctrl, int n_pad)
+                                                 const float4 *sm, unsigned short *tmp, const InnerArgs &ia,
+                                                 int *__restrict__ ctrl, int n_pad)
 {
     // i_begin - r.lo is a multiple of 32, so tid & 31 is the lane the gather kernels give the atom
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
@@ -476,82 +468,78 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
         const int nno = ia.nn_o[i];
         const int ng = ((nno & 0xffff) + 3) >> 2;
         const uint2 *row = ia.olist + i;
-        // pass 1: membership of every candidate (fp32 predicate of D:A6), class populations
-        unsigned long long pop = 0ull;
+        // pass 1: the candidates that pass the fp32 predicate of D:A6, in candidate order
         int m = 0, seen = 0;
-        {
-            uint2 q0 = ng > 0 ? __ldcs(row) : make_uint2(0u, 0u);
-            uint2 q1 = ng > 1 ? __ldcs(row + (size_t)n_pad) : make_uint2(0u, 0u);
-            unsigned word = 0u;
-            for (int g = 0; g < ng; ++g) {
-                const uint2 jj = (g & 1) ? q1 : q0;
-                const uint2 nx = g + 2 < ng ? __ldcs(row + (size_t)(g + 2) * n_pad) : make_uint2(0u, 0u);
-                if (g & 1) q1 = nx; else q0 = nx;
-                const unsigned e[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
-                float d2[4];
+        auto group = [&](const uint2 jj) {
+            const unsigned e[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
+            float d2[4];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const float4 pj = lds_rec(sm, e[q]);
-                    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                    d2[q] = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
-                }
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    if (d2[q] < ia.rl2) {          // padding entries point at the sentinel and fail
-                        if (m < ia.kmax) {
-                            word |= 1u << (((g & 7) << 2) + q);
-                            pop += 1ull << (((e[q] >> 4) & 7u) << 3);
-                            ++m;
-                        }
-                        ++seen;
-                    }
-                }
-                if ((g & 7) == 7 || g == ng - 1) {
-                    msk[(g >> 3) * nthr + tid] = word;
-                    word = 0u;
-                }
+            for (int q = 0; q < 4; ++q) {
+                const float4 pj = lds_rec(sm, e[q]);
+                const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                d2[q] = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
             }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (d2[q] < ia.rl2) {          // padding entries point at the sentinel and fail
+                    if (m < ia.kmax) { tmp[TMP_AT(m)] = (unsigned short)e[q]; ++m; }
+                    ++seen;
+                }
+        };
+        {
+            auto ld = [&](int g) { return g < ng ? __ldcs(row + (size_t)g * n_pad) : make_uint2(0u, 0u); };
+            uint2 q0 = ld(0), q1 = ld(1), q2 = ld(2), q3 = ld(3);
+            int g = 0;
+            for (; g + 4 <= ng; g += 4) {
+                uint2 jj = q0; q0 = ld(g + 4); group(jj);
+                jj = q1; q1 = ld(g + 5); group(jj);
+                jj = q2; q2 = ld(g + 6); group(jj);
+                jj = q3; q3 = ld(g + 7); group(jj);
+            }
+            if (g < ng) group(q0);
+            if (g + 1 < ng) group(q1);
+            if (g + 2 < ng) group(q2);
         }
         over = over || seen > ia.kmax;
         maxc = max(maxc, seen);
-        // pass 2: placement of the members
-        const int L = m >> 3;                 // full rounds
-        unsigned long long cur = 0ull;        // members of each class placed so far
-        int hc = -1, hj = L, tail = L << 3;   // free-position generator: class streams shorter than L, then the tail
-        for (int g = 0; g < ng; ++g) {
-            const unsigned bits = (msk[(g >> 3) * nthr + tid] >> ((g & 7) << 2)) & 15u;
-            if (!bits) continue;
-            const uint2 jj = row[(size_t)g * n_pad];          // again, from L2
-            const unsigned e4[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
+        // entries per class and first entry of each class (packed bytes), rotated so that byte s is class lane + s
+        unsigned long long npk = 0ull;
+        for (int k = 0; k < m; ++k) npk += 1ull << (((tmp[TMP_AT(k)] >> 4) & 7u) << 3);
+        unsigned long long opk = 0ull;
+        int nmax = 0;
+        {
+            unsigned run = 0;
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                if (!((bits >> q) & 1u)) continue;
-                const unsigned e = e4[q];
-                const int c = (e >> 4) & 7;
-                const int j = (int)byte_of(cur, c);
-                cur += 1ull << (c << 3);
-                int p;
-                if (j < L) {
-                    p = (j << 3) + ((c - lane) & 7);
-                } else {
-                    while (hj >= L && hc < 8) {
-                        ++hc;
-                        hj = hc < 8 ? (int)byte_of(pop, hc) : L;
-                    }
-                    if (hc < 8) { p = (hj << 3) + ((hc - lane) & 7); ++hj; }
-                    else p = tail++;
-                }
-                out[p * nthr + tid] = (unsigned short)e;
+            for (int c = 0; c < 8; ++c) {
+                const unsigned n_c = byte_of(npk, c);
+                opk |= (unsigned long long)run << (c << 3);
+                run += n_c;
+                nmax = max(nmax, (int)n_c);
             }
         }
-        const int mpad = (m + 3) & ~3;
-        for (int k = m; k < mpad; ++k) out[k * nthr + tid] = 0;      // unused entries = 0 = the sentinel
+        const unsigned long long nrot = rotr64_bytes(npk, lane), orot = rotr64_bytes(opk, lane);
+        int n_s[8], o_s[8];
+#pragma unroll
+        for (int sft = 0; sft < 8; ++sft) { n_s[sft] = (int)byte_of(nrot, sft); o_s[sft] = (int)byte_of(orot, sft); }
+        // pass 2: round j takes the j-th entry of classes lane, lane + 1, ... that still have one
         uint2 *dst = ia.nl + i;
-        for (int g = 0; g < (mpad >> 2); ++g) {
-            const unsigned a0 = out[(4 * g) * nthr + tid], a1 = out[(4 * g + 1) * nthr + tid];
-            const unsigned a2 = out[(4 * g + 2) * nthr + tid], a3 = out[(4 * g + 3) * nthr + tid];
-            dst[(size_t)g * n_pad] = make_uint2(a0 | (a1 << 16), a2 | (a3 << 16));
+        unsigned w0 = 0u, w1 = 0u;
+        int p = 0;
+        for (int j = 0; j < nmax; ++j) {
+#pragma unroll
+            for (int sft = 0; sft < 8; ++sft)
+                if (j < n_s[sft]) {
+                    const int k = o_s[sft] + j;
+                    const unsigned v = (unsigned)tmp[TMP_AT(k)] << ((p & 1) << 4);
+                    if (p & 2) w1 |= v; else w0 |= v;
+                    if ((p & 3) == 3) {
+                        dst[(size_t)(p >> 2) * n_pad] = make_uint2(w0, w1);
+                        w0 = w1 = 0u;
+                    }
+                    ++p;
+                }
         }
+        if (p & 3) dst[(size_t)(p >> 2) * n_pad] = make_uint2(w0, w1);      // unused entries = 0 = the sentinel
         ia.nn[i] = m | (nno & 0x7fff0000);
         ia.pos_build[i] = pi;
         const float4 po = ia.pos_outer[i];
@@ -568,17 +556,15 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
 }
 
 // inner build of the dirty replicas: work list 0, every tile cut into pieces of blockDim.x own atoms
-__global__ void __launch_bounds__(512)
+__global__ void __launch_bounds__(kInnerThreads)
 k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, const int *__restrict__ cell_start,
-             const float4 *__restrict__ pos, InnerArgs ia, int *__restrict__ ctrl, int n_pad, int s_cap, int nsplit,
-             int mask_words)
+             const float4 *__restrict__ pos, InnerArgs ia, int *__restrict__ ctrl, int n_pad, int s_cap, int nsplit)
 {
     extern __shared__ float4 smem_f4[];
     __shared__ unsigned long long s_bar;
     const int nu = work[0] * nsplit;
     if ((int)blockIdx.x >= nu) return;
-    unsigned *msk = reinterpret_cast<unsigned *>(smem_f4 + s_cap + 1);
-    unsigned short *out = reinterpret_cast<unsigned short *>(msk + (size_t)mask_words * blockDim.x);
+    unsigned short *tmp = reinterpret_cast<unsigned short *>(smem_f4 + s_cap + 1);
     TileFill tf = tile_fill_init(&s_bar);
     for (int u = blockIdx.x; u < nu; u += gridDim.x) {
         const TileDesc t = tiles[work[2 + u / nsplit]];
@@ -593,7 +579,7 @@ k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, c
         fill_tile(smem_f4, pos, r.halo_lo, r.nh, tf);
         // the last piece also takes whatever a tile holds beyond the headroom it was sized with
         const int i_end = (u % nsplit) == nsplit - 1 ? r.hi : min(i_begin + (int)blockDim.x, r.hi);
-        tile_inner_build(t, r, i_begin, i_end, smem_f4, msk, out, ia, ctrl, n_pad);
+        tile_inner_build(t, r, i_begin, i_end, smem_f4, tmp, ia, ctrl, n_pad);
     }
 }
 
@@ -917,16 +903,7 @@ int gather_grid(const tbsma_ctx *c, int mode)
     if (mode != TBSMA_TILES_DIRTY) return c->n_tiles;
     return c->n_tiles < 4 * c->n_sm ? c->n_tiles : 4 * c->n_sm;
 }
-int inner_mask_words(const tbsma_ctx *c) { return (c->kmax_o / 4 + 7) / 8; }
-size_t inner_bytes_per_thread(const tbsma_ctx *c) { return (size_t)c->kmax * 2 + (size_t)inner_mask_words(c) * 4; }
-int inner_threads(const tbsma_ctx *c)
-{
-    int t = (int)((200 * 1024 - gather_smem(c)) / inner_bytes_per_thread(c)) & ~31;
-    if (t > 512) t = 512;
-    if (t < 32) t = 32;
-    return t;
-}
-size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + inner_bytes_per_thread(c) * inner_threads(c); }
+size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + (size_t)kInnerThreads * c->kmax * 2; }
 InnerArgs inner_args(const tbsma_ctx *c)
 {
     InnerArgs ia;
@@ -1087,13 +1064,16 @@ cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st)
 
 cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, cudaStream_t st)
 {
-    const int nt = inner_threads(c);
-    int nsplit = (c->own_cap + nt - 1) / nt;
+    int nsplit = (c->own_cap + kInnerThreads - 1) / kInnerThreads;
     if (nsplit < 1) nsplit = 1;
     const int64_t units = (int64_t)c->n_tiles * nsplit;
-    const int grid = (int)(units < 2 * (int64_t)c->n_sm ? units : 2 * (int64_t)c->n_sm);
-    k_tile_inner<<<grid, nt, inner_smem(c), st>>>(c->d_tiles, c->d_work, c->d_cell_start, pos, inner_args(c), c->d_ctrl,
-                                                  c->n_pad, c->tile_cap, nsplit, inner_mask_words(c));
+    const size_t sm = inner_smem(c);
+    // one CTA per SM: the kernel runs beside the gather passes of the other replicas (second stream) and is latency
+    // bound, so it should leave the shared memory of an SM to them
+    const int64_t cap = c->n_sm;
+    const int grid = (int)(units < cap ? units : cap);
+    k_tile_inner<<<grid, kInnerThreads, sm, st>>>(c->d_tiles, c->d_work, c->d_cell_start, pos, inner_args(c), c->d_ctrl,
+                                                  c->n_pad, c->tile_cap, nsplit);
     c->launches++;
     return cudaGetLastError();
 }
