@@ -167,6 +167,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel-steps", type=int, default=60, help="steps of the per-kernel CUDA-event timing pass")
+    ap.add_argument("--plain-graph", action="store_true",
+                    help="capture the step without the conditional node (Nsight Compute cannot profile kernel nodes "
+                         "of graphs that hold conditional nodes): for the ncu passes under profiles/")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -212,6 +215,8 @@ def main():
 
     w = make_workload(args.config, rank, args.replicas)
     ctx = B.make_context(w)
+    if args.plain_graph:
+        ctx.set_graph(True, conditional=False)
     st = B.DeviceState(w, dev)
     stream = torch.cuda.Stream(device=dev)
     K, Wm = args.steps, args.warmup

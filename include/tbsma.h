@@ -186,15 +186,36 @@ int tbsma_set_outer_skin(tbsma_ctx *ctx, double outer_skin);
  * 32, <= 512, default 256).  Takes effect at the next tbsma_build_cells. */
 int tbsma_set_tile(tbsma_ctx *ctx, int32_t layers_per_tile, int32_t threads);
 
-/* md_run replays one captured step as a CUDA graph when enabled (default 1) and the stream is
- * not the legacy default stream. */
+/* md_run replays one captured step as a CUDA graph when `enable` != 0 (default 2) and the stream is not the legacy
+ * default stream.  enable = 2: in the shared-memory variant the kernels that renew cells and candidates (needed in a
+ * few steps only, decided on the device) are the body of a conditional IF node of that graph, so that nothing is
+ * launched for them otherwise; enable = 1: plain graph, those kernels are launched every step and return at once
+ * when there is nothing to do (Nsight Compute cannot profile the kernel nodes of a graph that holds conditional
+ * nodes, so profiles are taken with 1); 0: no graph.  Results are identical in all three. */
 int tbsma_set_graph(tbsma_ctx *ctx, int32_t enable);
 
-/* Shared-memory variant only: when enabled (default 1) an MD step runs the neighbour rebuild of the replicas that
- * need one, followed by their two gather passes, on a second stream of the context, concurrently with the gather
- * passes of all other replicas on `stream` (replicas never interact); both are joined before the step ends, so the
- * caller sees ordinary stream semantics.  Results are bitwise identical either way. */
+/* Shared-memory variant only.  The list of a replica is renewed in one of two ways: with new cells and candidates
+ * (rare, see tbsma_set_outer_skin), ahead of the gather passes of that step; or re-filtered from its candidates.
+ * When `enable` (default 1, margin 0.03 A) the second kind is asked for as soon as an atom has moved
+ * skin/2 - margin and is written to the second half of the list buffers WHILE the gather passes of the same step
+ * still read the previous list (valid until skin/2), on a second stream of the context when
+ * tbsma_set_overlap is on; the step's last kernel swaps the halves.  margin must exceed the largest distance an
+ * atom moves in one step (0.03 A = 13 sigma_v dt at 298 K, dt = 2 fs); SKIN_VIOLATED is raised if an atom was found
+ * beyond skin/2 with its old list still in use.  Off (or margin 0, or a fixed rebuild cadence): every rebuild
+ * precedes the gather passes.  Membership of the lists is decided by the predicate of D:A6 either way. */
+int tbsma_set_async(tbsma_ctx *ctx, int32_t enable, double margin);
+
+/* Shared-memory variant only: when enabled (default 1) tbsma_md_step / tbsma_md_run use a second stream of the
+ * context for the asynchronous list renewal above; both streams are joined before the step ends, so the caller sees
+ * ordinary stream semantics.  Off: the same kernels run one after the other on `stream`. */
 int tbsma_set_overlap(tbsma_ctx *ctx, int32_t enable);
+
+/* Replicas built together (all of them, by tbsma_build_neighbors) that share a temperature would all need their
+ * next list at nearly the same step, and again one period later.  When enabled (default 1, more than one replica)
+ * replica r rebuilds for the first time as soon as an atom has moved f_r skin/2, f_r = 0.3 + 0.7 frac(0.618 r), and
+ * at skin/2 as usual ever after, which spreads the rebuild load evenly over the steps.  Rebuilding early is always
+ * valid (D:A14): results change only by the fp32 summation order.  Takes effect at the next tbsma_build_neighbors. */
+int tbsma_set_stagger(tbsma_ctx *ctx, int32_t enable);
 
 /* Per-kernel-class timing of tbsma_md_step / tbsma_md_run with CUDA events recorded on the
  * launching stream (graph replay is off while enabled; at most 512 steps are recorded).

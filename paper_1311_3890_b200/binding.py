@@ -20,7 +20,7 @@ EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
-    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_outer_skin",
+    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_async", "tbsma_set_outer_skin",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
 
@@ -77,6 +77,8 @@ def lib():
         L.tbsma_set_tile.argtypes = [vp, i32, i32]
         L.tbsma_set_graph.argtypes = [vp, i32]
         L.tbsma_set_overlap.argtypes = [vp, i32]
+        L.tbsma_set_stagger.argtypes = [vp, i32]
+        L.tbsma_set_async.argtypes = [vp, i32, dbl]
         L.tbsma_set_outer_skin.argtypes = [vp, dbl]
         L.tbsma_set_timing.argtypes = [vp, i32]
         L.tbsma_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
@@ -220,11 +222,17 @@ class Context:
     def set_tile(self, layers_per_tile, threads):
         _check(lib().tbsma_set_tile(self._h, int(layers_per_tile), int(threads)), "tbsma_set_tile")
 
-    def set_graph(self, enable):
-        _check(lib().tbsma_set_graph(self._h, int(bool(enable))), "tbsma_set_graph")
+    def set_graph(self, enable, conditional=True):
+        _check(lib().tbsma_set_graph(self._h, (2 if conditional else 1) if enable else 0), "tbsma_set_graph")
 
     def set_outer_skin(self, outer_skin):
         _check(lib().tbsma_set_outer_skin(self._h, float(outer_skin)), "tbsma_set_outer_skin")
+
+    def set_stagger(self, enable):
+        _check(lib().tbsma_set_stagger(self._h, int(bool(enable))), "tbsma_set_stagger")
+
+    def set_async(self, enable, margin=0.03):
+        _check(lib().tbsma_set_async(self._h, int(bool(enable)), float(margin)), "tbsma_set_async")
 
     def set_overlap(self, enable):
         _check(lib().tbsma_set_overlap(self._h, int(bool(enable))), "tbsma_set_overlap")

@@ -36,7 +36,8 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_geom); cudaFree(c->d_atom_rep); cudaFree(c->d_cell_count); cudaFree(c->d_cell_start);
     cudaFree(c->d_cell_of); cudaFree(c->d_slot); cudaFree(c->d_order); cudaFree(c->d_pos_build);
     cudaFree(c->d_tmp4); cudaFree(c->d_tmp_tag); cudaFree(c->d_nlist); cudaFree(c->d_nn); cudaFree(c->d_xs);
-    cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters);
+    cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters); cudaFree(c->d_stagger); cudaFree(c->d_cur);
+    c->d_stagger = nullptr; c->d_cur = nullptr;
     cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_newslot); cudaFree(c->d_oldof);
     cudaFree(c->d_nn_tmp); cudaFree(c->d_tmp_pos);
     cudaFree(c->d_tile_first); cudaFree(c->d_work);
@@ -165,11 +166,19 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
     a.c2 = (float)sqrt(1.0 - c1 * c1);
     a.sigma_scale = (float)sqrt(TBSMA_KB * TBSMA_ACC / c->prm.mass_amu);
     a.skin_half2 = (float)(0.25 * c->skin * c->skin);
+    a.trigger2 = a.skin_half2;
+    const bool tiles = c->active_variant == 2;
+    const bool async = tiles && c->async_inner && c->list_bufs == 2 && rebuild_every <= 0 &&
+                       0.5 * c->skin > c->async_margin && c->async_margin > 0.0;
+    if (async) a.trigger2 = (float)((0.5 * c->skin - c->async_margin) * (0.5 * c->skin - c->async_margin));
+    a.cur = c->d_cur;
+    a.pb_stride = c->n_pad;
     a.thermostat = gamma > 0.0;
     a.rebuild_every = rebuild_every;
     a.step_base = step0;
     a.T = T; a.seed = seed; a.disp0 = disp0; a.rate = rate;
     a.want_outer = c->active_variant == 2 ? c->d_want_outer : nullptr;
+    a.stagger = c->d_stagger;
     a.e_rep = e_rep; a.w_rep = w_rep; a.ekin = ekin;
     KickArgs kk;
     kk.vel = vel; kk.kick = a.kick; kk.ke_scale = (float)(0.5 * c->prm.mass_amu / TBSMA_ACC); kk.ekin = ekin;
@@ -178,35 +187,70 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         if (c->timing && c->tev && c->tev_steps < TBSMA_TIMING_MAX_STEPS) ev = c->tev + 6 * (c->tev_steps++);
         if (ev) CK(cudaEventRecord(ev[0], st));
         CK(tbsma_launch_integrate_pre(c, pos, vel, force, tag, a, st));
-        if (c->active_variant == 2 && c->overlap && !c->timing && c->aux_stream && c->R > 1) {
-            // fork: the replicas that keep their lists go straight to the two gather passes on `st`; the rebuild
-            // chain of the others, then their gather passes, run on the high-priority second stream
-            cudaStream_t s2 = c->aux_stream;
-            CK(cudaEventRecord(c->ev_fork, st));
-            CK(cudaStreamWaitEvent(s2, c->ev_fork, 0));
-            CK(tbsma_launch_tile_worklist(c, s2));
-            CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, s2));
-            CK(tbsma_launch_tile_inner(c, pos, s2));
-            CK(tbsma_launch_density_tile(c, pos, TBSMA_TILES_DIRTY, s2));
-            CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, TBSMA_TILES_DIRTY, s2));
-            CK(cudaEventRecord(c->ev_join, s2));
-            CK(tbsma_launch_density_tile(c, pos, TBSMA_TILES_CLEAN, st));
-            CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, TBSMA_TILES_CLEAN, st));
-            CK(cudaStreamWaitEvent(st, c->ev_join, 0));
-            CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
-            continue;
-        }
         if (ev) CK(cudaEventRecord(ev[1], st));
-        if (c->active_variant == 2) CK(tbsma_launch_tile_worklist(c, st));
-        CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
-        if (c->active_variant == 2) CK(tbsma_launch_tile_inner(c, pos, st));
+        bool forked = false;
+        if (tiles) {
+            // Replicas whose atoms moved far enough get a new list.  With new cells and candidates (dirty == 2, rare)
+            // the rebuild precedes the gather passes, which then read the freshly written half of the list buffers.
+            // A list that is only re-filtered from its candidates (dirty == 1) is, when `async`, asked for `margin`
+            // early and written to the other half while the gather passes of this step still read the old one, on a
+            // second stream; the step's last kernel swaps the halves.
+            cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+            cudaGraph_t cg = nullptr;
+            const cudaGraphNode_t *deps = nullptr;
+            size_t n_deps = 0;
+            cudaGraphConditionalHandle cond = 0;
+            bool use_cond = false;
+            if (st && c->use_cond && c->body_stream &&
+                cudaStreamGetCaptureInfo(st, &cap, nullptr, &cg, &deps, &n_deps) == cudaSuccess &&
+                cap == cudaStreamCaptureStatusActive && cg)
+                use_cond = cudaGraphConditionalHandleCreate(&cond, cg, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+            CK(tbsma_launch_tile_worklist(c, st, (unsigned long long)cond, use_cond ? 1 : 0));
+            if (async && c->overlap && !c->timing && c->aux_stream) {
+                CK(cudaEventRecord(c->ev_fork, st));
+                CK(cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
+                CK(tbsma_launch_tile_inner(c, pos, 0, c->aux_stream));
+                CK(cudaEventRecord(c->ev_join, c->aux_stream));
+                forked = true;
+            }
+            if (use_cond) {
+                // IF (a replica needs new cells and candidates) { chain; its inner lists }: nothing is launched otherwise
+                CK(cudaStreamGetCaptureInfo(st, &cap, nullptr, &cg, &deps, &n_deps));
+                cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+                np.type = cudaGraphNodeTypeConditional;
+                np.conditional.handle = cond;
+                np.conditional.type = cudaGraphCondTypeIf;
+                np.conditional.size = 1;
+                cudaGraphNode_t cnode;
+                CK(cudaGraphAddNode(&cnode, cg, deps, n_deps, &np));
+                cudaGraph_t body = np.conditional.phGraph_out[0];
+                CK(cudaStreamBeginCaptureToGraph(c->body_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+                const int64_t before = c->launches;
+                cudaError_t e1 = tbsma_launch_rebuild(c, pos, vel, tag, true, true, c->body_stream);
+                cudaError_t e2 = tbsma_launch_tile_inner(c, pos, 1, c->body_stream);
+                c->launches = before;      // kernels of the body are not counted: they run in a few steps only
+                cudaGraph_t body_out = nullptr;
+                CK(cudaStreamEndCapture(c->body_stream, &body_out));
+                CK(e1);
+                CK(e2);
+                CK(cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies));
+            } else {
+                CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
+                CK(tbsma_launch_tile_inner(c, pos, 1, st));
+            }
+            if (!forked) CK(tbsma_launch_tile_inner(c, pos, 0, st));
+        } else {
+            CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
+        }
+        const int sync_level = async ? 2 : 1;
         if (ev) CK(cudaEventRecord(ev[2], st));
-        if (c->active_variant == 2) CK(tbsma_launch_density_tile(c, pos, TBSMA_TILES_ALL, st));
+        if (tiles) CK(tbsma_launch_density_tile(c, pos, sync_level, st));
         else CK(tbsma_launch_density(c, pos, st));
         if (ev) CK(cudaEventRecord(ev[3], st));
-        if (c->active_variant == 2) CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, TBSMA_TILES_ALL, st));
+        if (tiles) CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, sync_level, st));
         else CK(tbsma_launch_force(c, force, e_rep, w_rep, kk, st));
         if (ev) CK(cudaEventRecord(ev[4], st));
+        if (forked) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
         CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
         if (ev) CK(cudaEventRecord(ev[5], st));
     }
@@ -253,6 +297,10 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->tile_threads = 256;
     c->use_graph = 1;
     c->overlap = 1;
+    c->stagger = 1;
+    c->use_cond = 1;
+    c->async_inner = 1;
+    c->async_margin = 0.03;
     {
         int lo_prio = 0, hi_prio = 0;
         cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio);
@@ -264,6 +312,7 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
             free(c);
             return TBSMA_ECUDA;
         }
+        if (cudaStreamCreateWithFlags(&c->body_stream, cudaStreamNonBlocking) != cudaSuccess) c->body_stream = nullptr;
     }
     int sm = 0;
     if (cudaDeviceGetAttribute(&sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sm < 1) sm = 148;
@@ -281,6 +330,7 @@ int tbsma_destroy(tbsma_ctx *c)
     free_staging(c);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
     if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+    if (c->body_stream) cudaStreamDestroy(c->body_stream);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->tev) {
@@ -332,6 +382,24 @@ int tbsma_set_graph(tbsma_ctx *c, int32_t enable)
 {
     if (!c) return TBSMA_EINVAL;
     c->use_graph = enable != 0;
+    c->use_cond = enable != 1;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    return TBSMA_OK;
+}
+
+int tbsma_set_stagger(tbsma_ctx *c, int32_t enable)
+{
+    if (!c) return TBSMA_EINVAL;
+    c->stagger = enable != 0;
+    return TBSMA_OK;
+}
+
+int tbsma_set_async(tbsma_ctx *c, int32_t enable, double margin)
+{
+    if (!c || margin < 0.0) return TBSMA_EINVAL;
+    c->async_inner = enable != 0;
+    c->async_margin = margin;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     return TBSMA_OK;
 }
 
@@ -422,9 +490,12 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     cudaError_t e = cudaSuccess;
 #define DA(ptr, cnt) if (e == cudaSuccess) e = dalloc(&(ptr), (cnt))
     DA(c->d_geom, (size_t)R); DA(c->d_atom_rep, n); DA(c->d_cell_of, n); DA(c->d_slot, n); DA(c->d_order, n);
-    DA(c->d_pos_build, n); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
-    DA(c->d_nlist, (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, n); DA(c->d_xs, n);
-    DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8);
+    c->list_bufs = c->any_periodic ? 1 : 2;   // the tile variant (non-periodic systems only) double-buffers its lists
+    const size_t nb = (size_t)c->list_bufs;
+    DA(c->d_pos_build, nb * c->n_pad); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
+    DA(c->d_nlist, nb * (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, nb * c->n_pad); DA(c->d_xs, n);
+    DA(c->d_cur, (size_t)R);
+    DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8); DA(c->d_stagger, (size_t)R);
     DA(c->d_maxpop, (size_t)R); DA(c->d_hbase, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
     DA(c->d_tmp_pos, n);
 #undef DA
@@ -436,9 +507,11 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     e = cudaMemcpy(c->d_atom_rep, rep, sizeof(int32_t) * n, cudaMemcpyHostToDevice);
     free(rep);
     if (e == cudaSuccess) e = cudaMemset(c->d_dirty, 0, sizeof(int32_t) * R);
+    if (e == cudaSuccess) e = cudaMemset(c->d_stagger, 0, sizeof(float) * R);
     if (e == cudaSuccess) e = cudaMemset(c->d_ctrl, 0, sizeof(int32_t) * 8);
     if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, sizeof(unsigned long long) * 8);
-    if (e == cudaSuccess) e = cudaMemset(c->d_nn, 0, sizeof(int32_t) * (n ? n : 1));
+    if (e == cudaSuccess) e = cudaMemset(c->d_nn, 0, sizeof(int32_t) * nb * (c->n_pad ? c->n_pad : 1));
+    if (e == cudaSuccess) e = cudaMemset(c->d_cur, 0, sizeof(int32_t) * R);
     if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
     c->cell_w = 0.0;
     c->kmax_o = c->kmax;
@@ -477,8 +550,9 @@ int tbsma_build_neighbors(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_t
     CK(tbsma_launch_mark_all_dirty(c, st));
     if (c->active_variant == 2) CK(tbsma_launch_tile_worklist(c, st));
     CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, false, true, st));
-    if (c->active_variant == 2) CK(tbsma_launch_tile_inner(c, (const float4 *)d_pos, st));
+    if (c->active_variant == 2) CK(tbsma_launch_tile_inner(c, (const float4 *)d_pos, 1, st));
     CK(tbsma_launch_finish_step(c, 0, st));
+    CK(tbsma_launch_set_stagger(c, st));
     c->list_built = 1;
     return TBSMA_OK;
 }
@@ -493,8 +567,8 @@ int tbsma_compute(tbsma_ctx *c, const float *d_pos, float *d_force_energy, doubl
     if (c->n == 0) return TBSMA_OK;
     KickArgs kk = {nullptr, 0.f, 0.f, nullptr};
     if (c->active_variant == 2) {
-        CK(tbsma_launch_density_tile(c, (const float4 *)d_pos, TBSMA_TILES_ALL, st));
-        CK(tbsma_launch_force_tile(c, (float4 *)d_force_energy, d_e, d_w, kk, TBSMA_TILES_ALL, st));
+        CK(tbsma_launch_density_tile(c, (const float4 *)d_pos, 1, st));
+        CK(tbsma_launch_force_tile(c, (float4 *)d_force_energy, d_e, d_w, kk, 1, st));
     } else {
         CK(tbsma_launch_density(c, (const float4 *)d_pos, st));
         CK(tbsma_launch_force(c, (float4 *)d_force_energy, d_e, d_w, kk, st));

@@ -81,11 +81,12 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
     }
     pos[i] = p;
     vel[i] = v;
-    const float4 pb = pos_build[i];
+    const float4 pb = pos_build[(size_t)a.cur[r] * a.pb_stride + i];
     const float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
     const float d2 = dx * dx + dy * dy + dz * dz;
     const bool cadence = a.rebuild_every > 0 && (step % (unsigned long long)a.rebuild_every) == 0ull;
-    if (d2 > a.skin_half2 || cadence) {
+    if (d2 > a.skin_half2 && a.trigger2 < a.skin_half2) atomicOr(ctrl + 1, (int)TBSMA_FLAG_SKIN_VIOLATED);
+    if (d2 > a.trigger2 * a.stagger[r] || cadence) {
         // level 2 = cells + candidate list too (tile variant, decided at the replica's previous rebuild)
         const int level = (a.want_outer && a.want_outer[r]) ? 2 : 1;
         dirty[r] = level;
@@ -97,6 +98,7 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
 
 // end of step: statistics, clear the dirty flags, advance the in-run step offset
 __global__ void k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl, int *__restrict__ want_outer,
+                              float *__restrict__ stagger, int *__restrict__ cur, int swap,
                               unsigned long long *__restrict__ counters, int R, int advance, int count_step)
 {
     __shared__ int s_cnt, s_cnt2;
@@ -106,7 +108,7 @@ __global__ void k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl, i
         int mine = 0, mine2 = 0;
         for (int r = threadIdx.x; r < R; r += blockDim.x) {
             const int d = dirty[r];
-            if (d) { ++mine; dirty[r] = 0; }
+            if (d) { ++mine; dirty[r] = 0; stagger[r] = 1.0f; if (swap) cur[r] ^= 1; }
             if (d == 2) ++mine2;
         }
         if (mine) atomicAdd(&s_cnt, mine);
@@ -123,7 +125,30 @@ __global__ void k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl, i
     }
 }
 
+// Replicas that are built together (all of them, at the start of a run) and share a temperature would all ask
+// for their next list at nearly the same step, and again one period later: steps with a hundred rebuilds
+// between steps with none.  Rebuilding early is always valid, so until its first rebuild replica r uses the
+// fraction f_r^2 of (skin/2)^2, f_r = 0.3 + 0.7 frac(r phi): the rebuild phases start out spread evenly.
+__global__ void k_set_stagger(float *__restrict__ stagger, int R, int enable)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    float f = 1.0f;
+    if (enable && R > 1) {
+        const float u = (float)r * 0.6180339887f;
+        f = 0.3f + 0.7f * (u - floorf(u));
+    }
+    stagger[r] = f * f;
+}
+
 }  // namespace
+
+cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st)
+{
+    k_set_stagger<<<(c->R + 255) / 256, 256, 0, st>>>(c->d_stagger, c->R, c->stagger);
+    c->launches++;
+    return cudaGetLastError();
+}
 
 cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, const float4 *force,
                                        const int32_t *tag, const StepArgs &a, cudaStream_t st)
@@ -139,7 +164,7 @@ cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, c
 cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st)
 {
     k_finish_step<<<1, 256, 0, st>>>(c->d_dirty, c->d_ctrl, c->active_variant == 2 ? c->d_want_outer : nullptr,
-                                     c->d_counters, c->R, advance_offset & 1,
+                                     c->d_stagger, c->d_cur, c->list_bufs == 2 && c->active_variant == 2, c->d_counters, c->R, advance_offset & 1,
                                      (advance_offset >> 1) & 1);
     c->launches++;
     return cudaGetLastError();

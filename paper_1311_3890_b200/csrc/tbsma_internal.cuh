@@ -131,6 +131,16 @@ struct tbsma_ctx {
     float4 *d_xs;           // n: (x, y, z, 1/sqrt(rho)) written by the density pass
     // device: control
     int32_t *d_dirty;       // R: replica needs a rebuild
+    // Tile variant: list, counts and build positions exist twice (buffer b at offset b * stride of the same
+    // allocation).  Replica r reads buffer cur[r]; a rebuild writes the other one and the step's last kernel swaps,
+    // so the filter pass of a replica can run beside the gather passes that still use its previous list.
+    int list_bufs;          // 1 or 2
+    int32_t *d_cur;         // R: buffer in use (all 0 when list_bufs == 1)
+    int async_inner;        // enabled (default 1): see tbsma_set_async
+    double async_margin;    // A: the list is renewed once an atom has moved skin/2 - margin
+    float *d_stagger;       // R: factor on (skin/2)^2 until the replica's first rebuild (spreads the rebuilds of
+                            // replicas that start together over the steps); 1 afterwards
+    int stagger;            // enabled (default 1)
     int32_t *d_ctrl;        // [0] any replica dirty, [1] status flags, [2] max neighbours seen, [3] any dirty == 2
     unsigned long long *d_counters; // [0] step offset inside md_run, [1] replica builds, [2] build passes, [3] steps,
                                     // [4..5] count_pairs scratch, [6] replica builds that redid cells + candidates
@@ -154,6 +164,8 @@ struct tbsma_ctx {
     // md step of the tile variant: rebuild chain + rebuilt replicas on a second (high-priority) stream
     int overlap;               // enabled (default 1)
     cudaStream_t aux_stream;
+    cudaStream_t body_stream;  // captures the body of the conditional node of a captured step
+    int use_cond;              // captured steps wrap the cells + candidates chain in an IF node (default 1)
     cudaEvent_t ev_fork, ev_join;
     // optional per-kernel-class timing with CUDA events on the launching stream
     int timing;
@@ -192,19 +204,17 @@ cudaError_t tbsma_launch_count_pairs(tbsma_ctx *c, const float4 *pos, unsigned l
 // shared-memory tile variant (tbsma_tile.cu)
 int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st);   // host: sizes the tiles from the binned cells (synchronises)
 cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t *tag, cudaStream_t st);
-cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st);   // tiles of the dirty replicas, from the flags
-cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, cudaStream_t st);   // inner lists of dirty replicas
+// tiles of the dirty replicas, from the flags; use_cond: also sets the graph conditional `cond` (any replica with dirty == 2)
+cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st, unsigned long long cond = 0ull, int use_cond = 0);
+// inner lists of the replicas on work list `which` (0: dirty == 1, 1: dirty == 2), written to the buffer not in use
+cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, int which, cudaStream_t st);
 cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float4 *vel, const int32_t *tag,
                                     cudaStream_t st);
-// mode: which tiles a gather launch processes.  The md step runs the tiles of the replicas that are NOT being
-// rebuilt on the main stream while the rebuild chain and then the tiles of the rebuilt replicas run on a second
-// stream (replicas never interact, so the two halves are independent).
-#define TBSMA_TILES_ALL 0
-#define TBSMA_TILES_CLEAN 1
-#define TBSMA_TILES_DIRTY 2
-cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int mode, cudaStream_t st);
+// sync_level: the gather passes read the freshly written half of the list buffers for replicas with
+// dirty >= sync_level (their rebuild ran ahead of the launch), the half in use for all others.
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st);
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kick,
-                                    int mode, cudaStream_t st);
+                                    int sync_level, cudaStream_t st);
 cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
                                             cudaStream_t st);
 cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsigned long long *d_out2,
@@ -212,7 +222,10 @@ cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsig
 // integrator (tbsma_integrate.cu)
 struct StepArgs {
     float half_dt, kick, c1, c2, sigma_scale;  // sigma_v = sigma_scale * sqrt(T)
-    float skin_half2;
+    float skin_half2;        // (skin/2)^2: beyond it the list in use is no longer guaranteed
+    float trigger2;          // displacement^2 that asks for a new list (= skin_half2 unless lists are renewed one step late)
+    const int *cur;          // per replica: which half of pos_build belongs to the list in use
+    int pb_stride;           // float4 elements between the two halves of pos_build
     int thermostat;          // gamma > 0
     int rebuild_every;
     unsigned long long step_base;
@@ -221,8 +234,10 @@ struct StepArgs {
     const double *disp0;     // nullable
     const double *rate;      // nullable
     const int *want_outer;   // nullable (tile variant): replicas whose next rebuild redoes cells + candidates
+    const float *stagger;    // per replica factor on skin_half2
     double *e_rep, *w_rep, *ekin;  // zeroed here for the force pass; nullable
 };
 cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, const float4 *force,
                                        const int32_t *tag, const StepArgs &a, cudaStream_t st);
 cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st);
+cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st);

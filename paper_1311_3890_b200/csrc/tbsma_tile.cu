@@ -73,10 +73,11 @@ __global__ void k_layer_maxpop(const RepGeom *__restrict__ geom, const int *__re
 
 // ---- worklists.  Only a few per cent of the replicas rebuild in a given step, so the kernels that
 // work on them loop over a list of their tiles instead of launching one (mostly idle) CTA per tile.
-// work[0] = tiles of replicas with dirty >= 1, work[1] = with dirty == 2, then the two tile lists.
+// work[0] = tiles of replicas with dirty == 1 (new list from the old candidates), work[1] = with dirty == 2
+// (new cells and candidates first), then the two tile lists.
 __global__ void __launch_bounds__(256)
 k_tile_worklist(const int *__restrict__ dirty, const int *__restrict__ tile_first, int *__restrict__ work, int R,
-                int n_tiles)
+                int n_tiles, cudaGraphConditionalHandle cond, int use_cond)
 {
     __shared__ int s_base[2], s_warp[2][8];
     if (threadIdx.x < 2) s_base[threadIdx.x] = 0;
@@ -86,7 +87,7 @@ k_tile_worklist(const int *__restrict__ dirty, const int *__restrict__ tile_firs
         const int r = r0 + threadIdx.x;
         const int d = r < R ? dirty[r] : 0;
         const int f = r < R ? tile_first[r] : 0, nt = r < R ? tile_first[r + 1] - f : 0;
-        int v[2] = {d >= 1 ? nt : 0, d == 2 ? nt : 0}, incl[2];
+        int v[2] = {d == 1 ? nt : 0, d == 2 ? nt : 0}, incl[2];
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
             int x = v[k];
@@ -115,6 +116,8 @@ k_tile_worklist(const int *__restrict__ dirty, const int *__restrict__ tile_firs
         __syncthreads();
     }
     if (threadIdx.x < 2) work[threadIdx.x] = s_base[threadIdx.x];
+    // inside a captured step the cells + candidates chain is the body of an IF node: skipped unless a replica needs it
+    if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, s_base[1] > 0 ? 1u : 0u);
 }
 
 // ---- K1: scan.  Cell-ordered positions of the tile + halo in shared memory; every own atom scans
@@ -233,8 +236,10 @@ __device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { retur
 // ---- K2: finish.  One thread per FINAL slot of the tile: reads the temporary row of the atom that
 // moves there, translates every partner to its final position (byte offset of its record in the
 // tile's shared-memory image, record k at (k + 1) * 16, the sentinel at 0), and writes the row sorted
-// by CLASS (bank group of the record = record index mod 8; stable inside a class): the inner build
-// keeps this order when it filters, so its kept entries come out grouped by class as well.
+// by CLASS (bank group of the record = record index mod 8; stable inside a class), starting with the
+// class equal to the atom's lane mod 8: the inner build keeps this order when it filters, so its kept
+// entries come out grouped by class as well, and while it gathers the candidates the eight lanes served by
+// one shared-memory wavefront are (mostly) on eight different classes instead of all on class 0.
 struct FinishArgs {
     const int *cell_start;
     const uint2 *nl_tmp;
@@ -267,14 +272,15 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs 
         const int cnt = nnv & 0xffff;
         const uint2 *src = nl_tmp + a;
         const int ng = (cnt + 3) >> 2;
-        // pass A: population of the 8 classes (packed bytes; kmax <= 248)
+        const unsigned lane = (unsigned)(ip - r.lo) & 31u;     // the lane the inner build and the gather passes give this atom
+        // pass A: population of the 8 classes, counted from the lane's own (packed bytes; kmax <= 248)
         unsigned long long pop = 0ull;
         for (int g = 0; g < ng; ++g) {
             const uint2 w = src[(size_t)g * n_pad];
             const unsigned e[4] = {w.x & 0xffffu, w.x >> 16, w.y & 0xffffu, w.y >> 16};
 #pragma unroll
             for (int q = 0; q < 4; ++q)
-                if (4 * g + q < cnt) pop += 1ull << (((map[e[q]] >> 4) & 7) << 3);
+                if (4 * g + q < cnt) pop += 1ull << ((((map[e[q]] >> 4) - lane) & 7) << 3);
         }
         unsigned long long off = 0ull;
         {
@@ -291,7 +297,7 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs 
             for (int q = 0; q < 4; ++q)
                 if (4 * g + q < cnt) {
                     const unsigned m = map[e[q]];
-                    const int c = (m >> 4) & 7;
+                    const int c = ((m >> 4) - lane) & 7;
                     const unsigned idx = byte_of(off, c) + byte_of(cur, c);
                     cur += 1ull << (c << 3);
                     scr[idx * nthr + tid] = (unsigned short)m;
@@ -406,14 +412,68 @@ __device__ __forceinline__ float4 lds_rec(const float4 *sm, unsigned byte_off)
     return *reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(sm) + byte_off);
 }
 
-__device__ __forceinline__ float rho_term_t(const float4 &pi, const float4 &pj, const PairConst &pc)
+// ---- packed fp32 arithmetic.  sm_100 has two-wide fp32 instructions (FADD2 / FMUL2 / FFMA2 on a pair of
+// registers): the same flops per cycle as the scalar forms but half the issue slots, and both gather passes
+// are bound by issue slots and the MUFU pipe, not by flops.  Two neighbours are evaluated side by side;
+// every component sees exactly the operations of the scalar form (same roundings, D:A6 included).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk(float lo, float hi)
 {
-    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6 order
-    const float rinv = rsqrt_approx(d2);
-    const float t = __fmaf_rn(d2, rinv, -pc.r0f);                                // r - r0
-    const float e = ex2_approx(__fmaf_rn(pc.aq, t, pc.b_rho));                   // xi^2 e^{-2q x}
-    return d2 < pc.rc2 ? e : 0.f;
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpk(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+#define TBSMA_T_OUT 1.0e6f   // r - r0 of a pair outside the cutoff: every exponential of the pair becomes exactly 0
+
+// d2 (D:A6 order), 1/r and t = r - r0 of two neighbours; t = TBSMA_T_OUT outside the cutoff
+struct Pair2 {
+    f32x2 dx, dy, dz, rinv, t;
+};
+__device__ __forceinline__ Pair2 pair2(const float4 &pi, const float4 &pa, const float4 &pb, const PairConst &pc)
+{
+    Pair2 P;
+    P.dx = pk(pi.x - pa.x, pi.x - pb.x);
+    P.dy = pk(pi.y - pa.y, pi.y - pb.y);
+    P.dz = pk(pi.z - pa.z, pi.z - pb.z);
+    const f32x2 d2 = fma2(P.dz, P.dz, fma2(P.dy, P.dy, mul2(P.dx, P.dx)));
+    float d2a, d2b;
+    unpk(d2, d2a, d2b);
+    P.rinv = pk(rsqrt_approx(d2a), rsqrt_approx(d2b));
+    const f32x2 t = fma2(d2, P.rinv, pk(-pc.r0f, -pc.r0f));      // r - r0
+    float ta, tb;
+    unpk(t, ta, tb);
+    P.t = pk(d2a < pc.rc2 ? ta : TBSMA_T_OUT, d2b < pc.rc2 ? tb : TBSMA_T_OUT);
+    return P;
+}
+
+// xi^2 e^{-2q x} of two neighbours added to the two running sums in rho2
+__device__ __forceinline__ f32x2 rho_term2(const float4 &pi, const float4 &pa, const float4 &pb, const PairConst &pc,
+                                           f32x2 rho2)
+{
+    const Pair2 P = pair2(pi, pa, pb, pc);
+    const f32x2 arg = fma2(pk(pc.aq, pc.aq), P.t, pk(pc.b_rho, pc.b_rho));
+    float a0, a1;
+    unpk(arg, a0, a1);
+    return add2(rho2, pk(ex2_approx(a0), ex2_approx(a1)));
 }
 
 
@@ -435,9 +495,12 @@ __device__ __forceinline__ float rho_term_t(const float4 &pi, const float4 &pj, 
 struct InnerArgs {
     const uint2 *olist;      // candidates (class-sorted rows)
     const int *nn_o;
-    uint2 *nl;               // out: inner list
-    int *nn;                 // out: count | flag << 16
-    float4 *pos_build;       // out
+    uint2 *nl;               // out: inner list            } both halves; the half NOT in use by the replica
+    int *nn;                 // out: count | flag << 16    } is written (the last kernel of the step swaps)
+    float4 *pos_build;       // out                        }
+    const int *cur;          // per replica: half in use
+    size_t nl_stride;        // uint2 elements between the halves of nl
+    int n_stride;            // elements between the halves of nn and pos_build
     const float4 *pos_outer;
     int *want_outer;         // per replica
     int kmax;                // inner capacity
@@ -446,15 +509,7 @@ struct InnerArgs {
 
 constexpr int kInnerThreads = 256;   // one atom per thread, kmax u16 of shared-memory scratch each
 
-__device__ __forceinline__ unsigned long long rotr64_bytes(unsigned long long v, int nbytes)
-{
-    const int s = (nbytes & 7) << 3;
-    return s ? (v >> s) | (v << (64 - s)) : v;
-}
-
-// tmp: element k of thread t at [((k >> 1) * nthr + t) * 2 + (k & 1)]: a thread's entries stay in one bank,
-// so the lanes of a warp never conflict, whatever k each of them is at
-#define TMP_AT(k) ((((k) >> 1) * nthr + tid) * 2 + ((k) & 1))
+// tmp: element k of thread t at [k * nthr + t], kmax + 1 rows (row kmax takes what does not fit)
 __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRange &r, int i_begin, int i_end,
                                                  const float4 *sm, unsigned short *tmp, const InnerArgs &ia,
                                                  int *__restrict__ ctrl, int n_pad)
@@ -463,13 +518,19 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     int maxc = 0;
     bool want = false, viol = false, over = false;
+    const int ob = ia.cur[t.rep] ^ 1;                  // the half to write
+    uint2 *nl_out = ia.nl + (size_t)ob * ia.nl_stride;
+    int *nn_out = ia.nn + (size_t)ob * ia.n_stride;
+    float4 *pb_out = ia.pos_build + (size_t)ob * ia.n_stride;
+    unsigned short *col = tmp + tid;
     for (int i = i_begin + tid; i < i_end; i += nthr) {
         const float4 pi = sm[i - r.halo_lo + 1];
         const int nno = ia.nn_o[i];
         const int ng = ((nno & 0xffff) + 3) >> 2;
         const uint2 *row = ia.olist + i;
-        // pass 1: the candidates that pass the fp32 predicate of D:A6, in candidate order
-        int m = 0, seen = 0;
+        // pass 1: the candidates that pass the fp32 predicate of D:A6, in candidate order.  Branch-free: every
+        // candidate is stored at the current end of the column, the end advances for the members only.
+        int m = 0;
         auto group = [&](const uint2 jj) {
             const unsigned e[4] = {jj.x & 0xffffu, jj.x >> 16, jj.y & 0xffffu, jj.y >> 16};
             float d2[4];
@@ -480,11 +541,10 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
                 d2[q] = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
-                if (d2[q] < ia.rl2) {          // padding entries point at the sentinel and fail
-                    if (m < ia.kmax) { tmp[TMP_AT(m)] = (unsigned short)e[q]; ++m; }
-                    ++seen;
-                }
+            for (int q = 0; q < 4; ++q) {
+                col[min(m, ia.kmax) * nthr] = (unsigned short)e[q];
+                m += d2[q] < ia.rl2 ? 1 : 0;       // padding entries point at the sentinel and fail
+            }
         };
         {
             auto ld = [&](int g) { return g < ng ? __ldcs(row + (size_t)g * n_pad) : make_uint2(0u, 0u); };
@@ -500,48 +560,50 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
             if (g + 1 < ng) group(q1);
             if (g + 2 < ng) group(q2);
         }
-        over = over || seen > ia.kmax;
-        maxc = max(maxc, seen);
-        // entries per class and first entry of each class (packed bytes), rotated so that byte s is class lane + s
+        over = over || m > ia.kmax;
+        maxc = max(maxc, m);
+        m = min(m, ia.kmax);
+        // entries per class, byte s = class lane + s (the order the classes are stored in), and where each run starts
         unsigned long long npk = 0ull;
-        for (int k = 0; k < m; ++k) npk += 1ull << (((tmp[TMP_AT(k)] >> 4) & 7u) << 3);
-        unsigned long long opk = 0ull;
-        int nmax = 0;
+        for (int k = 0; k < m; ++k) npk += 1ull << ((((col[k * nthr] >> 4) - (unsigned)lane) & 7u) << 3);
+        unsigned long long orot = 0ull;
+        int n_s[8];
         {
             unsigned run = 0;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const unsigned n_c = byte_of(npk, c);
-                opk |= (unsigned long long)run << (c << 3);
-                run += n_c;
-                nmax = max(nmax, (int)n_c);
+            for (int sft = 0; sft < 8; ++sft) {
+                n_s[sft] = (int)byte_of(npk, sft);
+                orot |= (unsigned long long)run << (sft << 3);
+                run += (unsigned)n_s[sft];
             }
         }
-        const unsigned long long nrot = rotr64_bytes(npk, lane), orot = rotr64_bytes(opk, lane);
-        int n_s[8], o_s[8];
+        // pass 2: round j takes the j-th entry of the classes lane, lane + 1, ... that still have one.  One loop
+        // iteration per list entry (the lanes of a warp have lists of nearly equal length): the classes of round j
+        // are the set bits of `act`.
+        uint2 *dst = nl_out + i;
+        unsigned long long w = 0ull;
+        int j = 0;
+        unsigned act = 0u;
 #pragma unroll
-        for (int sft = 0; sft < 8; ++sft) { n_s[sft] = (int)byte_of(nrot, sft); o_s[sft] = (int)byte_of(orot, sft); }
-        // pass 2: round j takes the j-th entry of classes lane, lane + 1, ... that still have one
-        uint2 *dst = ia.nl + i;
-        unsigned w0 = 0u, w1 = 0u;
-        int p = 0;
-        for (int j = 0; j < nmax; ++j) {
+        for (int sft = 0; sft < 8; ++sft) act |= (n_s[sft] > 0 ? 1u : 0u) << sft;
+        for (int p = 0; p < m; ++p) {
+            const int sft = __ffs((int)act) - 1;
+            act &= act - 1u;
+            const int k = (int)((unsigned)(orot >> (sft << 3)) & 0xffu) + j;
+            w |= (unsigned long long)col[k * nthr] << ((p & 3) << 4);
+            if ((p & 3) == 3) {
+                dst[(size_t)(p >> 2) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));
+                w = 0ull;
+            }
+            if (act == 0u) {       // next round
+                ++j;
 #pragma unroll
-            for (int sft = 0; sft < 8; ++sft)
-                if (j < n_s[sft]) {
-                    const int k = o_s[sft] + j;
-                    const unsigned v = (unsigned)tmp[TMP_AT(k)] << ((p & 1) << 4);
-                    if (p & 2) w1 |= v; else w0 |= v;
-                    if ((p & 3) == 3) {
-                        dst[(size_t)(p >> 2) * n_pad] = make_uint2(w0, w1);
-                        w0 = w1 = 0u;
-                    }
-                    ++p;
-                }
+                for (int s2 = 0; s2 < 8; ++s2) act |= (n_s[s2] > j ? 1u : 0u) << s2;
+            }
         }
-        if (p & 3) dst[(size_t)(p >> 2) * n_pad] = make_uint2(w0, w1);      // unused entries = 0 = the sentinel
-        ia.nn[i] = m | (nno & 0x7fff0000);
-        ia.pos_build[i] = pi;
+        if (m & 3) dst[(size_t)(m >> 2) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));   // unused = 0 = sentinel
+        nn_out[i] = m | (nno & 0x7fff0000);
+        pb_out[i] = pi;
         const float4 po = ia.pos_outer[i];
         const float ox = pi.x - po.x, oy = pi.y - po.y, oz = pi.z - po.z;
         const float o2 = ox * ox + oy * oy + oz * oz;
@@ -555,19 +617,21 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
     if (over) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
 }
 
-// inner build of the dirty replicas: work list 0, every tile cut into pieces of blockDim.x own atoms
+// inner build of the replicas on work list `which`, every tile cut into pieces of blockDim.x own atoms
 __global__ void __launch_bounds__(kInnerThreads)
 k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, const int *__restrict__ cell_start,
-             const float4 *__restrict__ pos, InnerArgs ia, int *__restrict__ ctrl, int n_pad, int s_cap, int nsplit)
+             const float4 *__restrict__ pos, InnerArgs ia, int *__restrict__ ctrl, int n_pad, int s_cap, int nsplit,
+             int which, int n_tiles)
 {
     extern __shared__ float4 smem_f4[];
     __shared__ unsigned long long s_bar;
-    const int nu = work[0] * nsplit;
+    const int *__restrict__ wl = work + 2 + which * n_tiles;
+    const int nu = work[which] * nsplit;
     if ((int)blockIdx.x >= nu) return;
     unsigned short *tmp = reinterpret_cast<unsigned short *>(smem_f4 + s_cap + 1);
     TileFill tf = tile_fill_init(&s_bar);
     for (int u = blockIdx.x; u < nu; u += gridDim.x) {
-        const TileDesc t = tiles[work[2 + u / nsplit]];
+        const TileDesc t = tiles[wl[u / nsplit]];
         const TileRange r = tile_range(t, cell_start);
         const int i_begin = r.lo + (u % nsplit) * blockDim.x;
         if (i_begin >= r.hi) continue;
@@ -625,14 +689,12 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
         const float4 pi = sm[i - r.halo_lo + 1];
         const int ng = ((nn[i] & 0xffff) + 3) >> 2;
         const uint2 *row = nl + i;
-        float rho0 = 0.f, rho1 = 0.f;
+        f32x2 rho2 = pk(0.f, 0.f);
         auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
             const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
-            rho0 += rho_term_t(pi, p0, pc);
-            rho1 += rho_term_t(pi, p1, pc);
-            rho0 += rho_term_t(pi, p2, pc);
-            rho1 += rho_term_t(pi, p3, pc);
+            rho2 = rho_term2(pi, p0, p1, pc, rho2);
+            rho2 = rho_term2(pi, p2, p3, pc, rho2);
         };
         // three rows in flight, rotated by unrolling (a register move would wait for the newest load)
         uint2 q0 = ld_row(row, 0, ng, n_pad), q1 = ld_row(row, 1, ng, n_pad), q2 = ld_row(row, 2, ng, n_pad);
@@ -646,62 +708,80 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
             group(q0);
             if (g + 1 < ng) group(q1);
         }
+        float rho0, rho1;
+        unpk(rho2, rho0, rho1);
         const float rho = rho0 + rho1;
         const float s = rho > 0.f ? 1.0f / sqrtf(rho) : 0.f;     // once per atom, IEEE (D:A5 for rho = 0)
         xs[i] = make_float4(pi.x, pi.y, pi.z, s);
     }
 }
 
-// mode ALL / CLEAN: one CTA per tile (CLEAN skips the replicas being rebuilt); mode DIRTY: the CTAs loop over
-// work list 0.  nn and nl are read-only here: they were written by an earlier kernel.
+// Which half of the list buffers a tile reads: the one its replica has in use, or, when the replica's list has
+// just been rebuilt ahead of this launch (dirty >= sync_level), the other one (the step's last kernel swaps).
+struct ListSel {
+    const int *cur, *dirty;
+    int sync_level;          // 1: every rebuild of this step precedes the gather passes; 2: only those with new candidates
+    size_t nl_stride;
+    int n_stride;
+};
+__device__ __forceinline__ int list_half(const ListSel &ls, int rep)
+{
+    return ls.cur[rep] ^ (ls.dirty[rep] >= ls.sync_level ? 1 : 0);
+}
+
+// one CTA per tile.  nn and nl are read-only here: they were written by an earlier kernel (or, the half not read,
+// are being written by the filter pass running beside this launch).
 __global__ void __launch_bounds__(512, 2)
 k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
                const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
-               float4 *__restrict__ xs, int *__restrict__ ctrl, const int *__restrict__ dirty,
-               const int *__restrict__ work, int mode, int n_pad, int s_cap, PairConst pc)
+               float4 *__restrict__ xs, int *__restrict__ ctrl, ListSel ls, int n_pad, int s_cap, PairConst pc)
 {
     __shared__ unsigned long long s_bar;
-    if (mode == TBSMA_TILES_DIRTY) {
-        const int nw = work[0];
-        if ((int)blockIdx.x >= nw) return;
-        TileFill tf = tile_fill_init(&s_bar);
-        for (int w = blockIdx.x; w < nw; w += gridDim.x) {
-            __syncthreads();
-            density_tile(tiles[work[2 + w]], cell_start, pos, nl, nn, xs, ctrl, n_pad, s_cap, pc, tf);
-        }
-        return;
-    }
     const TileDesc t = tiles[blockIdx.x];
-    if (mode == TBSMA_TILES_CLEAN && dirty[t.rep]) return;
+    const int h = list_half(ls, t.rep);
     TileFill tf = tile_fill_init(&s_bar);
-    density_tile(t, cell_start, pos, nl, nn, xs, ctrl, n_pad, s_cap, pc, tf);
+    density_tile(t, cell_start, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad, s_cap,
+                 pc, tf);
 }
 
+// running sums of stage 2, two lanes each (even / odd neighbours), added up once per atom
 struct AccT {
-    float fx, fy, fz, er;
-    float wxx, wyy, wzz, wxy, wxz, wyz;
+    f32x2 fx, fy, fz, er;
+    f32x2 wxx, wyy, wzz, wxy, wxz, wyz;
 };
 
+// Two neighbours of atom i (pi.w = s_i, pa.w / pb.w = s_j):
+//   F_i += [ (2Ap/r0) e^{-p x} - (q xi^2/r0) e^{-2q x} (s_i + s_j) ] d_ij / r_ij   (derivative of Eq.1-3)
+// and the repulsive sum of Eq.2.  Outside the cutoff t = TBSMA_T_OUT makes both exponentials exactly 0.
 template <bool VIRIAL>
-__device__ __forceinline__ void force_term_t(const float4 &pi, const float4 &pj, const PairConst &pc, AccT &a)
+__device__ __forceinline__ void force_term2(const float4 &pi, const float4 &pa, const float4 &pb, const PairConst &pc,
+                                            AccT &a)
 {
-    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-    const bool in = d2 < pc.rc2;
-    const float rinv = rsqrt_approx(d2);
-    const float t = __fmaf_rn(d2, rinv, -pc.r0f);
-    float er = ex2_approx(__fmaf_rn(pc.ap, t, pc.b_rep));          // (2Ap/r0) e^{-p x}
-    const float eb = ex2_approx(__fmaf_rn(pc.aq, t, pc.b_band));   // (q xi^2/r0) e^{-2q x}
-    float fp = (er - eb * (pi.w + pj.w)) * rinv;                   // -dE/dr / r
-    fp = in ? fp : 0.f;
-    er = in ? er : 0.f;
-    a.fx = __fmaf_rn(fp, dx, a.fx); a.fy = __fmaf_rn(fp, dy, a.fy); a.fz = __fmaf_rn(fp, dz, a.fz);
-    a.er += er;
+    const Pair2 P = pair2(pi, pa, pb, pc);
+    const f32x2 ar = fma2(pk(pc.ap, pc.ap), P.t, pk(pc.b_rep, pc.b_rep));
+    const f32x2 ab = fma2(pk(pc.aq, pc.aq), P.t, pk(pc.b_band, pc.b_band));
+    float ar0, ar1, ab0, ab1;
+    unpk(ar, ar0, ar1);
+    unpk(ab, ab0, ab1);
+    const f32x2 er = pk(ex2_approx(ar0), ex2_approx(ar1));          // (2Ap/r0) e^{-p x}
+    const f32x2 eb = pk(ex2_approx(ab0), ex2_approx(ab1));          // (q xi^2/r0) e^{-2q x}
+    const f32x2 nss = pk(-pi.w - pa.w, -pi.w - pb.w);               // -(s_i + s_j)
+    const f32x2 fp = mul2(fma2(eb, nss, er), P.rinv);               // -dE/dr / r
+    a.fx = fma2(fp, P.dx, a.fx);
+    a.fy = fma2(fp, P.dy, a.fy);
+    a.fz = fma2(fp, P.dz, a.fz);
+    a.er = add2(a.er, er);
     if (VIRIAL) {
-        const float fx = __fmul_rn(fp, dx), fy = __fmul_rn(fp, dy), fz = __fmul_rn(fp, dz);
-        a.wxx = __fmaf_rn(dx, fx, a.wxx); a.wyy = __fmaf_rn(dy, fy, a.wyy); a.wzz = __fmaf_rn(dz, fz, a.wzz);
-        a.wxy = __fmaf_rn(dx, fy, a.wxy); a.wxz = __fmaf_rn(dx, fz, a.wxz); a.wyz = __fmaf_rn(dy, fz, a.wyz);
+        const f32x2 fx = mul2(fp, P.dx), fy = mul2(fp, P.dy), fz = mul2(fp, P.dz);
+        a.wxx = fma2(P.dx, fx, a.wxx); a.wyy = fma2(P.dy, fy, a.wyy); a.wzz = fma2(P.dz, fz, a.wzz);
+        a.wxy = fma2(P.dx, fy, a.wxy); a.wxz = fma2(P.dx, fz, a.wxz); a.wyz = fma2(P.dy, fz, a.wyz);
     }
+}
+__device__ __forceinline__ float sum2(f32x2 v)
+{
+    float lo, hi;
+    unpk(v, lo, hi);
+    return lo + hi;
 }
 
 __device__ __forceinline__ double warp_sum_d(double v)
@@ -757,14 +837,13 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
         const int nni = nn[i];
         const int ng = ((nni & 0xffff) + 3) >> 2;
         const uint2 *row = nl + i;
-        AccT a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        const f32x2 z2 = pk(0.f, 0.f);
+        AccT a = {z2, z2, z2, z2, z2, z2, z2, z2, z2, z2};
         auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
             const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
-            force_term_t<VIRIAL>(pi, p0, pc, a);
-            force_term_t<VIRIAL>(pi, p1, pc, a);
-            force_term_t<VIRIAL>(pi, p2, pc, a);
-            force_term_t<VIRIAL>(pi, p3, pc, a);
+            force_term2<VIRIAL>(pi, p0, p1, pc, a);
+            force_term2<VIRIAL>(pi, p2, p3, pc, a);
         };
         uint2 q0 = ld_row(row, 0, ng, n_pad), q1 = ld_row(row, 1, ng, n_pad), q2 = ld_row(row, 2, ng, n_pad);
         int g = 0;
@@ -777,22 +856,23 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
             group(q0);
             if (g + 1 < ng) group(q1);
         }
+        const float fx = sum2(a.fx), fy = sum2(a.fy), fz = sum2(a.fz);
         const float sqrt_rho = pi.w > 0.f ? 1.0f / pi.w : 0.f;
-        const float ei = __fmaf_rn(a.er, pc.e_rep_scale, -sqrt_rho);   // Eq.1-3: E_R^i + E_B^i
-        force[i] = make_float4(a.fx, a.fy, a.fz, ei);
-        bad = bad || !isfinite(a.fx + a.fy + a.fz + ei);
+        const float ei = __fmaf_rn(sum2(a.er), pc.e_rep_scale, -sqrt_rho);   // Eq.1-3: E_R^i + E_B^i
+        force[i] = make_float4(fx, fy, fz, ei);
+        bad = bad || !isfinite(fx + fy + fz + ei);
         se += (double)ei;
         if (KICK && (nni >> 16) == 0) {       // final B of the step, dynamic atoms only
             float4 v = kk.vel[i];
-            v.x = __fmaf_rn(kk.kick, a.fx, v.x);
-            v.y = __fmaf_rn(kk.kick, a.fy, v.y);
-            v.z = __fmaf_rn(kk.kick, a.fz, v.z);
+            v.x = __fmaf_rn(kk.kick, fx, v.x);
+            v.y = __fmaf_rn(kk.kick, fy, v.y);
+            v.z = __fmaf_rn(kk.kick, fz, v.z);
             kk.vel[i] = v;
             sk += (double)(kk.ke_scale * (v.x * v.x + v.y * v.y + v.z * v.z));
         }
         if (VIRIAL) {
-            sw[0] += 0.5 * (double)a.wxx; sw[1] += 0.5 * (double)a.wyy; sw[2] += 0.5 * (double)a.wzz;
-            sw[3] += 0.5 * (double)a.wxy; sw[4] += 0.5 * (double)a.wxz; sw[5] += 0.5 * (double)a.wyz;
+            sw[0] += 0.5 * (double)sum2(a.wxx); sw[1] += 0.5 * (double)sum2(a.wyy); sw[2] += 0.5 * (double)sum2(a.wzz);
+            sw[3] += 0.5 * (double)sum2(a.wxy); sw[4] += 0.5 * (double)sum2(a.wxz); sw[5] += 0.5 * (double)sum2(a.wyz);
         }
     }
     if (bad) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NONFINITE);
@@ -809,25 +889,14 @@ __global__ void __launch_bounds__(512, 2)
 k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
              const float4 *__restrict__ xs, const uint2 *__restrict__ nl, const int *__restrict__ nn,
              float4 *__restrict__ force, double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk,
-             int *__restrict__ ctrl, const int *__restrict__ dirty, const int *__restrict__ work, int mode,
-             int n_pad, int s_cap, PairConst pc)
+             int *__restrict__ ctrl, ListSel ls, int n_pad, int s_cap, PairConst pc)
 {
     __shared__ unsigned long long s_bar;
-    if (mode == TBSMA_TILES_DIRTY) {
-        const int nw = work[0];
-        if ((int)blockIdx.x >= nw) return;
-        TileFill tf = tile_fill_init(&s_bar);
-        for (int w = blockIdx.x; w < nw; w += gridDim.x) {
-            __syncthreads();
-            force_tile<VIRIAL, KICK>(tiles[work[2 + w]], cell_start, xs, nl, nn, force, e_rep, w_rep, kk, ctrl, n_pad,
-                                     s_cap, pc, tf);
-        }
-        return;
-    }
     const TileDesc t = tiles[blockIdx.x];
-    if (mode == TBSMA_TILES_CLEAN && dirty[t.rep]) return;
+    const int h = list_half(ls, t.rep);
     TileFill tf = tile_fill_init(&s_bar);
-    force_tile<VIRIAL, KICK>(t, cell_start, xs, nl, nn, force, e_rep, w_rep, kk, ctrl, n_pad, s_cap, pc, tf);
+    force_tile<VIRIAL, KICK>(t, cell_start, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force, e_rep,
+                             w_rep, kk, ctrl, n_pad, s_cap, pc, tf);
 }
 
 // ---- inspection (parity tests, bench statistics) ----------------------------------------------
@@ -838,11 +907,15 @@ __device__ __forceinline__ unsigned entry_of(const uint2 *__restrict__ nl, int n
     return (k & 1) ? (h >> 16) : (h & 0xffffu);
 }
 
-__global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *__restrict__ nl,
-                                     const int *__restrict__ nn, const int *__restrict__ hbase,
+__global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *__restrict__ nl0,
+                                     const int *__restrict__ nn0, const int *__restrict__ hbase,
+                                     const int *__restrict__ atom_rep, const int *__restrict__ cur, size_t nl_stride,
                                      int *__restrict__ counts, int *__restrict__ list, int n, int n_pad, int kmax)
 {
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int h = cur[atom_rep[i]];
+        const uint2 *nl = nl0 + (size_t)h * nl_stride;
+        const int *nn = nn0 + (size_t)h * n_pad;
         const int t = tag[i];
         const int cnt = nn[i] & 0xffff;
         counts[t] = cnt;
@@ -851,12 +924,16 @@ __global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *_
     }
 }
 
-__global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *__restrict__ nl,
-                                   const int *__restrict__ nn, const int *__restrict__ hbase,
+__global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *__restrict__ nl0,
+                                   const int *__restrict__ nn0, const int *__restrict__ hbase,
+                                   const int *__restrict__ atom_rep, const int *__restrict__ cur, size_t nl_stride,
                                    unsigned long long *__restrict__ out, int n, int n_pad, float rc2)
 {
     unsigned long long entries = 0, inside = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const int h = cur[atom_rep[i]];
+        const uint2 *nl = nl0 + (size_t)h * nl_stride;
+        const int *nn = nn0 + (size_t)h * n_pad;
         const float4 pi = pos[i];
         const int cnt = nn[i] & 0xffff;
         entries += cnt;
@@ -897,13 +974,7 @@ size_t finish_smem(const tbsma_ctx *c)
     return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax_o * finish_threads(c) * 2;
 }
 size_t gather_smem(const tbsma_ctx *c) { return (size_t)(c->tile_cap + 1) * 16; }
-// grid of a gather launch: one CTA per tile, or (mode DIRTY) enough CTAs to loop over the work list
-int gather_grid(const tbsma_ctx *c, int mode)
-{
-    if (mode != TBSMA_TILES_DIRTY) return c->n_tiles;
-    return c->n_tiles < 4 * c->n_sm ? c->n_tiles : 4 * c->n_sm;
-}
-size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + (size_t)kInnerThreads * c->kmax * 2; }
+size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + (size_t)kInnerThreads * (c->kmax + 1) * 2; }
 InnerArgs inner_args(const tbsma_ctx *c)
 {
     InnerArgs ia;
@@ -912,6 +983,9 @@ InnerArgs inner_args(const tbsma_ctx *c)
     ia.nl = reinterpret_cast<uint2 *>(c->d_nlist);
     ia.nn = c->d_nn;
     ia.pos_build = c->d_pos_build;
+    ia.cur = c->d_cur;
+    ia.nl_stride = (size_t)(c->kmax / 4) * c->n_pad;
+    ia.n_stride = c->n_pad;
     ia.pos_outer = c->d_pos_outer;
     ia.want_outer = c->d_want_outer;
     ia.kmax = c->kmax;
@@ -1055,25 +1129,29 @@ cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int3
     return cudaGetLastError();
 }
 
-cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st)
+cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st, unsigned long long cond, int use_cond)
 {
-    k_tile_worklist<<<1, 256, 0, st>>>(c->d_dirty, c->d_tile_first, c->d_work, c->R, c->n_tiles);
+    k_tile_worklist<<<1, 256, 0, st>>>(c->d_dirty, c->d_tile_first, c->d_work, c->R, c->n_tiles,
+                                       (cudaGraphConditionalHandle)cond, use_cond);
     c->launches++;
     return cudaGetLastError();
 }
 
-cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, cudaStream_t st)
+cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, int which, cudaStream_t st)
 {
     int nsplit = (c->own_cap + kInnerThreads - 1) / kInnerThreads;
     if (nsplit < 1) nsplit = 1;
     const int64_t units = (int64_t)c->n_tiles * nsplit;
     const size_t sm = inner_smem(c);
-    // one CTA per SM: the kernel runs beside the gather passes of the other replicas (second stream) and is latency
-    // bound, so it should leave the shared memory of an SM to them
-    const int64_t cap = c->n_sm;
+    // list 0 is worked on beside the gather passes of the step (second stream): two CTAs per SM leave most of the
+    // shared memory and registers to them; list 1 (and the first build of everything) runs alone
+    int per_sm = which == 0 ? 2 : (int)((200 * 1024) / (sm + 1024));
+    if (per_sm > 4) per_sm = 4;
+    if (per_sm < 1) per_sm = 1;
+    const int64_t cap = (int64_t)per_sm * c->n_sm;
     const int grid = (int)(units < cap ? units : cap);
     k_tile_inner<<<grid, kInnerThreads, sm, st>>>(c->d_tiles, c->d_work, c->d_cell_start, pos, inner_args(c), c->d_ctrl,
-                                                  c->n_pad, c->tile_cap, nsplit);
+                                                  c->n_pad, c->tile_cap, nsplit, which, c->n_tiles);
     c->launches++;
     return cudaGetLastError();
 }
@@ -1086,26 +1164,37 @@ cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float
     return cudaGetLastError();
 }
 
-cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int mode, cudaStream_t st)
+static ListSel list_sel(const tbsma_ctx *c, int sync_level)
 {
-    const int g = gather_grid(c, mode);
-    k_density_tile<<<g, c->tile_threads, gather_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos,
-                                                              reinterpret_cast<const uint2 *>(c->d_nlist), c->d_nn,
-                                                              c->d_xs, c->d_ctrl, c->d_dirty, c->d_work, mode, c->n_pad,
-                                                              c->tile_cap, c->pc);
+    ListSel ls;
+    ls.cur = c->d_cur;
+    ls.dirty = c->d_dirty;
+    ls.sync_level = sync_level;
+    ls.nl_stride = (size_t)(c->kmax / 4) * c->n_pad;
+    ls.n_stride = c->n_pad;
+    return ls;
+}
+
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st)
+{
+    k_density_tile<<<c->n_tiles, c->tile_threads, gather_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos,
+                                                                       reinterpret_cast<const uint2 *>(c->d_nlist),
+                                                                       c->d_nn, c->d_xs, c->d_ctrl, list_sel(c, sync_level),
+                                                                       c->n_pad, c->tile_cap, c->pc);
     c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kk,
-                                    int mode, cudaStream_t st)
+                                    int sync_level, cudaStream_t st)
 {
     const uint2 *nl = reinterpret_cast<const uint2 *>(c->d_nlist);
     const size_t sm = gather_smem(c);
-    const int g = gather_grid(c, mode), b = c->tile_threads;
+    const int g = c->n_tiles, b = c->tile_threads;
+    const ListSel ls = list_sel(c, sync_level);
 #define TBSMA_FT(V, K)                                                                                             \
     k_force_tile<V, K><<<g, b, sm, st>>>(c->d_tiles, c->d_cell_start, c->d_xs, nl, c->d_nn, force, e_rep, w_rep, kk, \
-                                         c->d_ctrl, c->d_dirty, c->d_work, mode, c->n_pad, c->tile_cap, c->pc)
+                                         c->d_ctrl, ls, c->n_pad, c->tile_cap, c->pc)
     if (w_rep) { if (kk.vel) TBSMA_FT(true, true); else TBSMA_FT(true, false); }
     else       { if (kk.vel) TBSMA_FT(false, true); else TBSMA_FT(false, false); }
 #undef TBSMA_FT
@@ -1117,7 +1206,8 @@ cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, in
                                             cudaStream_t st)
 {
     k_get_neighbors_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(tag, reinterpret_cast<const uint2 *>(c->d_nlist),
-                                                                   c->d_nn, c->d_hbase, counts, list, (int)c->n,
+                                                                   c->d_nn, c->d_hbase, c->d_atom_rep, c->d_cur,
+                                                                   (size_t)(c->kmax / 4) * c->n_pad, counts, list, (int)c->n,
                                                                    c->n_pad, c->kmax);
     c->launches++;
     return cudaGetLastError();
@@ -1127,7 +1217,8 @@ cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsig
                                           cudaStream_t st)
 {
     k_count_pairs_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(pos, reinterpret_cast<const uint2 *>(c->d_nlist),
-                                                                 c->d_nn, c->d_hbase, d_out2, (int)c->n, c->n_pad,
+                                                                 c->d_nn, c->d_hbase, c->d_atom_rep, c->d_cur,
+                                                                 (size_t)(c->kmax / 4) * c->n_pad, d_out2, (int)c->n, c->n_pad,
                                                                  c->pc.rc2);
     c->launches++;
     return cudaGetLastError();

@@ -28,13 +28,14 @@ def B():
 VARIANTS = [1, 2]     # 1 = global-gather lists, 2 = shared-memory tiles (non-periodic replicas only)
 
 
-def setup(B, w, max_nb=96, variant=0, tile=None):
+def setup(B, w, max_nb=96, variant=0, tile=None, stagger=True):
     if variant == 2 and np.any(w.periodic):
         pytest.skip("the shared-memory tile variant is for non-periodic replicas")
     ctx = B.make_context(w, max_nb)
     ctx.set_variant(variant)
     if tile:
         ctx.set_tile(*tile)
+    ctx.set_stagger(stagger)
     st = B.DeviceState(w)
     ctx.build_cells(st.pos, st.vel, st.tag)
     ctx.build_neighbors(st.pos, st.vel, st.tag)
@@ -196,10 +197,12 @@ def test_call_order_and_arguments(B):
     assert e.value.code == B.EINVAL
 
 
-def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None, overlap=True):
-    ctx, st = setup(B, w, variant=variant, tile=tile)
+def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None, overlap=True,
+               stagger=True, async_inner=True):
+    ctx, st = setup(B, w, variant=variant, tile=tile, stagger=stagger)
     ctx.set_graph(graph)
     ctx.set_overlap(overlap)
+    ctx.set_async(async_inner)
     ctx.compute(st.pos, st.force, st.e_rep, None)
     stream = torch.cuda.Stream()
     stream.wait_stream(torch.cuda.current_stream())
@@ -282,14 +285,16 @@ def test_md_step_equals_md_run_and_graph_bitwise(B, variant):
 
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_replicas_are_independent_and_ragged_batch_matches_single_runs(B, variant):
+    # staggering (tbsma_set_stagger) makes a replica's FIRST rebuild depend on its index in the batch, which changes the
+    # fp32 summation order, not the physics: switched off here because this test compares bits
     w = W.config4(4, seed=21)
     n_steps = 60
-    _, st = run_gpu_md(B, w, n_steps, variant=variant)
+    _, st = run_gpu_md(B, w, n_steps, variant=variant, stagger=False)
     xb = st.untag(st.pos)
     assert len(set(np.diff(w.offsets))) > 1        # really ragged
     for r in range(w.n_replicas):
         single = w.take(r, r + 1)
-        _, ss = run_gpu_md(B, single, n_steps, variant=variant)
+        _, ss = run_gpu_md(B, single, n_steps, variant=variant, stagger=False)
         s = slice(w.offsets[r], w.offsets[r + 1])
         assert np.array_equal(xb[s], ss.untag(ss.pos))          # bit-identical: no cross-replica effect
 
