@@ -577,28 +577,37 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
                 run += (unsigned)n_s[sft];
             }
         }
-        // pass 2: round j takes the j-th entry of the classes lane, lane + 1, ... that still have one.  One loop
-        // iteration per list entry (the lanes of a warp have lists of nearly equal length): the classes of round j
-        // are the set bits of `act`.
+        // pass 2: position 8 j + s takes the j-th entry of class lane + s for j < L = m / 8.  A class with fewer than
+        // L entries leaves holes; they, and the positions from 8 L on, take the entries beyond the L-th of the longer
+        // classes, in stored order.
         uint2 *dst = nl_out + i;
         unsigned long long w = 0ull;
-        int j = 0;
-        unsigned act = 0u;
+        const int L = m >> 3;
+        int sc = 0, sj = L;
+        auto next_surplus = [&]() {
+            while (sj >= (int)byte_of(npk, sc)) { ++sc; sj = L; }
+            return (int)byte_of(orot, sc) + sj++;
+        };
+        int o_s[8];
 #pragma unroll
-        for (int sft = 0; sft < 8; ++sft) act |= (n_s[sft] > 0 ? 1u : 0u) << sft;
-        for (int p = 0; p < m; ++p) {
-            const int sft = __ffs((int)act) - 1;
-            act &= act - 1u;
-            const int k = (int)((unsigned)(orot >> (sft << 3)) & 0xffu) + j;
+        for (int sft = 0; sft < 8; ++sft) o_s[sft] = (int)byte_of(orot, sft);
+        for (int j = 0; j < L; ++j) {
+#pragma unroll
+            for (int sft = 0; sft < 8; ++sft) {
+                const int k = n_s[sft] > j ? o_s[sft] + j : next_surplus();
+                w |= (unsigned long long)col[k * nthr] << ((sft & 3) << 4);
+                if ((sft & 3) == 3) {
+                    dst[(size_t)(2 * j + (sft >> 2)) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));
+                    w = 0ull;
+                }
+            }
+        }
+        for (int p = L << 3; p < m; ++p) {
+            const int k = next_surplus();
             w |= (unsigned long long)col[k * nthr] << ((p & 3) << 4);
             if ((p & 3) == 3) {
                 dst[(size_t)(p >> 2) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));
                 w = 0ull;
-            }
-            if (act == 0u) {       // next round
-                ++j;
-#pragma unroll
-                for (int s2 = 0; s2 < 8; ++s2) act |= (n_s[s2] > j ? 1u : 0u) << s2;
             }
         }
         if (m & 3) dst[(size_t)(m >> 2) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));   // unused = 0 = sentinel
