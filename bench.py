@@ -278,14 +278,20 @@ def main():
                 "density_pass": {"achieved": ach_dens, "frac": ach_dens / peak, "avg_launch_ms": per_kernel_ms["density"]},
                 "whole_step": {"achieved": ach_step, "frac": ach_step / peak, "bytes_per_atom_step": step_bytes / w.n_atoms},
                 "per_kernel_ms": per_kernel_ms, "timed_steps": tsteps}
-    traffic_file = os.path.join(ROOT, "profiles", "force_kernel_dram_bytes.json")
+    # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu capture
+    traffic_file = os.path.join(ROOT, "profiles", "r1c_force_kernel_traffic.csv")
     if os.path.exists(traffic_file):
         try:
-            tf = json.load(open(traffic_file))
-            if tf.get("workload") == w.name:
-                roofline["traffic"] = tf.get("dram_bytes_per_launch")
+            import csv
+            for row in csv.DictReader(open(traffic_file)):
+                if row["workload"] == w.name and row["kernel"].startswith("k_force"):
+                    roofline["traffic"] = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+                    roofline["traffic_source"] = row["source"]
         except Exception:
             pass
+    roofline["note"] = ("HBM is the designated roofline (BASELINE.json); with 16-bit lists the gather passes move less than "
+                        "the algorithmic bytes and are bound by the shared-memory data pipe and the MUFU pipe "
+                        "(profiles/r1c_ncu_full_summary.md)")
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -334,6 +340,9 @@ def main():
                        "rebuild": "displacement > skin/2 per replica" if not w.rebuild_every else f"every {w.rebuild_every} steps",
                        "mean_list_length": n_l, "mean_steps_between_rebuilds": k_eff,
                        "l2": "inputs larger than L2 (index list %.0f MB per pass)" % (entries * 4 / 1e6),
+                       "variant": {1: "global gather (int32 list)", 2: "shared-memory tiles (u16 lists)"}.get(ctx.get_variant()),
+                       "list_renewal": "asynchronous, margin 0.03 A, second stream" if ctx.get_variant() == 2 and not w.rebuild_every else "ahead of the gather passes",
+                       "graph": "plain" if args.plain_graph else "conditional node around the cells+candidates chain",
                        "parallelism": "replicas only" if world > 1 else "1 gpu"},
             "pair_interactions_per_s": pair_rate,
             "clocks": sampler.summary(t_host0, t_host1),

@@ -198,9 +198,9 @@ def test_call_order_and_arguments(B):
 
 
 def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None, overlap=True,
-               stagger=True, async_inner=True):
+               stagger=True, async_inner=True, conditional=True):
     ctx, st = setup(B, w, variant=variant, tile=tile, stagger=stagger)
-    ctx.set_graph(graph)
+    ctx.set_graph(graph, conditional=conditional)
     ctx.set_overlap(overlap)
     ctx.set_async(async_inner)
     ctx.compute(st.pos, st.force, st.e_rep, None)
@@ -319,6 +319,77 @@ def test_two_stream_overlap_is_bitwise_identical(B, graph):
     assert ca.status() == 0 and cb.status() == 0
     md = run_oracle_md(w, n_steps)
     assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+
+
+def test_async_list_renewal_changes_cost_not_results(B):
+    """tbsma_set_async: lists re-filtered one step early into the second half of the buffers, beside the gather passes
+    that still read the old half, give the same physics as lists renewed ahead of the gather passes; and the list in
+    use after the run still covers the cutoff sphere (forces from it match the oracle at the final positions)"""
+    w = W.config3(6, seed=13, length=60.0)
+    n_steps = 120
+    ca, a = run_gpu_md(B, w, n_steps, variant=2, async_inner=True)
+    cb, b = run_gpu_md(B, w, n_steps, variant=2, async_inner=False)
+    sa, sb = ca.get_stats(), cb.get_stats()
+    assert sa["n_replica_builds"] >= sb["n_replica_builds"] >= 4      # asked for 0.03 A earlier: never fewer
+    assert ca.status() == 0 and cb.status() == 0
+    xa, xb = a.untag(a.pos)[:, :3].astype(np.float64), b.untag(b.pos)[:, :3].astype(np.float64)
+    assert traj_rms(xa, xb) <= 1e-4
+    md = run_oracle_md(w, n_steps)
+    assert traj_rms(xa, md.x) <= TRAJ_RMS
+    for ctx, st in ((ca, a), (cb, b)):
+        ctx.compute(st.pos, st.force, st.e_rep, None)
+        torch.cuda.synchronize()
+        x = st.untag(st.pos)
+        o = oracle.compute(x[:, :3].astype(np.float64), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi,
+                           periodic=w.periodic)
+        f = st.untag(st.force)
+        err = np.linalg.norm(f[:, :3] - o["f"], axis=1)
+        assert np.all(err <= F_ABS + F_REL * np.linalg.norm(o["f"], axis=1))
+        assert np.allclose(st.e_rep.cpu().numpy(), o["e_rep"], rtol=E_REL, atol=0)
+
+
+def test_conditional_graph_node_is_bitwise_identical(B):
+    """tbsma_set_graph 2 vs 1: wrapping the cells + candidates chain in an IF node of the captured step changes which
+    kernels are launched, not one bit of the results; S = 0.5 forces that chain to run in some steps"""
+    w = W.config3(4, seed=17, length=60.0)
+
+    def run(cond):
+        ctx = B.make_context(w)
+        ctx.set_variant(2)
+        ctx.set_outer_skin(0.5)
+        ctx.set_graph(True, conditional=cond)
+        st = B.DeviceState(w)
+        ctx.build_cells(st.pos, st.vel, st.tag)
+        ctx.build_neighbors(st.pos, st.vel, st.tag)
+        ctx.compute(st.pos, st.force, st.e_rep, None)
+        stream = torch.cuda.Stream()
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, 100, None, st.slab_rate,
+                       0, st.e_rep, None, st.ekin)
+        torch.cuda.synchronize()
+        assert ctx.status() == 0
+        return ctx.get_stats(), st
+
+    sa, a = run(True)
+    sb, b = run(False)
+    assert sa == sb and sa["n_candidate_builds"] >= 1
+    for name in ("pos", "vel", "force"):
+        assert np.array_equal(a.untag(getattr(a, name)), b.untag(getattr(b, name))), name
+
+
+def test_stagger_spreads_the_first_rebuilds(B):
+    """tbsma_set_stagger: replicas that start together and share a temperature rebuild in the same few steps; with
+    the first threshold scaled per replica the same number of steps sees more, smaller rebuild passes"""
+    w = W.config4(16, seed=19)       # sixteen 298 K wires
+    n_steps = 30
+    ca, a = run_gpu_md(B, w, n_steps, variant=2, stagger=True)
+    cb, b = run_gpu_md(B, w, n_steps, variant=2, stagger=False)
+    sa, sb = ca.get_stats(), cb.get_stats()
+    assert sa["n_build_passes"] > sb["n_build_passes"] >= 1
+    assert ca.status() == 0 and cb.status() == 0
+    xa, xb = a.untag(a.pos)[:, :3].astype(np.float64), b.untag(b.pos)[:, :3].astype(np.float64)
+    assert traj_rms(xa, xb) <= 1e-4
 
 
 @pytest.mark.parametrize("outer_skin", [0.0, 0.5, 2.0])
