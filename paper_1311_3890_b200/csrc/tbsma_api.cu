@@ -206,13 +206,6 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
                 cap == cudaStreamCaptureStatusActive && cg)
                 use_cond = cudaGraphConditionalHandleCreate(&cond, cg, 0, cudaGraphCondAssignDefault) == cudaSuccess;
             CK(tbsma_launch_tile_worklist(c, st, (unsigned long long)cond, use_cond ? 1 : 0));
-            if (async && c->overlap && !c->timing && c->aux_stream) {
-                CK(cudaEventRecord(c->ev_fork, st));
-                CK(cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
-                CK(tbsma_launch_tile_inner(c, pos, 0, c->aux_stream));
-                CK(cudaEventRecord(c->ev_join, c->aux_stream));
-                forked = true;
-            }
             if (use_cond) {
                 // IF (a replica needs new cells and candidates) { chain; its inner lists }: nothing is launched otherwise
                 CK(cudaStreamGetCaptureInfo(st, &cap, nullptr, &cg, &deps, &n_deps));
@@ -237,6 +230,15 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
             } else {
                 CK(tbsma_launch_rebuild(c, pos, vel, tag, true, true, st));
                 CK(tbsma_launch_tile_inner(c, pos, 1, st));
+            }
+            // (after the chain: idle, its kernels take 1.5 us each on an empty GPU, but each would wait for room on every SM
+            // behind a filter kernel already running)
+            if (async && c->overlap && !c->timing && c->aux_stream) {
+                CK(cudaEventRecord(c->ev_fork, st));
+                CK(cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
+                CK(tbsma_launch_tile_inner(c, pos, 0, c->aux_stream));
+                CK(cudaEventRecord(c->ev_join, c->aux_stream));
+                forked = true;
             }
             if (!forked) CK(tbsma_launch_tile_inner(c, pos, 0, st));
         } else {

@@ -318,7 +318,13 @@ cudaError_t tbsma_launch_rebuild(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t
         k_cell_scan<<<c->R, scan_threads, 0, st>>>(c->d_geom, dv, c->d_cell_count, c->d_cell_start);
         k_scatter<<<ga, kThreads, 0, st>>>(c->d_atom_rep, dv, c->d_cell_start,
                                            c->d_cell_of, c->d_slot, c->d_order, n);
-        k_cell_sort<<<dim3(c->R, kSortSplit), 256, 0, st>>>(c->d_geom, dv, c->d_cell_start, tag, c->d_order);
+        // a warp sorts one cell at a time: enough CTAs per replica that a batch of few, large replicas fills the GPU too
+        int split = (8 * c->n_sm + c->R - 1) / c->R;
+        if (split < kSortSplit) split = kSortSplit;
+        const int64_t by_cells = (c->n_cells / c->R + 7) / 8;      // no more CTAs than cells / 8 warps
+        if (split > by_cells) split = (int)(by_cells > 0 ? by_cells : 1);
+        if (split > 65535) split = 65535;
+        k_cell_sort<<<dim3(c->R, split), 256, 0, st>>>(c->d_geom, dv, c->d_cell_start, tag, c->d_order);
         // d_slot is free after the scatter: reuse it for the cell id of every sorted slot
         k_reorder_gather<<<ga, kThreads, 0, st>>>(pos, vel, tag, c->d_atom_rep, c->d_geom, dv,
                                                   c->d_order, c->d_cell_of, c->d_tmp_pos,
