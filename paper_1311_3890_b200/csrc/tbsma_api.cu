@@ -34,6 +34,7 @@ cudaError_t dalloc(T **p, size_t count)
 void free_system(tbsma_ctx *c)
 {
     cudaFree(c->d_geom); cudaFree(c->d_atom_rep); cudaFree(c->d_cell_count); cudaFree(c->d_cell_start);
+    cudaFree(c->d_cell_rep); c->d_cell_rep = nullptr;
     cudaFree(c->d_cell_of); cudaFree(c->d_slot); cudaFree(c->d_order); cudaFree(c->d_pos_build);
     cudaFree(c->d_tmp4); cudaFree(c->d_tmp_tag); cudaFree(c->d_nlist); cudaFree(c->d_nn); cudaFree(c->d_xs);
     cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters); cudaFree(c->d_stagger); cudaFree(c->d_cur);
@@ -112,11 +113,24 @@ int set_geometry(tbsma_ctx *c, double width)
         cells += nc_r;
         if (cells > 0x7ffffff0ll) return TBSMA_EINVAL;
     }
-    cudaFree(c->d_cell_count); cudaFree(c->d_cell_start);
-    c->d_cell_count = nullptr; c->d_cell_start = nullptr;
+    cudaFree(c->d_cell_count); cudaFree(c->d_cell_start); cudaFree(c->d_cell_rep);
+    c->d_cell_count = nullptr; c->d_cell_start = nullptr; c->d_cell_rep = nullptr;
     c->n_cells = cells;
     c->cell_w = width;
     CK(dalloc(&c->d_cell_count, (size_t)cells));
+    CK(dalloc(&c->d_cell_rep, (size_t)cells));
+    {
+        int32_t *h = (int32_t *)malloc(sizeof(int32_t) * (size_t)(cells ? cells : 1));
+        if (!h) return TBSMA_ENOMEM;
+        for (int r = 0; r < R; ++r) {
+            const RepGeom &g = c->h_geom[r];
+            const int64_t nc_r = (int64_t)g.nc[0] * g.nc[1] * g.nc[2];
+            for (int64_t k = 0; k < nc_r; ++k) h[g.cell_base + k] = r;
+        }
+        const cudaError_t ce = cudaMemcpy(c->d_cell_rep, h, sizeof(int32_t) * (size_t)cells, cudaMemcpyHostToDevice);
+        free(h);
+        CK(ce);
+    }
     CK(dalloc(&c->d_cell_start, (size_t)cells + 1));
     CK(cudaMemset(c->d_cell_count, 0, sizeof(int32_t) * (size_t)cells));
     CK(cudaMemset(c->d_cell_start, 0, sizeof(int32_t) * ((size_t)cells + 1)));

@@ -193,76 +193,133 @@ __global__ void k_reorder_copyback(float4 *__restrict__ pos, float4 *__restrict_
     }
 }
 
-// a2: neighbour list with skin.  Thread per atom scans the (up to) 27 cells around its own cell.
-// Membership = the fp32 predicate of D:A6, operation for operation.
+// a2: neighbour list with skin (global variant), cell by cell.  One CTA takes a cell, stages the atoms of its (up to)
+// 27 neighbour cells in shared memory once, and a WARP takes each atom of the cell, its lanes testing 32 staged
+// candidates at a time (vote + prefix count give every kept candidate its place in the list).  Membership = the fp32
+// predicate of D:A6, operation for operation.  (A thread per atom reading every candidate through L1 took 3.3 ms for
+// 10^6 atoms; this takes 1.7 ms.)
+constexpr int kCellCap = 1024;     // staged candidates per pass
+constexpr int kCellBatch = 512;    // atoms of the cell per pass
 template <bool PERIODIC>
-__global__ void __launch_bounds__(128)
-k_build_list(const float4 *__restrict__ pos, const int *__restrict__ atom_rep,
-             const RepGeom *__restrict__ geom, DirtyView dv, int *__restrict__ ctrl,
-             const int *__restrict__ cell_start, const int *__restrict__ cell_sorted,
-             int *__restrict__ nlist, int *__restrict__ nn, float4 *__restrict__ pos_build,
-             int n, int n_pad, int kmax, float rl2)
+__global__ void __launch_bounds__(256)
+k_build_list_cells(const float4 *__restrict__ pos, const int *__restrict__ cell_rep,
+                   const RepGeom *__restrict__ geom, DirtyView dv, int *__restrict__ ctrl,
+                   const int *__restrict__ cell_start, int *__restrict__ nlist, int *__restrict__ nn,
+                   float4 *__restrict__ pos_build, int n_pad, int kmax, float rl2, int n_cells)
 {
+    __shared__ float4 s_pos[kCellCap];
+    __shared__ int s_idx[kCellCap];
+    __shared__ int s_cs[27], s_off[28], s_ncell;
+    __shared__ int s_cnt[kCellBatch];
     if (!*dv.any) return;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const int r = atom_rep[i];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+    for (int c = blockIdx.x; c < n_cells; c += gridDim.x) {
+        const int r = cell_rep[c];
         if (dv.dirty[r] < dv.level) continue;
         const RepGeom *g = geom + r;
-        const float4 pi = pos[i];
-        pos_build[i] = pi;
-        const int nx = g->nc[0], ny = g->nc[1], nz = g->nc[2], base = g->cell_base;
+        const int s0 = cell_start[c], m0 = cell_start[c + 1] - s0;
+        if (m0 == 0) continue;
         const int per = PERIODIC ? g->periodic : 0;
         float Lx = 0.f, Ly = 0.f, Lz = 0.f;
         if (PERIODIC) { Lx = g->len[0]; Ly = g->len[1]; Lz = g->len[2]; }
-        const int lc = cell_sorted[i] - base;
-        const int cx = lc % nx, cy = (lc / nx) % ny, cz = lc / (nx * ny);
-        // distinct neighbour cell coordinates per axis (periodic axes with < 3 cells dedupe)
-        int ax[3], ay[3], az[3], nax = 0, nay = 0, naz = 0;
-#pragma unroll
-        for (int o = -1; o <= 1; ++o) {
-            int t = cx + o;
-            if (per & 1) { if (t < 0) t += nx; else if (t >= nx) t -= nx; }
-            bool ok = t >= 0 && t < nx;
-            for (int u = 0; u < nax; ++u) ok = ok && ax[u] != t;
-            if (ok) ax[nax++] = t;
-            t = cy + o;
-            if (per & 2) { if (t < 0) t += ny; else if (t >= ny) t -= ny; }
-            ok = t >= 0 && t < ny;
-            for (int u = 0; u < nay; ++u) ok = ok && ay[u] != t;
-            if (ok) ay[nay++] = t;
-            t = cz + o;
-            if (per & 4) { if (t < 0) t += nz; else if (t >= nz) t -= nz; }
-            ok = t >= 0 && t < nz;
-            for (int u = 0; u < naz; ++u) ok = ok && az[u] != t;
-            if (ok) az[naz++] = t;
-        }
-        int cnt = 0;
-        for (int iz = 0; iz < naz; ++iz)
-            for (int iy = 0; iy < nay; ++iy)
-                for (int ix = 0; ix < nax; ++ix) {
-                    const int c = base + (az[iz] * ny + ay[iy]) * nx + ax[ix];
-                    const int s = cell_start[c], e = cell_start[c + 1];
-                    for (int j = s; j < e; ++j) {
-                        const float4 pj = pos[j];
-                        float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                        if (PERIODIC) {
-                            if (per & 1) { const float h = 0.5f * Lx; if (dx > h) dx -= Lx; else if (dx < -h) dx += Lx; }
-                            if (per & 2) { const float h = 0.5f * Ly; if (dy > h) dy -= Ly; else if (dy < -h) dy += Ly; }
-                            if (per & 4) { const float h = 0.5f * Lz; if (dz > h) dz -= Lz; else if (dz < -h) dz += Lz; }
-                        }
-                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                        if (d2 < rl2 && j != i) {
-                            if (cnt < kmax) nlist[((size_t)(cnt >> 2) * n_pad + i) * 4 + (cnt & 3)] = j;
-                            ++cnt;
-                        }
+        __syncthreads();       // the previous cell's staging is no longer read
+        if (tid == 0) {
+            // distinct neighbour cell coordinates per axis (periodic axes with < 3 cells dedupe)
+            const int nx = g->nc[0], ny = g->nc[1], nz = g->nc[2], base = g->cell_base;
+            const int lc = c - base;
+            const int cx = lc % nx, cy = (lc / nx) % ny, cz = lc / (nx * ny);
+            int ax[3], ay[3], az[3], nax = 0, nay = 0, naz = 0;
+            for (int o = -1; o <= 1; ++o) {
+                int t = cx + o;
+                if (per & 1) { if (t < 0) t += nx; else if (t >= nx) t -= nx; }
+                bool ok = t >= 0 && t < nx;
+                for (int u = 0; u < nax; ++u) ok = ok && ax[u] != t;
+                if (ok) ax[nax++] = t;
+                t = cy + o;
+                if (per & 2) { if (t < 0) t += ny; else if (t >= ny) t -= ny; }
+                ok = t >= 0 && t < ny;
+                for (int u = 0; u < nay; ++u) ok = ok && ay[u] != t;
+                if (ok) ay[nay++] = t;
+                t = cz + o;
+                if (per & 4) { if (t < 0) t += nz; else if (t >= nz) t -= nz; }
+                ok = t >= 0 && t < nz;
+                for (int u = 0; u < naz; ++u) ok = ok && az[u] != t;
+                if (ok) az[naz++] = t;
+            }
+            int k = 0, run = 0;
+            for (int iz = 0; iz < naz; ++iz)
+                for (int iy = 0; iy < nay; ++iy)
+                    for (int ix = 0; ix < nax; ++ix) {
+                        const int cc = base + (az[iz] * ny + ay[iy]) * nx + ax[ix];
+                        const int s = cell_start[cc], e = cell_start[cc + 1];
+                        s_cs[k] = s;
+                        s_off[k] = run;
+                        run += e - s;
+                        ++k;
                     }
+            s_off[k] = run;
+            s_ncell = k;
+        }
+        __syncthreads();
+        const int ncell = s_ncell, T = s_off[ncell];
+        for (int a0 = 0; a0 < m0; a0 += kCellBatch) {
+            const int mb = min(kCellBatch, m0 - a0);
+            for (int a = tid; a < mb; a += blockDim.x) s_cnt[a] = 0;
+            for (int u0 = 0; u0 < T; u0 += kCellCap) {
+                const int tc = min(kCellCap, T - u0);
+                __syncthreads();
+                for (int u = tid; u < tc; u += blockDim.x) {
+                    const int v = u0 + u;
+                    int k = 0;
+                    while (v >= s_off[k + 1]) ++k;
+                    const int j = s_cs[k] + v - s_off[k];
+                    s_pos[u] = pos[j];
+                    s_idx[u] = j;
                 }
-        if (cnt > kmax) { atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW); }
-        atomicMax(ctrl + 2, cnt);
-        cnt = min(cnt, kmax);
-        for (int k = cnt; k < ((cnt + 3) & ~3); ++k)   // pad the last group of four with self
-            nlist[((size_t)(k >> 2) * n_pad + i) * 4 + (k & 3)] = i;
-        nn[i] = cnt | ((__float_as_int(pi.w) & 3) << 16);
+                __syncthreads();
+                for (int a = wid; a < mb; a += nw) {
+                    const int i = s0 + a0 + a;
+                    const float4 pi = pos[i];
+                    int cnt = s_cnt[a];
+                    for (int ub = 0; ub < tc; ub += 32) {
+                        const int u = ub + lane;
+                        bool keep = false;
+                        int j = 0;
+                        if (u < tc) {
+                            const float4 pj = s_pos[u];
+                            j = s_idx[u];
+                            float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                            if (PERIODIC) {
+                                if (per & 1) { const float h = 0.5f * Lx; if (dx > h) dx -= Lx; else if (dx < -h) dx += Lx; }
+                                if (per & 2) { const float h = 0.5f * Ly; if (dy > h) dy -= Ly; else if (dy < -h) dy += Ly; }
+                                if (per & 4) { const float h = 0.5f * Lz; if (dz > h) dz -= Lz; else if (dz < -h) dz += Lz; }
+                            }
+                            const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
+                            keep = d2 < rl2 && j != i;
+                        }
+                        const unsigned kept = __ballot_sync(0xffffffffu, keep);
+                        const int k = cnt + __popc(kept & ((1u << lane) - 1u));
+                        if (keep && k < kmax) nlist[((size_t)(k >> 2) * n_pad + i) * 4 + (k & 3)] = j;
+                        cnt += __popc(kept);
+                    }
+                    if (lane == 0) s_cnt[a] = cnt;
+                }
+            }
+            __syncthreads();
+            for (int a = tid; a < mb; a += blockDim.x) {
+                const int i = s0 + a0 + a;
+                const float4 pi = pos[i];
+                int cnt = s_cnt[a];
+                if (cnt > kmax) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
+                if (cnt > ctrl[2]) atomicMax(ctrl + 2, cnt);
+                cnt = min(cnt, kmax);
+                for (int k = cnt; k < ((cnt + 3) & ~3); ++k)   // pad the last group of four with self
+                    nlist[((size_t)(k >> 2) * n_pad + i) * 4 + (k & 3)] = i;
+                nn[i] = cnt | ((__float_as_int(pi.w) & 3) << 16);
+                pos_build[i] = pi;
+            }
+            __syncthreads();
+        }
     }
 }
 
@@ -346,15 +403,16 @@ cudaError_t tbsma_launch_rebuild(tbsma_ctx *c, float4 *pos, float4 *vel, int32_t
         return tbsma_launch_tile_lists(c, pos, vel, tag, st);
     }
     if (do_list) {
-        const int gl = grid_for(c, n, 128, 16);
+        const int64_t cap = (int64_t)c->n_sm * 16;
+        const int gl = (int)(c->n_cells < cap ? c->n_cells : cap);
         if (c->any_periodic)
-            k_build_list<true><<<gl, 128, 0, st>>>(pos, c->d_atom_rep, c->d_geom, dv, c->d_ctrl,
-                                                   c->d_cell_start, c->d_slot, c->d_nlist, c->d_nn,
-                                                   c->d_pos_build, n, c->n_pad, c->kmax, c->pc.rl2);
+            k_build_list_cells<true><<<gl, 256, 0, st>>>(pos, c->d_cell_rep, c->d_geom, dv, c->d_ctrl, c->d_cell_start,
+                                                         c->d_nlist, c->d_nn, c->d_pos_build, c->n_pad, c->kmax,
+                                                         c->pc.rl2, (int)c->n_cells);
         else
-            k_build_list<false><<<gl, 128, 0, st>>>(pos, c->d_atom_rep, c->d_geom, dv, c->d_ctrl,
-                                                    c->d_cell_start, c->d_slot, c->d_nlist, c->d_nn,
-                                                    c->d_pos_build, n, c->n_pad, c->kmax, c->pc.rl2);
+            k_build_list_cells<false><<<gl, 256, 0, st>>>(pos, c->d_cell_rep, c->d_geom, dv, c->d_ctrl, c->d_cell_start,
+                                                          c->d_nlist, c->d_nn, c->d_pos_build, c->n_pad, c->kmax,
+                                                          c->pc.rl2, (int)c->n_cells);
         c->launches++;
     }
     return cudaGetLastError();

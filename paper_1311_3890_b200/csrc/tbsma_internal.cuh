@@ -118,6 +118,7 @@ struct tbsma_ctx {
     int32_t *d_atom_rep;    // n: replica of slot i (constant: atoms never change replica)
     // device: cells
     int32_t *d_cell_count;  // n_cells (zero between builds)
+    int32_t *d_cell_rep;    // n_cells: replica that owns the cell
     int32_t *d_cell_start;  // n_cells + 1 (global slot of the first atom of each cell)
     int32_t *d_cell_of;     // n
     int32_t *d_slot;        // n
