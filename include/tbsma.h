@@ -210,6 +210,16 @@ int tbsma_set_async(tbsma_ctx *ctx, int32_t enable, double margin);
  * ordinary stream semantics.  Off: the same kernels run one after the other on `stream`. */
 int tbsma_set_overlap(tbsma_ctx *ctx, int32_t enable);
 
+/* Shared-memory variant: where the records of a tile sit in its shared-memory image.  The gather passes read one
+ * 16-byte record per neighbour and lane; eight lanes are served at a time and collide unless their records lie in
+ * eight different bank groups (image index mod 8).  The list of every atom is ordered so that they do, as far as the
+ * atom's neighbours are spread evenly over the eight groups.  enable = 1 (default): the records get their image index
+ * from the COLOUR of the cell of side `cell` (Angstrom; 0 = r0 / sqrt 2, the (100) plane spacing of the fcc crystal the
+ * potential describes) their position falls in, (ix + 2 iy + 3 iz) mod 8: on a crystal every neighbourhood then holds
+ * nearly equal numbers of each group.  enable = 0: slot order.  Any placement gives the same lists as SETS and the same
+ * forces up to the fp32 summation order.  Takes effect when candidates are next rebuilt (tbsma_build_neighbors). */
+int tbsma_set_balance(tbsma_ctx *ctx, int32_t enable, double cell);
+
 /* Replicas built together (all of them, by tbsma_build_neighbors) that share a temperature would all need their
  * next list at nearly the same step, and again one period later.  When enabled (default 1, more than one replica)
  * replica r rebuilds for the first time as soon as an atom has moved f_r skin/2, f_r = 0.3 + 0.7 frac(0.618 r), and

@@ -20,7 +20,7 @@ EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
-    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_async", "tbsma_set_outer_skin",
+    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
 
@@ -79,6 +79,7 @@ def lib():
         L.tbsma_set_overlap.argtypes = [vp, i32]
         L.tbsma_set_stagger.argtypes = [vp, i32]
         L.tbsma_set_async.argtypes = [vp, i32, dbl]
+        L.tbsma_set_balance.argtypes = [vp, i32, dbl]
         L.tbsma_set_outer_skin.argtypes = [vp, dbl]
         L.tbsma_set_timing.argtypes = [vp, i32]
         L.tbsma_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
@@ -230,6 +231,9 @@ class Context:
 
     def set_stagger(self, enable):
         _check(lib().tbsma_set_stagger(self._h, int(bool(enable))), "tbsma_set_stagger")
+
+    def set_balance(self, enable, cell=0.0):
+        _check(lib().tbsma_set_balance(self._h, int(bool(enable)), float(cell)), "tbsma_set_balance")
 
     def set_async(self, enable, margin=0.03):
         _check(lib().tbsma_set_async(self._h, int(bool(enable)), float(margin)), "tbsma_set_async")

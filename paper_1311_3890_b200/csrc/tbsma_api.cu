@@ -39,7 +39,9 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_tmp4); cudaFree(c->d_tmp_tag); cudaFree(c->d_nlist); cudaFree(c->d_nn); cudaFree(c->d_xs);
     cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters); cudaFree(c->d_stagger); cudaFree(c->d_cur);
     c->d_stagger = nullptr; c->d_cur = nullptr;
-    cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_newslot); cudaFree(c->d_oldof);
+    cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_tileof); cudaFree(c->d_img); cudaFree(c->d_inv);
+    c->d_tileof = nullptr; c->d_img = nullptr; c->d_inv = nullptr;
+    cudaFree(c->d_newslot); cudaFree(c->d_oldof);
     cudaFree(c->d_nn_tmp); cudaFree(c->d_tmp_pos);
     cudaFree(c->d_tile_first); cudaFree(c->d_work);
     c->d_tile_first = nullptr; c->d_work = nullptr;
@@ -314,6 +316,8 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->use_graph = 1;
     c->overlap = 1;
     c->stagger = 1;
+    c->balance = 1;
+    c->class_h = params->r0 / sqrt(2.0);
     c->use_cond = 1;
     c->async_inner = 1;
     c->async_margin = 0.03;
@@ -400,6 +404,14 @@ int tbsma_set_graph(tbsma_ctx *c, int32_t enable)
     c->use_graph = enable != 0;
     c->use_cond = enable != 1;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    return TBSMA_OK;
+}
+
+int tbsma_set_balance(tbsma_ctx *c, int32_t enable, double cell)
+{
+    if (!c || cell < 0.0) return TBSMA_EINVAL;
+    c->balance = enable != 0;
+    c->class_h = cell > 0.0 ? cell : c->prm.r0 / sqrt(2.0);
     return TBSMA_OK;
 }
 
@@ -512,7 +524,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     DA(c->d_nlist, nb * (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, nb * c->n_pad); DA(c->d_xs, n);
     DA(c->d_cur, (size_t)R);
     DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8); DA(c->d_stagger, (size_t)R);
-    DA(c->d_maxpop, (size_t)R); DA(c->d_hbase, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
+    DA(c->d_maxpop, (size_t)R); DA(c->d_hbase, n); DA(c->d_tileof, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
     DA(c->d_tmp_pos, n);
 #undef DA
     if (e != cudaSuccess) { free_system(c); return map_cuda(e); }

@@ -104,6 +104,12 @@ struct tbsma_ctx {
     int own_cap;           // own atoms a tile may hold (sizes the split of the inner build)
     int32_t *d_maxpop;  // R: largest layer population of each replica (measured at build_cells)
     int32_t *d_hbase;   // n: first halo slot of the tile that owns slot i
+    int32_t *d_tileof;  // n: the tile that owns slot i
+    unsigned short *d_img;  // n_tiles x tile_cap: image index of every halo record of a tile (k_tile_place)
+    unsigned short *d_inv;  // n_tiles x img_cap: the inverse
+    int img_cap;        // records of a tile image, sentinel and spare room of the colour classes included
+    int balance;        // records placed by colour (default 1) or in slot order
+    double class_h;     // side of the colour cells (default r0 / sqrt 2)
     int32_t *d_newslot; // n: cell-order slot -> final slot
     int32_t *d_oldof;   // n: final slot -> cell-order slot
     int32_t *d_nn_tmp;  // n

@@ -231,6 +231,80 @@ k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ work, in
     }
 }
 
+// ---- K1b: placement of the halo records in the tile's shared-memory image.  The bank group ("class") a record is
+// read from is its image index mod 8, and the gather passes read without bank conflicts only as far as every atom's
+// neighbours are spread EVENLY over the eight classes (position p of lane l reads class (l + p) mod 8; a class that
+// runs out leaves a hole that collides with a neighbour lane).  With the records simply in slot order the classes
+// of an atom's ~70 neighbours are as good as random: 8.8 +- 2.8 per class, 7 holes per atom.  Here every atom gets a
+// COLOUR from the cell of side h (default r0 / sqrt 2, the spacing of the (100) planes of the fcc lattice the
+// potential describes) its position falls in, (ix + 2 iy + 3 iz) mod 8, and the image holds the records of colour c
+// at indices 8 j + c + 1 (j = rank among the tile's records of that colour, in slot order; index 0 = sentinel).  On a
+// crystal every sphere then holds nearly equal numbers of each colour (1 - 3 holes per atom); on a disordered
+// system the colours are no worse than random.  Any placement is CORRECT: lists hold image offsets, whatever they are.
+struct PlaceArgs {
+    const int *cell_start, *oldof;
+    const float4 *pos_sorted;        // cell-ordered positions of this rebuild
+    const RepGeom *geom;
+    unsigned short *img, *inv;       // per tile: halo-local final index -> image index, and back
+    int img_stride, inv_stride;      // tile_cap, img_cap
+    int img_cap;                     // records an image may hold (sentinel included)
+    float inv_h;                     // 1 / h; 0 = slot order (colour = index mod 8)
+    int *ctrl;
+};
+
+__global__ void __launch_bounds__(256)
+k_tile_place(const TileDesc *__restrict__ tiles, const int *__restrict__ work, int n_tiles, PlaceArgs A)
+{
+    __shared__ unsigned char s_col[TBSMA_TILE_MAX_RECORDS + 1];
+    __shared__ int s_count[8], s_fallback;
+    const int nw = work[1];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int w = blockIdx.x; w < nw; w += gridDim.x) {
+        const int ti = work[2 + n_tiles + w];
+        const TileDesc t = tiles[ti];
+        const TileRange r = tile_range(t, A.cell_start);
+        if (r.hi <= r.lo || r.nh > A.img_stride) continue;
+        const RepGeom *g = A.geom + t.rep;
+        unsigned short *img = A.img + (size_t)ti * A.img_stride, *inv = A.inv + (size_t)ti * A.inv_stride;
+        __syncthreads();
+        if (tid == 0) s_fallback = 0;
+        for (int pass = 0; pass < 2; ++pass) {
+            // pass 0: colours from the positions; pass 1 (only if they filled the image too unevenly): slot order
+            for (int k = tid; k < r.nh; k += blockDim.x) {
+                int col = k & 7;
+                if (pass == 0 && A.inv_h > 0.f) {
+                    const float4 p = A.pos_sorted[A.oldof[r.halo_lo + k]];
+                    const int ix = __float2int_rd((p.x - g->lo[0]) * A.inv_h), iy = __float2int_rd((p.y - g->lo[1]) * A.inv_h);
+                    const int iz = __float2int_rd((p.z - g->lo[2]) * A.inv_h);
+                    col = (ix + 2 * iy + 3 * iz) & 7;
+                }
+                s_col[k] = (unsigned char)col;
+            }
+            __syncthreads();
+            if (wid < 8) {         // warp c ranks the records of colour c in slot order
+                int run = 0;
+                for (int kb = 0; kb < r.nh; kb += 32) {
+                    const int k = kb + lane;
+                    const bool mine = k < r.nh && s_col[k] == wid;
+                    const unsigned m = __ballot_sync(0xffffffffu, mine);
+                    if (mine) {
+                        const int idx = 8 * (run + __popc(m & ((1u << lane) - 1u))) + wid + 1;
+                        if (idx < A.img_cap) { img[k] = (unsigned short)idx; inv[idx] = (unsigned short)k; }
+                    }
+                    run += __popc(m);
+                }
+                if (lane == 0) {
+                    s_count[wid] = run;
+                    if (8 * (run - 1) + wid + 1 >= A.img_cap) s_fallback = 1;
+                }
+            }
+            __syncthreads();
+            if (!s_fallback || pass == 1) break;
+            __syncthreads();
+        }
+    }
+}
+
 __device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { return (unsigned)(v >> (c << 3)) & 0xffu; }
 
 // ---- K2: finish.  One thread per FINAL slot of the tile: reads the temporary row of the atom that
@@ -245,11 +319,13 @@ struct FinishArgs {
     const uint2 *nl_tmp;
     const int *nn_tmp, *newslot, *oldof;
     uint2 *nl;
-    int *nn, *hbase;
+    int *nn, *hbase, *tileof;
+    const unsigned short *img;   // image placement of every tile (k_tile_place)
+    int img_stride;
     int n_pad, s_cap;
 };
 
-__device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs &A)
+__device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const FinishArgs &A)
 {
     const int *__restrict__ cell_start = A.cell_start;
     const uint2 *__restrict__ nl_tmp = A.nl_tmp;
@@ -263,8 +339,9 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs 
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo || r.nh > s_cap) return;
     const int tid = threadIdx.x, nthr = blockDim.x;
+    const unsigned short *__restrict__ img = A.img + (size_t)ti * A.img_stride;
     for (int k = tid; k < r.nh; k += blockDim.x)
-        map[k] = (unsigned short)((newslot[r.halo_lo + k] - r.halo_lo + 1) << 4);
+        map[k] = (unsigned short)((unsigned)img[newslot[r.halo_lo + k] - r.halo_lo] << 4);
     __syncthreads();
     for (int ip = r.lo + tid; ip < r.hi; ip += blockDim.x) {
         const int a = oldof[ip];
@@ -313,6 +390,7 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, const FinishArgs 
         }
         nn[ip] = nnv;
         hbase[ip] = r.halo_lo;
+        A.tileof[ip] = ti;
     }
 }
 
@@ -322,7 +400,8 @@ k_tile_finish(const TileDesc *__restrict__ tiles, const int *__restrict__ work, 
     const int nw = work[1];
     for (int w = blockIdx.x; w < nw; w += gridDim.x) {
         __syncthreads();
-        finish_tile(tiles[work[2 + n_tiles + w]], A);
+        const int ti = work[2 + n_tiles + w];
+        finish_tile(tiles[ti], ti, A);
     }
 }
 
@@ -363,48 +442,29 @@ __global__ void k_stage_copy(const float4 *__restrict__ pos, const float4 *__res
 // the loops need no self / padding test), record k + 1 is the atom at slot halo_lo + k.
 #define TBSMA_SENTINEL 1.0e9f
 
-// The image is one contiguous run of records, so a single bulk copy (cp.async.bulk, the 1-D form of
-// TMA) issued by one thread moves it; everybody waits on the mbarrier the copy completes on.  The
-// caller has made sure (__syncthreads) that nobody still reads a previous image.  `phase` is the
-// parity of the barrier, flipped by every fill.
-struct TileFill {
-    unsigned long long *bar;
-    unsigned phase;
-};
-
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ TileFill tile_fill_init(unsigned long long *bar)
+// The records of the halo go to the image indices k_tile_place chose for them (see there): one coalesced read of
+// the slot range, scattered 16-byte stores.  The caller has made sure (__syncthreads) that nobody still reads a
+// previous image.  (A contiguous image was one cp.async.bulk; spreading the records over the bank groups is worth
+// more than the copy engine: a third fewer shared-memory wavefronts in the gather passes.)
+__device__ __forceinline__ void fill_image(float4 *sm, const float4 *__restrict__ src,
+                                           const unsigned short *__restrict__ img, int halo_lo, int nh)
 {
-    if (threadIdx.x == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(bar)) : "memory");
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (threadIdx.x == 0) sm[0] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
+    // eight records per thread and round, all sixteen loads in flight before the first store
+    const int nthr = blockDim.x;
+    for (int k0 = threadIdx.x; k0 < nh; k0 += 8 * nthr) {
+        float4 rec[8];
+        unsigned short at[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int k = k0 + u * nthr;
+            if (k < nh) { at[u] = img[k]; rec[u] = src[halo_lo + k]; }
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            if (k0 + u * nthr < nh) sm[at[u]] = rec[u];
     }
     __syncthreads();
-    TileFill f;
-    f.bar = bar;
-    f.phase = 0u;
-    return f;
-}
-
-__device__ __forceinline__ void fill_tile(float4 *sm, const float4 *__restrict__ src, int halo_lo, int nh, TileFill &f)
-{
-    const unsigned bar = smem_u32(f.bar);
-    if (threadIdx.x == 0) {
-        sm[0] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
-        const unsigned bytes = (unsigned)nh * 16u;
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic reads of the image vs. this write
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                     ::"r"(smem_u32(sm + 1)), "l"(src + halo_lo), "r"(bytes), "r"(bar) : "memory");
-    }
-    unsigned done;
-    do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-                     "selp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(bar), "r"(f.phase) : "memory");
-    } while (!done);
-    f.phase ^= 1u;
 }
 
 __device__ __forceinline__ float4 lds_rec(const float4 *sm, unsigned byte_off)
@@ -499,6 +559,8 @@ struct InnerArgs {
     int *nn;                 // out: count | flag << 16    } is written (the last kernel of the step swaps)
     float4 *pos_build;       // out                        }
     const int *cur;          // per replica: half in use
+    const unsigned short *img;   // image placement of every tile (k_tile_place)
+    int img_stride, img_cap;
     size_t nl_stride;        // uint2 elements between the halves of nl
     int n_stride;            // elements between the halves of nn and pos_build
     const float4 *pos_outer;
@@ -511,8 +573,8 @@ constexpr int kInnerThreads = 256;   // one atom per thread, kmax u16 of shared-
 
 // tmp: element k of thread t at [k * nthr + t], kmax + 1 rows (row kmax takes what does not fit)
 __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRange &r, int i_begin, int i_end,
-                                                 const float4 *sm, unsigned short *tmp, const InnerArgs &ia,
-                                                 int *__restrict__ ctrl, int n_pad)
+                                                 const float4 *sm, const float4 *__restrict__ pos, unsigned short *tmp,
+                                                 const InnerArgs &ia, int *__restrict__ ctrl, int n_pad)
 {
     // i_begin - r.lo is a multiple of 32, so tid & 31 is the lane the gather kernels give the atom
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
@@ -524,7 +586,7 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
     float4 *pb_out = ia.pos_build + (size_t)ob * ia.n_stride;
     unsigned short *col = tmp + tid;
     for (int i = i_begin + tid; i < i_end; i += nthr) {
-        const float4 pi = sm[i - r.halo_lo + 1];
+        const float4 pi = pos[i];
         const int nno = ia.nn_o[i];
         const int ng = ((nno & 0xffff) + 3) >> 2;
         const uint2 *row = ia.olist + i;
@@ -633,14 +695,13 @@ k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, c
              int which, int n_tiles)
 {
     extern __shared__ float4 smem_f4[];
-    __shared__ unsigned long long s_bar;
     const int *__restrict__ wl = work + 2 + which * n_tiles;
     const int nu = work[which] * nsplit;
     if ((int)blockIdx.x >= nu) return;
-    unsigned short *tmp = reinterpret_cast<unsigned short *>(smem_f4 + s_cap + 1);
-    TileFill tf = tile_fill_init(&s_bar);
+    unsigned short *tmp = reinterpret_cast<unsigned short *>(smem_f4 + ia.img_cap);
     for (int u = blockIdx.x; u < nu; u += gridDim.x) {
-        const TileDesc t = tiles[wl[u / nsplit]];
+        const int ti = wl[u / nsplit];
+        const TileDesc t = tiles[ti];
         const TileRange r = tile_range(t, cell_start);
         const int i_begin = r.lo + (u % nsplit) * blockDim.x;
         if (i_begin >= r.hi) continue;
@@ -649,10 +710,10 @@ k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, c
             continue;
         }
         __syncthreads();
-        fill_tile(smem_f4, pos, r.halo_lo, r.nh, tf);
+        fill_image(smem_f4, pos, ia.img + (size_t)ti * ia.img_stride, r.halo_lo, r.nh);
         // the last piece also takes whatever a tile holds beyond the headroom it was sized with
         const int i_end = (u % nsplit) == nsplit - 1 ? r.hi : min(i_begin + (int)blockDim.x, r.hi);
-        tile_inner_build(t, r, i_begin, i_end, smem_f4, tmp, ia, ctrl, n_pad);
+        tile_inner_build(t, r, i_begin, i_end, smem_f4, pos, tmp, ia, ctrl, n_pad);
     }
 }
 
@@ -678,7 +739,7 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
                                              const float4 *__restrict__ pos, const uint2 *__restrict__ nl,
                                              const int *__restrict__ nn, float4 *__restrict__ xs,
                                              int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
-                                             TileFill &tf)
+                                             const unsigned short *__restrict__ img)
 {
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
@@ -690,12 +751,12 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
     __shared__ int s_next;
     const float4 *sm = smem_f4;
     if (threadIdx.x == 0) s_next = 0;
-    fill_tile(smem_f4, pos, r.halo_lo, r.nh, tf);
+    fill_image(smem_f4, pos, img, r.halo_lo, r.nh);
     const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
     for (int ch = next_chunk(&s_next); ch < nchunk; ch = next_chunk(&s_next)) {
         const int i = r.lo + (ch << 5) + lane;
         if (i >= r.hi) continue;
-        const float4 pi = sm[i - r.halo_lo + 1];
+        const float4 pi = pos[i];
         const int ng = ((nn[i] & 0xffff) + 3) >> 2;
         const uint2 *row = nl + i;
         f32x2 rho2 = pk(0.f, 0.f);
@@ -732,6 +793,8 @@ struct ListSel {
     int sync_level;          // 1: every rebuild of this step precedes the gather passes; 2: only those with new candidates
     size_t nl_stride;
     int n_stride;
+    const unsigned short *img;   // image placement of every tile (k_tile_place)
+    int img_stride;
 };
 __device__ __forceinline__ int list_half(const ListSel &ls, int rep)
 {
@@ -745,12 +808,10 @@ k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_
                const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
                float4 *__restrict__ xs, int *__restrict__ ctrl, ListSel ls, int n_pad, int s_cap, PairConst pc)
 {
-    __shared__ unsigned long long s_bar;
     const TileDesc t = tiles[blockIdx.x];
     const int h = list_half(ls, t.rep);
-    TileFill tf = tile_fill_init(&s_bar);
     density_tile(t, cell_start, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad, s_cap,
-                 pc, tf);
+                 pc, ls.img + (size_t)blockIdx.x * ls.img_stride);
 }
 
 // running sums of stage 2, two lanes each (even / odd neighbours), added up once per atom
@@ -822,7 +883,7 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
                                            const int *__restrict__ nn, float4 *__restrict__ force,
                                            double *__restrict__ e_rep, double *__restrict__ w_rep, const KickArgs &kk,
                                            int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
-                                           TileFill &tf)
+                                           const unsigned short *__restrict__ img)
 {
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
@@ -835,14 +896,14 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
     __shared__ int s_next;
     const float4 *sm = smem_f4;
     if (threadIdx.x == 0) s_next = 0;
-    fill_tile(smem_f4, xs, r.halo_lo, r.nh, tf);
+    fill_image(smem_f4, xs, img, r.halo_lo, r.nh);
     double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     bool bad = false;
     const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
     for (int ch = next_chunk(&s_next); ch < nchunk; ch = next_chunk(&s_next)) {
         const int i = r.lo + (ch << 5) + lane;
         if (i >= r.hi) continue;
-        const float4 pi = sm[i - r.halo_lo + 1];
+        const float4 pi = xs[i];
         const int nni = nn[i];
         const int ng = ((nni & 0xffff) + 3) >> 2;
         const uint2 *row = nl + i;
@@ -900,12 +961,10 @@ k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
              float4 *__restrict__ force, double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk,
              int *__restrict__ ctrl, ListSel ls, int n_pad, int s_cap, PairConst pc)
 {
-    __shared__ unsigned long long s_bar;
     const TileDesc t = tiles[blockIdx.x];
     const int h = list_half(ls, t.rep);
-    TileFill tf = tile_fill_init(&s_bar);
     force_tile<VIRIAL, KICK>(t, cell_start, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force, e_rep,
-                             w_rep, kk, ctrl, n_pad, s_cap, pc, tf);
+                             w_rep, kk, ctrl, n_pad, s_cap, pc, ls.img + (size_t)blockIdx.x * ls.img_stride);
 }
 
 // ---- inspection (parity tests, bench statistics) ----------------------------------------------
@@ -918,8 +977,10 @@ __device__ __forceinline__ unsigned entry_of(const uint2 *__restrict__ nl, int n
 
 __global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *__restrict__ nl0,
                                      const int *__restrict__ nn0, const int *__restrict__ hbase,
-                                     const int *__restrict__ atom_rep, const int *__restrict__ cur, size_t nl_stride,
-                                     int *__restrict__ counts, int *__restrict__ list, int n, int n_pad, int kmax)
+                                     const int *__restrict__ tileof, const unsigned short *__restrict__ inv,
+                                     int inv_stride, const int *__restrict__ atom_rep, const int *__restrict__ cur,
+                                     size_t nl_stride, int *__restrict__ counts, int *__restrict__ list, int n,
+                                     int n_pad, int kmax)
 {
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int h = cur[atom_rep[i]];
@@ -929,14 +990,16 @@ __global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *_
         const int cnt = nn[i] & 0xffff;
         counts[t] = cnt;
         for (int k = 0; k < cnt; ++k)
-            list[(size_t)t * kmax + k] = tag[hbase[i] + (int)(entry_of(nl, n_pad, i, k) >> 4) - 1];
+            list[(size_t)t * kmax + k] =
+                tag[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, n_pad, i, k) >> 4)]];
     }
 }
 
 __global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *__restrict__ nl0,
                                    const int *__restrict__ nn0, const int *__restrict__ hbase,
-                                   const int *__restrict__ atom_rep, const int *__restrict__ cur, size_t nl_stride,
-                                   unsigned long long *__restrict__ out, int n, int n_pad, float rc2)
+                                   const int *__restrict__ tileof, const unsigned short *__restrict__ inv,
+                                   int inv_stride, const int *__restrict__ atom_rep, const int *__restrict__ cur,
+                                   size_t nl_stride, unsigned long long *__restrict__ out, int n, int n_pad, float rc2)
 {
     unsigned long long entries = 0, inside = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
@@ -947,7 +1010,7 @@ __global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *
         const int cnt = nn[i] & 0xffff;
         entries += cnt;
         for (int k = 0; k < cnt; ++k) {
-            const float4 pj = pos[hbase[i] + (int)(entry_of(nl, n_pad, i, k) >> 4) - 1];
+            const float4 pj = pos[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, n_pad, i, k) >> 4)]];
             const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
             inside += d2 < rc2;
@@ -982,7 +1045,7 @@ size_t finish_smem(const tbsma_ctx *c)
 {
     return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax_o * finish_threads(c) * 2;
 }
-size_t gather_smem(const tbsma_ctx *c) { return (size_t)(c->tile_cap + 1) * 16; }
+size_t gather_smem(const tbsma_ctx *c) { return (size_t)c->img_cap * 16; }
 size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + (size_t)kInnerThreads * (c->kmax + 1) * 2; }
 InnerArgs inner_args(const tbsma_ctx *c)
 {
@@ -993,6 +1056,9 @@ InnerArgs inner_args(const tbsma_ctx *c)
     ia.nn = c->d_nn;
     ia.pos_build = c->d_pos_build;
     ia.cur = c->d_cur;
+    ia.img = c->d_img;
+    ia.img_stride = c->tile_cap;
+    ia.img_cap = c->img_cap;
     ia.nl_stride = (size_t)(c->kmax / 4) * c->n_pad;
     ia.n_stride = c->n_pad;
     ia.pos_outer = c->d_pos_outer;
@@ -1081,8 +1147,8 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     }
     first[R] = (int)k;
     free(Lr);
-    cudaFree(c->d_tiles); cudaFree(c->d_tile_first); cudaFree(c->d_work);
-    c->d_tiles = nullptr; c->d_tile_first = nullptr; c->d_work = nullptr;
+    cudaFree(c->d_tiles); cudaFree(c->d_tile_first); cudaFree(c->d_work); cudaFree(c->d_img); cudaFree(c->d_inv);
+    c->d_tiles = nullptr; c->d_tile_first = nullptr; c->d_work = nullptr; c->d_img = nullptr; c->d_inv = nullptr;
     e = cudaMalloc((void **)&c->d_tiles, sizeof(TileDesc) * (size_t)(n_tiles ? n_tiles : 1));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_tile_first, sizeof(int) * (size_t)(R + 1));
     if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_work, sizeof(int) * (size_t)(2 + 2 * n_tiles));
@@ -1094,7 +1160,14 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     free(first);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? TBSMA_ENOMEM : TBSMA_ECUDA;
     c->n_tiles = (int)n_tiles;
-    c->tile_cap = rec_cap < cap ? rec_cap : cap;   // shared-memory image sized to the largest halo expected
+    c->tile_cap = rec_cap < cap ? rec_cap : cap;   // halo records a tile may hold
+    // image: the sentinel + eight colour classes of records (k_tile_place); room for classes 1/8 + 64 fuller than even
+    c->img_cap = c->tile_cap + c->tile_cap / 8 + 64 + 1;
+    if (c->img_cap > TBSMA_TILE_MAX_RECORDS + 1) c->img_cap = TBSMA_TILE_MAX_RECORDS + 1;
+    if (c->img_cap < c->tile_cap + 1) c->img_cap = c->tile_cap + 1;
+    e = cudaMalloc((void **)&c->d_img, sizeof(unsigned short) * (size_t)(n_tiles ? n_tiles : 1) * c->tile_cap);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_inv, sizeof(unsigned short) * (size_t)(n_tiles ? n_tiles : 1) * c->img_cap);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? TBSMA_ENOMEM : TBSMA_ECUDA;
     c->tile_cell_cap = (cell_cap + 3) & ~3;
     c->own_cap = own_cap;
     // opt in to > 48 KB of dynamic shared memory
@@ -1127,14 +1200,21 @@ cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int3
     sa.s_cap = c->tile_cap; sa.cell_cap = c->tile_cell_cap;
     FinishArgs fa;
     fa.cell_start = c->d_cell_start; fa.nl_tmp = ol_tmp; fa.nn_tmp = c->d_nn_tmp; fa.newslot = c->d_newslot;
-    fa.oldof = c->d_oldof; fa.nl = ol; fa.nn = c->d_nn_o; fa.hbase = c->d_hbase; fa.n_pad = c->n_pad;
+    fa.oldof = c->d_oldof; fa.nl = ol; fa.nn = c->d_nn_o; fa.hbase = c->d_hbase; fa.tileof = c->d_tileof;
+    fa.img = c->d_img; fa.img_stride = c->tile_cap; fa.n_pad = c->n_pad;
     fa.s_cap = c->tile_cap;
+    PlaceArgs pa;
+    pa.cell_start = c->d_cell_start; pa.oldof = c->d_oldof; pa.pos_sorted = c->d_tmp_pos; pa.geom = c->d_geom;
+    pa.img = c->d_img; pa.inv = c->d_inv; pa.img_stride = c->tile_cap; pa.inv_stride = c->img_cap;
+    pa.img_cap = c->img_cap; pa.inv_h = c->balance && c->class_h > 0.0 ? (float)(1.0 / c->class_h) : 0.f;
+    pa.ctrl = c->d_ctrl;
     const int gw = c->n_tiles < 2 * c->n_sm ? c->n_tiles : 2 * c->n_sm;
     k_tile_scan<<<gw, kScanThreads, scan_smem(c), st>>>(c->d_tiles, c->d_work, c->n_tiles, sa);
+    k_tile_place<<<gw, 256, 0, st>>>(c->d_tiles, c->d_work, c->n_tiles, pa);
     k_tile_finish<<<gw, finish_threads(c), finish_smem(c), st>>>(c->d_tiles, c->d_work, c->n_tiles, fa);
     k_tile_permute<<<grid_for(c, n, 256, 8), 256, 0, st>>>(pos, vel, tag, c->d_pos_outer, c->d_atom_rep, dv,
                                                           c->d_oldof, c->d_tmp_pos, c->d_tmp4, c->d_tmp_tag, n);
-    c->launches += 3;
+    c->launches += 4;
     return cudaGetLastError();
 }
 
@@ -1181,6 +1261,8 @@ static ListSel list_sel(const tbsma_ctx *c, int sync_level)
     ls.sync_level = sync_level;
     ls.nl_stride = (size_t)(c->kmax / 4) * c->n_pad;
     ls.n_stride = c->n_pad;
+    ls.img = c->d_img;
+    ls.img_stride = c->tile_cap;
     return ls;
 }
 
@@ -1215,7 +1297,8 @@ cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, in
                                             cudaStream_t st)
 {
     k_get_neighbors_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(tag, reinterpret_cast<const uint2 *>(c->d_nlist),
-                                                                   c->d_nn, c->d_hbase, c->d_atom_rep, c->d_cur,
+                                                                   c->d_nn, c->d_hbase, c->d_tileof, c->d_inv, c->img_cap,
+                                                                   c->d_atom_rep, c->d_cur,
                                                                    (size_t)(c->kmax / 4) * c->n_pad, counts, list, (int)c->n,
                                                                    c->n_pad, c->kmax);
     c->launches++;
@@ -1226,7 +1309,8 @@ cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsig
                                           cudaStream_t st)
 {
     k_count_pairs_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(pos, reinterpret_cast<const uint2 *>(c->d_nlist),
-                                                                 c->d_nn, c->d_hbase, c->d_atom_rep, c->d_cur,
+                                                                 c->d_nn, c->d_hbase, c->d_tileof, c->d_inv, c->img_cap,
+                                                                 c->d_atom_rep, c->d_cur,
                                                                  (size_t)(c->kmax / 4) * c->n_pad, d_out2, (int)c->n, c->n_pad,
                                                                  c->pc.rc2);
     c->launches++;
