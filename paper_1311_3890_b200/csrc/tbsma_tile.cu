@@ -309,7 +309,7 @@ __device__ __forceinline__ unsigned byte_of(unsigned long long v, int c) { retur
 
 // ---- K2: finish.  One thread per FINAL slot of the tile: reads the temporary row of the atom that
 // moves there, translates every partner to its final position (byte offset of its record in the
-// tile's shared-memory image, record k at (k + 1) * 16, the sentinel at 0), and writes the row sorted
+// tile's shared-memory image, 16 x the index k_tile_place gave it, the sentinel at 0), and writes the row sorted
 // by CLASS (bank group of the record = record index mod 8; stable inside a class), starting with the
 // class equal to the atom's lane mod 8: the inner build keeps this order when it filters, so its kept
 // entries come out grouped by class as well, and while it gathers the candidates the eight lanes served by
@@ -445,7 +445,7 @@ __global__ void k_stage_copy(const float4 *__restrict__ pos, const float4 *__res
 // The records of the halo go to the image indices k_tile_place chose for them (see there): one coalesced read of
 // the slot range, scattered 16-byte stores.  The caller has made sure (__syncthreads) that nobody still reads a
 // previous image.  (A contiguous image was one cp.async.bulk; spreading the records over the bank groups is worth
-// more than the copy engine: a third fewer shared-memory wavefronts in the gather passes.)
+// more than the copy engine: a fifth fewer shared-memory wavefronts in the gather passes, 62 % fewer bank conflicts.)
 __device__ __forceinline__ void fill_image(float4 *sm, const float4 *__restrict__ src,
                                            const unsigned short *__restrict__ img, int halo_lo, int nh)
 {
