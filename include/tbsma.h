@@ -205,9 +205,12 @@ int tbsma_set_graph(tbsma_ctx *ctx, int32_t enable);
  * precedes the gather passes.  Membership of the lists is decided by the predicate of D:A6 either way. */
 int tbsma_set_async(tbsma_ctx *ctx, int32_t enable, double margin);
 
-/* Shared-memory variant only: when enabled (default 1) tbsma_md_step / tbsma_md_run use a second stream of the
- * context for the asynchronous list renewal above; both streams are joined before the step ends, so the caller sees
- * ordinary stream semantics.  Off: the same kernels run one after the other on `stream`. */
+/* Shared-memory variant only: how the asynchronous list renewal above runs beside the gather passes.
+ * 2 (default): on `stream` itself, the density pass launched as a PROGRAMMATIC DEPENDENT of the filter kernel (which
+ * signals griddepcontrol.launch_dependents at once; the density pass reads the half of the list buffers the filter
+ * kernel does not write), so that both run together without a second stream; 1: the filter kernel on a second,
+ * high-priority stream of the context, forked and joined inside the step; 0: the same kernels one after the other.
+ * The caller sees ordinary stream semantics in all three; results are bitwise identical. */
 int tbsma_set_overlap(tbsma_ctx *ctx, int32_t enable);
 
 /* Shared-memory variant: where the records of a tile sit in its shared-memory image.  The gather passes read one

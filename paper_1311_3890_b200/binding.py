@@ -239,7 +239,7 @@ class Context:
         _check(lib().tbsma_set_async(self._h, int(bool(enable)), float(margin)), "tbsma_set_async")
 
     def set_overlap(self, enable):
-        _check(lib().tbsma_set_overlap(self._h, int(bool(enable))), "tbsma_set_overlap")
+        _check(lib().tbsma_set_overlap(self._h, int(enable)), "tbsma_set_overlap")
 
     def set_timing(self, enable):
         _check(lib().tbsma_set_timing(self._h, int(bool(enable))), "tbsma_set_timing")

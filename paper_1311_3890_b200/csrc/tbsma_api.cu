@@ -204,7 +204,7 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         if (ev) CK(cudaEventRecord(ev[0], st));
         CK(tbsma_launch_integrate_pre(c, pos, vel, force, tag, a, st));
         if (ev) CK(cudaEventRecord(ev[1], st));
-        bool forked = false;
+        bool forked = false, early = false, joined = false;
         if (tiles) {
             // Replicas whose atoms moved far enough get a new list.  With new cells and candidates (dirty == 2, rare)
             // the rebuild precedes the gather passes, which then read the freshly written half of the list buffers.
@@ -249,7 +249,12 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
             }
             // (after the chain: idle, its kernels take 1.5 us each on an empty GPU, but each would wait for room on every SM
             // behind a filter kernel already running)
-            if (async && c->overlap && !c->timing && c->aux_stream) {
+            if (async && c->overlap == 2 && !c->timing && st) {
+                CK(tbsma_launch_tile_inner(c, pos, 0, st));
+                early = true;
+                forked = true;       // (nothing to join: same stream)
+                joined = true;
+            } else if (async && c->overlap && !c->timing && c->aux_stream) {
                 CK(cudaEventRecord(c->ev_fork, st));
                 CK(cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
                 CK(tbsma_launch_tile_inner(c, pos, 0, c->aux_stream));
@@ -262,13 +267,13 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         }
         const int sync_level = async ? 2 : 1;
         if (ev) CK(cudaEventRecord(ev[2], st));
-        if (tiles) CK(tbsma_launch_density_tile(c, pos, sync_level, st));
+        if (tiles) CK(tbsma_launch_density_tile(c, pos, sync_level, st, early));
         else CK(tbsma_launch_density(c, pos, st));
         if (ev) CK(cudaEventRecord(ev[3], st));
         if (tiles) CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, sync_level, st));
         else CK(tbsma_launch_force(c, force, e_rep, w_rep, kk, st));
         if (ev) CK(cudaEventRecord(ev[4], st));
-        if (forked) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
+        if (forked && !joined) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
         CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
         if (ev) CK(cudaEventRecord(ev[5], st));
     }
@@ -314,7 +319,7 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->tile_layers = 2;
     c->tile_threads = 256;
     c->use_graph = 1;
-    c->overlap = 1;
+    c->overlap = 2;
     c->stagger = 1;
     c->balance = 1;
     c->class_h = params->r0 / sqrt(2.0);
@@ -434,7 +439,7 @@ int tbsma_set_async(tbsma_ctx *c, int32_t enable, double margin)
 int tbsma_set_overlap(tbsma_ctx *c, int32_t enable)
 {
     if (!c) return TBSMA_EINVAL;
-    c->overlap = enable != 0;
+    c->overlap = enable;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     return TBSMA_OK;
 }

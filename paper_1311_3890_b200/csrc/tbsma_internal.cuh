@@ -219,7 +219,8 @@ cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float
                                     cudaStream_t st);
 // sync_level: the gather passes read the freshly written half of the list buffers for replicas with
 // dirty >= sync_level (their rebuild ran ahead of the launch), the half in use for all others.
-cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st);
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st,
+                                      bool early = false);
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kick,
                                     int sync_level, cudaStream_t st);
 cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,

@@ -695,6 +695,9 @@ k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, c
              int which, int n_tiles)
 {
     extern __shared__ float4 smem_f4[];
+    // the density pass may be launched as a programmatic dependent of this kernel (it reads the half of the list
+    // buffers this kernel does not write): let it start at once
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     const int *__restrict__ wl = work + 2 + which * n_tiles;
     const int nu = work[which] * nsplit;
     if ((int)blockIdx.x >= nu) return;
@@ -1266,14 +1269,25 @@ static ListSel list_sel(const tbsma_ctx *c, int sync_level)
     return ls;
 }
 
-cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st)
+// early: the launch may begin while the kernel before it on the stream (the filter pass of the replicas renewing
+// their lists, whose output this launch does not read) is still running: programmatic dependent launch
+cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st, bool early)
 {
-    k_density_tile<<<c->n_tiles, c->tile_threads, gather_smem(c), st>>>(c->d_tiles, c->d_cell_start, pos,
-                                                                       reinterpret_cast<const uint2 *>(c->d_nlist),
-                                                                       c->d_nn, c->d_xs, c->d_ctrl, list_sel(c, sync_level),
-                                                                       c->n_pad, c->tile_cap, c->pc);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(c->n_tiles);
+    cfg.blockDim = dim3(c->tile_threads);
+    cfg.dynamicSmemBytes = gather_smem(c);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = early ? 1 : 0;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, k_density_tile, (const TileDesc *)c->d_tiles, (const int *)c->d_cell_start,
+                                             pos, reinterpret_cast<const uint2 *>(c->d_nlist), (const int *)c->d_nn, c->d_xs,
+                                             c->d_ctrl, list_sel(c, sync_level), c->n_pad, c->tile_cap, c->pc);
     c->launches++;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kk,

@@ -197,7 +197,7 @@ def test_call_order_and_arguments(B):
     assert e.value.code == B.EINVAL
 
 
-def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None, overlap=True,
+def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None, overlap=2,
                stagger=True, async_inner=True, conditional=True):
     ctx, st = setup(B, w, variant=variant, tile=tile, stagger=stagger)
     ctx.set_graph(graph, conditional=conditional)
@@ -299,14 +299,16 @@ def test_replicas_are_independent_and_ragged_batch_matches_single_runs(B, varian
         assert np.array_equal(xb[s], ss.untag(ss.pos))          # bit-identical: no cross-replica effect
 
 
+@pytest.mark.parametrize("overlap", [1, 2])
 @pytest.mark.parametrize("graph", [True, False])
-def test_two_stream_overlap_is_bitwise_identical(B, graph):
-    """the rebuild chain + rebuilt replicas on the second stream (tbsma_set_overlap) change nothing: a batch with
-    10 K and 298 K replicas (so that some rebuild while others do not) gives the same bits either way"""
+def test_overlapped_list_renewal_is_bitwise_identical(B, graph, overlap):
+    """the filter pass beside the gather passes (tbsma_set_overlap: 1 = second stream, 2 = the density pass launched as
+    its programmatic dependent) changes nothing: a batch with 10 K and 298 K replicas (so that some rebuild while
+    others do not) gives the same bits as the same kernels one after the other"""
     w = W.config3(6, seed=11, length=60.0)
     n_steps = 80
-    ca, a = run_gpu_md(B, w, n_steps, variant=2, graph=graph, overlap=True, virial=True)
-    cb, b = run_gpu_md(B, w, n_steps, variant=2, graph=graph, overlap=False, virial=True)
+    ca, a = run_gpu_md(B, w, n_steps, variant=2, graph=graph, overlap=overlap, virial=True)
+    cb, b = run_gpu_md(B, w, n_steps, variant=2, graph=graph, overlap=0, virial=True)
     sa, sb = ca.get_stats(), cb.get_stats()
     assert sa == sb
     assert 0 < sa["n_replica_builds"] < w.n_replicas * n_steps and sa["n_build_passes"] < n_steps
