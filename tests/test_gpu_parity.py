@@ -571,17 +571,17 @@ def test_md_run_host_matches_device_path(B):
     assert e[0] == pytest.approx(st.e_rep.item(), rel=1e-12) and k[0] == pytest.approx(st.ekin.item(), rel=1e-12)
 
 
-@pytest.mark.parametrize("which", ["config3", "config5a"])
+@pytest.mark.parametrize("which", ["config3", "config4", "config5a", "config5b"])
 def test_full_size_sampled_parity(B, which):
     """BASELINE full sizes, in the configuration bench.py times: sampled atoms recomputed one by one
     by the oracle from scratch (brute force over the whole replica)."""
-    w = W.config3() if which == "config3" else W.config5a()
+    w = {"config3": W.config3, "config4": W.config4, "config5a": W.config5a, "config5b": W.config5b}[which]()
     ctx, st = setup(B, w)
     ctx.compute(st.pos, st.force, st.e_rep, None)
     torch.cuda.synchronize()
     assert ctx.status() == 0
     rng = np.random.default_rng(0)
-    m = 48 if which == "config3" else 24
+    m = 48 if which in ("config3", "config4") else 24
     idx = np.sort(rng.choice(w.n_atoms, m, replace=False))
     s = oracle.compute_sample(w.x64(), w.r_cut, idx, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, periodic=w.periodic)
     fe = st.untag(st.force)
@@ -595,13 +595,42 @@ def test_full_size_sampled_parity(B, which):
     entries, pairs = ctx.count_pairs(st.pos)
     assert entries % 2 == 0 and pairs % 2 == 0
     # whole-replica energy against the linked-cell oracle for one replica / a 10^6-atom box
-    if which == "config3":
-        r = 200
+    if which in ("config3", "config4"):
+        r = 200 if which == "config3" else 1234
         sub = w.take(r, r + 1)
         oc = oracle.compute(sub.x64(), w.r_cut, lo=sub.box_lo, hi=sub.box_hi, cells=True)
         assert abs(st.e_rep[r].item() - oc["e_rep"][0]) <= E_REL * abs(oc["e_rep"][0])
+    elif which == "config5b":
+        oc = oracle.compute(w.x64(), w.r_cut, lo=w.box_lo, hi=w.box_hi, cells=True)
+        assert abs(st.e_rep[0].item() - oc["e_rep"][0]) <= E_REL * abs(oc["e_rep"][0])
+        assert_forces(f, oc["f"])
+        assert pairs == oc["n_pairs_directed"]
     else:
         oc = oracle.compute(w.x64(), w.r_cut, lo=w.box_lo, hi=w.box_hi, periodic=1, cells=True)
         assert abs(st.e_rep[0].item() - oc["e_rep"][0]) <= E_REL * abs(oc["e_rep"][0])
         assert_forces(f, oc["f"])
         assert pairs == oc["n_pairs_directed"]
+
+
+def test_full_size_trajectory_in_bench_configuration(B):
+    """config 3 at full size with every default bench.py runs with (tile variant, colour placement, staggered first
+    rebuilds, asynchronous list renewal beside the gather passes, conditional graph node): 40 steps, then three replicas
+    (a 10 K one, a 298 K one that has rebuilt its list, the last one) are compared with the oracle run of that replica
+    ALONE -- positions, velocities, per-replica energies"""
+    w = W.config3()
+    n_steps = 40
+    ctx, st = run_gpu_md(B, w, n_steps)
+    assert ctx.status() == 0 and ctx.get_variant() == 2
+    stats = ctx.get_stats()
+    assert stats["n_replica_builds"] >= 128          # every 298 K replica has renewed its list at least once
+    x = st.untag(st.pos)[:, :3].astype(np.float64)
+    v = st.untag(st.vel)[:, :3].astype(np.float64)
+    e_rep, ekin = st.e_rep.cpu().numpy(), st.ekin.cpu().numpy()
+    for r in (5, 200, 255):
+        sub = w.take(r, r + 1)
+        md = run_oracle_md(sub, n_steps)
+        sl = slice(w.offsets[r], w.offsets[r + 1])
+        assert traj_rms(x[sl], md.x) <= TRAJ_RMS
+        assert np.abs(v[sl] - md.v).max() < 2e-5
+        assert abs(e_rep[r] - md.e_rep[0]) <= 10 * E_REL * abs(md.e_rep[0])     # 40 steps of fp32 drift, not one evaluation
+        assert abs(ekin[r] - md.ekin_rep[0]) <= 2e-3 * md.ekin_rep[0]
