@@ -52,6 +52,11 @@ def make_workload(cfg, rank=0, replicas=None):
         return W.config5a(64, 5 + seed_shift)
     if cfg == "5b":
         return W.config5b(6 + seed_shift)
+    if cfg.startswith("paper"):       # paper:k:T[:replicas], e.g. paper:12:10 = the largest row of the paper's Table 2
+        f = cfg.split(":")
+        k = int(f[1]) if len(f) > 1 else 1
+        T = float(f[2]) if len(f) > 2 else 10.0
+        return W.paper_wire(k, T, replicas or (int(f[3]) if len(f) > 3 else 1), 7 + seed_shift)
     raise SystemExit(f"unknown --config {cfg}")
 
 
@@ -161,7 +166,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=60)
-    ap.add_argument("--config", default="3", choices=["1", "2", "3", "4", "5a", "5b"])
+    ap.add_argument("--config", default="3",
+                    help="1, 2, 3, 4, 5a, 5b (BASELINE.json configs) or paper:k:T[:replicas] (shapes of the paper's Table 2)")
     ap.add_argument("--replicas", type=int, default=None, help="override the replica count of config 3/4")
     ap.add_argument("--impl", default="tbsma", choices=["tbsma", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

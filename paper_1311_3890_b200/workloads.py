@@ -243,6 +243,26 @@ def config4(n_rep=2048, seed=4):
                           seed, jitter_layers=True, cfg=4)
 
 
+def paper_wire(k=1, T=10.0, n_rep=1, seed=7):
+    """The shapes of the paper's own benchmark (Table 2): unstretched [100] Au wires of
+    D0 = 3.1 nm and L0 = 20.4 k nm (8 850 k atoms; the paper's sizes are 8 823 + 8 850 (k - 1), with a 27-atom notch that
+    is left out here), r_cut = 5.8 A, buffer 0.29 A, dt = 2 fs, at 10 K or 298 K, not pulled.  The paper's
+    thermostat is Nose-Hoover; Langevin (gamma = 1/ps) stands in for it.  n_rep > 1 batches identical wires with their own
+    seeds (the paper runs one per GPU)."""
+    x = fcc_wire(31.0, 204.0 * k)
+    fl = np.zeros(len(x), np.int32)
+    wires, flags, vels, seeds = [], [], [], []
+    for r in range(n_rep):
+        s = seed * 100003 + r
+        wires.append(x); flags.append(fl); seeds.append(s)
+        vels.append(maxwell_velocities(len(x), T, s, fl == 0))
+    w = _assemble(f"paper_table2_{n_rep}x_wire_3.1x{20.4 * k:.1f}nm_{T:g}K", wires, flags, vels, [T] * n_rep, seeds,
+                  [0.0] * n_rep, 1e-3, meta=dict(config="paper", k=k))
+    w.r_cut = 5.8
+    w.skin = 0.29
+    return w
+
+
 def config5a(ncell=64, seed=5):
     """BASELINE config 5 (bulk): periodic FCC ncell^3 cells, sigma = 0.05 A displacements,
     NVE, neighbour rebuild every 10 steps.  ncell = 64 -> 1 048 576 atoms."""
