@@ -5,7 +5,7 @@
 // atoms ordered along the wire axis.  With cells numbered z-slowest, a run of z-layers of
 // cells ("tile") and its one-layer halo are CONTIGUOUS index ranges, so one CTA can stage every
 // position its atoms will ever gather (a few thousand records) in shared memory with one coalesced
-// copy and serve all neighbour gathers from there.  That allows
+// read of the range and serve all neighbour gathers from there.  That allows
 //   * 16-bit neighbour entries (byte offsets into the tile's shared-memory image): half the list
 //     bytes of the int32 list, which is the dominant HBM stream of both passes;
 //   * atoms ordered inside each layer by neighbour count (longest lists first), so the 32 lanes of
@@ -13,17 +13,22 @@
 //     core atoms 86);
 //   * each atom's list ordered so that at step p lane l reads a record of bank group (l + p) mod 8:
 //     the eight lanes served by one shared-memory wavefront of a 128-bit load then hit eight
-//     different 16-byte bank groups (summation order is free, A15).
+//     different 16-byte bank groups (summation order is free, A15);
+//   * the records placed in the image by the colour of a spatial hash (k_tile_place), so that every
+//     atom's neighbours are spread evenly over the eight bank groups and that order has few holes.
 // Membership is the fp32 predicate of D:A6, operation for operation, as in tbsma_cells.cu.
 //
 // Two-level lists.  Scanning 27 cells costs about five force passes per atom, and at 298 K a replica
 // needs a fresh list every ~12 steps (fewer rebuilds are why 10 K runs faster).  So the cell
-// scan builds a CANDIDATE list with the larger radius r_cut + skin + S (S = outer_skin, 1 A): K1-K3
-// below, rarely.  The list the gather passes read (radius r_cut + skin, the paper's r_buff list)
-// is filtered from the candidates by the tile that owns the atom (k_tile_inner) in the step in which
-// the replica's atoms moved more than skin/2: ~2.3 candidates per kept entry instead of ~9.  A candidate list stays valid while no atom moved more than S/2 since
-// it was built; the inner build checks that (status flag) and asks for new candidates one rebuild
-// earlier (want_outer).  Slots (and so the u16 offsets) only change when candidates are rebuilt.
+// scan builds a CANDIDATE list with the larger radius r_cut + skin + S (S = outer_skin, 2 A by default):
+// K1 (scan), K1b (place), K2 (finish), K3 (permute) below, rarely.  The list the gather passes read
+// (radius r_cut + skin, the paper's r_buff list) is filtered from the candidates by the tile that
+// owns the atom (k_tile_inner) when the replica's atoms have moved skin/2 (less a margin when the filter
+// pass runs beside the gather passes, tbsma_set_async): ~2.7 candidates per kept entry instead of ~9.
+// A candidate list stays valid while no atom moved more than S/2 since it was built; the inner build
+// checks that (status flag) and asks for new candidates one rebuild earlier (want_outer).  Slots (and
+// so the u16 offsets) only change when candidates are rebuilt.  The list, its counts and its build
+// positions exist twice (ListSel): a renewal writes the half not in use, the step's last kernel swaps.
 #include "tbsma_internal.cuh"
 
 namespace {
