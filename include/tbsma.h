@@ -148,6 +148,17 @@ int tbsma_md_run_host(tbsma_ctx *ctx, float *h_pos, float *h_vel, float *h_force
                       const double *h_slab_disp0, const double *h_slab_rate, int32_t rebuild_every,
                       double *h_replica_energy, double *h_replica_virial, double *h_replica_ekin);
 
+/* Observables of the tensile tests.  Eq.5 is garbled in the source (D:A11); it stands for the virial
+ * stress  sigma_ab = -(W_ab + K_ab) / V,  tension positive, with W_ab the virial tbsma_compute / tbsma_md_step return,
+ * K_ab = sum_i m v_a v_b over the dynamic atoms, and V the constant "hard-sphere" volume of the wire, which is the
+ * caller's: tbsma_kinetic_tensor writes K of every replica (n_replicas x 6 doubles, eV, xx yy zz xy xz yz) for the
+ * velocities in d_vel (flags from d_pos); tbsma_stress combines them (d_k may be NULL = 0 K) with d_volume
+ * (n_replicas doubles, A^3) into d_sigma (n_replicas x 6, eV/A^3; 1 eV/A^3 = 160.21766208 GPa).  Strain (Eq.4)
+ * is (L - L0) / L0 with L - L0 the slab displacement the caller itself supplies to tbsma_md_step. */
+int tbsma_kinetic_tensor(tbsma_ctx *ctx, const float *d_pos, const float *d_vel, double *d_replica_kinetic, void *stream);
+int tbsma_stress(tbsma_ctx *ctx, const double *d_replica_virial, const double *d_replica_kinetic,
+                 const double *d_volume, double *d_sigma, void *stream);
+
 /* Neighbour lists in TAG space for parity checks: d_counts[t] and d_list[t*max_neighbors + k]
  * (k < count, unsorted) for the atom whose tag is t.  d_tag as left by tbsma_build_cells. */
 int tbsma_get_neighbors(tbsma_ctx *ctx, const int32_t *d_tag, int32_t *d_counts, int32_t *d_list,

@@ -3,7 +3,8 @@
 TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's
 cpu_baseline / --impl reference legs.  Never imported by paper_1311_3890_b200 (the product),
 and it imports nothing from it.  Every function is a thin marshalling layer; all arithmetic
-is in the C file, which cites the paper line by line.
+is in the C file, which cites the paper line by line (the observables of P:79-87 -- kinetic
+tensor, virial stress, strain -- are plain numpy in oracle/observables.py).
 """
 import ctypes as C
 import os

@@ -19,7 +19,7 @@ FLAG_NLIST_OVERFLOW, FLAG_OUT_OF_BOX, FLAG_NONFINITE, FLAG_SKIN_VIOLATED, FLAG_T
 EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
-    "tbsma_count_pairs", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
+    "tbsma_count_pairs", "tbsma_kinetic_tensor", "tbsma_stress", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
     "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
@@ -68,6 +68,8 @@ def lib():
         L.tbsma_md_run.argtypes = [vp, vp, vp, vp, vp, dbl, vp, dbl, vp, C.c_uint64, i64, vp, vp, i32, vp, vp, vp, vp]
         L.tbsma_md_run_host.argtypes = [vp, vp, vp, vp, vp, dbl, vp, dbl, vp, C.c_uint64, i64, vp, vp, i32, vp, vp, vp]
         L.tbsma_get_neighbors.argtypes = [vp, vp, vp, vp, vp]
+        L.tbsma_kinetic_tensor.argtypes = [vp, vp, vp, vp, vp]
+        L.tbsma_stress.argtypes = [vp, vp, vp, vp, vp, vp]
         L.tbsma_count_pairs.argtypes = [vp, vp, C.POINTER(i64), C.POINTER(i64), vp]
         L.tbsma_status.argtypes = [vp, C.POINTER(C.c_uint32)]
         L.tbsma_clear_status.argtypes = [vp]
@@ -189,6 +191,12 @@ class Context:
                                        _hp(T), float(gamma_per_fs), _hp(seed), int(step0), int(n_steps),
                                        _hp(slab_disp0), _hp(slab_rate), int(rebuild_every), _hp(replica_energy),
                                        _hp(replica_virial), _hp(replica_ekin)), "tbsma_md_run_host")
+
+    def kinetic_tensor(self, pos, vel, k_rep, stream=None):
+        _check(lib().tbsma_kinetic_tensor(self._h, _dp(pos), _dp(vel), _dp(k_rep), _stream(stream)), "tbsma_kinetic_tensor")
+
+    def stress(self, w_rep, k_rep, volume, sigma, stream=None):
+        _check(lib().tbsma_stress(self._h, _dp(w_rep), _dp(k_rep), _dp(volume), _dp(sigma), _stream(stream)), "tbsma_stress")
 
     def get_neighbors(self, tag, counts, nlist, stream=None):
         _check(lib().tbsma_get_neighbors(self._h, _dp(tag), _dp(counts), _dp(nlist), _stream(stream)),

@@ -724,6 +724,24 @@ int tbsma_md_run_host(tbsma_ctx *c, float *h_pos, float *h_vel, float *h_force, 
     return TBSMA_OK;
 }
 
+int tbsma_kinetic_tensor(tbsma_ctx *c, const float *d_pos, const float *d_vel, double *d_k, void *stream)
+{
+    if (!c || !d_pos || !d_vel || !d_k) return TBSMA_EINVAL;
+    if (!c->d_geom) return TBSMA_ESTATE;
+    if (c->n == 0) return TBSMA_OK;
+    CK(tbsma_launch_kinetic_tensor(c, (const float4 *)d_pos, (const float4 *)d_vel, d_k, (cudaStream_t)stream));
+    return TBSMA_OK;
+}
+
+int tbsma_stress(tbsma_ctx *c, const double *d_w, const double *d_k, const double *d_volume, double *d_sigma, void *stream)
+{
+    if (!c || !d_w || !d_volume || !d_sigma) return TBSMA_EINVAL;
+    if (!c->d_geom) return TBSMA_ESTATE;
+    if (c->R == 0) return TBSMA_OK;
+    CK(tbsma_launch_stress(c, d_w, d_k, d_volume, d_sigma, (cudaStream_t)stream));
+    return TBSMA_OK;
+}
+
 int tbsma_get_neighbors(tbsma_ctx *c, const int32_t *d_tag, int32_t *d_counts, int32_t *d_list, void *stream)
 {
     if (!c || !d_tag || !d_counts || !d_list) return TBSMA_EINVAL;

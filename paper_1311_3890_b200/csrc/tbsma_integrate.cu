@@ -141,7 +141,71 @@ __global__ void k_set_stagger(float *__restrict__ stagger, int R, int enable)
     stagger[r] = f * f;
 }
 
+// ---- observables of the tensile tests (Eq.5 as read in D:A11) -----------------------
+// K_ab = sum_i m v_i,a v_i,b over the dynamic atoms of every replica (eV; xx yy zz xy xz yz).  Atoms of a replica are
+// contiguous, so nearly every warp belongs to one replica: warp shuffle sums, one fp64 atomic per warp and component.
+__global__ void __launch_bounds__(256)
+k_kinetic_tensor(const float4 *__restrict__ pos, const float4 *__restrict__ vel, const int *__restrict__ atom_rep,
+                 double *__restrict__ k_rep, double m_over_c, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    int r = -1;
+    double k[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    if (i < n) {
+        r = atom_rep[i];
+        if ((__float_as_int(pos[i].w) & 3) == 0) {
+            const float4 v = vel[i];
+            const double vx = v.x, vy = v.y, vz = v.z;
+            k[0] = m_over_c * vx * vx; k[1] = m_over_c * vy * vy; k[2] = m_over_c * vz * vz;
+            k[3] = m_over_c * vx * vy; k[4] = m_over_c * vx * vz; k[5] = m_over_c * vy * vz;
+        }
+    }
+    const int r0 = __shfl_sync(0xffffffffu, r, 0);
+    const bool uniform = __all_sync(0xffffffffu, r == r0);
+    if (uniform) {
+        if (r0 < 0) return;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+            double s = k[c];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) atomicAdd(k_rep + 6 * (size_t)r0 + c, s);
+        }
+    } else if (r >= 0) {
+#pragma unroll
+        for (int c = 0; c < 6; ++c) atomicAdd(k_rep + 6 * (size_t)r + c, k[c]);
+    }
+}
+
+// sigma_ab = -(W_ab + K_ab) / V, tension positive
+__global__ void k_stress(const double *__restrict__ w_rep, const double *__restrict__ k_rep,
+                         const double *__restrict__ volume, double *__restrict__ sigma, int R)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= 6 * R) return;
+    sigma[q] = -(w_rep[q] + (k_rep ? k_rep[q] : 0.0)) / volume[q / 6];
+}
+
 }  // namespace
+
+cudaError_t tbsma_launch_kinetic_tensor(tbsma_ctx *c, const float4 *pos, const float4 *vel, double *k_rep, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(k_rep, 0, sizeof(double) * 6 * (size_t)c->R, st);
+    if (e != cudaSuccess) return e;
+    const int n = (int)c->n;
+    k_kinetic_tensor<<<(n + 255) / 256, 256, 0, st>>>(pos, vel, c->d_atom_rep, k_rep, c->prm.mass_amu / TBSMA_ACC, n);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_stress(tbsma_ctx *c, const double *w_rep, const double *k_rep, const double *volume,
+                                double *sigma, cudaStream_t st)
+{
+    k_stress<<<(6 * c->R + 255) / 256, 256, 0, st>>>(w_rep, k_rep, volume, sigma, c->R);
+    c->launches++;
+    return cudaGetLastError();
+}
 
 cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st)
 {

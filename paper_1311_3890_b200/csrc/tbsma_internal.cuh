@@ -249,3 +249,6 @@ cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, c
                                        const int32_t *tag, const StepArgs &a, cudaStream_t st);
 cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st);
 cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st);
+cudaError_t tbsma_launch_kinetic_tensor(tbsma_ctx *c, const float4 *pos, const float4 *vel, double *k_rep, cudaStream_t st);
+cudaError_t tbsma_launch_stress(tbsma_ctx *c, const double *w_rep, const double *k_rep, const double *volume,
+                                double *sigma, cudaStream_t st);

@@ -634,3 +634,39 @@ def test_full_size_trajectory_in_bench_configuration(B):
         assert np.abs(v[sl] - md.v).max() < 2e-5
         assert abs(e_rep[r] - md.e_rep[0]) <= 10 * E_REL * abs(md.e_rep[0])     # 40 steps of fp32 drift, not one evaluation
         assert abs(ekin[r] - md.ekin_rep[0]) <= 2e-3 * md.ekin_rep[0]
+
+
+def test_stress_and_kinetic_tensor_match_oracle(B):
+    """tbsma_kinetic_tensor / tbsma_stress (Eq.5 as read in A11) after 30 Langevin steps with grips and pulling: K from
+    the same fp32 velocities to rounding, tr K = 2 E_kin of the force pass, sigma = -(W + K) / V against the numpy
+    oracle fed with the fp64 oracle's virial of the final positions"""
+    from oracle import observables as ob
+    w = W.config3(4, seed=23, length=60.0)
+    ctx, st = run_gpu_md(B, w, 30, virial=True)
+    R = w.n_replicas
+    k = torch.full((R, 6), -1.0, dtype=torch.float64, device="cuda")
+    sig = torch.zeros(R, 6, dtype=torch.float64, device="cuda")
+    n_r = np.diff(w.offsets).astype(np.float64)
+    vol = n_r * W.A_LATTICE ** 3 / 4          # one fcc atomic volume per atom, held constant (P:87)
+    d_vol = torch.from_numpy(vol).cuda()
+    ctx.kinetic_tensor(st.pos, st.vel, k)
+    ctx.stress(st.w_rep, k, d_vol, sig)
+    torch.cuda.synchronize()
+    v = st.untag(st.vel)[:, :3].astype(np.float64)
+    x = st.untag(st.pos)
+    K = ob.kinetic_tensor(v, w.flags, w.offsets, oracle.au_params().mass_amu)
+    kg = k.cpu().numpy()
+    assert np.allclose(kg, K, rtol=1e-11, atol=1e-12)
+    assert np.allclose(kg[:, :3].sum(1), 2 * st.ekin.cpu().numpy(), rtol=1e-6)      # the force pass sums E_kin in fp32 terms
+    o = oracle.compute(x[:, :3].astype(np.float64), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi,
+                       periodic=w.periodic)
+    s_ref = ob.stress(o["w_rep"], K, vol)
+    sg = sig.cpu().numpy()
+    scale = (np.abs(o["w_rep"][:, :3]).sum(1) + n_r * 1e-3) / vol
+    assert np.all(np.abs(sg - s_ref) <= 2e-5 * scale[:, None])
+    # a stretched wire at 298 K is under tension along its axis: a few GPa
+    assert np.all(sg[R // 2:, 2] * ob.EV_PER_A3_IN_GPA > 0)
+    # 0 K stress: K = NULL
+    ctx.stress(st.w_rep, None, d_vol, sig)
+    torch.cuda.synchronize()
+    assert np.allclose(sig.cpu().numpy(), -st.w_rep.cpu().numpy() / vol[:, None], rtol=1e-14, atol=0)

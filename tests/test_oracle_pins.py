@@ -437,3 +437,40 @@ def test_grips_are_rigid_and_placed():                         # readings A10, A
     # kinetic energy counts dynamic atoms only
     ek = 0.5 * MASS / ACC * (md.v[dyn] ** 2).sum()
     assert md.ekin_rep[0] == pytest.approx(ek, rel=1e-13)
+
+
+# ---------------------------------------------------------------- observables (Eq.4-5, reading A11)
+def test_stress_hydrostatic_part_is_minus_dE_dV_of_the_lattice_sum():
+    """perfect fcc bulk, no motion: -tr(sigma)/3 = p = -dE/dV with E(a) the hand-written shell sum, V = a^3 / 4 per atom"""
+    from oracle import observables as ob
+    a, nshell, ncell = 4.08, 5, 4
+    x, L = bulk(a, ncell)
+    o = oracle.compute(x, 7.0, lo=0.0, hi=np.float32(L), periodic=1, fp32_pred=False)
+    n = len(x)
+    V = float(np.float32(L)) ** 3
+    sig = ob.stress(o["w_rep"], np.zeros((1, 6)), np.array([V]))[0]
+    h = 1e-5
+    ae = float(np.float32(L)) / ncell           # the oracle's box length is the fp32 value
+    dE_da = (lattice_energy(ae + h, nshell)[0] - lattice_energy(ae - h, nshell)[0]) / (2 * h)    # per atom
+    p_ref = -dE_da / (3 * ae * ae / 4)                                                           # dV/da = 3 a^2 / 4 per atom
+    assert -(sig[0] + sig[1] + sig[2]) / 3 == pytest.approx(p_ref, rel=2e-5)
+    assert sig[0] == pytest.approx(sig[1], rel=1e-6) and sig[0] == pytest.approx(sig[2], rel=1e-6)   # cubic symmetry
+    assert np.abs(sig[3:]).max() < 1e-9 * n
+    # a = 4.08 is 0.03 % above the zero-pressure lattice constant: slight tension
+    assert 0 < sig[2] * ob.EV_PER_A3_IN_GPA < 0.5
+
+
+def test_kinetic_tensor_trace_and_ideal_gas_pressure():
+    """tr K = 2 E_kin (E_kin from the C oracle's MD state), and without forces -tr(sigma)/3 = (N - 1) kB T / V for
+    Maxwell velocities rescaled to T exactly with the centre of mass at rest (reading A13)"""
+    from oracle import observables as ob
+    w = W.config2(length=60.0)
+    md = oracle.MD(w.x64(), w.v64(), w.flags, w.r_cut, lo=w.box_lo, hi=w.box_hi, zref=w.vel4[:, 3].astype(np.float64))
+    K = ob.kinetic_tensor(w.v64(), w.flags, w.offsets, oracle.au_params().mass_amu)
+    assert K[0, :3].sum() == pytest.approx(2 * md.ekin_rep[0], rel=1e-12)
+    n_dyn = int((w.flags == 0).sum())
+    kT = 8.617333262e-5 * float(w.T[0])
+    V = 1234.5
+    sig = ob.stress(np.zeros((1, 6)), K, np.array([V]))[0]
+    assert -(sig[:3].sum()) / 3 == pytest.approx((n_dyn - 1) * kT / V, rel=1e-6)
+    assert ob.strain(np.array([110.0]), 100.0)[0] == pytest.approx(0.1)
