@@ -219,7 +219,8 @@ int tbsma_set_async(tbsma_ctx *ctx, int32_t enable, double margin);
 /* Shared-memory variant only: how the asynchronous list renewal above runs beside the gather passes.
  * 2 (default): on `stream` itself, the density pass launched as a PROGRAMMATIC DEPENDENT of the filter kernel (which
  * signals griddepcontrol.launch_dependents at once; the density pass reads the half of the list buffers the filter
- * kernel does not write), so that both run together without a second stream; 1: the filter kernel on a second,
+ * kernel does not write, and executes griddepcontrol.wait before it exits, so that whatever follows it also follows the
+ * filter kernel), so that both run together without a second stream; 1: the filter kernel on a second,
  * high-priority stream of the context, forked and joined inside the step; 0: the same kernels one after the other.
  * The caller sees ordinary stream semantics in all three; results are bitwise identical. */
 int tbsma_set_overlap(tbsma_ctx *ctx, int32_t enable);

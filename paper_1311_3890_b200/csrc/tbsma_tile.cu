@@ -820,6 +820,10 @@ k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_
     const int h = list_half(ls, t.rep);
     density_tile(t, cell_start, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad, s_cap,
                  pc, ls.img + (size_t)blockIdx.x * ls.img_stride);
+    // Launched as a programmatic dependent of the filter kernel this pass starts early and reads nothing of it; but the
+    // kernels after it (force pass, then the swap of the list halves) are ordered after THIS kernel only, so it must
+    // not complete before the filter kernel has (a no-op for an ordinary launch).
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // running sums of stage 2, two lanes each (even / odd neighbours), added up once per atom

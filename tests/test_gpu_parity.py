@@ -670,3 +670,20 @@ def test_stress_and_kinetic_tensor_match_oracle(B):
     ctx.stress(st.w_rep, None, d_vol, sig)
     torch.cuda.synchronize()
     assert np.allclose(sig.cpu().numpy(), -st.w_rep.cpu().numpy() / vol[:, None], rtol=1e-14, atol=0)
+
+
+@pytest.mark.parametrize("overlap", [1, 2])
+def test_overlapped_renewal_waits_for_a_long_filter_pass(B, overlap):
+    """512 hot replicas built together and NOT staggered all renew their lists in the same step: the filter pass then
+    outlasts both gather passes beside it.  The step must still not swap the list halves before it has finished
+    (two streams: join event; programmatic dependent launch: the density pass waits for its primary before it exits).
+    Same bits as the kernels one after the other."""
+    w = W.config4(512, seed=29)
+    n_steps = 30
+    ca, a = run_gpu_md(B, w, n_steps, variant=2, overlap=overlap, stagger=False)
+    cb, b = run_gpu_md(B, w, n_steps, variant=2, overlap=0, stagger=False)
+    sa, sb = ca.get_stats(), cb.get_stats()
+    assert sa == sb and sa["n_replica_builds"] >= 512 and sa["n_build_passes"] <= 20     # bunched in a few steps
+    assert ca.status() == 0 and cb.status() == 0
+    for name in ("pos", "vel", "force"):
+        assert np.array_equal(a.untag(getattr(a, name)), b.untag(getattr(b, name))), name
