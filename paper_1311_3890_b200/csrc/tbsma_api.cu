@@ -369,6 +369,7 @@ int tbsma_destroy(tbsma_ctx *c)
 int tbsma_set_variant(tbsma_ctx *c, int32_t variant)
 {
     if (!c || variant < 0 || variant > 2) return TBSMA_EINVAL;
+    c->epoch++;
     c->variant = variant;
     c->cells_built = c->list_built = 0;   // lists must be rebuilt for the new variant
     return TBSMA_OK;
@@ -381,6 +382,7 @@ int tbsma_set_tile(tbsma_ctx *c, int32_t layers_per_tile, int32_t threads)
     if (!c || layers_per_tile < 1 || layers_per_tile > TBSMA_TILE_MAX_LAYERS || threads < 32 || threads > 512 ||
         (threads & 31))
         return TBSMA_EINVAL;
+    c->epoch++;
     c->tile_layers = layers_per_tile;
     c->tile_threads = threads;
     c->cells_built = c->list_built = 0;
@@ -390,6 +392,7 @@ int tbsma_set_tile(tbsma_ctx *c, int32_t layers_per_tile, int32_t threads)
 int tbsma_set_outer_skin(tbsma_ctx *c, double outer_skin)
 {
     if (!c || !(outer_skin >= 0.0) || !(outer_skin <= 16.0)) return TBSMA_EINVAL;
+    c->epoch++;
     if (c->d_olist) {
         cudaDeviceSynchronize();
         cudaFree(c->d_tile_first); cudaFree(c->d_work);
@@ -406,6 +409,7 @@ int tbsma_set_outer_skin(tbsma_ctx *c, double outer_skin)
 int tbsma_set_graph(tbsma_ctx *c, int32_t enable)
 {
     if (!c) return TBSMA_EINVAL;
+    c->epoch++;
     c->use_graph = enable != 0;
     c->use_cond = enable != 1;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
@@ -415,6 +419,7 @@ int tbsma_set_graph(tbsma_ctx *c, int32_t enable)
 int tbsma_set_balance(tbsma_ctx *c, int32_t enable, double cell)
 {
     if (!c || cell < 0.0) return TBSMA_EINVAL;
+    c->epoch++;
     c->balance = enable != 0;
     c->class_h = cell > 0.0 ? cell : c->prm.r0 / sqrt(2.0);
     return TBSMA_OK;
@@ -423,6 +428,7 @@ int tbsma_set_balance(tbsma_ctx *c, int32_t enable, double cell)
 int tbsma_set_stagger(tbsma_ctx *c, int32_t enable)
 {
     if (!c) return TBSMA_EINVAL;
+    c->epoch++;
     c->stagger = enable != 0;
     return TBSMA_OK;
 }
@@ -430,6 +436,7 @@ int tbsma_set_stagger(tbsma_ctx *c, int32_t enable)
 int tbsma_set_async(tbsma_ctx *c, int32_t enable, double margin)
 {
     if (!c || margin < 0.0) return TBSMA_EINVAL;
+    c->epoch++;
     c->async_inner = enable != 0;
     c->async_margin = margin;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
@@ -439,6 +446,7 @@ int tbsma_set_async(tbsma_ctx *c, int32_t enable, double margin)
 int tbsma_set_overlap(tbsma_ctx *c, int32_t enable)
 {
     if (!c) return TBSMA_EINVAL;
+    c->epoch++;
     c->overlap = enable;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
     return TBSMA_OK;
@@ -447,6 +455,7 @@ int tbsma_set_overlap(tbsma_ctx *c, int32_t enable)
 int tbsma_set_timing(tbsma_ctx *c, int32_t enable)
 {
     if (!c) return TBSMA_EINVAL;
+    c->epoch++;
     if (enable && !c->tev) {
         c->tev = (cudaEvent_t *)calloc(6 * TBSMA_TIMING_MAX_STEPS, sizeof(cudaEvent_t));
         if (!c->tev) return TBSMA_ENOMEM;
@@ -483,6 +492,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     if (!c || n_atoms < 0 || n_atoms > 0x7ffffff0ll || n_replicas < 1 || !h_off || !h_lo || !h_hi || !h_per ||
         max_neighbors < 1 || max_neighbors > 4096)
         return TBSMA_EINVAL;
+    c->epoch++;
     if (h_off[0] != 0 || h_off[n_replicas] != n_atoms) return TBSMA_EINVAL;
     for (int r = 0; r < n_replicas; ++r)
         if (h_off[r + 1] < h_off[r]) return TBSMA_EINVAL;
@@ -556,6 +566,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
 int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, void *stream)
 {
     if (!c || !d_pos || !d_tag) return TBSMA_EINVAL;
+    c->epoch++;
     if (!c->d_geom) return TBSMA_ESTATE;
     if (c->n == 0) { c->cells_built = 1; return TBSMA_OK; }
     cudaStream_t st = (cudaStream_t)stream;
@@ -577,6 +588,7 @@ int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, 
 int tbsma_build_neighbors(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, void *stream)
 {
     if (!c || !d_pos || !d_tag) return TBSMA_EINVAL;
+    c->epoch++;
     if (!c->d_geom || !c->cells_built) return TBSMA_ESTATE;
     if (c->n == 0) { c->list_built = 1; return TBSMA_OK; }
     cudaStream_t st = (cudaStream_t)stream;
@@ -652,6 +664,7 @@ int tbsma_md_run(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energy
         key.p[0] = pos; key.p[1] = vel; key.p[2] = force; key.p[3] = d_tag; key.p[4] = d_T; key.p[5] = seed;
         key.p[6] = d_disp0; key.p[7] = d_rate; key.p[8] = d_e; key.p[9] = d_w; key.p[10] = d_k;
         key.dt = dt_fs; key.gamma = gamma_per_fs; key.step0 = step0; key.rebuild_every = rebuild_every;
+        key.epoch = c->epoch;
         if (!c->graph_exec || memcmp(&key, &c->graph_key, sizeof(key)) != 0) {
             if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
             cudaGraph_t g = nullptr;

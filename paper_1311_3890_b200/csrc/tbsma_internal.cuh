@@ -66,7 +66,7 @@ struct GraphKey {          // arguments a cached one-step CUDA graph was capture
     double dt, gamma;
     unsigned long long step0;
     int rebuild_every;
-    int pad;
+    int epoch;             // tbsma_ctx::epoch when captured: any call that re-sizes, re-allocates or re-tunes bumps it
 };
 
 struct tbsma_ctx {
@@ -161,6 +161,7 @@ struct tbsma_ctx {
     int s_R;
 
     int cells_built, list_built;
+    int epoch;                 // bumped by every call after which a captured step would hold stale arguments
     int64_t launches;
     // md_run: one step captured as a CUDA graph and replayed
     int use_graph;
