@@ -235,6 +235,18 @@ int tbsma_set_overlap(tbsma_ctx *ctx, int32_t enable);
  * forces up to the fp32 summation order.  Takes effect when candidates are next rebuilt (tbsma_build_neighbors). */
 int tbsma_set_balance(tbsma_ctx *ctx, int32_t enable, double cell);
 
+/* Thermostat of tbsma_md_step / tbsma_md_run.  kind 0 (default): Langevin with the friction passed to those calls
+ * (BASELINE.json's substitution).  kind 1: Nose-Hoover, the paper's, which gives neither discretisation nor
+ * thermostat mass (D:A17): one variable xi per replica, d xi/dt = (2K - g kB T)/Q, dv/dt = F/m - xi v, Q = g kB T
+ * tau_fs^2, g = 3 N_dyn, integrated as B A N A B with N: xi += (dt/2)(2K - g kB T)/Q; v *= exp(-xi dt); K *= s^2;
+ * xi += (dt/2)(2K - g kB T)/Q, K the kinetic energy of the dynamic atoms after the opening kick (summed by a kernel of
+ * its own at the start of every step).  gamma_per_fs and d_seed of the step calls are ignored, d_T is the target.  xi
+ * and eta (d eta/dt = xi; E + K + Q xi^2/2 + g kB T eta is conserved) live in the context, start at 0 and are reset by
+ * this call and by tbsma_set_system; tbsma_get_thermostat copies them to the host (n_replicas doubles each,
+ * synchronises). */
+int tbsma_set_thermostat(tbsma_ctx *ctx, int32_t kind, double tau_fs);
+int tbsma_get_thermostat(tbsma_ctx *ctx, double *h_xi, double *h_eta);
+
 /* Replicas built together (all of them, by tbsma_build_neighbors) that share a temperature would all need their
  * next list at nearly the same step, and again one period later.  When enabled (default 1, more than one replica)
  * replica r rebuilds for the first time as soon as an atom has moved f_r skin/2, f_r = 0.3 + 0.7 frac(0.618 r), and

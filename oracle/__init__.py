@@ -4,7 +4,8 @@ TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.
 cpu_baseline / --impl reference legs.  Never imported by paper_1311_3890_b200 (the product),
 and it imports nothing from it.  Every function is a thin marshalling layer; all arithmetic
 is in the C file, which cites the paper line by line (the observables of P:79-87 -- kinetic
-tensor, virial stress, strain -- are plain numpy in oracle/observables.py).
+tensor, virial stress, strain -- are plain numpy in oracle/observables.py, and the paper's
+Nose-Hoover thermostat in oracle/nose_hoover.py on top of this module's forces).
 """
 import ctypes as C
 import os

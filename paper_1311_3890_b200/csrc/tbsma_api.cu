@@ -38,7 +38,8 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_cell_of); cudaFree(c->d_slot); cudaFree(c->d_order); cudaFree(c->d_pos_build);
     cudaFree(c->d_tmp4); cudaFree(c->d_tmp_tag); cudaFree(c->d_nlist); cudaFree(c->d_nn); cudaFree(c->d_xs);
     cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters); cudaFree(c->d_stagger); cudaFree(c->d_cur);
-    c->d_stagger = nullptr; c->d_cur = nullptr;
+    cudaFree(c->d_nh); cudaFree(c->d_kmid); cudaFree(c->d_nh_scale);
+    c->d_stagger = nullptr; c->d_cur = nullptr; c->d_nh = nullptr; c->d_kmid = nullptr; c->d_nh_scale = nullptr;
     cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_tileof); cudaFree(c->d_img); cudaFree(c->d_inv);
     c->d_tileof = nullptr; c->d_img = nullptr; c->d_inv = nullptr;
     cudaFree(c->d_newslot); cudaFree(c->d_oldof);
@@ -189,7 +190,9 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
     if (async) a.trigger2 = (float)((0.5 * c->skin - c->async_margin) * (0.5 * c->skin - c->async_margin));
     a.cur = c->d_cur;
     a.pb_stride = c->n_pad;
-    a.thermostat = gamma > 0.0;
+    const bool nose_hoover = c->thermostat_kind == 1;
+    a.thermostat = !nose_hoover && gamma > 0.0;
+    a.nh_scale = nose_hoover ? c->d_nh_scale : nullptr;
     a.rebuild_every = rebuild_every;
     a.step_base = step0;
     a.T = T; a.seed = seed; a.disp0 = disp0; a.rate = rate;
@@ -202,6 +205,7 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         cudaEvent_t *ev = nullptr;
         if (c->timing && c->tev && c->tev_steps < TBSMA_TIMING_MAX_STEPS) ev = c->tev + 6 * (c->tev_steps++);
         if (ev) CK(cudaEventRecord(ev[0], st));
+        if (nose_hoover) CK(tbsma_launch_nose_hoover(c, pos, vel, force, a, dt, st));
         CK(tbsma_launch_integrate_pre(c, pos, vel, force, tag, a, st));
         if (ev) CK(cudaEventRecord(ev[1], st));
         bool forked = false, early = false, joined = false;
@@ -396,8 +400,8 @@ int tbsma_set_outer_skin(tbsma_ctx *c, double outer_skin)
     if (c->d_olist) {
         cudaDeviceSynchronize();
         cudaFree(c->d_tile_first); cudaFree(c->d_work);
-    c->d_tile_first = nullptr; c->d_work = nullptr;
-    cudaFree(c->d_olist); cudaFree(c->d_nn_o); cudaFree(c->d_pos_outer); cudaFree(c->d_want_outer);
+        c->d_tile_first = nullptr; c->d_work = nullptr;
+        cudaFree(c->d_olist); cudaFree(c->d_nn_o); cudaFree(c->d_pos_outer); cudaFree(c->d_want_outer);
         c->d_olist = nullptr; c->d_nn_o = nullptr; c->d_pos_outer = nullptr; c->d_want_outer = nullptr;
     }
     c->outer_skin = outer_skin;
@@ -422,6 +426,30 @@ int tbsma_set_balance(tbsma_ctx *c, int32_t enable, double cell)
     c->epoch++;
     c->balance = enable != 0;
     c->class_h = cell > 0.0 ? cell : c->prm.r0 / sqrt(2.0);
+    return TBSMA_OK;
+}
+
+int tbsma_set_thermostat(tbsma_ctx *c, int32_t kind, double tau_fs)
+{
+    if (!c || kind < 0 || kind > 1 || (kind == 1 && !(tau_fs > 0.0))) return TBSMA_EINVAL;
+    c->epoch++;
+    c->thermostat_kind = kind;
+    c->nh_tau = tau_fs;
+    if (c->d_nh) CK(cudaMemset(c->d_nh, 0, sizeof(double) * 2 * (size_t)c->R));
+    return TBSMA_OK;
+}
+
+int tbsma_get_thermostat(tbsma_ctx *c, double *h_xi, double *h_eta)
+{
+    if (!c || !h_xi || !h_eta) return TBSMA_EINVAL;
+    if (!c->d_nh) return TBSMA_ESTATE;
+    CK(cudaDeviceSynchronize());
+    double *h = (double *)malloc(sizeof(double) * 2 * (size_t)(c->R ? c->R : 1));
+    if (!h) return TBSMA_ENOMEM;
+    const cudaError_t e = cudaMemcpy(h, c->d_nh, sizeof(double) * 2 * (size_t)c->R, cudaMemcpyDeviceToHost);
+    for (int r = 0; r < c->R && e == cudaSuccess; ++r) { h_xi[r] = h[2 * r]; h_eta[r] = h[2 * r + 1]; }
+    free(h);
+    CK(e);
     return TBSMA_OK;
 }
 
@@ -537,7 +565,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     const size_t nb = (size_t)c->list_bufs;
     DA(c->d_pos_build, nb * c->n_pad); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
     DA(c->d_nlist, nb * (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, nb * c->n_pad); DA(c->d_xs, n);
-    DA(c->d_cur, (size_t)R);
+    DA(c->d_cur, (size_t)R); DA(c->d_nh, 2 * (size_t)R); DA(c->d_kmid, 2 * (size_t)R); DA(c->d_nh_scale, (size_t)R);
     DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8); DA(c->d_stagger, (size_t)R);
     DA(c->d_maxpop, (size_t)R); DA(c->d_hbase, n); DA(c->d_tileof, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
     DA(c->d_tmp_pos, n);
@@ -555,6 +583,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     if (e == cudaSuccess) e = cudaMemset(c->d_counters, 0, sizeof(unsigned long long) * 8);
     if (e == cudaSuccess) e = cudaMemset(c->d_nn, 0, sizeof(int32_t) * nb * (c->n_pad ? c->n_pad : 1));
     if (e == cudaSuccess) e = cudaMemset(c->d_cur, 0, sizeof(int32_t) * R);
+    if (e == cudaSuccess) e = cudaMemset(c->d_nh, 0, sizeof(double) * 2 * R);
     if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
     c->cell_w = 0.0;
     c->kmax_o = c->kmax;
@@ -626,7 +655,8 @@ int tbsma_md_step(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energ
                   const double *d_slab_disp, double *d_e, double *d_w, double *d_k, void *stream)
 {
     if (!c || !d_pos || !d_vel || !d_force_energy || !d_tag || !(dt_fs > 0.0) || !(gamma_per_fs >= 0.0)) return TBSMA_EINVAL;
-    if (gamma_per_fs > 0.0 && (!d_T || !d_seed)) return TBSMA_EINVAL;
+    if (c && c->thermostat_kind == 0 && gamma_per_fs > 0.0 && (!d_T || !d_seed)) return TBSMA_EINVAL;
+    if (c && c->thermostat_kind == 1 && !d_T) return TBSMA_EINVAL;
     if (!c->d_geom || !c->list_built) return TBSMA_ESTATE;
     if (c->n == 0) return TBSMA_OK;
     return run_steps(c, (float4 *)d_pos, (float4 *)d_vel, (float4 *)d_force_energy, d_tag, dt_fs, d_T, gamma_per_fs,
@@ -642,7 +672,8 @@ int tbsma_md_run(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energy
     if (!c || !d_pos || !d_vel || !d_force_energy || !d_tag || !(dt_fs > 0.0) || !(gamma_per_fs >= 0.0) ||
         n_steps < 0 || rebuild_every < 0)
         return TBSMA_EINVAL;
-    if (gamma_per_fs > 0.0 && (!d_T || !d_seed)) return TBSMA_EINVAL;
+    if (c && c->thermostat_kind == 0 && gamma_per_fs > 0.0 && (!d_T || !d_seed)) return TBSMA_EINVAL;
+    if (c && c->thermostat_kind == 1 && !d_T) return TBSMA_EINVAL;
     if (!c->d_geom || !c->list_built) return TBSMA_ESTATE;
     if (c->n == 0 || n_steps == 0) return TBSMA_OK;
     cudaStream_t st = (cudaStream_t)stream;

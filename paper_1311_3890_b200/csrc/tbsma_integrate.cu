@@ -64,7 +64,10 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
         const float4 f = force[i];
         v.x = __fmaf_rn(a.kick, f.x, v.x); v.y = __fmaf_rn(a.kick, f.y, v.y); v.z = __fmaf_rn(a.kick, f.z, v.z);
         p.x = __fmaf_rn(a.half_dt, v.x, p.x); p.y = __fmaf_rn(a.half_dt, v.y, p.y); p.z = __fmaf_rn(a.half_dt, v.z, p.z);
-        if (a.thermostat) {
+        if (a.nh_scale) {              // N of B A N A B (Nose-Hoover, k_nh_update): v *= exp(-xi dt)
+            const float sc = a.nh_scale[r];
+            v.x *= sc; v.y *= sc; v.z *= sc;
+        } else if (a.thermostat) {
             const unsigned trel = (unsigned)(tag[i] - geom[r].atom_begin);
             const float3 g = gauss3(a.seed[r], trel, step);
             const float sg = a.c2 * a.sigma_scale * sqrtf(a.T[r]);
@@ -141,6 +144,64 @@ __global__ void k_set_stagger(float *__restrict__ stagger, int R, int enable)
     stagger[r] = f * f;
 }
 
+// ---- Nose-Hoover (the paper's thermostat; reading A17): B A N A B with one variable xi per replica,
+//   N:  xi += (dt/2)(2K - g kB T)/Q;  v *= s = exp(-xi dt);  K *= s^2;  xi += (dt/2)(2K - g kB T)/Q;   Q = g kB T tau^2,
+// K = kinetic energy of the dynamic atoms AFTER the opening kick, g = 3 N_dyn.  K needs all atoms of the replica, so it
+// is summed by a kernel of its own from (v, F) with the kick of k_integrate_pre, operation for operation; a thread per
+// replica then advances xi and eta (d eta/dt = xi: the conserved quantity is E + K + Q xi^2/2 + g kB T eta) and leaves
+// the scale for the integrator.
+__global__ void __launch_bounds__(256)
+k_nh_kinetic(const float4 *__restrict__ pos, const float4 *__restrict__ vel, const float4 *__restrict__ force,
+             const int *__restrict__ atom_rep, double *__restrict__ kmid, float kick, double half_m_over_c, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    int r = -1;
+    double k = 0.0, cnt = 0.0;
+    if (i < n) {
+        r = atom_rep[i];
+        if ((__float_as_int(pos[i].w) & 3) == 0) {
+            const float4 v = vel[i], f = force[i];
+            const double vx = __fmaf_rn(kick, f.x, v.x), vy = __fmaf_rn(kick, f.y, v.y), vz = __fmaf_rn(kick, f.z, v.z);
+            k = half_m_over_c * (vx * vx + vy * vy + vz * vz);
+            cnt = 1.0;
+        }
+    }
+    const int r0 = __shfl_sync(0xffffffffu, r, 0);
+    if (__all_sync(0xffffffffu, r == r0)) {
+        if (r0 < 0) return;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            k += __shfl_xor_sync(0xffffffffu, k, o);
+            cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+        }
+        if (lane == 0) { atomicAdd(kmid + 2 * (size_t)r0, k); atomicAdd(kmid + 2 * (size_t)r0 + 1, cnt); }
+    } else if (r >= 0) {
+        atomicAdd(kmid + 2 * (size_t)r, k);
+        atomicAdd(kmid + 2 * (size_t)r + 1, cnt);
+    }
+}
+
+__global__ void k_nh_update(const double *__restrict__ kmid, const float *__restrict__ T, double *__restrict__ nh,
+                            float *__restrict__ scale, double dt, double tau, int R)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    const double K = kmid[2 * r], g = 3.0 * kmid[2 * r + 1];
+    const double gkt = g * TBSMA_KB * (double)T[r];
+    double s = 1.0;
+    if (gkt > 0.0 && tau > 0.0) {
+        const double Q = gkt * tau * tau;
+        double xi = nh[2 * r];
+        xi += 0.5 * dt * (2.0 * K - gkt) / Q;
+        s = exp(-xi * dt);
+        nh[2 * r + 1] += xi * dt;
+        xi += 0.5 * dt * (2.0 * K * s * s - gkt) / Q;
+        nh[2 * r] = xi;
+    }
+    scale[r] = (float)s;
+}
+
 // ---- observables of the tensile tests (Eq.5 as read in D:A11) -----------------------
 // K_ab = sum_i m v_i,a v_i,b over the dynamic atoms of every replica (eV; xx yy zz xy xz yz).  Atoms of a replica are
 // contiguous, so nearly every warp belongs to one replica: warp shuffle sums, one fp64 atomic per warp and component.
@@ -188,6 +249,19 @@ __global__ void k_stress(const double *__restrict__ w_rep, const double *__restr
 }
 
 }  // namespace
+
+cudaError_t tbsma_launch_nose_hoover(tbsma_ctx *c, const float4 *pos, const float4 *vel, const float4 *force,
+                                     const StepArgs &a, double dt, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(c->d_kmid, 0, sizeof(double) * 2 * (size_t)c->R, st);
+    if (e != cudaSuccess) return e;
+    const int n = (int)c->n;
+    k_nh_kinetic<<<(n + 255) / 256, 256, 0, st>>>(pos, vel, force, c->d_atom_rep, c->d_kmid, a.kick,
+                                                 0.5 * c->prm.mass_amu / TBSMA_ACC, n);
+    k_nh_update<<<(c->R + 127) / 128, 128, 0, st>>>(c->d_kmid, a.T, c->d_nh, c->d_nh_scale, dt, c->nh_tau, c->R);
+    c->launches += 2;
+    return cudaGetLastError();
+}
 
 cudaError_t tbsma_launch_kinetic_tensor(tbsma_ctx *c, const float4 *pos, const float4 *vel, double *k_rep, cudaStream_t st)
 {

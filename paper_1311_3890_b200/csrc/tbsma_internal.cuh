@@ -160,6 +160,12 @@ struct tbsma_ctx {
     int64_t s_n;
     int s_R;
 
+    // Nose-Hoover thermostat (the paper's; tbsma_set_thermostat): one variable per replica
+    int thermostat_kind;       // 0 Langevin (gamma of tbsma_md_step), 1 Nose-Hoover
+    double nh_tau;             // fs: Q = g kB T tau^2
+    double *d_nh;              // 2 R: xi, eta
+    double *d_kmid;            // 2 R: kinetic energy after the opening kick, number of dynamic atoms
+    float *d_nh_scale;         // R
     int cells_built, list_built;
     int epoch;                 // bumped by every call after which a captured step would hold stale arguments
     int64_t launches;
@@ -244,12 +250,15 @@ struct StepArgs {
     const double *rate;      // nullable
     const int *want_outer;   // nullable (tile variant): replicas whose next rebuild redoes cells + candidates
     const float *stagger;    // per replica factor on skin_half2
+    const float *nh_scale;   // nullable: Nose-Hoover velocity scale of this step per replica (replaces the O part)
     double *e_rep, *w_rep, *ekin;  // zeroed here for the force pass; nullable
 };
 cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, const float4 *force,
                                        const int32_t *tag, const StepArgs &a, cudaStream_t st);
 cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st);
 cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st);
+cudaError_t tbsma_launch_nose_hoover(tbsma_ctx *c, const float4 *pos, const float4 *vel, const float4 *force,
+                                     const StepArgs &a, double dt, cudaStream_t st);
 cudaError_t tbsma_launch_kinetic_tensor(tbsma_ctx *c, const float4 *pos, const float4 *vel, double *k_rep, cudaStream_t st);
 cudaError_t tbsma_launch_stress(tbsma_ctx *c, const double *w_rep, const double *k_rep, const double *volume,
                                 double *sigma, cudaStream_t st);

@@ -687,3 +687,42 @@ def test_overlapped_renewal_waits_for_a_long_filter_pass(B, overlap):
     assert ca.status() == 0 and cb.status() == 0
     for name in ("pos", "vel", "force"):
         assert np.array_equal(a.untag(getattr(a, name)), b.untag(getattr(b, name))), name
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_nose_hoover_trajectory_matches_oracle(B, variant):
+    """tbsma_set_thermostat(1, tau): the paper's thermostat (reading A17) as B A N A B; two replicas of the same
+    wire started at 300 K with targets 150 K and 450 K, 100 steps, against oracle/nose_hoover.py"""
+    from oracle.nose_hoover import NoseHooverMD
+    base = W.config1()
+    n = base.n_atoms
+    v = W.maxwell_velocities(n, 300.0, 5, np.ones(n, bool))
+    w = W._assemble("nh_2x_wire_3x6nm", [base.x64(), base.x64()], [np.zeros(n, np.int32)] * 2, [v, v], [150.0, 450.0],
+                    [1, 2], [0.0, 0.0], 0.0)
+    tau, n_steps = 50.0, 100
+    ctx, st = setup(B, w, variant=variant)
+    ctx.set_thermostat(1, tau)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, 0.0, st.seed, 0, n_steps, None, None, 0, st.e_rep, None,
+                   st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    nh = NoseHooverMD(w.x64(), w.v64(), w.flags, w.r_cut, w.T.astype(np.float64), tau, lo=w.box_lo, hi=w.box_hi,
+                      offsets=w.offsets)
+    for s in range(n_steps):
+        nh.step(w.dt)
+    xg = st.untag(st.pos)[:, :3].astype(np.float64)
+    vg = st.untag(st.vel)[:, :3].astype(np.float64)
+    assert traj_rms(xg, nh.x) <= TRAJ_RMS
+    assert np.abs(vg - nh.v).max() < 2e-5
+    xi, eta = ctx.get_thermostat()
+    assert np.allclose(xi, nh.xi, rtol=2e-4, atol=1e-8) and np.allclose(eta, nh.eta, rtol=2e-4, atol=1e-7)
+    assert eta[0] > 0 > eta[1]                    # net cooling of the first replica, net heating of the second
+    ek = st.ekin.cpu().numpy()
+    assert np.allclose(ek, nh.kinetic(), rtol=1e-4)
+    # back to Langevin / velocity Verlet: the thermostat state is reset
+    ctx.set_thermostat(0)
+    assert np.all(ctx.get_thermostat()[0] == 0)

@@ -474,3 +474,37 @@ def test_kinetic_tensor_trace_and_ideal_gas_pressure():
     sig = ob.stress(np.zeros((1, 6)), K, np.array([V]))[0]
     assert -(sig[:3].sum()) / 3 == pytest.approx((n_dyn - 1) * kT / V, rel=1e-6)
     assert ob.strain(np.array([110.0]), 100.0)[0] == pytest.approx(0.1)
+
+
+# ---------------------------------------------------------------- Nose-Hoover (reading A17)
+def test_nose_hoover_conserved_quantity_reduction_to_verlet_and_temperature():
+    from oracle.nose_hoover import NoseHooverMD, KB
+    w = W.config1()
+    x, v = w.x64(), W.maxwell_velocities(w.n_atoms, 300.0, 5, np.ones(w.n_atoms, bool))
+    # (a) tau -> infinity and xi = 0: velocity Verlet, the same numbers as the C oracle's gamma = 0 step
+    nh = NoseHooverMD(x, v, w.flags, w.r_cut, 300.0, 1e30, lo=w.box_lo, hi=w.box_hi)
+    md = oracle.MD(x, v, w.flags, w.r_cut, lo=w.box_lo, hi=w.box_hi)
+    for s in range(5):
+        nh.step(w.dt)
+        md.step(w.dt, 0.0, 0.0, 1, s)
+    assert np.abs(nh.x - md.x).max() < 1e-12 and np.abs(nh.v - md.v).max() < 1e-14
+    # (b) H' = E + K + Q xi^2 / 2 + g kT eta is conserved; the thermostat pulls a 300 K start towards 150 K
+    nh = NoseHooverMD(x, v, w.flags, w.r_cut, 150.0, 50.0, lo=w.box_lo, hi=w.box_hi)
+    h0 = nh.conserved()[0]
+    k0 = nh.kinetic()[0]
+    temps = []
+    for s in range(300):
+        nh.step(w.dt)
+        temps.append(2 * nh.kinetic()[0] / (nh.g[0] * KB))
+    assert abs(nh.conserved()[0] - h0) < 2e-5 * w.n_atoms           # eV; truncation jumps of the cutoff included (A4)
+    assert abs(nh.xi[0]) > 0 and nh.kinetic()[0] < k0
+    assert abs(np.mean(temps[150:]) - 150.0) < 25.0
+    # (c) time reversal: flip v and xi, step back
+    nh2 = NoseHooverMD(x, v, w.flags, w.r_cut, 150.0, 50.0, lo=w.box_lo, hi=w.box_hi)
+    for s in range(20):
+        nh2.step(w.dt)
+    nh2.v *= -1.0
+    nh2.xi *= -1.0
+    for s in range(20):
+        nh2.step(w.dt)
+    assert np.abs(nh2.x - x).max() < 1e-9
