@@ -347,7 +347,7 @@ def main():
                        "mean_list_length": n_l, "mean_steps_between_rebuilds": k_eff,
                        "l2": "inputs larger than L2 (index list %.0f MB per pass)" % (entries * 4 / 1e6),
                        "variant": {1: "global gather (int32 list)", 2: "shared-memory tiles (u16 lists)"}.get(ctx.get_variant()),
-                       "list_renewal": "asynchronous, margin 0.03 A, second stream" if ctx.get_variant() == 2 and not w.rebuild_every else "ahead of the gather passes",
+                       "list_renewal": "asynchronous, margin 0.03 A, beside the gather passes (density pass = programmatic dependent of the filter kernel)" if ctx.get_variant() == 2 and not w.rebuild_every else "ahead of the gather passes",
                        "graph": "plain" if args.plain_graph else "conditional node around the cells+candidates chain",
                        "parallelism": "replicas only" if world > 1 else "1 gpu"},
             "pair_interactions_per_s": pair_rate,
