@@ -108,6 +108,7 @@ struct tbsma_ctx {
     unsigned short *d_img;  // n_tiles x tile_cap: image index of every halo record of a tile (k_tile_place)
     unsigned short *d_inv;  // n_tiles x img_cap: the inverse
     int img_cap;        // records of a tile image, sentinel and spare room of the colour classes included
+    size_t have_tiles, have_first, have_work, have_img, have_inv;   // bytes allocated for the five tile tables
     int balance;        // records placed by colour (default 1) or in slot order
     double class_h;     // side of the colour cells (default r0 / sqrt 2)
     int32_t *d_newslot; // n: cell-order slot -> final slot

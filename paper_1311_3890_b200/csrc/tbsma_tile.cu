@@ -1159,11 +1159,27 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     }
     first[R] = (int)k;
     free(Lr);
-    cudaFree(c->d_tiles); cudaFree(c->d_tile_first); cudaFree(c->d_work); cudaFree(c->d_img); cudaFree(c->d_inv);
-    c->d_tiles = nullptr; c->d_tile_first = nullptr; c->d_work = nullptr; c->d_img = nullptr; c->d_inv = nullptr;
-    e = cudaMalloc((void **)&c->d_tiles, sizeof(TileDesc) * (size_t)(n_tiles ? n_tiles : 1));
-    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_tile_first, sizeof(int) * (size_t)(R + 1));
-    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_work, sizeof(int) * (size_t)(2 + 2 * n_tiles));
+    // the tables keep their allocations from one tbsma_build_cells to the next while they are large enough
+    // (tbsma_md_run_host rebuilds the cells in every call)
+    auto ensure = [](void **p, size_t *have, size_t need) -> cudaError_t {
+        if (*p && *have >= need) return cudaSuccess;
+        cudaFree(*p);
+        *p = nullptr;
+        *have = 0;
+        const cudaError_t err = cudaMalloc(p, need);
+        if (err == cudaSuccess) *have = need;
+        return err;
+    };
+    const size_t nt1 = (size_t)(n_tiles ? n_tiles : 1);
+    const int new_tile_cap = rec_cap < cap ? rec_cap : cap;
+    int new_img_cap = new_tile_cap + new_tile_cap / 8 + 64 + 1;
+    if (new_img_cap > TBSMA_TILE_MAX_RECORDS + 1) new_img_cap = TBSMA_TILE_MAX_RECORDS + 1;
+    if (new_img_cap < new_tile_cap + 1) new_img_cap = new_tile_cap + 1;
+    e = ensure((void **)&c->d_tiles, &c->have_tiles, sizeof(TileDesc) * nt1);
+    if (e == cudaSuccess) e = ensure((void **)&c->d_tile_first, &c->have_first, sizeof(int) * (size_t)(R + 1));
+    if (e == cudaSuccess) e = ensure((void **)&c->d_work, &c->have_work, sizeof(int) * (size_t)(2 + 2 * n_tiles));
+    if (e == cudaSuccess) e = ensure((void **)&c->d_img, &c->have_img, sizeof(unsigned short) * nt1 * new_tile_cap);
+    if (e == cudaSuccess) e = ensure((void **)&c->d_inv, &c->have_inv, sizeof(unsigned short) * nt1 * new_img_cap);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d_work, 0, sizeof(int) * (size_t)(2 + 2 * n_tiles), st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tiles, h, sizeof(TileDesc) * (size_t)n_tiles, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tile_first, first, sizeof(int) * (size_t)(R + 1), cudaMemcpyHostToDevice, st);
@@ -1172,14 +1188,9 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     free(first);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? TBSMA_ENOMEM : TBSMA_ECUDA;
     c->n_tiles = (int)n_tiles;
-    c->tile_cap = rec_cap < cap ? rec_cap : cap;   // halo records a tile may hold
+    c->tile_cap = new_tile_cap;   // halo records a tile may hold
     // image: the sentinel + eight colour classes of records (k_tile_place); room for classes 1/8 + 64 fuller than even
-    c->img_cap = c->tile_cap + c->tile_cap / 8 + 64 + 1;
-    if (c->img_cap > TBSMA_TILE_MAX_RECORDS + 1) c->img_cap = TBSMA_TILE_MAX_RECORDS + 1;
-    if (c->img_cap < c->tile_cap + 1) c->img_cap = c->tile_cap + 1;
-    e = cudaMalloc((void **)&c->d_img, sizeof(unsigned short) * (size_t)(n_tiles ? n_tiles : 1) * c->tile_cap);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&c->d_inv, sizeof(unsigned short) * (size_t)(n_tiles ? n_tiles : 1) * c->img_cap);
-    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? TBSMA_ENOMEM : TBSMA_ECUDA;
+    c->img_cap = new_img_cap;
     c->tile_cell_cap = (cell_cap + 3) & ~3;
     c->own_cap = own_cap;
     // opt in to > 48 KB of dynamic shared memory
