@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(256)
 k_tile_place(const TileDesc *__restrict__ tiles, const int *__restrict__ work, int n_tiles, PlaceArgs A)
 {
     __shared__ unsigned char s_col[TBSMA_TILE_MAX_RECORDS + 1];
-    __shared__ int s_count[8], s_fallback;
+    __shared__ int s_fallback;
     const int nw = work[1];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     for (int w = blockIdx.x; w < nw; w += gridDim.x) {
@@ -298,10 +298,7 @@ k_tile_place(const TileDesc *__restrict__ tiles, const int *__restrict__ work, i
                     }
                     run += __popc(m);
                 }
-                if (lane == 0) {
-                    s_count[wid] = run;
-                    if (8 * (run - 1) + wid + 1 >= A.img_cap) s_fallback = 1;
-                }
+                if (lane == 0 && 8 * (run - 1) + wid + 1 >= A.img_cap) s_fallback = 1;
             }
             __syncthreads();
             if (!s_fallback || pass == 1) break;
