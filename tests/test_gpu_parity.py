@@ -726,3 +726,35 @@ def test_nose_hoover_trajectory_matches_oracle(B, variant):
     # back to Langevin / velocity Verlet: the thermostat state is reset
     ctx.set_thermostat(0)
     assert np.all(ctx.get_thermostat()[0] == 0)
+
+
+@pytest.mark.parametrize("balance,cell", [(0, 0.0), (1, 0.0), (1, 0.9), (1, 6.0)])
+def test_image_placement_changes_cost_not_results(B, balance, cell):
+    """tbsma_set_balance: records placed in the tile image in slot order, by the default 2.04 A colour cells, or by
+    cells that fit the lattice badly -- the neighbour sets are the oracle's, bit for bit, after the build and after
+    60 steps with rebuilds, and the trajectory is the oracle's"""
+    w = W.config3(3, seed=31, length=60.0)
+    ctx = B.make_context(w)
+    ctx.set_variant(2)
+    ctx.set_balance(balance, cell)
+    st = B.DeviceState(w)
+    ctx.build_cells(st.pos, st.vel, st.tag)
+    ctx.build_neighbors(st.pos, st.vel, st.tag)
+    cg, lg = gpu_neighbors(B, ctx, st)
+    co, lo = oracle.neighbors(w.pos4, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+    assert_same_sets(cg, lg, co, lo)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    n_steps = 60
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate,
+                   1, st.e_rep, None, st.ekin)          # rebuild_every = 1: the lists are those of the final positions
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    cg, lg = gpu_neighbors(B, ctx, st)
+    xf = st.untag(st.pos)
+    co, lo = oracle.neighbors(xf, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+    assert_same_sets(cg, lg, co, lo)
+    md = run_oracle_md(w, n_steps)
+    assert traj_rms(xf[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
