@@ -173,6 +173,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel-steps", type=int, default=60, help="steps of the per-kernel CUDA-event timing pass")
+    ap.add_argument("--outer-skin", type=float, default=None,
+                    help="buffer radius S of the candidate lists of the tile variant (tbsma_set_outer_skin; library default if omitted)")
     ap.add_argument("--plain-graph", action="store_true",
                     help="capture the step without the conditional node (Nsight Compute cannot profile kernel nodes "
                          "of graphs that hold conditional nodes): for the ncu passes under profiles/")
@@ -223,6 +225,8 @@ def main():
     ctx = B.make_context(w)
     if args.plain_graph:
         ctx.set_graph(True, conditional=False)
+    if args.outer_skin is not None:
+        ctx.set_outer_skin(args.outer_skin)
     st = B.DeviceState(w, dev)
     stream = torch.cuda.Stream(device=dev)
     K, Wm = args.steps, args.warmup

@@ -184,7 +184,7 @@ int tbsma_get_stats(tbsma_ctx *ctx, tbsma_stats *h_out); /* synchronises */
 int tbsma_set_variant(tbsma_ctx *ctx, int32_t variant);
 int tbsma_get_variant(const tbsma_ctx *ctx);
 
-/* Shared-memory variant: buffer radius S of the CANDIDATE list (default 2.0 A).  The cell scan collects every
+/* Shared-memory variant: buffer radius S of the CANDIDATE list (default 2.5 A).  The cell scan collects every
  * pair within r_cut + skin + S, once; while no atom has moved more than S/2 since then, the replica's list
  * (radius r_cut + skin) is re-filtered from those candidates whenever its atoms have moved more than skin/2
  * (inside the density pass of that step).  Membership of the list is decided by the predicate of D:A6 either way,

@@ -319,7 +319,7 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->device = dev;
     c->variant = 0;
     c->active_variant = 1;
-    c->outer_skin = 2.0;
+    c->outer_skin = 2.5;
     c->tile_layers = 2;
     c->tile_threads = 256;
     c->use_graph = 1;

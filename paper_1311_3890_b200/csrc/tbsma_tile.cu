@@ -20,7 +20,7 @@
 //
 // Two-level lists.  Scanning 27 cells costs about five force passes per atom, and at 298 K a replica
 // needs a fresh list every ~12 steps (fewer rebuilds are why 10 K runs faster).  So the cell
-// scan builds a CANDIDATE list with the larger radius r_cut + skin + S (S = outer_skin, 2 A by default):
+// scan builds a CANDIDATE list with the larger radius r_cut + skin + S (S = outer_skin, 2.5 A by default):
 // K1 (scan), K1b (place), K2 (finish), K3 (permute) below, rarely.  The list the gather passes read
 // (radius r_cut + skin, the paper's r_buff list) is filtered from the candidates by the tile that
 // owns the atom (k_tile_inner) when the replica's atoms have moved skin/2 (less a margin when the filter
