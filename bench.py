@@ -289,7 +289,7 @@ def main():
                 "whole_step": {"achieved": ach_step, "frac": ach_step / peak, "bytes_per_atom_step": step_bytes / w.n_atoms},
                 "per_kernel_ms": per_kernel_ms, "timed_steps": tsteps}
     # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu capture
-    traffic_file = os.path.join(ROOT, "profiles", "r1d_force_kernel_traffic.csv")
+    traffic_file = os.path.join(ROOT, "profiles", "r1e_force_kernel_traffic.csv")
     if os.path.exists(traffic_file):
         try:
             import csv
@@ -301,7 +301,7 @@ def main():
             pass
     roofline["note"] = ("HBM is the designated roofline (BASELINE.json); with 16-bit lists the gather passes move less than "
                         "the algorithmic bytes and are bound by the shared-memory data pipe and the MUFU pipe "
-                        "(profiles/r1d_ncu_full_summary.md)")
+                        "(profiles/r1e_ncu_full_summary.md)")
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
