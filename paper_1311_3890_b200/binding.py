@@ -149,7 +149,7 @@ class Context:
         except Exception:
             pass
 
-    def set_system(self, offsets, box_lo, box_hi, periodic, max_neighbors=96):
+    def set_system(self, offsets, box_lo, box_hi, periodic, max_neighbors=112):
         offsets = np.ascontiguousarray(offsets, dtype=np.int32)
         R = len(offsets) - 1
         lo = np.ascontiguousarray(np.broadcast_to(np.asarray(box_lo, np.float32), (R, 3)))
@@ -300,7 +300,7 @@ class DeviceState:
         return out
 
 
-def make_context(w, max_neighbors=96, params=None):
+def make_context(w, max_neighbors=112, params=None):
     """Context sized for a Workload."""
     ctx = Context(params, r_cut=w.r_cut, skin=w.skin)
     ctx.set_system(w.offsets, w.box_lo, w.box_hi, w.periodic, max_neighbors)
