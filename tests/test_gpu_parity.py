@@ -758,3 +758,21 @@ def test_image_placement_changes_cost_not_results(B, balance, cell):
     assert_same_sets(cg, lg, co, lo)
     md = run_oracle_md(w, n_steps)
     assert traj_rms(xf[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+
+
+def test_long_run_keeps_a_clean_status_word(B):
+    """1500 steps of sixteen 24 nm wires at 298 K under tension (about 120 list renewals per replica, the ends relaxing,
+    the wire stretching): no list, candidate or tile overflow, no skin violation, nothing non-finite, and the kinetic
+    temperature stays at the thermostat's"""
+    w = W.config3(16, seed=37)
+    w.T[:] = 298.0
+    w.vel4[:, :3] = np.concatenate([W.maxwell_velocities(int(n), 298.0, 1000 + r, w.flags[w.offsets[r]:w.offsets[r + 1]] == 0)
+                                    for r, n in enumerate(np.diff(w.offsets))]).astype(np.float32)
+    ctx, st = run_gpu_md(B, w, 1500)
+    assert ctx.status() == 0
+    s = ctx.get_stats()
+    assert s["n_replica_builds"] > 16 * 60 and s["max_neighbors_seen"] <= 112
+    assert bool(torch.isfinite(st.pos).all()) and bool(torch.isfinite(st.vel).all())
+    n_dyn = np.array([(w.flags[w.offsets[r]:w.offsets[r + 1]] == 0).sum() for r in range(w.n_replicas)])
+    T_kin = 2 * st.ekin.cpu().numpy() / (3 * n_dyn * 8.617333262e-5)
+    assert np.all(np.abs(T_kin - 298.0) < 15.0)
