@@ -476,6 +476,34 @@ def test_kinetic_tensor_trace_and_ideal_gas_pressure():
     assert ob.strain(np.array([110.0]), 100.0)[0] == pytest.approx(0.1)
 
 
+def test_kinetic_tensor_off_diagonal_order_by_hand():
+    """K_ab = sum_i m v_a v_b (Eq.5's kinetic term as read in D:A11) with the six components in the order
+    xx yy zz xy xz yz: three atoms with hand-set velocities whose six sums are all different numbers, worked out here
+    term by term, plus a grip atom that must not count (D:A12) and a second replica that must not mix in."""
+    from oracle import observables as ob
+    v = np.array([[1.0, 2.0, 3.0],        # replica 0, dynamic
+                  [-2.0, 5.0, 7.0],       # replica 0, dynamic
+                  [11.0, -13.0, 17.0],    # replica 0, dynamic
+                  [100.0, 100.0, 100.0],  # replica 0, grip: excluded
+                  [0.5, -0.25, 2.0]])     # replica 1, dynamic
+    flags = np.array([0, 0, 0, 2, 0], dtype=np.int32)
+    offsets = np.array([0, 4, 5], dtype=np.int32)
+    mass = 3.0 * ACC                       # m / ACC = 3 exactly
+    K = ob.kinetic_tensor(v, flags, offsets, mass)
+    # sums over atoms 0..2:  xx = 1 + 4 + 121;  yy = 4 + 25 + 169;  zz = 9 + 49 + 289
+    #                         xy = 2 - 10 - 143;  xz = 3 - 14 + 187;  yz = 6 + 35 - 221
+    expect0 = 3.0 * np.array([126.0, 198.0, 347.0, -151.0, 176.0, -180.0])
+    expect1 = 3.0 * np.array([0.25, 0.0625, 4.0, -0.125, 1.0, -0.5])
+    assert np.allclose(K[0], expect0, rtol=0, atol=1e-12)
+    assert np.allclose(K[1], expect1, rtol=0, atol=1e-12)
+    assert len(set(np.round(expect0, 9))) == 6       # a swapped pair of components cannot pass
+    # and the stress built from it keeps the order: sigma_ab = -(W_ab + K_ab) / V
+    Wv = np.array([[1.0, 2.0, 3.0, 4.0, 5.0, 6.0], [0.0] * 6])
+    sig = ob.stress(Wv, K, np.array([2.0, 4.0]))
+    assert np.allclose(sig[0], -(Wv[0] + expect0) / 2.0, rtol=0, atol=1e-12)
+    assert np.allclose(sig[1], -expect1 / 4.0, rtol=0, atol=1e-12)
+
+
 # ---------------------------------------------------------------- Nose-Hoover (SURVEY 8(f) f1; P:71, reading A17)
 def test_nose_hoover_conserved_quantity_reduction_to_verlet_and_temperature():
     from oracle.nose_hoover import NoseHooverMD, KB
