@@ -111,6 +111,9 @@ int tbsma_build_neighbors(tbsma_ctx *ctx, float *d_pos, float *d_vel, int32_t *d
  * d_ij,a f_ij,b in the order xx yy zz xy xz yz (potential part of Eq.5; D:A11). */
 int tbsma_compute(tbsma_ctx *ctx, const float *d_pos, float *d_force_energy,
                   double *d_replica_energy, double *d_replica_virial, void *stream);
+/* (Shared-memory variant: the per-replica sums of tbsma_compute / tbsma_md_step / tbsma_md_run are added in a fixed
+ * order -- the 32 atoms of a chunk by a shuffle tree, the chunks of a CTA in chunk order, the CTAs of a replica in tile
+ * order -- and are bitwise repeatable from run to run; the global variant adds them with fp64 atomics.) */
 
 /* One MD step of every replica (thermostat D:A8 = BAOAB Langevin, gamma = 0 is exactly
  * velocity Verlet):  B A O A, neighbour rebuild of the replicas whose atoms moved more than
@@ -198,6 +201,13 @@ int tbsma_set_outer_skin(tbsma_ctx *ctx, double outer_skin);
  * 32, <= 512, default 256).  Takes effect at the next tbsma_build_cells. */
 int tbsma_set_tile(tbsma_ctx *ctx, int32_t layers_per_tile, int32_t threads);
 
+/* Shared-memory variant: CTAs of the two gather kernels per tile.  0 (default) = automatic: one, unless the batch has
+ * too few tiles to fill the GPU (a single 3 nm x 6 nm wire is 3 tiles), in which case several CTAs share a tile -- each
+ * stages the tile image and takes a share of its 32-atom chunks -- until there are about eight CTAs per SM or one chunk
+ * per CTA.  Changes cost and the order of the per-replica sums, nothing else.  Takes effect at the next
+ * tbsma_build_cells. */
+int tbsma_set_tile_split(tbsma_ctx *ctx, int32_t ctas_per_tile);
+
 /* md_run replays one captured step as a CUDA graph when `enable` != 0 (default 2) and the stream is not the legacy
  * default stream.  enable = 2: in the shared-memory variant the kernels that renew cells and candidates (needed in a
  * few steps only, decided on the device) are the body of a conditional IF node of that graph, so that nothing is
@@ -241,12 +251,18 @@ int tbsma_set_balance(tbsma_ctx *ctx, int32_t enable, double cell);
  * thermostat mass (D:A17): one variable xi per replica, d xi/dt = (2K - g kB T)/Q, dv/dt = F/m - xi v, Q = g kB T
  * tau_fs^2, g = 3 N_dyn, integrated as B A N A B with N: xi += (dt/2)(2K - g kB T)/Q; v *= exp(-xi dt); K *= s^2;
  * xi += (dt/2)(2K - g kB T)/Q, K the kinetic energy of the dynamic atoms after the opening kick (summed by a kernel of
- * its own at the start of every step).  gamma_per_fs and d_seed of the step calls are ignored, d_T is the target.  xi
+ * its own at the start of every step, in a fixed order: runs of 256 consecutive atoms by a tree, the runs of a replica in
+ * order).  gamma_per_fs and d_seed of the step calls are ignored, d_T is the target.  xi
  * and eta (d eta/dt = xi; E + K + Q xi^2/2 + g kB T eta is conserved) live in the context, start at 0 and are reset by
  * this call and by tbsma_set_system; tbsma_get_thermostat copies them to the host (n_replicas doubles each,
  * synchronises). */
 int tbsma_set_thermostat(tbsma_ctx *ctx, int32_t kind, double tau_fs);
 int tbsma_get_thermostat(tbsma_ctx *ctx, double *h_xi, double *h_eta);
+/* Restores xi and eta (n_replicas doubles each, HOST pointers; synchronises): with pos, vel, force, tag and the step
+ * number, which are the caller's, that is the whole state of a Nose-Hoover run.  (The per-replica kinetic energy that drives
+ * xi is added in a fixed order, so a run repeats bit for bit; a run resumed in a new context rebuilds its neighbour lists
+ * at the restart, i.e. continues with another fp32 summation order: same physics, not the same bits.) */
+int tbsma_set_thermostat_state(tbsma_ctx *ctx, const double *h_xi, const double *h_eta);
 
 /* Replicas built together (all of them, by tbsma_build_neighbors) that share a temperature would all need their
  * next list at nearly the same step, and again one period later.  When enabled (default 1, more than one replica)

@@ -20,7 +20,7 @@ EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_kinetic_tensor", "tbsma_stress", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
-    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin",
+    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_thermostat_state", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin", "tbsma_set_tile_split",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
 
@@ -82,9 +82,11 @@ def lib():
         L.tbsma_set_stagger.argtypes = [vp, i32]
         L.tbsma_set_thermostat.argtypes = [vp, i32, dbl]
         L.tbsma_get_thermostat.argtypes = [vp, vp, vp]
+        L.tbsma_set_thermostat_state.argtypes = [vp, vp, vp]
         L.tbsma_set_async.argtypes = [vp, i32, dbl]
         L.tbsma_set_balance.argtypes = [vp, i32, dbl]
         L.tbsma_set_outer_skin.argtypes = [vp, dbl]
+        L.tbsma_set_tile_split.argtypes = [vp, i32]
         L.tbsma_set_timing.argtypes = [vp, i32]
         L.tbsma_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.tbsma_launch_count.argtypes = [vp]
@@ -239,6 +241,9 @@ class Context:
     def set_outer_skin(self, outer_skin):
         _check(lib().tbsma_set_outer_skin(self._h, float(outer_skin)), "tbsma_set_outer_skin")
 
+    def set_tile_split(self, ctas_per_tile):
+        _check(lib().tbsma_set_tile_split(self._h, int(ctas_per_tile)), "tbsma_set_tile_split")
+
     def set_thermostat(self, kind, tau_fs=0.0):
         _check(lib().tbsma_set_thermostat(self._h, int(kind), float(tau_fs)), "tbsma_set_thermostat")
 
@@ -246,6 +251,12 @@ class Context:
         xi, eta = np.zeros(self.R), np.zeros(self.R)
         _check(lib().tbsma_get_thermostat(self._h, _hp(xi), _hp(eta)), "tbsma_get_thermostat")
         return xi, eta
+
+    def set_thermostat_state(self, xi, eta):
+        xi = np.ascontiguousarray(xi, dtype=np.float64)
+        eta = np.ascontiguousarray(eta, dtype=np.float64)
+        assert len(xi) == self.R and len(eta) == self.R
+        _check(lib().tbsma_set_thermostat_state(self._h, _hp(xi), _hp(eta)), "tbsma_set_thermostat_state")
 
     def set_stagger(self, enable):
         _check(lib().tbsma_set_stagger(self._h, int(bool(enable))), "tbsma_set_stagger")

@@ -38,10 +38,12 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_cell_of); cudaFree(c->d_slot); cudaFree(c->d_order); cudaFree(c->d_pos_build);
     cudaFree(c->d_tmp4); cudaFree(c->d_tmp_tag); cudaFree(c->d_nlist); cudaFree(c->d_nn); cudaFree(c->d_xs);
     cudaFree(c->d_dirty); cudaFree(c->d_ctrl); cudaFree(c->d_counters); cudaFree(c->d_stagger); cudaFree(c->d_cur);
-    cudaFree(c->d_nh); cudaFree(c->d_kmid); cudaFree(c->d_nh_scale);
+    cudaFree(c->d_nh); cudaFree(c->d_kmid); cudaFree(c->d_nh_scale); cudaFree(c->d_blk_rep); cudaFree(c->d_blk_first);
     c->d_stagger = nullptr; c->d_cur = nullptr; c->d_nh = nullptr; c->d_kmid = nullptr; c->d_nh_scale = nullptr;
+    c->d_blk_rep = nullptr; c->d_blk_first = nullptr; c->n_blk = 0;
     cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_tileof); cudaFree(c->d_img); cudaFree(c->d_inv);
     c->d_tileof = nullptr; c->d_img = nullptr; c->d_inv = nullptr;
+    cudaFree(c->d_cta_sums); c->d_cta_sums = nullptr; c->have_sums = 0;
     cudaFree(c->d_newslot); cudaFree(c->d_oldof);
     cudaFree(c->d_nn_tmp); cudaFree(c->d_tmp_pos);
     cudaFree(c->d_tile_first); cudaFree(c->d_work);
@@ -173,9 +175,10 @@ int ensure_variant_resources(tbsma_ctx *c)
 int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *tag, double dt, const float *T,
               double gamma, const unsigned long long *seed, unsigned long long step0, int64_t n_steps,
               const double *disp0, const double *rate, int rebuild_every, double *e_rep, double *w_rep,
-              double *ekin, bool advance, cudaStream_t st)
+              double *ekin, bool advance, cudaStream_t st, bool step_on_device = false)
 {
     StepArgs a;
+    a.step_on_device = step_on_device ? 1 : 0;
     a.half_dt = (float)(0.5 * dt);
     a.kick = (float)(0.5 * dt * TBSMA_ACC / c->prm.mass_amu);
     const double c1 = exp(-gamma * dt);
@@ -205,6 +208,18 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         cudaEvent_t *ev = nullptr;
         if (c->timing && c->tev && c->tev_steps < TBSMA_TIMING_MAX_STEPS) ev = c->tev + 6 * (c->tev_steps++);
         if (ev) CK(cudaEventRecord(ev[0], st));
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        cudaGraph_t cg = nullptr;
+        const cudaGraphNode_t *deps = nullptr;
+        size_t n_deps = 0;
+        cudaGraphConditionalHandle cond = 0;
+        bool use_cond = false;
+        if (tiles) {
+            if (st && c->use_cond && c->body_stream &&
+                cudaStreamGetCaptureInfo(st, &cap, nullptr, &cg, &deps, &n_deps) == cudaSuccess &&
+                cap == cudaStreamCaptureStatusActive && cg)
+                use_cond = cudaGraphConditionalHandleCreate(&cond, cg, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+        }
         if (nose_hoover) CK(tbsma_launch_nose_hoover(c, pos, vel, force, a, dt, st));
         CK(tbsma_launch_integrate_pre(c, pos, vel, force, tag, a, st));
         if (ev) CK(cudaEventRecord(ev[1], st));
@@ -215,16 +230,6 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
             // A list that is only re-filtered from its candidates (dirty == 1) is, when `async`, asked for `margin`
             // early and written to the other half while the gather passes of this step still read the old one, on a
             // second stream; the step's last kernel swaps the halves.
-            cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-            cudaGraph_t cg = nullptr;
-            const cudaGraphNode_t *deps = nullptr;
-            size_t n_deps = 0;
-            cudaGraphConditionalHandle cond = 0;
-            bool use_cond = false;
-            if (st && c->use_cond && c->body_stream &&
-                cudaStreamGetCaptureInfo(st, &cap, nullptr, &cg, &deps, &n_deps) == cudaSuccess &&
-                cap == cudaStreamCaptureStatusActive && cg)
-                use_cond = cudaGraphConditionalHandleCreate(&cond, cg, 0, cudaGraphCondAssignDefault) == cudaSuccess;
             CK(tbsma_launch_tile_worklist(c, st, (unsigned long long)cond, use_cond ? 1 : 0));
             if (use_cond) {
                 // IF (a replica needs new cells and candidates) { chain; its inner lists }: nothing is launched otherwise
@@ -274,11 +279,12 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         if (tiles) CK(tbsma_launch_density_tile(c, pos, sync_level, st, early));
         else CK(tbsma_launch_density(c, pos, st));
         if (ev) CK(cudaEventRecord(ev[3], st));
-        if (tiles) CK(tbsma_launch_force_tile(c, force, e_rep, w_rep, kk, sync_level, st));
+        if (tiles) CK(tbsma_launch_force_tile(c, force, w_rep != nullptr, kk, sync_level, st));
         else CK(tbsma_launch_force(c, force, e_rep, w_rep, kk, st));
         if (ev) CK(cudaEventRecord(ev[4], st));
         if (forked && !joined) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
-        CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st));
+        CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st,
+                                    tiles ? tbsma_tile_sums(c, e_rep, ekin, w_rep) : TileSums()));
         if (ev) CK(cudaEventRecord(ev[5], st));
     }
     return TBSMA_OK;
@@ -393,6 +399,15 @@ int tbsma_set_tile(tbsma_ctx *c, int32_t layers_per_tile, int32_t threads)
     return TBSMA_OK;
 }
 
+int tbsma_set_tile_split(tbsma_ctx *c, int32_t ctas_per_tile)
+{
+    if (!c || ctas_per_tile < 0 || ctas_per_tile > 128) return TBSMA_EINVAL;
+    c->epoch++;
+    c->tile_split_req = ctas_per_tile;
+    c->cells_built = c->list_built = 0;
+    return TBSMA_OK;
+}
+
 int tbsma_set_outer_skin(tbsma_ctx *c, double outer_skin)
 {
     if (!c || !(outer_skin >= 0.0) || !(outer_skin <= 16.0)) return TBSMA_EINVAL;
@@ -448,6 +463,20 @@ int tbsma_get_thermostat(tbsma_ctx *c, double *h_xi, double *h_eta)
     if (!h) return TBSMA_ENOMEM;
     const cudaError_t e = cudaMemcpy(h, c->d_nh, sizeof(double) * 2 * (size_t)c->R, cudaMemcpyDeviceToHost);
     for (int r = 0; r < c->R && e == cudaSuccess; ++r) { h_xi[r] = h[2 * r]; h_eta[r] = h[2 * r + 1]; }
+    free(h);
+    CK(e);
+    return TBSMA_OK;
+}
+
+int tbsma_set_thermostat_state(tbsma_ctx *c, const double *h_xi, const double *h_eta)
+{
+    if (!c || !h_xi || !h_eta) return TBSMA_EINVAL;
+    if (!c->d_nh) return TBSMA_ESTATE;
+    CK(cudaDeviceSynchronize());
+    double *h = (double *)malloc(sizeof(double) * 2 * (size_t)(c->R ? c->R : 1));
+    if (!h) return TBSMA_ENOMEM;
+    for (int r = 0; r < c->R; ++r) { h[2 * r] = h_xi[r]; h[2 * r + 1] = h_eta[r]; }
+    const cudaError_t e = cudaMemcpy(c->d_nh, h, sizeof(double) * 2 * (size_t)c->R, cudaMemcpyHostToDevice);
     free(h);
     CK(e);
     return TBSMA_OK;
@@ -565,7 +594,11 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     const size_t nb = (size_t)c->list_bufs;
     DA(c->d_pos_build, nb * c->n_pad); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
     DA(c->d_nlist, nb * (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, nb * c->n_pad); DA(c->d_xs, n);
-    DA(c->d_cur, (size_t)R); DA(c->d_nh, 2 * (size_t)R); DA(c->d_kmid, 2 * (size_t)R); DA(c->d_nh_scale, (size_t)R);
+    int64_t n_blk = 0;
+    for (int r = 0; r < R; ++r) n_blk += (h_off[r + 1] - h_off[r] + 255) / 256;
+    c->n_blk = (int)n_blk;
+    DA(c->d_cur, (size_t)R); DA(c->d_nh, 2 * (size_t)R); DA(c->d_kmid, 2 * (size_t)n_blk); DA(c->d_nh_scale, (size_t)R);
+    DA(c->d_blk_rep, (size_t)n_blk); DA(c->d_blk_first, (size_t)R + 1);
     DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8); DA(c->d_stagger, (size_t)R);
     DA(c->d_maxpop, (size_t)R); DA(c->d_hbase, n); DA(c->d_tileof, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
     DA(c->d_tmp_pos, n);
@@ -577,6 +610,20 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
         for (int64_t i = h_off[r]; i < h_off[r + 1]; ++i) rep[i] = r;
     e = cudaMemcpy(c->d_atom_rep, rep, sizeof(int32_t) * n, cudaMemcpyHostToDevice);
     free(rep);
+    {   // runs of 256 consecutive atoms of one replica (ordered sums of the Nose-Hoover kinetic energy)
+        int32_t *br = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_blk ? n_blk : 1));
+        int32_t *bf = (int32_t *)malloc(sizeof(int32_t) * (size_t)(R + 1));
+        if (!br || !bf) { free(br); free(bf); free_system(c); return TBSMA_ENOMEM; }
+        int64_t k = 0;
+        for (int r = 0; r < R; ++r) {
+            bf[r] = (int32_t)k;
+            for (int64_t b = 0; b < (h_off[r + 1] - h_off[r] + 255) / 256; ++b) br[k++] = r;
+        }
+        bf[R] = (int32_t)k;
+        if (e == cudaSuccess) e = cudaMemcpy(c->d_blk_rep, br, sizeof(int32_t) * (size_t)n_blk, cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(c->d_blk_first, bf, sizeof(int32_t) * (size_t)(R + 1), cudaMemcpyHostToDevice);
+        free(br); free(bf);
+    }
     if (e == cudaSuccess) e = cudaMemset(c->d_dirty, 0, sizeof(int32_t) * R);
     if (e == cudaSuccess) e = cudaMemset(c->d_stagger, 0, sizeof(float) * R);
     if (e == cudaSuccess) e = cudaMemset(c->d_ctrl, 0, sizeof(int32_t) * 8);
@@ -606,6 +653,9 @@ int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, 
         if (rc0) return rc0;
     }
     c->active_variant = (c->variant != 1 && !c->any_periodic) ? 2 : 1;   // provisional: selects the dirty level
+    // every list is rebuilt from here on: all replicas start from half 0 of the list buffers again (the global variant
+    // only ever uses half 0; after a run in the tile variant some replicas would otherwise still point at half 1)
+    CK(cudaMemsetAsync(c->d_cur, 0, sizeof(int32_t) * (size_t)c->R, st));
     CK(tbsma_launch_mark_all_dirty(c, st));
     CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, true, false, st));
     const int rc = tbsma_tile_setup(c, st);   // picks the gather variant for these cells (synchronises)
@@ -642,7 +692,8 @@ int tbsma_compute(tbsma_ctx *c, const float *d_pos, float *d_force_energy, doubl
     KickArgs kk = {nullptr, 0.f, 0.f, nullptr};
     if (c->active_variant == 2) {
         CK(tbsma_launch_density_tile(c, (const float4 *)d_pos, 1, st));
-        CK(tbsma_launch_force_tile(c, (float4 *)d_force_energy, d_e, d_w, kk, 1, st));
+        CK(tbsma_launch_force_tile(c, (float4 *)d_force_energy, d_w != nullptr, kk, 1, st));
+        CK(tbsma_launch_reduce_replicas(c, d_e, nullptr, d_w, st));
     } else {
         CK(tbsma_launch_density(c, (const float4 *)d_pos, st));
         CK(tbsma_launch_force(c, (float4 *)d_force_energy, d_e, d_w, kk, st));
@@ -694,15 +745,15 @@ int tbsma_md_run(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energy
         memset(&key, 0, sizeof(key));
         key.p[0] = pos; key.p[1] = vel; key.p[2] = force; key.p[3] = d_tag; key.p[4] = d_T; key.p[5] = seed;
         key.p[6] = d_disp0; key.p[7] = d_rate; key.p[8] = d_e; key.p[9] = d_w; key.p[10] = d_k;
-        key.dt = dt_fs; key.gamma = gamma_per_fs; key.step0 = step0; key.rebuild_every = rebuild_every;
+        key.dt = dt_fs; key.gamma = gamma_per_fs; key.rebuild_every = rebuild_every;
         key.epoch = c->epoch;
         if (!c->graph_exec || memcmp(&key, &c->graph_key, sizeof(key)) != 0) {
             if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
             cudaGraph_t g = nullptr;
             CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
             const int64_t before = c->launches;
-            int rc = run_steps(c, pos, vel, force, d_tag, dt_fs, d_T, gamma_per_fs, seed, step0, 1, d_disp0, d_rate,
-                               rebuild_every, d_e, d_w, d_k, true, st);
+            int rc = run_steps(c, pos, vel, force, d_tag, dt_fs, d_T, gamma_per_fs, seed, 0, 1, d_disp0, d_rate,
+                               rebuild_every, d_e, d_w, d_k, true, st, true);
             cudaError_t e = cudaStreamEndCapture(st, &g);
             c->graph_launches_per_step = c->launches - before;
             c->launches = before;
@@ -713,6 +764,8 @@ int tbsma_md_run(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energy
             if (e != cudaSuccess) { c->graph_exec = nullptr; return map_cuda(e); }
             c->graph_key = key;
         }
+        // the captured step reads the number of the run's first step from the device: one graph serves every step0
+        CK(tbsma_launch_set_step_base(c, step0, st));
         for (int64_t s = 0; s < n_steps; ++s) CK(cudaGraphLaunch(c->graph_exec, st));
         c->launches += c->graph_launches_per_step * n_steps;
     }

@@ -54,9 +54,9 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
         if (a.ekin) a.ekin[i] = 0.0;
         if (a.w_rep) for (int k = 0; k < 6; ++k) a.w_rep[6 * i + k] = 0.0;
     }
-    if (i >= n) return;
+    if (i < n) {
     const unsigned long long off = counters[0];
-    const unsigned long long step = a.step_base + off;
+    const unsigned long long step = (a.step_on_device ? counters[7] : a.step_base) + off;
     const int r = atom_rep[i];
     float4 p = pos[i], v = vel[i];
     const int flag = __float_as_int(p.w) & 3;
@@ -89,7 +89,10 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
     const float d2 = dx * dx + dy * dy + dz * dz;
     const bool cadence = a.rebuild_every > 0 && (step % (unsigned long long)a.rebuild_every) == 0ull;
     if (d2 > a.skin_half2 && a.trigger2 < a.skin_half2) atomicOr(ctrl + 1, (int)TBSMA_FLAG_SKIN_VIOLATED);
-    if (d2 > a.trigger2 * a.stagger[r] || cadence) {
+    // (the staggered first rebuild is for displacement-triggered lists only: with a fixed cadence an early trigger
+    // would be reported as a violated skin)
+    const float trig2 = a.rebuild_every > 0 ? a.trigger2 : a.trigger2 * a.stagger[r];
+    if (d2 > trig2 || cadence) {
         // level 2 = cells + candidate list too (tile variant, decided at the replica's previous rebuild)
         const int level = (a.want_outer && a.want_outer[r]) ? 2 : 1;
         dirty[r] = level;
@@ -97,14 +100,18 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
         if (level == 2) ctrl[3] = 1;
         if (a.rebuild_every > 0 && !cadence) atomicOr(ctrl + 1, (int)TBSMA_FLAG_SKIN_VIOLATED);
     }
+    }
 }
 
 // end of step: statistics, clear the dirty flags, advance the in-run step offset
-__global__ void k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl, int *__restrict__ want_outer,
-                              float *__restrict__ stagger, int *__restrict__ cur, int swap,
-                              unsigned long long *__restrict__ counters, int R, int advance, int count_step)
+__global__ void __launch_bounds__(256)
+k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl, int *__restrict__ want_outer,
+              float *__restrict__ stagger, int *__restrict__ cur, int swap,
+              unsigned long long *__restrict__ counters, int R, int advance, int count_step, TileSums ts)
 {
     __shared__ int s_cnt, s_cnt2;
+    tbsma_reduce_replicas(ts, R);      // a6 of the tile variant: per-replica E, E_kin, W in a fixed order (all CTAs)
+    if (blockIdx.x != 0) return;       // the bookkeeping below is CTA 0's
     if (threadIdx.x == 0) { s_cnt = 0; s_cnt2 = 0; }
     __syncthreads();
     if (ctrl[0]) {
@@ -150,44 +157,53 @@ __global__ void k_set_stagger(float *__restrict__ stagger, int R, int enable)
 // is summed by a kernel of its own from (v, F) with the kick of k_integrate_pre, operation for operation; a thread per
 // replica then advances xi and eta (d eta/dt = xi: the conserved quantity is E + K + Q xi^2/2 + g kB T eta) and leaves
 // the scale for the integrator.
+// One CTA per run of 256 consecutive atoms of ONE replica (the runs are laid out by tbsma_set_system: blk_first[r] is
+// the first run of replica r), a fixed tree inside the CTA, and k_nh_update adds the runs of a replica in order: the
+// kinetic energy that drives xi is bitwise repeatable, and with it the whole Nose-Hoover trajectory.
 __global__ void __launch_bounds__(256)
 k_nh_kinetic(const float4 *__restrict__ pos, const float4 *__restrict__ vel, const float4 *__restrict__ force,
-             const int *__restrict__ atom_rep, double *__restrict__ kmid, float kick, double half_m_over_c, int n)
+             const int *__restrict__ blk_rep, const int *__restrict__ blk_first, const RepGeom *__restrict__ geom,
+             double *__restrict__ kpart, float kick, double half_m_over_c)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    int r = -1;
+    __shared__ double red[2][256];
+    const int j = blockIdx.x, r = blk_rep[j];
+    const int i = geom[r].atom_begin + 256 * (j - blk_first[r]) + (int)threadIdx.x;
     double k = 0.0, cnt = 0.0;
-    if (i < n) {
-        r = atom_rep[i];
-        if ((__float_as_int(pos[i].w) & 3) == 0) {
-            const float4 v = vel[i], f = force[i];
-            const double vx = __fmaf_rn(kick, f.x, v.x), vy = __fmaf_rn(kick, f.y, v.y), vz = __fmaf_rn(kick, f.z, v.z);
-            k = half_m_over_c * (vx * vx + vy * vy + vz * vz);
-            cnt = 1.0;
-        }
+    if (i < geom[r].atom_end && (__float_as_int(pos[i].w) & 3) == 0) {
+        const float4 v = vel[i], f = force[i];
+        const double vx = __fmaf_rn(kick, f.x, v.x), vy = __fmaf_rn(kick, f.y, v.y), vz = __fmaf_rn(kick, f.z, v.z);
+        k = half_m_over_c * (vx * vx + vy * vy + vz * vz);
+        cnt = 1.0;
     }
-    const int r0 = __shfl_sync(0xffffffffu, r, 0);
-    if (__all_sync(0xffffffffu, r == r0)) {
-        if (r0 < 0) return;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            k += __shfl_xor_sync(0xffffffffu, k, o);
-            cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    red[0][threadIdx.x] = k;
+    red[1][threadIdx.x] = cnt;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            red[0][threadIdx.x] += red[0][threadIdx.x + o];
+            red[1][threadIdx.x] += red[1][threadIdx.x + o];
         }
-        if (lane == 0) { atomicAdd(kmid + 2 * (size_t)r0, k); atomicAdd(kmid + 2 * (size_t)r0 + 1, cnt); }
-    } else if (r >= 0) {
-        atomicAdd(kmid + 2 * (size_t)r, k);
-        atomicAdd(kmid + 2 * (size_t)r + 1, cnt);
+        __syncthreads();
     }
+    if (threadIdx.x == 0) { kpart[2 * (size_t)j] = red[0][0]; kpart[2 * (size_t)j + 1] = red[1][0]; }
 }
 
-__global__ void k_nh_update(const double *__restrict__ kmid, const float *__restrict__ T, double *__restrict__ nh,
-                            float *__restrict__ scale, double dt, double tau, int R)
+// a warp per replica: K and the number of dynamic atoms from the runs (lane l adds runs l, l + 32, ... in order, then a
+// shuffle tree), then lane 0 advances xi and eta
+__global__ void __launch_bounds__(256)
+k_nh_update(const double *__restrict__ kpart, const int *__restrict__ blk_first, const float *__restrict__ T,
+            double *__restrict__ nh, float *__restrict__ scale, double dt, double tau, int R)
 {
-    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)blockIdx.x * 8 + (int)(threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (r >= R) return;
-    const double K = kmid[2 * r], g = 3.0 * kmid[2 * r + 1];
+    double K = 0.0, nd = 0.0;
+    for (int j = blk_first[r] + lane; j < blk_first[r + 1]; j += 32) { K += kpart[2 * (size_t)j]; nd += kpart[2 * (size_t)j + 1]; }
+    for (int o = 16; o > 0; o >>= 1) {
+        K += __shfl_xor_sync(0xffffffffu, K, o);
+        nd += __shfl_xor_sync(0xffffffffu, nd, o);
+    }
+    if (lane != 0) return;
+    const double g = 3.0 * nd;
     const double gkt = g * TBSMA_KB * (double)T[r];
     double s = 1.0;
     if (gkt > 0.0 && tau > 0.0) {
@@ -253,12 +269,10 @@ __global__ void k_stress(const double *__restrict__ w_rep, const double *__restr
 cudaError_t tbsma_launch_nose_hoover(tbsma_ctx *c, const float4 *pos, const float4 *vel, const float4 *force,
                                      const StepArgs &a, double dt, cudaStream_t st)
 {
-    cudaError_t e = cudaMemsetAsync(c->d_kmid, 0, sizeof(double) * 2 * (size_t)c->R, st);
-    if (e != cudaSuccess) return e;
-    const int n = (int)c->n;
-    k_nh_kinetic<<<(n + 255) / 256, 256, 0, st>>>(pos, vel, force, c->d_atom_rep, c->d_kmid, a.kick,
-                                                 0.5 * c->prm.mass_amu / TBSMA_ACC, n);
-    k_nh_update<<<(c->R + 127) / 128, 128, 0, st>>>(c->d_kmid, a.T, c->d_nh, c->d_nh_scale, dt, c->nh_tau, c->R);
+    if (c->n_blk == 0) return cudaSuccess;
+    k_nh_kinetic<<<c->n_blk, 256, 0, st>>>(pos, vel, force, c->d_blk_rep, c->d_blk_first, c->d_geom, c->d_kmid, a.kick,
+                                           0.5 * c->prm.mass_amu / TBSMA_ACC);
+    k_nh_update<<<(c->R + 7) / 8, 256, 0, st>>>(c->d_kmid, c->d_blk_first, a.T, c->d_nh, c->d_nh_scale, dt, c->nh_tau, c->R);
     c->launches += 2;
     return cudaGetLastError();
 }
@@ -281,6 +295,15 @@ cudaError_t tbsma_launch_stress(tbsma_ctx *c, const double *w_rep, const double 
     return cudaGetLastError();
 }
 
+__global__ void k_set_u64(unsigned long long *p, unsigned long long v) { *p = v; }
+
+cudaError_t tbsma_launch_set_step_base(tbsma_ctx *c, unsigned long long step0, cudaStream_t st)
+{
+    k_set_u64<<<1, 1, 0, st>>>(c->d_counters + 7, step0);
+    c->launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st)
 {
     k_set_stagger<<<(c->R + 255) / 256, 256, 0, st>>>(c->d_stagger, c->R, c->stagger);
@@ -299,11 +322,11 @@ cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, c
     return cudaGetLastError();
 }
 
-cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st)
+cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st, TileSums ts)
 {
-    k_finish_step<<<1, 256, 0, st>>>(c->d_dirty, c->d_ctrl, c->active_variant == 2 ? c->d_want_outer : nullptr,
+    k_finish_step<<<ts.cta_sums ? tbsma_reduce_grid(c->R) : 1, 256, 0, st>>>(c->d_dirty, c->d_ctrl, c->active_variant == 2 ? c->d_want_outer : nullptr,
                                      c->d_stagger, c->d_cur, c->list_bufs == 2 && c->active_variant == 2, c->d_counters, c->R, advance_offset & 1,
-                                     (advance_offset >> 1) & 1);
+                                     (advance_offset >> 1) & 1, ts);
     c->launches++;
     return cudaGetLastError();
 }

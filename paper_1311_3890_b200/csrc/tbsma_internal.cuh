@@ -64,7 +64,6 @@ struct DirtyView {
 struct GraphKey {          // arguments a cached one-step CUDA graph was captured with
     const void *p[11];
     double dt, gamma;
-    unsigned long long step0;
     int rebuild_every;
     int epoch;             // tbsma_ctx::epoch when captured: any call that re-sizes, re-allocates or re-tunes bumps it
 };
@@ -102,6 +101,10 @@ struct tbsma_ctx {
     int32_t *d_work;       // [0] tiles of replicas with dirty >= 1, [1] with dirty == 2, then the two tile lists
                            // (n_tiles entries each), rebuilt every step by k_tile_worklist
     int own_cap;           // own atoms a tile may hold (sizes the split of the inner build)
+    int tile_nsplit;       // CTAs of the gather kernels per tile (> 1 when the tiles are too few to fill the GPU)
+    int tile_split_req;    // requested by tbsma_set_tile_split (0 = automatic)
+    double *d_cta_sums;    // n_tiles x tile_nsplit x 8: E, E_kin, W (xx yy zz xy xz yz) of every CTA of the force pass
+    size_t have_sums;
     int32_t *d_maxpop;  // R: largest layer population of each replica (measured at build_cells)
     int32_t *d_hbase;   // n: first halo slot of the tile that owns slot i
     int32_t *d_tileof;  // n: the tile that owns slot i
@@ -151,7 +154,8 @@ struct tbsma_ctx {
     int stagger;            // enabled (default 1)
     int32_t *d_ctrl;        // [0] any replica dirty, [1] status flags, [2] max neighbours seen, [3] any dirty == 2
     unsigned long long *d_counters; // [0] step offset inside md_run, [1] replica builds, [2] build passes, [3] steps,
-                                    // [4..5] count_pairs scratch, [6] replica builds that redid cells + candidates
+                                    // [4..5] count_pairs scratch, [6] replica builds that redid cells + candidates,
+                                    // [7] step number of the first step of the md_run in flight (captured steps read it)
     // host staging for *_host entry point
     float4 *s_pos, *s_vel, *s_force;
     int32_t *s_tag;
@@ -165,7 +169,11 @@ struct tbsma_ctx {
     int thermostat_kind;       // 0 Langevin (gamma of tbsma_md_step), 1 Nose-Hoover
     double nh_tau;             // fs: Q = g kB T tau^2
     double *d_nh;              // 2 R: xi, eta
-    double *d_kmid;            // 2 R: kinetic energy after the opening kick, number of dynamic atoms
+    double *d_kmid;            // 2 n_blk: kinetic energy after the opening kick and number of dynamic atoms of every run
+                               // of 256 consecutive atoms of a replica
+    int32_t *d_blk_rep;        // n_blk: replica of the run
+    int32_t *d_blk_first;      // R + 1: first run of every replica
+    int n_blk;
     float *d_nh_scale;         // R
     int cells_built, list_built;
     int epoch;                 // bumped by every call after which a captured step would hold stale arguments
@@ -204,6 +212,65 @@ inline DirtyView tbsma_dirty_view(const tbsma_ctx *c)
 }
 cudaError_t tbsma_launch_get_neighbors(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
                                        cudaStream_t st);
+// a6 in the tile variant: per-replica sums from the sums the CTAs of the force pass left, in tile order
+struct TileSums {
+    const double *cta_sums;   // nullptr: nothing to do
+    const int *tile_first;    // R + 1
+    int nsplit;
+    double *e_rep, *ekin, *w_rep;   // each nullable
+};
+#ifdef __CUDACC__
+// Called by all threads of every CTA of a grid of tbsma_reduce_grid(R) CTAs of 256 threads.  Many replicas: a warp per
+// replica, lane l adds the replica's CTAs l, l + 32, ... in order and a shuffle tree adds the lanes.  Few replicas (one
+// long wire has thousands of tiles): CTA 0 takes one replica at a time, thread t adds CTAs t, t + 256, ... and a fixed
+// tree adds the threads.  Either way the order is fixed: bitwise repeatable.
+inline int tbsma_reduce_grid(int R) { return R >= 64 ? (R + 7) / 8 : 1; }
+__device__ inline void tbsma_reduce_replicas(const TileSums &ts, int R)
+{
+    if (!ts.cta_sums) return;
+    const int nq = ts.w_rep ? 8 : 2;
+    if (R >= 64) {
+        const int r = (int)blockIdx.x * 8 + (int)(threadIdx.x >> 5), lane = threadIdx.x & 31;
+        if (r >= R) return;
+        double acc[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        const int j0 = ts.tile_first[r] * ts.nsplit, j1 = ts.tile_first[r + 1] * ts.nsplit;
+        for (int j = j0 + lane; j < j1; j += 32)
+            for (int q = 0; q < nq; ++q) acc[q] += ts.cta_sums[8 * (size_t)j + q];
+        for (int q = 0; q < nq; ++q)
+            for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+        if (lane == 0) {
+            if (ts.e_rep) ts.e_rep[r] = acc[0];
+            if (ts.ekin) ts.ekin[r] = acc[1];
+            if (ts.w_rep)
+                for (int q = 0; q < 6; ++q) ts.w_rep[6 * (size_t)r + q] = acc[2 + q];
+        }
+        return;
+    }
+    if (blockIdx.x != 0) return;
+    __shared__ double red[8][256];
+    for (int r = 0; r < R; ++r) {
+        double acc[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        const int j0 = ts.tile_first[r] * ts.nsplit, j1 = ts.tile_first[r + 1] * ts.nsplit;
+        for (int j = j0 + (int)threadIdx.x; j < j1; j += 256)
+            for (int q = 0; q < nq; ++q) acc[q] += ts.cta_sums[8 * (size_t)j + q];
+        __syncthreads();
+        for (int q = 0; q < nq; ++q) red[q][threadIdx.x] = acc[q];
+        __syncthreads();
+        for (int o = 128; o > 0; o >>= 1) {
+            if ((int)threadIdx.x < o)
+                for (int q = 0; q < nq; ++q) red[q][threadIdx.x] += red[q][threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) {
+            if (ts.e_rep) ts.e_rep[r] = red[0][0];
+            if (ts.ekin) ts.ekin[r] = red[1][0];
+            if (ts.w_rep)
+                for (int q = 0; q < 6; ++q) ts.w_rep[6 * (size_t)r + q] = red[2 + q][0];
+        }
+    }
+}
+#endif
+
 // forces (tbsma_force.cu)
 struct KickArgs {
     float4 *vel;          // nullptr = no fused half kick
@@ -229,8 +296,12 @@ cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float
 // dirty >= sync_level (their rebuild ran ahead of the launch), the half in use for all others.
 cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st,
                                       bool early = false);
-cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kick,
-                                    int sync_level, cudaStream_t st);
+// leaves the sums of every CTA in d_cta_sums (virial: with W); per-replica sums by tbsma_launch_reduce_replicas or,
+// inside an MD step, by k_finish_step
+cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, bool virial, KickArgs kick, int sync_level,
+                                    cudaStream_t st);
+TileSums tbsma_tile_sums(const tbsma_ctx *c, double *e_rep, double *ekin, double *w_rep);
+cudaError_t tbsma_launch_reduce_replicas(tbsma_ctx *c, double *e_rep, double *ekin, double *w_rep, cudaStream_t st);
 cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
                                             cudaStream_t st);
 cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsigned long long *d_out2,
@@ -245,6 +316,7 @@ struct StepArgs {
     int thermostat;          // gamma > 0
     int rebuild_every;
     unsigned long long step_base;
+    int step_on_device;      // the step number of the run's first step is d_counters[7], not step_base (captured steps)
     const float *T;
     const unsigned long long *seed;
     const double *disp0;     // nullable
@@ -256,8 +328,9 @@ struct StepArgs {
 };
 cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, const float4 *force,
                                        const int32_t *tag, const StepArgs &a, cudaStream_t st);
-cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st);
+cudaError_t tbsma_launch_finish_step(tbsma_ctx *c, int advance_offset, cudaStream_t st, TileSums ts = TileSums());
 cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st);
+cudaError_t tbsma_launch_set_step_base(tbsma_ctx *c, unsigned long long step0, cudaStream_t st);
 cudaError_t tbsma_launch_nose_hoover(tbsma_ctx *c, const float4 *pos, const float4 *vel, const float4 *force,
                                      const StepArgs &a, double dt, cudaStream_t st);
 cudaError_t tbsma_launch_kinetic_tensor(tbsma_ctx *c, const float4 *pos, const float4 *vel, double *k_rep, cudaStream_t st);

@@ -739,12 +739,14 @@ __device__ __forceinline__ uint2 ld_row(const uint2 *row, int g, int ng, int n_p
     return g < ng ? __ldcs(row + (size_t)g * n_pad) : make_uint2(0u, 0u);
 }
 
-// stage 1 (Eq.1): rho_i over the list, s_i = rho_i^(-1/2) packed with the position
+// stage 1 (Eq.1): rho_i over the list, s_i = rho_i^(-1/2) packed with the position.
+// SPLIT: the CTA takes part `part` of `nsplit` of the tile's chunks (small batches); otherwise all of them
+template <bool SPLIT>
 __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__restrict__ cell_start,
                                              const float4 *__restrict__ pos, const uint2 *__restrict__ nl,
                                              const int *__restrict__ nn, float4 *__restrict__ xs,
                                              int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
-                                             const unsigned short *__restrict__ img)
+                                             const unsigned short *__restrict__ img, int part, int nsplit)
 {
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
@@ -752,13 +754,21 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
         if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
         return;
     }
+    // this CTA's share of the tile's 32-atom chunks (all of them unless the batch is too small to fill the GPU)
+    // (the range lives in shared memory: the loops below have no register to spare)
     extern __shared__ float4 smem_f4[];
-    __shared__ int s_next;
+    __shared__ int s_next, s_end;
+    {
+        const int nchunk_all = (r.hi - r.lo + 31) >> 5;
+        const int cb = SPLIT ? nchunk_all * part / nsplit : 0, ce = SPLIT ? nchunk_all * (part + 1) / nsplit : nchunk_all;
+        if (ce <= cb) return;
+        if (threadIdx.x == 0) { s_next = cb; s_end = ce; }
+    }
     const float4 *sm = smem_f4;
-    if (threadIdx.x == 0) s_next = 0;
     fill_image(smem_f4, pos, img, r.halo_lo, r.nh);
-    const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
-    for (int ch = next_chunk(&s_next); ch < nchunk; ch = next_chunk(&s_next)) {
+    const int lane = threadIdx.x & 31;
+    const int nchunk = (r.hi - r.lo + 31) >> 5;
+    for (int ch = next_chunk(&s_next); ch < (SPLIT ? s_end : nchunk); ch = next_chunk(&s_next)) {
         const int i = r.lo + (ch << 5) + lane;
         if (i >= r.hi) continue;
         const float4 pi = pos[i];
@@ -800,23 +810,26 @@ struct ListSel {
     int n_stride;
     const unsigned short *img;   // image placement of every tile (k_tile_place)
     int img_stride;
+    int nsplit;                  // CTAs per tile (> 1 when the tiles are too few to fill the GPU)
 };
 __device__ __forceinline__ int list_half(const ListSel &ls, int rep)
 {
     return ls.cur[rep] ^ (ls.dirty[rep] >= ls.sync_level ? 1 : 0);
 }
 
-// one CTA per tile.  nn and nl are read-only here: they were written by an earlier kernel (or, the half not read,
+// one CTA per tile (or per part of a tile, ls.nsplit).  nn and nl are read-only here: they were written by an earlier kernel (or, the half not read,
 // are being written by the filter pass running beside this launch).
+template <bool SPLIT>
 __global__ void __launch_bounds__(512, 2)
 k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
                const float4 *__restrict__ pos, const uint2 *__restrict__ nl, const int *__restrict__ nn,
                float4 *__restrict__ xs, int *__restrict__ ctrl, ListSel ls, int n_pad, int s_cap, PairConst pc)
 {
-    const TileDesc t = tiles[blockIdx.x];
+    const int ti = SPLIT ? (int)blockIdx.x / ls.nsplit : (int)blockIdx.x, part = SPLIT ? (int)blockIdx.x % ls.nsplit : 0;
+    const TileDesc t = tiles[ti];
     const int h = list_half(ls, t.rep);
-    density_tile(t, cell_start, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad, s_cap,
-                 pc, ls.img + (size_t)blockIdx.x * ls.img_stride);
+    density_tile<SPLIT>(t, cell_start, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad, s_cap,
+                 pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit);
     // Launched as a programmatic dependent of the filter kernel this pass starts early and reads nothing of it; but the
     // kernels after it (force pass, then the swap of the list halves) are ordered after THIS kernel only, so it must
     // not complete before the filter kernel has (a no-op for an ordinary launch).
@@ -870,30 +883,25 @@ __device__ __forceinline__ double warp_sum_d(double v)
     return v;
 }
 
-// a6: CTA-wide fp64 sum -> one atomic per CTA (a tile belongs to exactly one replica)
-__device__ __forceinline__ void cta_add(double *dst, double v, double *red)
-{
-    v = warp_sum_d(v);
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    __syncthreads();
-    if (lane == 0) red[wid] = v;
-    __syncthreads();
-    if (wid == 0) {
-        double x = lane < nw ? red[lane] : 0.0;
-        x = warp_sum_d(x);
-        if (lane == 0) atomicAdd(dst, x);
-    }
-}
+// a6.  Per-replica sums are ORDER-FIXED, so that energies, virials and kinetic energies are bitwise repeatable: the 32
+// atoms of a chunk are added by a shuffle tree, the chunks of a CTA in chunk order (whichever warp happened to work on
+// them), and tbsma_reduce_replicas (tbsma_internal.cuh) adds the CTAs of a replica in tile order.  No atomics.
+constexpr int kMaxChunks = (TBSMA_TILE_MAX_RECORDS + 31) / 32 + 1;
 
 // stage 2 (Eq.1-3, Eq.5): forces, per-atom energy, virial, closing half kick, E_kin
-template <bool VIRIAL, bool KICK>
+template <bool VIRIAL, bool KICK, bool SPLIT>
 __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restrict__ cell_start,
                                            const float4 *__restrict__ xs, const uint2 *__restrict__ nl,
-                                           const int *__restrict__ nn, float4 *__restrict__ force,
-                                           double *__restrict__ e_rep, double *__restrict__ w_rep, const KickArgs &kk,
+                                           const int *__restrict__ nn, float4 *__restrict__ force, const KickArgs &kk,
                                            int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
-                                           const unsigned short *__restrict__ img)
+                                           const unsigned short *__restrict__ img, int part, int nsplit,
+                                           double *__restrict__ my_sums)
 {
+    constexpr int NQ = VIRIAL ? 8 : 2;
+    __shared__ double s_part[NQ][kMaxChunks];
+    const int lane = threadIdx.x & 31;
+    // every CTA leaves its sums (E, E_kin, W): zero if it has nothing to do
+    if (threadIdx.x < NQ) my_sums[threadIdx.x] = 0.0;
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
     if (r.nh > s_cap) {
@@ -901,17 +909,20 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
         return;
     }
     extern __shared__ float4 smem_f4[];
-    __shared__ double red[32];
-    __shared__ int s_next;
+    __shared__ int s_next, s_end, s_begin;
+    {
+        const int nchunk_all = (r.hi - r.lo + 31) >> 5;
+        const int cb = SPLIT ? nchunk_all * part / nsplit : 0, ce = SPLIT ? nchunk_all * (part + 1) / nsplit : nchunk_all;
+        if (ce <= cb) return;
+        if (threadIdx.x == 0) { s_next = cb; s_end = ce; s_begin = cb; }
+    }
     const float4 *sm = smem_f4;
-    if (threadIdx.x == 0) s_next = 0;
     fill_image(smem_f4, xs, img, r.halo_lo, r.nh);
-    double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     bool bad = false;
-    const int nchunk = (r.hi - r.lo + 31) >> 5, lane = threadIdx.x & 31;
-    for (int ch = next_chunk(&s_next); ch < nchunk; ch = next_chunk(&s_next)) {
+    for (int ch = next_chunk(&s_next); ch < s_end; ch = next_chunk(&s_next)) {
         const int i = r.lo + (ch << 5) + lane;
-        if (i >= r.hi) continue;
+        double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        if (i < r.hi) {
         const float4 pi = xs[i];
         const int nni = nn[i];
         const int ng = ((nni & 0xffff) + 3) >> 2;
@@ -940,40 +951,72 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
         const float ei = __fmaf_rn(sum2(a.er), pc.e_rep_scale, -sqrt_rho);   // Eq.1-3: E_R^i + E_B^i
         force[i] = make_float4(fx, fy, fz, ei);
         bad = bad || !isfinite(fx + fy + fz + ei);
-        se += (double)ei;
+        se = (double)ei;
         if (KICK && (nni >> 16) == 0) {       // final B of the step, dynamic atoms only
             float4 v = kk.vel[i];
             v.x = __fmaf_rn(kk.kick, fx, v.x);
             v.y = __fmaf_rn(kk.kick, fy, v.y);
             v.z = __fmaf_rn(kk.kick, fz, v.z);
             kk.vel[i] = v;
-            sk += (double)(kk.ke_scale * (v.x * v.x + v.y * v.y + v.z * v.z));
+            sk = (double)(kk.ke_scale * (v.x * v.x + v.y * v.y + v.z * v.z));
         }
         if (VIRIAL) {
-            sw[0] += 0.5 * (double)sum2(a.wxx); sw[1] += 0.5 * (double)sum2(a.wyy); sw[2] += 0.5 * (double)sum2(a.wzz);
-            sw[3] += 0.5 * (double)sum2(a.wxy); sw[4] += 0.5 * (double)sum2(a.wxz); sw[5] += 0.5 * (double)sum2(a.wyz);
+            sw[0] = 0.5 * (double)sum2(a.wxx); sw[1] = 0.5 * (double)sum2(a.wyy); sw[2] = 0.5 * (double)sum2(a.wzz);
+            sw[3] = 0.5 * (double)sum2(a.wxy); sw[4] = 0.5 * (double)sum2(a.wxz); sw[5] = 0.5 * (double)sum2(a.wyz);
+        }
+        }
+        // the chunk's sums, by a fixed tree
+        __syncwarp();
+        se = warp_sum_d(se);
+        if (KICK) sk = warp_sum_d(sk);
+        if (VIRIAL) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) sw[k] = warp_sum_d(sw[k]);
+        }
+        if (lane == 0) {
+            const int c = ch - s_begin;
+            s_part[0][c] = se;
+            s_part[1][c] = sk;
+            if (VIRIAL) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k) s_part[(2 + k) % NQ][c] = sw[k];
+            }
         }
     }
     if (bad) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NONFINITE);
-    if (e_rep) cta_add(e_rep + t.rep, se, red);
-    if (KICK && kk.ekin) cta_add(kk.ekin + t.rep, sk, red);
-    if (VIRIAL) {
+    __syncthreads();
+    // the CTA's sums: chunks in chunk order (lane l takes chunks l, l + 32, ...; then a fixed tree)
+    if (threadIdx.x < 32) {
 #pragma unroll
-        for (int k = 0; k < 6; ++k) cta_add(w_rep + 6 * (size_t)t.rep + k, sw[k], red);
+        for (int q = 0; q < NQ; ++q) {
+            double v = 0.0;
+            for (int c = lane; c < s_end - s_begin; c += 32) v += s_part[q][c];
+            v = warp_sum_d(v);
+            if (lane == 0) my_sums[q] = v;
+        }
     }
 }
 
-template <bool VIRIAL, bool KICK>
+template <bool VIRIAL, bool KICK, bool SPLIT>
 __global__ void __launch_bounds__(512, 2)
 k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_start,
              const float4 *__restrict__ xs, const uint2 *__restrict__ nl, const int *__restrict__ nn,
-             float4 *__restrict__ force, double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk,
+             float4 *__restrict__ force, double *__restrict__ cta_sums, KickArgs kk,
              int *__restrict__ ctrl, ListSel ls, int n_pad, int s_cap, PairConst pc)
 {
-    const TileDesc t = tiles[blockIdx.x];
+    const int ti = SPLIT ? (int)blockIdx.x / ls.nsplit : (int)blockIdx.x, part = SPLIT ? (int)blockIdx.x % ls.nsplit : 0;
+    const TileDesc t = tiles[ti];
     const int h = list_half(ls, t.rep);
-    force_tile<VIRIAL, KICK>(t, cell_start, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force, e_rep,
-                             w_rep, kk, ctrl, n_pad, s_cap, pc, ls.img + (size_t)blockIdx.x * ls.img_stride);
+    force_tile<VIRIAL, KICK, SPLIT>(t, cell_start, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force, kk,
+                             ctrl, n_pad, s_cap, pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit,
+                             cta_sums + 8 * (size_t)blockIdx.x);
+}
+
+// per-replica sums of the CTA sums, in tile order (tbsma_compute; inside an MD step k_finish_step does it)
+__global__ void __launch_bounds__(256)
+k_reduce_replicas(TileSums ts, int R)
+{
+    tbsma_reduce_replicas(ts, R);
 }
 
 // ---- inspection (parity tests, bench statistics) ----------------------------------------------
@@ -1177,6 +1220,19 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     if (e == cudaSuccess) e = ensure((void **)&c->d_work, &c->have_work, sizeof(int) * (size_t)(2 + 2 * n_tiles));
     if (e == cudaSuccess) e = ensure((void **)&c->d_img, &c->have_img, sizeof(unsigned short) * nt1 * new_tile_cap);
     if (e == cudaSuccess) e = ensure((void **)&c->d_inv, &c->have_inv, sizeof(unsigned short) * nt1 * new_img_cap);
+    // Few tiles (one or a few small wires): several CTAs share a tile, each filling the image and taking a share of the
+    // 32-atom chunks, until the CTAs fill the GPU about twice (or every CTA is down to one chunk).
+    int nsplit = 1;
+    {
+        const int slots = 8 * c->n_sm;
+        int est_chunks = (own_cap * 4 / 5 + 31) / 32;     // own_cap carries 25 % headroom
+        if (est_chunks < 1) est_chunks = 1;
+        if (n_tiles > 0 && n_tiles < slots) nsplit = (int)((slots + n_tiles - 1) / n_tiles);
+        if (nsplit > est_chunks) nsplit = est_chunks;
+        if (c->tile_split_req > 0) nsplit = c->tile_split_req;
+        if (nsplit < 1) nsplit = 1;
+    }
+    if (e == cudaSuccess) e = ensure((void **)&c->d_cta_sums, &c->have_sums, sizeof(double) * 8 * nt1 * (size_t)nsplit);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d_work, 0, sizeof(int) * (size_t)(2 + 2 * n_tiles), st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tiles, h, sizeof(TileDesc) * (size_t)n_tiles, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tile_first, first, sizeof(int) * (size_t)(R + 1), cudaMemcpyHostToDevice, st);
@@ -1185,6 +1241,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     free(first);
     if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? TBSMA_ENOMEM : TBSMA_ECUDA;
     c->n_tiles = (int)n_tiles;
+    c->tile_nsplit = nsplit;
     c->tile_cap = new_tile_cap;   // halo records a tile may hold
     // image: the sentinel + eight colour classes of records (k_tile_place); room for classes 1/8 + 64 fuller than even
     c->img_cap = new_img_cap;
@@ -1196,11 +1253,13 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_tile_inner, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)inner_smem(c));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tile_finish, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_fin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_density_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_force_tile<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);
+#define TBSMA_ATTR(K) if (e == cudaSuccess) e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g)
+    TBSMA_ATTR(k_density_tile<false>); TBSMA_ATTR(k_density_tile<true>);
+    TBSMA_ATTR((k_force_tile<false, false, false>)); TBSMA_ATTR((k_force_tile<false, true, false>));
+    TBSMA_ATTR((k_force_tile<true, false, false>)); TBSMA_ATTR((k_force_tile<true, true, false>));
+    TBSMA_ATTR((k_force_tile<false, false, true>)); TBSMA_ATTR((k_force_tile<false, true, true>));
+    TBSMA_ATTR((k_force_tile<true, false, true>)); TBSMA_ATTR((k_force_tile<true, true, true>));
+#undef TBSMA_ATTR
     if (e != cudaSuccess) return TBSMA_ECUDA;
     c->active_variant = 2;
     return TBSMA_OK;
@@ -1283,6 +1342,7 @@ static ListSel list_sel(const tbsma_ctx *c, int sync_level)
     ls.n_stride = c->n_pad;
     ls.img = c->d_img;
     ls.img_stride = c->tile_cap;
+    ls.nsplit = c->tile_nsplit;
     return ls;
 }
 
@@ -1291,7 +1351,7 @@ static ListSel list_sel(const tbsma_ctx *c, int sync_level)
 cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_level, cudaStream_t st, bool early)
 {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(c->n_tiles);
+    cfg.gridDim = dim3((unsigned)(c->n_tiles * c->tile_nsplit));
     cfg.blockDim = dim3(c->tile_threads);
     cfg.dynamicSmemBytes = gather_smem(c);
     cfg.stream = st;
@@ -1300,26 +1360,51 @@ cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = early ? 1 : 0;
-    const cudaError_t e = cudaLaunchKernelEx(&cfg, k_density_tile, (const TileDesc *)c->d_tiles, (const int *)c->d_cell_start,
-                                             pos, reinterpret_cast<const uint2 *>(c->d_nlist), (const int *)c->d_nn, c->d_xs,
-                                             c->d_ctrl, list_sel(c, sync_level), c->n_pad, c->tile_cap, c->pc);
+    const cudaError_t e =
+        c->tile_nsplit > 1
+            ? cudaLaunchKernelEx(&cfg, k_density_tile<true>, (const TileDesc *)c->d_tiles, (const int *)c->d_cell_start, pos,
+                                 reinterpret_cast<const uint2 *>(c->d_nlist), (const int *)c->d_nn, c->d_xs, c->d_ctrl,
+                                 list_sel(c, sync_level), c->n_pad, c->tile_cap, c->pc)
+            : cudaLaunchKernelEx(&cfg, k_density_tile<false>, (const TileDesc *)c->d_tiles, (const int *)c->d_cell_start, pos,
+                                 reinterpret_cast<const uint2 *>(c->d_nlist), (const int *)c->d_nn, c->d_xs, c->d_ctrl,
+                                 list_sel(c, sync_level), c->n_pad, c->tile_cap, c->pc);
     c->launches++;
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kk,
-                                    int sync_level, cudaStream_t st)
+cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, bool virial, KickArgs kk, int sync_level,
+                                    cudaStream_t st)
 {
     const uint2 *nl = reinterpret_cast<const uint2 *>(c->d_nlist);
     const size_t sm = gather_smem(c);
-    const int g = c->n_tiles, b = c->tile_threads;
+    const int g = c->n_tiles * c->tile_nsplit, b = c->tile_threads;
     const ListSel ls = list_sel(c, sync_level);
-#define TBSMA_FT(V, K)                                                                                             \
-    k_force_tile<V, K><<<g, b, sm, st>>>(c->d_tiles, c->d_cell_start, c->d_xs, nl, c->d_nn, force, e_rep, w_rep, kk, \
-                                         c->d_ctrl, ls, c->n_pad, c->tile_cap, c->pc)
-    if (w_rep) { if (kk.vel) TBSMA_FT(true, true); else TBSMA_FT(true, false); }
-    else       { if (kk.vel) TBSMA_FT(false, true); else TBSMA_FT(false, false); }
+#define TBSMA_FT(V, K, S)                                                                                          \
+    k_force_tile<V, K, S><<<g, b, sm, st>>>(c->d_tiles, c->d_cell_start, c->d_xs, nl, c->d_nn, force, c->d_cta_sums, kk, \
+                                            c->d_ctrl, ls, c->n_pad, c->tile_cap, c->pc)
+#define TBSMA_FT2(V, K) do { if (c->tile_nsplit > 1) TBSMA_FT(V, K, true); else TBSMA_FT(V, K, false); } while (0)
+    if (virial) { if (kk.vel) TBSMA_FT2(true, true); else TBSMA_FT2(true, false); }
+    else        { if (kk.vel) TBSMA_FT2(false, true); else TBSMA_FT2(false, false); }
+#undef TBSMA_FT2
 #undef TBSMA_FT
+    c->launches++;
+    return cudaGetLastError();
+}
+
+TileSums tbsma_tile_sums(const tbsma_ctx *c, double *e_rep, double *ekin, double *w_rep)
+{
+    TileSums ts;
+    ts.cta_sums = c->d_cta_sums;
+    ts.tile_first = c->d_tile_first;
+    ts.nsplit = c->tile_nsplit;
+    ts.e_rep = e_rep; ts.ekin = ekin; ts.w_rep = w_rep;
+    return ts;
+}
+
+cudaError_t tbsma_launch_reduce_replicas(tbsma_ctx *c, double *e_rep, double *ekin, double *w_rep, cudaStream_t st)
+{
+    if (!e_rep && !ekin && !w_rep) return cudaSuccess;
+    k_reduce_replicas<<<tbsma_reduce_grid(c->R), 256, 0, st>>>(tbsma_tile_sums(c, e_rep, ekin, w_rep), c->R);
     c->launches++;
     return cudaGetLastError();
 }

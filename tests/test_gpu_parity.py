@@ -314,13 +314,127 @@ def test_overlapped_list_renewal_is_bitwise_identical(B, graph, overlap):
     assert 0 < sa["n_replica_builds"] < w.n_replicas * n_steps and sa["n_build_passes"] < n_steps
     for name in ("pos", "vel", "force"):
         assert np.array_equal(a.untag(getattr(a, name)), b.untag(getattr(b, name))), name
-    # per-replica sums: one fp64 atomic per CTA, so the order (not the terms) may differ
-    assert np.allclose(a.e_rep.cpu().numpy(), b.e_rep.cpu().numpy(), rtol=1e-12, atol=0)
-    assert np.allclose(a.ekin.cpu().numpy(), b.ekin.cpu().numpy(), rtol=1e-12, atol=0)
-    assert np.allclose(a.w_rep.cpu().numpy(), b.w_rep.cpu().numpy(), rtol=1e-12, atol=1e-12)
+    # per-replica sums are added in a fixed order (chunk tree, chunks of a CTA in order, CTAs of a replica in tile order)
+    assert np.array_equal(a.e_rep.cpu().numpy(), b.e_rep.cpu().numpy())
+    assert np.array_equal(a.ekin.cpu().numpy(), b.ekin.cpu().numpy())
+    assert np.array_equal(a.w_rep.cpu().numpy(), b.w_rep.cpu().numpy())
     assert ca.status() == 0 and cb.status() == 0
     md = run_oracle_md(w, n_steps)
     assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+
+
+def test_per_replica_sums_are_bitwise_repeatable_and_tile_split_changes_only_their_order(B):
+    """a6 in the tile variant: the same run twice gives the same bits in E, E_kin and W of every replica (no atomics);
+    several CTAs per tile (tbsma_set_tile_split, what small batches get automatically) leave positions, velocities and
+    forces bit-identical and change the per-replica sums only by their fp64 summation order"""
+    w = W.config3(3, seed=17, length=60.0)
+    n_steps = 40
+
+    def run(split):
+        ctx, st = setup(B, w, variant=2)
+        if split is not None:
+            ctx.set_tile_split(split)
+            ctx.build_cells(st.pos, st.vel, st.tag)
+            ctx.build_neighbors(st.pos, st.vel, st.tag)
+        ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
+        torch.cuda.synchronize()
+        e0, w0 = st.e_rep.cpu().numpy().copy(), st.w_rep.cpu().numpy().copy()
+        stream = torch.cuda.Stream()
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate, 0,
+                       st.e_rep, st.w_rep, st.ekin)
+        torch.cuda.synchronize()
+        assert ctx.status() == 0
+        return dict(e0=e0, w0=w0, pos=st.untag(st.pos), vel=st.untag(st.vel), force=st.untag(st.force),
+                    e=st.e_rep.cpu().numpy().copy(), k=st.ekin.cpu().numpy().copy(), w=st.w_rep.cpu().numpy().copy())
+
+    a, b = run(None), run(None)
+    for key in a:
+        assert np.array_equal(a[key], b[key]), key
+    o = oracle.compute(w.x64(), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi)
+    assert np.all(np.abs(a["e0"] - o["e_rep"]) <= E_REL * np.abs(o["e_rep"]))
+    assert np.abs(a["w0"] - o["w_rep"]).max() <= 2e-5 * np.abs(o["w_rep"][:, :3]).sum(1).max()
+    for split in (1, 3, 7):
+        c = run(split)
+        for key in ("pos", "vel", "force"):
+            assert np.array_equal(a[key], c[key]), (split, key)
+        for key in ("e0", "w0", "e", "k", "w"):
+            assert np.allclose(a[key], c[key], rtol=1e-12, atol=1e-10), (split, key)
+
+
+def test_switching_to_the_global_variant_after_a_tile_run(B):
+    """after a run in the tile variant some replicas use the second half of the list buffers; rebuilding for the global
+    variant (which only has the first) on the same context must not leave them pointing there: no spurious rebuilds,
+    no SKIN_VIOLATED, same trajectory as a fresh global-variant context"""
+    w = W.config3(4, seed=19, length=60.0)
+    ctx, st = run_gpu_md(B, w, 60, variant=2)
+    assert ctx.get_variant() == 2 and ctx.get_stats()["n_replica_builds"] > w.n_replicas
+    ctx.set_variant(1)
+    ctx.build_cells(st.pos, st.vel, st.tag)
+    ctx.build_neighbors(st.pos, st.vel, st.tag)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    torch.cuda.synchronize()
+    assert ctx.get_variant() == 1
+    x0, v0 = st.untag(st.pos), st.untag(st.vel)
+    b0 = ctx.get_stats()["n_replica_builds"]
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 60, 5, None, None, 0, st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    assert ctx.get_stats()["n_replica_builds"] - b0 <= w.n_replicas      # not "every replica every step"
+    # reference: a fresh context in the global variant from the same state
+    w2 = W.Workload(w.name, x0.copy(), v0.copy(), w.offsets, w.box_lo, w.box_hi, w.periodic, w.T, w.seed, np.zeros_like(w.slab_rate),
+                    w.gamma, w.dt, w.r_cut, w.skin, 0, {})
+    ctx2, st2 = setup(B, w2, variant=1)
+    ctx2.compute(st2.pos, st2.force, st2.e_rep, None)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(stream):
+        ctx2.md_run(st2.pos, st2.vel, st2.force, st2.tag, w.dt, st2.T, w.gamma, st2.seed, 60, 5, None, None, 0, st2.e_rep, None, st2.ekin)
+    torch.cuda.synchronize()
+    assert np.array_equal(st.untag(st.pos)[:, :3], st2.untag(st2.pos)[:, :3])
+
+
+def test_fixed_cadence_with_several_replicas_and_chained_runs(B):
+    """rebuild_every > 0 on a batch: the staggered first rebuild (for displacement-triggered lists) must not fire and be
+    reported as a violated skin; and md_run called in pieces (step0 = 0, 7, 14, ...: one captured graph serves them
+    all, the step number of the run lives on the device) gives the bits of one long call"""
+    w = W.config3(4, seed=23, length=60.0)
+    w.rebuild_every = 10
+    n = 42
+    ca, a = run_gpu_md(B, w, n, variant=0)
+    assert ca.status() == 0
+    assert ca.get_stats()["n_build_passes"] == 1 + 5          # the explicit build + steps 0, 10, 20, 30, 40
+    ctx, st = setup(B, w)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    torch.cuda.synchronize()
+    stream = torch.cuda.Stream()
+    rate = st.slab_rate
+    with torch.cuda.stream(stream):
+        for s0 in range(0, n, 7):
+            m = min(7, n - s0)
+            disp0 = rate * float(s0)
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, s0, m, disp0, rate, w.rebuild_every,
+                       st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    assert np.array_equal(a.untag(a.pos), st.untag(st.pos))
+    # and with pieces long enough to go through the captured graph
+    ctx3, st3 = setup(B, w)
+    ctx3.compute(st3.pos, st3.force, st3.e_rep, None)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(stream):
+        for s0 in range(0, 40, 10):
+            ctx3.md_run(st3.pos, st3.vel, st3.force, st3.tag, w.dt, st3.T, w.gamma, st3.seed, s0, 10, st3.slab_rate * float(s0),
+                        st3.slab_rate, w.rebuild_every, st3.e_rep, None, st3.ekin)
+        ctx3.md_run(st3.pos, st3.vel, st3.force, st3.tag, w.dt, st3.T, w.gamma, st3.seed, 40, 2, st3.slab_rate * 40.0,
+                    st3.slab_rate, w.rebuild_every, st3.e_rep, None, st3.ekin)
+    torch.cuda.synchronize()
+    assert ctx3.status() == 0
+    assert np.array_equal(a.untag(a.pos), st3.untag(st3.pos))
+    assert np.array_equal(a.untag(a.vel), st3.untag(st3.vel))
 
 
 def test_async_list_renewal_changes_cost_not_results(B):
@@ -781,6 +895,38 @@ def test_nose_hoover_trajectory_matches_oracle(B, variant):
     assert eta[0] > 0 > eta[1]                    # net cooling of the first replica, net heating of the second
     ek = st.ekin.cpu().numpy()
     assert np.allclose(ek, nh.kinetic(), rtol=1e-4)
+    # bitwise repeatable (the kinetic energy that drives xi is added in a fixed order), and resumable: 60 steps, state
+    # out (pos, vel, force, tag are the caller's; xi, eta through the ABI), a NEW context, state in, 40 steps
+    def nh_run(pieces):
+        c2, s2 = setup(B, w, variant=variant)
+        c2.set_thermostat(1, tau)
+        c2.compute(s2.pos, s2.force, s2.e_rep, None)
+        torch.cuda.synchronize()
+        s0 = 0
+        for k, m in enumerate(pieces):
+            if k > 0:
+                xi2, eta2 = c2.get_thermostat()
+                c3 = B.make_context(w, max_neighbors=96)
+                c3.set_variant(variant)
+                c3.set_thermostat(1, tau)
+                c3.build_cells(s2.pos, s2.vel, s2.tag)
+                c3.build_neighbors(s2.pos, s2.vel, s2.tag)
+                c3.set_thermostat_state(xi2, eta2)
+                torch.cuda.synchronize()
+                c2 = c3
+            with torch.cuda.stream(stream):
+                c2.md_run(s2.pos, s2.vel, s2.force, s2.tag, w.dt, s2.T, 0.0, s2.seed, s0, m, None, None, 0, s2.e_rep, None,
+                          s2.ekin)
+            torch.cuda.synchronize()
+            s0 += m
+        return s2.untag(s2.pos), s2.untag(s2.vel), c2.get_thermostat()
+    xa, va, (xia, etaa) = nh_run([n_steps])
+    assert np.array_equal(xa, st.untag(st.pos)) and np.array_equal(va, st.untag(st.vel))
+    assert np.array_equal(xia, xi) and np.array_equal(etaa, eta)
+    # resumed in a new context the lists are rebuilt at step 60 (another fp32 summation order): same physics, not same bits
+    xb, vb, (xib, etab) = nh_run([60, 40])
+    assert np.abs(xb[:, :3] - xa[:, :3]).max() < 1e-4 and np.abs(vb[:, :3] - va[:, :3]).max() < 2e-6
+    assert np.allclose(xib, xia, rtol=1e-5, atol=1e-10) and np.allclose(etab, etaa, rtol=1e-5, atol=1e-9)
     # back to Langevin / velocity Verlet: the thermostat state is reset
     ctx.set_thermostat(0)
     assert np.all(ctx.get_thermostat()[0] == 0)
