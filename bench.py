@@ -63,7 +63,7 @@ def make_workload(cfg, rank=0, replicas=None):
 class ClockSampler(threading.Thread):
     """SM clock / throttle reasons sampled with NVML while the timed region runs."""
 
-    def __init__(self, index, period=0.02):
+    def __init__(self, index, period=0.002):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.stop_flag, self.ok = [], False, False
@@ -112,19 +112,21 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(seen), "samples": len(sel)}
 
 
-def cpu_oracle_rate(w, n_rep, n_steps):
-    """The oracle as it stands (brute force O(N^2) per replica, fp64, OpenMP), timed on a bounded
-    sample: the first n_rep replicas for n_steps MD steps.  Returns (atom-steps/s, cores, text)."""
+def cpu_oracle_rate(w, n_rep, n_steps, cells=True):
+    """The oracle as it stands (fp64, OpenMP), timed on a bounded sample: the first n_rep replicas for n_steps MD steps.
+    cells=True: its linked-cell path (SURVEY 8(d) "Oracle-CL", the fair CPU baseline); cells=False: the brute-force
+    O(N^2) path the parity tests use (SURVEY 8(d) "Oracle-BF").  Returns (atom-steps/s, cores, text)."""
     import oracle
     sub = w.take(0, min(n_rep, w.n_replicas))
     md = oracle.MD(sub.x64(), sub.v64(), sub.flags, sub.r_cut, offsets=sub.offsets, lo=sub.box_lo, hi=sub.box_hi,
-                   periodic=sub.periodic, fp32_pred=False, cells=False, zref=sub.vel4[:, 3].astype(np.float64))
+                   periodic=sub.periodic, fp32_pred=False, cells=cells, zref=sub.vel4[:, 3].astype(np.float64))
     t0 = time.perf_counter()
     for s in range(n_steps):
         md.step(sub.dt, sub.T.astype(np.float64), sub.gamma, sub.seed, s, slab_disp=sub.slab_rate * (s + 1))
     dt = time.perf_counter() - t0
+    how = "linked-cell fp64 OpenMP oracle (Oracle-CL)" if cells else "brute-force O(N^2) fp64 OpenMP oracle (Oracle-BF)"
     return sub.n_atoms * n_steps / dt, oracle.num_threads(), \
-        f"first {sub.n_replicas} replica(s) of {w.name} ({sub.n_atoms} atoms) x {n_steps} steps, brute-force O(N^2) oracle"
+        f"first {sub.n_replicas} replica(s) of {w.name} ({sub.n_atoms} atoms) x {n_steps} steps, {how}"
 
 
 def run_reference(args, rank):
@@ -133,11 +135,11 @@ def run_reference(args, rank):
         return
     w = make_workload(args.config, 0, replicas=2 if args.config in ("3", "4") else None)
     if args.config == "5a":
-        w = W.config5a(8, 5)     # 2 048-atom periodic block: the O(N^2) oracle cannot do 10^6 atoms per step
+        w = W.config5a(16, 5)    # 16 384-atom periodic block of the same lattice: a bounded sample of the 10^6-atom box
     sub = w.take(0, 1)
     import oracle
     md = oracle.MD(sub.x64(), sub.v64(), sub.flags, sub.r_cut, offsets=sub.offsets, lo=sub.box_lo, hi=sub.box_hi,
-                   periodic=sub.periodic, fp32_pred=False, cells=False, zref=sub.vel4[:, 3].astype(np.float64))
+                   periodic=sub.periodic, fp32_pred=False, cells=True, zref=sub.vel4[:, 3].astype(np.float64))
     s = 0
     for _ in range(args.warmup):
         md.step(sub.dt, sub.T.astype(np.float64), sub.gamma, sub.seed, s, slab_disp=sub.slab_rate * (s + 1))
@@ -148,7 +150,7 @@ def run_reference(args, rank):
         s += 1
     dt = time.perf_counter() - t0
     value = sub.n_atoms * args.steps / dt
-    sample = f"each step = 1 replica of {w.name} ({sub.n_atoms} atoms), brute-force O(N^2) fp64 oracle, OpenMP"
+    sample = f"each step = 1 replica of {w.name} ({sub.n_atoms} atoms), linked-cell fp64 OpenMP oracle (Oracle-CL)"
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
@@ -173,6 +175,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel-steps", type=int, default=60, help="steps of the per-kernel CUDA-event timing pass")
+    ap.add_argument("--preroll", type=int, default=300,
+                    help="declared, untimed steps before the warm-up: replicas built together rebuild together at first; "
+                         "the timed region should see the steady rebuild cadence, not that transient")
     ap.add_argument("--outer-skin", type=float, default=None,
                     help="buffer radius S of the candidate lists of the tile variant (tbsma_set_outer_skin; library default if omitted)")
     ap.add_argument("--plain-graph", action="store_true",
@@ -221,7 +226,13 @@ def main():
             return float(t.item())
         return float(x)
 
+    # Multi-GPU = replicas only: the job is one batch of world x R replicas, partitioned contiguously
+    # by sharding.replica_range; rank k owns replicas [r0, r1) and builds just those (seeds are a function of the global
+    # replica index through the per-rank seed shift), no data-path collective.
+    from paper_1311_3890_b200 import sharding
     w = make_workload(args.config, rank, args.replicas)
+    r0, r1 = sharding.replica_range(w.n_replicas * world, rank, world)
+    assert r1 - r0 == w.n_replicas
     ctx = B.make_context(w)
     if args.plain_graph:
         ctx.set_graph(True, conditional=False)
@@ -229,13 +240,20 @@ def main():
         ctx.set_outer_skin(args.outer_skin)
     st = B.DeviceState(w, dev)
     stream = torch.cuda.Stream(device=dev)
-    K, Wm = args.steps, args.warmup
+    K, Wm, P0 = args.steps, args.warmup, max(args.preroll, 0)
+
+    def run(step0, n):
+        """steps step0 .. step0 + n - 1; the pulled slab continues where the previous call left it"""
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, step0, n, st.slab_rate * float(step0),
+                   st.slab_rate, w.rebuild_every, st.e_rep, None, st.ekin)
+
     with torch.cuda.stream(stream):
         ctx.build_cells(st.pos, st.vel, st.tag)
         ctx.build_neighbors(st.pos, st.vel, st.tag)
         ctx.compute(st.pos, st.force, st.e_rep, None)
-        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, Wm, None, st.slab_rate,
-                   w.rebuild_every, st.e_rep, None, st.ekin)
+        if P0:
+            run(0, P0)
+        run(P0, Wm)
     sampler = ClockSampler(local_rank)
     sampler.start()
     barrier()
@@ -245,8 +263,7 @@ def main():
     t_host0 = time.perf_counter()
     with torch.cuda.stream(stream):
         ev0.record(stream)
-        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, Wm, K, None, st.slab_rate,
-                   w.rebuild_every, st.e_rep, None, st.ekin)
+        run(P0 + Wm, K)
         ev1.record(stream)
     barrier()
     t_host1 = time.perf_counter()
@@ -255,6 +272,9 @@ def main():
     launches = ctx.launch_count() - launches0
     stats1 = ctx.get_stats()
     status = ctx.status()
+    # the only traffic of the job: per-replica observables of the last step onto every rank (a few doubles per replica)
+    obs = sharding.gather_replica_values(np.stack([st.e_rep.cpu().numpy(), st.ekin.cpu().numpy()], axis=1),
+                                         w.n_replicas * world, rank, world, dist if world > 1 else None, dev if world > 1 else None)
     n_total = sum_over_ranks(w.n_atoms)
     value = n_total * K / (ms * 1e-3)
     entries, pairs = ctx.count_pairs(st.pos, stream)
@@ -267,17 +287,22 @@ def main():
     ctx.set_timing(True)
     ks = min(args.kernel_steps, 512)
     with torch.cuda.stream(stream):
-        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, Wm + K, ks, None, st.slab_rate,
-                   w.rebuild_every, st.e_rep, None, st.ekin)
+        run(P0 + Wm + K, ks)
     tms, tsteps = ctx.get_timing()
     ctx.set_timing(False)
     peak, peak_src = load_peaks()
     per_kernel_ms = {k: v / max(tsteps, 1) for k, v in tms.items()}
     # algorithmic bytes per launch: force pass 4 n_L + 40 B/atom,
-    # density pass 4 n_L + 24 B/atom, whole step 8 n_L + 160 + (4 n_L + 120)/K_eff B/atom
+    # density pass 4 n_L + 24 B/atom, whole step 8 n_L + 160 + (4 n_L + 120)/K_eff B/atom.  That budget is the survey's:
+    # an int32 list.  The tile variant streams 16-bit entries, so what it must move is less ("as_built" below, 2 B per
+    # entry): both are reported, and so is the DRAM traffic ncu measured.
     force_bytes = (4.0 * n_l + 40.0) * w.n_atoms
     dens_bytes = (4.0 * n_l + 24.0) * w.n_atoms
     step_bytes = (8.0 * n_l + 160.0 + (4.0 * n_l + 120.0) / k_eff) * w.n_atoms
+    eb = 2.0 if ctx.get_variant() == 2 else 4.0          # bytes per list entry of the variant that ran
+    force_bytes_built = (eb * n_l + 40.0) * w.n_atoms
+    dens_bytes_built = (eb * n_l + 24.0) * w.n_atoms
+    step_bytes_built = (2 * eb * n_l + 160.0 + (eb * n_l + 120.0) / k_eff) * w.n_atoms
     ach_force = force_bytes / (per_kernel_ms["force"] * 1e-3) / 1e9 if per_kernel_ms["force"] > 0 else 0.0
     ach_dens = dens_bytes / (per_kernel_ms["density"] * 1e-3) / 1e9 if per_kernel_ms["density"] > 0 else 0.0
     ach_step = step_bytes / (ms / K * 1e-3) / 1e9
@@ -287,16 +312,32 @@ def main():
                 "avg_launch_ms": per_kernel_ms["force"],
                 "density_pass": {"achieved": ach_dens, "frac": ach_dens / peak, "avg_launch_ms": per_kernel_ms["density"]},
                 "whole_step": {"achieved": ach_step, "frac": ach_step / peak, "bytes_per_atom_step": step_bytes / w.n_atoms},
-                "per_kernel_ms": per_kernel_ms, "timed_steps": tsteps}
+                "bytes_model": "SURVEY 8(d): int32 list, 4 B per entry (the designated budget; the tile variant stores 2 B entries)",
+                "as_built": {
+                    "bytes_per_list_entry": eb,
+                    "force_pass": {"bytes_per_launch": force_bytes_built,
+                                   "achieved": force_bytes_built / (per_kernel_ms["force"] * 1e-3) / 1e9 if per_kernel_ms["force"] > 0 else 0.0},
+                    "density_pass": {"bytes_per_launch": dens_bytes_built,
+                                     "achieved": dens_bytes_built / (per_kernel_ms["density"] * 1e-3) / 1e9 if per_kernel_ms["density"] > 0 else 0.0},
+                    "whole_step": {"bytes_per_atom_step": step_bytes_built / w.n_atoms,
+                                   "achieved": step_bytes_built / (ms / K * 1e-3) / 1e9}},
+                "per_kernel_ms": per_kernel_ms, "timed_steps": tsteps,
+                "per_kernel_note": "CUDA events between the kernel classes with graph replay and overlap OFF (kernels one "
+                                   "after the other); in the timed step the list renewal runs beside the gather passes, so "
+                                   "per_kernel_ms.rebuild is not what the step pays"}
+    for k in ("force_pass", "density_pass", "whole_step"):
+        roofline["as_built"][k]["frac"] = roofline["as_built"][k]["achieved"] / peak
     # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu capture
-    traffic_file = os.path.join(ROOT, "profiles", "r1e_force_kernel_traffic.csv")
+    # (a number from a committed capture, NOT measured in this run: it names the capture it comes from and is refreshed
+    # with every change of the kernel; null for workloads that have no capture)
+    traffic_file = os.path.join(ROOT, "profiles", "r2_force_kernel_traffic.csv")
     if os.path.exists(traffic_file):
         try:
             import csv
             for row in csv.DictReader(open(traffic_file)):
                 if row["workload"] == w.name and row["kernel"].startswith("k_force"):
                     roofline["traffic"] = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
-                    roofline["traffic_source"] = row["source"]
+                    roofline["traffic_from"] = "committed ncu capture: " + row["source"]
         except Exception:
             pass
     roofline["note"] = ("HBM is the designated roofline (BASELINE.json); with 16-bit lists the gather passes move less than "
@@ -330,15 +371,23 @@ def main():
                "call": "tbsma_md_run_host (H2D pos/vel/tag, cell+list build, initial forces, steps, D2H pos/vel/force/tag)"}
         ctx2.destroy()
 
-    cpu = None
+    cpu = cpu_bf = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        nrep, nst = (4, 8) if args.config in ("3",) else (8, 10) if args.config == "4" else (1, 10)
-        if args.config in ("5a", "5b"):
-            wc = W.config5a(8, 5) if args.config == "5a" else W.config2()
-            rate, cores, sample = cpu_oracle_rate(wc, 1, 10)
+        # bounded samples (about 10-20 s of CPU work together): the linked-cell oracle is the CPU baseline, the brute-force
+        # one (what the parity tests run) is reported beside it
+        nrep, nst = (8, 20) if args.config in ("3",) else (16, 40) if args.config == "4" else (1, 40)
+        if args.config == "5a":
+            wc = W.config5a(24, 5)
+            rate, cores, sample = cpu_oracle_rate(wc, 1, 10, cells=True)
+            rbf, _, sbf = cpu_oracle_rate(W.config5a(8, 5), 1, 10, cells=False)
+        elif args.config == "5b":
+            rate, cores, sample = cpu_oracle_rate(w, 1, 10, cells=True)
+            rbf, _, sbf = cpu_oracle_rate(W.config2(), 1, 10, cells=False)
         else:
-            rate, cores, sample = cpu_oracle_rate(w, nrep, nst)
+            rate, cores, sample = cpu_oracle_rate(w, nrep, nst, cells=True)
+            rbf, _, sbf = cpu_oracle_rate(w, 2 if args.config in ("3", "4") else 1, 4, cells=False)
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        cpu_bf = {"value": rbf, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sbf}
 
     if rank == 0:
         line = {
@@ -353,11 +402,14 @@ def main():
                        "variant": {1: "global gather (int32 list)", 2: "shared-memory tiles (u16 lists)"}.get(ctx.get_variant()),
                        "list_renewal": "asynchronous, margin 0.03 A, beside the gather passes (density pass = programmatic dependent of the filter kernel)" if ctx.get_variant() == 2 and not w.rebuild_every else "ahead of the gather passes",
                        "graph": "plain" if args.plain_graph else "conditional node around the cells+candidates chain",
+                       "preroll_steps": P0,
                        "parallelism": "replicas only" if world > 1 else "1 gpu"},
             "pair_interactions_per_s": pair_rate,
+            "observables": {"replicas": int(obs.shape[0]), "e_pot_eV_per_atom": float(obs[:, 0].sum() / n_total),
+                            "e_kin_eV_per_atom": float(obs[:, 1].sum() / n_total)},
             "clocks": sampler.summary(t_host0, t_host1),
             "e2e": e2e, "gpu_launches": int(launches), "status_flags": status,
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "cpu_baseline": cpu, "cpu_baseline_cl": cpu, "cpu_baseline_bf": cpu_bf,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
