@@ -95,7 +95,8 @@ int tbsma_set_system(tbsma_ctx *ctx, int64_t n_atoms, int32_t n_replicas,
 /* Cell binning (counting sort over replica x cell keys, stable by tag inside a cell) and in-place
  * reorder of d_pos, d_vel (nullable) and d_tag into cell order; positions on periodic axes are
  * wrapped into [lo, hi).  d_tag must hold the current tag of every slot (0..n-1 before the
- * first call).  Rebuilds every replica. */
+ * first call).  Rebuilds every replica.  The caller's force array is NOT permuted: after this call (and
+ * tbsma_build_neighbors) evaluate tbsma_compute before the next tbsma_md_step / tbsma_md_run. */
 int tbsma_build_cells(tbsma_ctx *ctx, float *d_pos, float *d_vel, int32_t *d_tag, void *stream);
 
 /* Neighbour list of every atom: all j != i of the same replica with |r_i - r_j| < r_cut + skin,

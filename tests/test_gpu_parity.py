@@ -911,6 +911,7 @@ def test_nose_hoover_trajectory_matches_oracle(B, variant):
                 c3.set_thermostat(1, tau)
                 c3.build_cells(s2.pos, s2.vel, s2.tag)
                 c3.build_neighbors(s2.pos, s2.vel, s2.tag)
+                c3.compute(s2.pos, s2.force, s2.e_rep, None)   # the build permuted pos / vel / tag, not the caller's forces
                 c3.set_thermostat_state(xi2, eta2)
                 torch.cuda.synchronize()
                 c2 = c3
