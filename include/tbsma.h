@@ -209,6 +209,16 @@ int tbsma_set_tile(tbsma_ctx *ctx, int32_t layers_per_tile, int32_t threads);
  * tbsma_build_cells. */
 int tbsma_set_tile_split(tbsma_ctx *ctx, int32_t ctas_per_tile);
 
+/* Shared-memory variant: how the two gather passes (P:59 stages 1 and 2) are launched.
+ *   1 (default) = persistent kernels: two CTAs of 16 warps per SM work through the tiles of the batch, each holding the
+ *       image of its NEXT tile while it works on the current one; warps move on to the next tile without a CTA-wide
+ *       barrier; the last tiles of a pass are split so that all CTAs finish together;
+ *       used for batches of at least four tiles per SM, smaller ones are run as under 0;
+ *   2, 3, 4 = persistent kernels whatever the batch size, with that many tile images per CTA (1 uses two);
+ *   0 = one CTA per tile (or per 1 / ctas_per_tile of a tile, tbsma_set_tile_split).
+ * Changes cost and the grouping of the per-replica fp64 sums, nothing else.  Takes effect at the next tbsma_build_cells. */
+int tbsma_set_gather(tbsma_ctx *ctx, int32_t mode);
+
 /* md_run replays one captured step as a CUDA graph when `enable` != 0 (default 2) and the stream is not the legacy
  * default stream.  enable = 2: in the shared-memory variant the kernels that renew cells and candidates (needed in a
  * few steps only, decided on the device) are the body of a conditional IF node of that graph, so that nothing is

@@ -20,7 +20,7 @@ EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_kinetic_tensor", "tbsma_stress", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
-    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_thermostat_state", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin", "tbsma_set_tile_split",
+    "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_thermostat_state", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin", "tbsma_set_tile_split", "tbsma_set_gather",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
 
@@ -87,6 +87,7 @@ def lib():
         L.tbsma_set_balance.argtypes = [vp, i32, dbl]
         L.tbsma_set_outer_skin.argtypes = [vp, dbl]
         L.tbsma_set_tile_split.argtypes = [vp, i32]
+        L.tbsma_set_gather.argtypes = [vp, i32]
         L.tbsma_set_timing.argtypes = [vp, i32]
         L.tbsma_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.tbsma_launch_count.argtypes = [vp]
@@ -243,6 +244,9 @@ class Context:
 
     def set_tile_split(self, ctas_per_tile):
         _check(lib().tbsma_set_tile_split(self._h, int(ctas_per_tile)), "tbsma_set_tile_split")
+
+    def set_gather(self, mode):
+        _check(lib().tbsma_set_gather(self._h, int(mode)), "tbsma_set_gather")
 
     def set_thermostat(self, kind, tau_fs=0.0):
         _check(lib().tbsma_set_thermostat(self._h, int(kind), float(tau_fs)), "tbsma_set_thermostat")

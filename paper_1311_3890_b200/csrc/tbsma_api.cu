@@ -328,6 +328,7 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->outer_skin = 2.5;
     c->tile_layers = 2;
     c->tile_threads = 256;
+    c->gather_mode = 1;
     c->use_graph = 1;
     c->overlap = 2;
     c->stagger = 1;
@@ -404,6 +405,16 @@ int tbsma_set_tile_split(tbsma_ctx *c, int32_t ctas_per_tile)
     if (!c || ctas_per_tile < 0 || ctas_per_tile > 128) return TBSMA_EINVAL;
     c->epoch++;
     c->tile_split_req = ctas_per_tile;
+    c->cells_built = c->list_built = 0;
+    return TBSMA_OK;
+}
+
+int tbsma_set_gather(tbsma_ctx *c, int32_t mode)
+{
+    if (!c || mode < 0 || mode > 4) return TBSMA_EINVAL;
+    c->epoch++;
+    c->gather_mode = mode != 0;
+    c->p_nb_req = mode >= 2 ? mode : 0;
     c->cells_built = c->list_built = 0;
     return TBSMA_OK;
 }

@@ -299,7 +299,7 @@ k_build_list_cells(const float4 *__restrict__ pos, const int *__restrict__ cell_
                         }
                         const unsigned kept = __ballot_sync(0xffffffffu, keep);
                         const int k = cnt + __popc(kept & ((1u << lane) - 1u));
-                        if (keep && k < kmax) nlist[((size_t)(k >> 2) * n_pad + i) * 4 + (k & 3)] = j;
+                        if (keep && k < kmax) nlist[(tbsma_lrow(i, kmax >> 2) + (size_t)(k >> 2) * TBSMA_LROW) * 4 + (k & 3)] = j;
                         cnt += __popc(kept);
                     }
                     if (lane == 0) s_cnt[a] = cnt;
@@ -314,7 +314,7 @@ k_build_list_cells(const float4 *__restrict__ pos, const int *__restrict__ cell_
                 if (cnt > ctrl[2]) atomicMax(ctrl + 2, cnt);
                 cnt = min(cnt, kmax);
                 for (int k = cnt; k < ((cnt + 3) & ~3); ++k)   // pad the last group of four with self
-                    nlist[((size_t)(k >> 2) * n_pad + i) * 4 + (k & 3)] = i;
+                    nlist[(tbsma_lrow(i, kmax >> 2) + (size_t)(k >> 2) * TBSMA_LROW) * 4 + (k & 3)] = i;
                 nn[i] = cnt | ((__float_as_int(pi.w) & 3) << 16);
                 pos_build[i] = pi;
             }
@@ -338,7 +338,7 @@ __global__ void k_get_neighbors(const int *__restrict__ tag, const int *__restri
         const int cnt = nn[i] & 0xffff;
         counts[t] = cnt;
         for (int k = 0; k < cnt; ++k)
-            list[(size_t)t * kmax + k] = tag[nlist[((size_t)(k >> 2) * n_pad + i) * 4 + (k & 3)]];
+            list[(size_t)t * kmax + k] = tag[nlist[(tbsma_lrow(i, kmax >> 2) + (size_t)(k >> 2) * TBSMA_LROW) * 4 + (k & 3)]];
     }
 }
 

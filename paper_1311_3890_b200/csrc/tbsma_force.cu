@@ -61,7 +61,7 @@ template <bool PERIODIC>
 __global__ void __launch_bounds__(kBlock)
 k_density(const float4 *__restrict__ pos, const int4 *__restrict__ nlist4, const int *__restrict__ nn,
           const int *__restrict__ atom_rep, const RepGeom *__restrict__ geom, float4 *__restrict__ xs,
-          int n, int n_pad, PairConst pc)
+          int n, int n_pad /* rows of capacity per atom, kmax / 4 */, PairConst pc)
 {
     const int i = blockIdx.x * kBlock + threadIdx.x;
     if (i >= n) return;
@@ -73,10 +73,10 @@ k_density(const float4 *__restrict__ pos, const int4 *__restrict__ nlist4, const
         b.Lx = g->len[0]; b.Ly = g->len[1]; b.Lz = g->len[2]; b.per = g->periodic;
     }
     const int ng = (cnt + 3) >> 2;
-    const int4 *row = nlist4 + i;
+    const int4 *row = nlist4 + tbsma_lrow(i, n_pad);
     float rho0 = 0.f, rho1 = 0.f;
     for (int g = 0; g < ng; ++g) {
-        const int4 jj = __ldcs(row + (size_t)g * n_pad);
+        const int4 jj = __ldcs(row + (size_t)g * TBSMA_LROW);
         const float4 p0 = pos[jj.x], p1 = pos[jj.y], p2 = pos[jj.z], p3 = pos[jj.w];
         rho0 += rho_term<PERIODIC>(pi, p0, jj.x != i, b, pc);
         rho1 += rho_term<PERIODIC>(pi, p1, jj.y != i, b, pc);
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(kBlock)
 k_force(const float4 *__restrict__ xs, const int4 *__restrict__ nlist4, const int *__restrict__ nn,
         const int *__restrict__ atom_rep, const RepGeom *__restrict__ geom, float4 *__restrict__ force,
         double *__restrict__ e_rep, double *__restrict__ w_rep, KickArgs kk, int *__restrict__ ctrl,
-        int n, int n_pad, PairConst pc)
+        int n, int n_pad /* rows of capacity per atom, kmax / 4 */, PairConst pc)
 {
     const int i0 = blockIdx.x * kBlock + threadIdx.x;
     const bool active = i0 < n;
@@ -158,10 +158,10 @@ k_force(const float4 *__restrict__ xs, const int4 *__restrict__ nlist4, const in
         b.Lx = g->len[0]; b.Ly = g->len[1]; b.Lz = g->len[2]; b.per = g->periodic;
     }
     const int ng = (cnt + 3) >> 2;
-    const int4 *row = nlist4 + i;
+    const int4 *row = nlist4 + tbsma_lrow(i, n_pad);
     Acc a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     for (int g = 0; g < ng; ++g) {
-        const int4 jj = __ldcs(row + (size_t)g * n_pad);
+        const int4 jj = __ldcs(row + (size_t)g * TBSMA_LROW);
         const float4 p0 = xs[jj.x], p1 = xs[jj.y], p2 = xs[jj.z], p3 = xs[jj.w];
         force_term<PERIODIC, VIRIAL>(pi, p0, jj.x != i, b, pc, a);
         force_term<PERIODIC, VIRIAL>(pi, p1, jj.y != i, b, pc, a);
@@ -202,7 +202,7 @@ template <bool PERIODIC>
 __global__ void k_count_pairs(const float4 *__restrict__ pos, const int *__restrict__ nlist,
                               const int *__restrict__ nn, const int *__restrict__ atom_rep,
                               const RepGeom *__restrict__ geom, unsigned long long *__restrict__ out,
-                              int n, int n_pad, float rc2)
+                              int n, int n_pad /* rows of capacity per atom */, float rc2)
 {
     unsigned long long entries = 0, inside = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
@@ -215,7 +215,7 @@ __global__ void k_count_pairs(const float4 *__restrict__ pos, const int *__restr
         }
         entries += cnt;
         for (int k = 0; k < cnt; ++k) {
-            const float4 pj = pos[nlist[((size_t)(k >> 2) * n_pad + i) * 4 + (k & 3)]];
+            const float4 pj = pos[nlist[(tbsma_lrow(i, n_pad) + (size_t)(k >> 2) * TBSMA_LROW) * 4 + (k & 3)]];
             float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
             min_image<PERIODIC>(dx, dy, dz, b);
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
@@ -234,9 +234,9 @@ cudaError_t tbsma_launch_density(tbsma_ctx *c, const float4 *pos, cudaStream_t s
     const int grid = (n + kBlock - 1) / kBlock;
     const int4 *nl = reinterpret_cast<const int4 *>(c->d_nlist);
     if (c->any_periodic)
-        k_density<true><<<grid, kBlock, 0, st>>>(pos, nl, c->d_nn, c->d_atom_rep, c->d_geom, c->d_xs, n, c->n_pad, c->pc);
+        k_density<true><<<grid, kBlock, 0, st>>>(pos, nl, c->d_nn, c->d_atom_rep, c->d_geom, c->d_xs, n, c->kmax / 4, c->pc);
     else
-        k_density<false><<<grid, kBlock, 0, st>>>(pos, nl, c->d_nn, c->d_atom_rep, c->d_geom, c->d_xs, n, c->n_pad, c->pc);
+        k_density<false><<<grid, kBlock, 0, st>>>(pos, nl, c->d_nn, c->d_atom_rep, c->d_geom, c->d_xs, n, c->kmax / 4, c->pc);
     c->launches++;
     return cudaGetLastError();
 }
@@ -249,10 +249,10 @@ static void launch_force_k(tbsma_ctx *c, float4 *force, double *e_rep, double *w
     const int4 *nl = reinterpret_cast<const int4 *>(c->d_nlist);
     if (kk.vel)
         k_force<PERIODIC, VIRIAL, true><<<grid, kBlock, 0, st>>>(c->d_xs, nl, c->d_nn, c->d_atom_rep, c->d_geom, force,
-                                                                 e_rep, w_rep, kk, c->d_ctrl, n, c->n_pad, c->pc);
+                                                                 e_rep, w_rep, kk, c->d_ctrl, n, c->kmax / 4, c->pc);
     else
         k_force<PERIODIC, VIRIAL, false><<<grid, kBlock, 0, st>>>(c->d_xs, nl, c->d_nn, c->d_atom_rep, c->d_geom, force,
-                                                                  e_rep, w_rep, kk, c->d_ctrl, n, c->n_pad, c->pc);
+                                                                  e_rep, w_rep, kk, c->d_ctrl, n, c->kmax / 4, c->pc);
 }
 
 cudaError_t tbsma_launch_force(tbsma_ctx *c, float4 *force, double *e_rep, double *w_rep, KickArgs kk,
@@ -275,9 +275,9 @@ cudaError_t tbsma_launch_count_pairs(tbsma_ctx *c, const float4 *pos, unsigned l
     int grid = (n + 255) / 256;
     if (grid > c->n_sm * 8) grid = c->n_sm * 8;
     if (c->any_periodic)
-        k_count_pairs<true><<<grid, 256, 0, st>>>(pos, c->d_nlist, c->d_nn, c->d_atom_rep, c->d_geom, d_out2, n, c->n_pad, c->pc.rc2);
+        k_count_pairs<true><<<grid, 256, 0, st>>>(pos, c->d_nlist, c->d_nn, c->d_atom_rep, c->d_geom, d_out2, n, c->kmax / 4, c->pc.rc2);
     else
-        k_count_pairs<false><<<grid, 256, 0, st>>>(pos, c->d_nlist, c->d_nn, c->d_atom_rep, c->d_geom, d_out2, n, c->n_pad, c->pc.rc2);
+        k_count_pairs<false><<<grid, 256, 0, st>>>(pos, c->d_nlist, c->d_nn, c->d_atom_rep, c->d_geom, d_out2, n, c->kmax / 4, c->pc.rc2);
     c->launches++;
     return cudaGetLastError();
 }

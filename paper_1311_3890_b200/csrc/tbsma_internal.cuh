@@ -50,6 +50,18 @@ struct TileDesc {
     int cell_base;    // first cell of the replica
     int pad;
 };
+// Layout of every neighbour list (int4 rows of the global variant, uint2 rows of the tile variant, candidates too):
+// "block-major".  A row is a group of four entries; the rows of the 32 atoms [32 b, 32 b + 32) are contiguous, row g of
+// atom i at element tbsma_lrow(i, kg) + 32 g, kg = rows of capacity per atom.  A warp's load of row g is one contiguous
+// 256 / 512-byte segment (two if its 32 atoms straddle a block), and ALL rows of a warp's atoms lie within a few KB:
+// with the rows of one atom a whole array pitch apart (the first layout) every row of a chunk was in another 2 MB page.
+#ifdef __CUDACC__
+__host__ __device__ __forceinline__ size_t tbsma_lrow(int i, int kg)
+{
+    return (size_t)(i >> 5) * ((size_t)kg << 5) + (size_t)(i & 31);
+}
+#endif
+#define TBSMA_LROW 32                // elements between consecutive rows of an atom
 #define TBSMA_TILE_MAX_LAYERS 8      // own layers per tile
 #define TBSMA_TILE_MAX_RECORDS 4095  // halo records per tile: (records + sentinel) * 16 B <= 64 KB, u16 byte offsets
 
@@ -104,6 +116,12 @@ struct tbsma_ctx {
     int tile_nsplit;       // CTAs of the gather kernels per tile (> 1 when the tiles are too few to fill the GPU)
     int tile_split_req;    // requested by tbsma_set_tile_split (0 = automatic)
     double *d_cta_sums;    // n_tiles x tile_nsplit x 8: E, E_kin, W (xx yy zz xy xz yz) of every CTA of the force pass
+    // persistent gather kernels: units = p_plain whole tiles, then the remaining tiles in p_S parts each
+    int gather_mode;       // 1 (default): persistent kernels (k_gather_persist); 0: one CTA per tile (or part of a tile)
+    int persist_ok;        // two images + sums of a CTA fit half an SM
+    int p_S, p_plain, p_units, p_max_chunks;
+    int p_tail_split;      // parts the last 2 n_sm tiles of a large batch are cut into (0 = whole)
+    int p_nb, p_nb_req;    // tile images per CTA (the next units' images are filled while the current one is worked on)
     size_t have_sums;
     int32_t *d_maxpop;  // R: largest layer population of each replica (measured at build_cells)
     int32_t *d_hbase;   // n: first halo slot of the tile that owns slot i
@@ -137,7 +155,8 @@ struct tbsma_ctx {
     float4 *d_tmp4;         // n: scratch for the in-place permutation of vel
     int32_t *d_tmp_tag;     // n
     // device: lists
-    int32_t *d_nlist;       // kmax/4 x n_pad x int4, group-major: entry k of atom i at ((k>>2)*n_pad+i)*4+(k&3)
+    int32_t *d_nlist;       // n_pad/32 blocks x kmax/4 rows x 32 atoms x int4 (tbsma_lrow): entry k of atom i at
+                            // (tbsma_lrow(i, kmax/4) + 32 (k>>2)) * 4 + (k&3)
     int32_t *d_nn;          // n: count | flag<<16
     float4 *d_xs;           // n: (x, y, z, 1/sqrt(rho)) written by the density pass
     // device: control

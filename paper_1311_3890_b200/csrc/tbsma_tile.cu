@@ -177,7 +177,7 @@ __device__ __forceinline__ void scan_tile(const TileDesc &t, const ScanArgs &A)
         const int lc = cell_sorted[a] - t.cell_base;
         const int cx = lc % nx, cy = (lc / nx) % ny, cz = lc / t.layer_cells;
         const int x0 = max(cx - 1, 0), x1 = min(cx + 1, nx - 1);
-        uint2 *row = nl_tmp + a;
+        uint2 *row = nl_tmp + tbsma_lrow(a, kmax >> 2);
         unsigned w0 = 0u, w1 = 0u;
         int cnt = 0, cnt_in = 0;     // candidates (d2 < ro2) and list members (d2 < rl2, orders the layer)
         for (int zz = max(cz - 1, 0); zz <= min(cz + 1, nz - 1); ++zz)
@@ -193,7 +193,7 @@ __device__ __forceinline__ void scan_tile(const TileDesc &t, const ScanArgs &A)
                             const unsigned v = (unsigned)j << ((cnt & 1) << 4);
                             if (cnt & 2) w1 |= v; else w0 |= v;
                             if ((cnt & 3) == 3) {
-                                row[(size_t)(cnt >> 2) * n_pad] = make_uint2(w0, w1);
+                                row[(size_t)(cnt >> 2) * TBSMA_LROW] = make_uint2(w0, w1);
                                 w0 = w1 = 0u;
                             }
                         }
@@ -204,7 +204,7 @@ __device__ __forceinline__ void scan_tile(const TileDesc &t, const ScanArgs &A)
             }
         if (cnt > kmax) atomicOr(ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
         cnt = min(cnt, kmax);
-        if (cnt & 3) row[(size_t)(cnt >> 2) * n_pad] = make_uint2(w0, w1);
+        if (cnt & 3) row[(size_t)(cnt >> 2) * TBSMA_LROW] = make_uint2(w0, w1);
         cnts[a - lo] = (unsigned short)cnt_in;
         nn_tmp[a] = cnt | ((__float_as_int(pi.w) & 3) << 16);
     }
@@ -325,6 +325,7 @@ struct FinishArgs {
     const unsigned short *img;   // image placement of every tile (k_tile_place)
     int img_stride;
     int n_pad, s_cap;
+    int kg_o;                    // rows of capacity per atom of the candidate list (kmax_o / 4)
 };
 
 __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const FinishArgs &A)
@@ -349,13 +350,13 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
         const int a = oldof[ip];
         const int nnv = nn_tmp[a];
         const int cnt = nnv & 0xffff;
-        const uint2 *src = nl_tmp + a;
+        const uint2 *src = nl_tmp + tbsma_lrow(a, A.kg_o);
         const int ng = (cnt + 3) >> 2;
         const unsigned lane = (unsigned)(ip - r.lo) & 31u;     // the lane the inner build and the gather passes give this atom
         // pass A: population of the 8 classes, counted from the lane's own (packed bytes; kmax <= 248)
         unsigned long long pop = 0ull;
         for (int g = 0; g < ng; ++g) {
-            const uint2 w = src[(size_t)g * n_pad];
+            const uint2 w = src[(size_t)g * TBSMA_LROW];
             const unsigned e[4] = {w.x & 0xffffu, w.x >> 16, w.y & 0xffffu, w.y >> 16};
 #pragma unroll
             for (int q = 0; q < 4; ++q)
@@ -370,7 +371,7 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
         // pass B: class-sorted copy in shared memory (column tid: conflict-free for any row)
         unsigned long long cur = 0ull;
         for (int g = 0; g < ng; ++g) {
-            const uint2 w = src[(size_t)g * n_pad];
+            const uint2 w = src[(size_t)g * TBSMA_LROW];
             const unsigned e[4] = {w.x & 0xffffu, w.x >> 16, w.y & 0xffffu, w.y >> 16};
 #pragma unroll
             for (int q = 0; q < 4; ++q)
@@ -383,12 +384,12 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
                 }
         }
         // rows of four entries, unused entries = 0 = the sentinel
-        uint2 *dst = nl + ip;
+        uint2 *dst = nl + tbsma_lrow(ip, A.kg_o);
         for (int g = 0; g < ng; ++g) {
             unsigned e[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) e[q] = 4 * g + q < cnt ? (unsigned)scr[(4 * g + q) * nthr + tid] : 0u;
-            dst[(size_t)g * n_pad] = make_uint2(e[0] | (e[1] << 16), e[2] | (e[3] << 16));
+            dst[(size_t)g * TBSMA_LROW] = make_uint2(e[0] | (e[1] << 16), e[2] | (e[3] << 16));
         }
         nn[ip] = nnv;
         hbase[ip] = r.halo_lo;
@@ -568,6 +569,7 @@ struct InnerArgs {
     const float4 *pos_outer;
     int *want_outer;         // per replica
     int kmax;                // inner capacity
+    int kg_o;                // rows of capacity per atom of the candidate list
     float rl2, want2, viol2;
 };
 
@@ -591,7 +593,7 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
         const float4 pi = pos[i];
         const int nno = ia.nn_o[i];
         const int ng = ((nno & 0xffff) + 3) >> 2;
-        const uint2 *row = ia.olist + i;
+        const uint2 *row = ia.olist + tbsma_lrow(i, ia.kg_o);
         // pass 1: the candidates that pass the fp32 predicate of D:A6, in candidate order.  Branch-free: every
         // candidate is stored at the current end of the column, the end advances for the members only.
         int m = 0;
@@ -611,7 +613,7 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
             }
         };
         {
-            auto ld = [&](int g) { return g < ng ? __ldcs(row + (size_t)g * n_pad) : make_uint2(0u, 0u); };
+            auto ld = [&](int g) { return g < ng ? __ldcs(row + (size_t)g * TBSMA_LROW) : make_uint2(0u, 0u); };
             uint2 q0 = ld(0), q1 = ld(1), q2 = ld(2), q3 = ld(3);
             int g = 0;
             for (; g + 4 <= ng; g += 4) {
@@ -644,7 +646,7 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
         // pass 2: position 8 j + s takes the j-th entry of class lane + s for j < L = m / 8.  A class with fewer than
         // L entries leaves holes; they, and the positions from 8 L on, take the entries beyond the L-th of the longer
         // classes, in stored order.
-        uint2 *dst = nl_out + i;
+        uint2 *dst = nl_out + tbsma_lrow(i, ia.kmax >> 2);
         unsigned long long w = 0ull;
         const int L = m >> 3;
         int sc = 0, sj = L;
@@ -661,7 +663,7 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
                 const int k = n_s[sft] > j ? o_s[sft] + j : next_surplus();
                 w |= (unsigned long long)col[k * nthr] << ((sft & 3) << 4);
                 if ((sft & 3) == 3) {
-                    dst[(size_t)(2 * j + (sft >> 2)) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));
+                    dst[(size_t)(2 * j + (sft >> 2)) * TBSMA_LROW] = make_uint2((unsigned)w, (unsigned)(w >> 32));
                     w = 0ull;
                 }
             }
@@ -670,11 +672,11 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
             const int k = next_surplus();
             w |= (unsigned long long)col[k * nthr] << ((p & 3) << 4);
             if ((p & 3) == 3) {
-                dst[(size_t)(p >> 2) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));
+                dst[(size_t)(p >> 2) * TBSMA_LROW] = make_uint2((unsigned)w, (unsigned)(w >> 32));
                 w = 0ull;
             }
         }
-        if (m & 3) dst[(size_t)(m >> 2) * n_pad] = make_uint2((unsigned)w, (unsigned)(w >> 32));   // unused = 0 = sentinel
+        if (m & 3) dst[(size_t)(m >> 2) * TBSMA_LROW] = make_uint2((unsigned)w, (unsigned)(w >> 32));   // unused = 0 = sentinel
         nn_out[i] = m | (nno & 0x7fff0000);
         pb_out[i] = pi;
         const float4 po = ia.pos_outer[i];
@@ -736,7 +738,7 @@ __device__ __forceinline__ int next_chunk(int *counter)
 
 __device__ __forceinline__ uint2 ld_row(const uint2 *row, int g, int ng, int n_pad)
 {
-    return g < ng ? __ldcs(row + (size_t)g * n_pad) : make_uint2(0u, 0u);
+    return g < ng ? __ldcs(row + (size_t)g * TBSMA_LROW) : make_uint2(0u, 0u);
 }
 
 // stage 1 (Eq.1): rho_i over the list, s_i = rho_i^(-1/2) packed with the position.
@@ -746,7 +748,7 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
                                              const float4 *__restrict__ pos, const uint2 *__restrict__ nl,
                                              const int *__restrict__ nn, float4 *__restrict__ xs,
                                              int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
-                                             const unsigned short *__restrict__ img, int part, int nsplit)
+                                             const unsigned short *__restrict__ img, int part, int nsplit, int kg)
 {
     const TileRange r = tile_range(t, cell_start);
     if (r.hi <= r.lo) return;
@@ -773,7 +775,7 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
         if (i >= r.hi) continue;
         const float4 pi = pos[i];
         const int ng = ((nn[i] & 0xffff) + 3) >> 2;
-        const uint2 *row = nl + i;
+        const uint2 *row = nl + tbsma_lrow(i, kg);
         f32x2 rho2 = pk(0.f, 0.f);
         auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
@@ -811,6 +813,7 @@ struct ListSel {
     const unsigned short *img;   // image placement of every tile (k_tile_place)
     int img_stride;
     int nsplit;                  // CTAs per tile (> 1 when the tiles are too few to fill the GPU)
+    int kg;                      // rows of capacity per atom of the list (kmax / 4)
 };
 __device__ __forceinline__ int list_half(const ListSel &ls, int rep)
 {
@@ -829,7 +832,7 @@ k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_
     const TileDesc t = tiles[ti];
     const int h = list_half(ls, t.rep);
     density_tile<SPLIT>(t, cell_start, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad, s_cap,
-                 pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit);
+                 pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit, ls.kg);
     // Launched as a programmatic dependent of the filter kernel this pass starts early and reads nothing of it; but the
     // kernels after it (force pass, then the swap of the list halves) are ordered after THIS kernel only, so it must
     // not complete before the filter kernel has (a no-op for an ordinary launch).
@@ -895,7 +898,7 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
                                            const int *__restrict__ nn, float4 *__restrict__ force, const KickArgs &kk,
                                            int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
                                            const unsigned short *__restrict__ img, int part, int nsplit,
-                                           double *__restrict__ my_sums)
+                                           double *__restrict__ my_sums, int kg)
 {
     constexpr int NQ = VIRIAL ? 8 : 2;
     __shared__ double s_part[NQ][kMaxChunks];
@@ -926,7 +929,7 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
         const float4 pi = xs[i];
         const int nni = nn[i];
         const int ng = ((nni & 0xffff) + 3) >> 2;
-        const uint2 *row = nl + i;
+        const uint2 *row = nl + tbsma_lrow(i, kg);
         const f32x2 z2 = pk(0.f, 0.f);
         AccT a = {z2, z2, z2, z2, z2, z2, z2, z2, z2, z2};
         auto group = [&](const uint2 jj) {
@@ -1009,7 +1012,350 @@ k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
     const int h = list_half(ls, t.rep);
     force_tile<VIRIAL, KICK, SPLIT>(t, cell_start, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force, kk,
                              ctrl, n_pad, s_cap, pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit,
-                             cta_sums + 8 * (size_t)blockIdx.x);
+                             cta_sums + 8 * (size_t)blockIdx.x, ls.kg);
+}
+
+// ---- persistent gather kernels ----------------------------------------------------------------------
+// One CTA of 16 warps per half SM for the whole pass.  Work comes in UNITS (a tile, or 1 / S of a tile's 32-atom chunks for
+// the last tiles of the pass and for batches with few tiles), claimed from a global counter.  A CTA holds TWO tile images:
+// while its warps work through the chunks of unit k the image of unit k + 1 is already in shared memory, and a warp that
+// finds no chunk left in unit k moves on to unit k + 1 AT ONCE -- no CTA-wide barrier at the end of a tile (8 % of the
+// warp time of the one-CTA-per-tile kernels: 25 chunks over 8 warps), no wait for an image fill (5 %), no partial last wave
+// of CTAs (6 %).  The last warp out of unit k adds the unit's sums in chunk order, claims unit k + 2 and fills the image
+// buffer unit k just vacated with cp.async (16 bytes per record, straight to the placed image index), completion
+// signalled on an mbarrier the warps wait on before they enter unit k + 2.
+struct PSlot {
+    int tile;            // < 0: the pass has run out of units
+    int lo, hi;          // own slots of the tile
+    int cb, ce;          // chunks [cb, ce) of the tile are this unit's
+    int half;            // which half of the list buffers the tile's replica reads
+    int sums;            // slot in cta_sums (force pass)
+    int pad;
+};
+constexpr int kPMaxBuf = 4;
+struct PShared {
+    unsigned long long full[kPMaxBuf];   // mbarriers: image + slot description of the buffer are in place
+    PSlot slot[kPMaxBuf];
+    int next[kPMaxBuf], done[kPMaxBuf];
+    int ended;
+};
+constexpr int kPThreads = 512;
+constexpr int kPWarps = kPThreads / 32;
+
+struct PUnits {
+    int n_units;     // n_plain whole tiles, then (n_tiles - n_plain) tiles in S parts each
+    int n_plain, S;
+    int max_chunks;  // capacity of the per-chunk sums of a unit
+};
+__device__ __forceinline__ void punit(const PUnits &U, int u, int &tile, int &part, int &nparts)
+{
+    if (u < U.n_plain) { tile = u; part = 0; nparts = 1; }
+    else { const int v = u - U.n_plain; tile = U.n_plain + v / U.S; part = v % U.S; nparts = U.S; }
+}
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *b, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *b)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity)
+{
+    const unsigned a = smem_u32(b);
+    unsigned ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+
+// description of unit u in slot b (lane 0 of the calling warp writes it); returns halo_lo and nh for the fill
+__device__ __forceinline__ bool pslot_describe(PSlot &S, const PUnits &U, int u, const TileDesc *__restrict__ tiles,
+                                               const int *__restrict__ cell_start, const ListSel &ls, int s_cap,
+                                               int *__restrict__ ctrl, int &tile, int &halo_lo, int &nh)
+{
+    int part, nparts;
+    punit(U, u, tile, part, nparts);
+    const TileDesc t = tiles[tile];
+    const TileRange r = tile_range(t, cell_start);
+    S.tile = tile;
+    S.lo = r.lo; S.hi = r.hi;
+    S.half = list_half(ls, t.rep);
+    S.sums = tile * U.S + part;
+    const int nchunk_all = (r.hi - r.lo + 31) >> 5;
+    S.cb = nchunk_all * part / nparts;
+    S.ce = nchunk_all * (part + 1) / nparts;
+    halo_lo = r.halo_lo; nh = r.nh;
+    bool ok = r.hi > r.lo && S.ce > S.cb;
+    if (r.nh > s_cap || S.ce - S.cb > U.max_chunks) {
+        atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
+        ok = false;
+    }
+    if (!ok) S.ce = S.cb;     // nothing to do (its sums are still written: zero)
+    return ok;
+}
+
+// image fill by ONE warp, asynchronous: every lane's copies arrive on `bar` when they have landed
+__device__ __forceinline__ void fill_image_async(float4 *sm, const float4 *__restrict__ src,
+                                                 const unsigned short *__restrict__ img, int halo_lo, int nh,
+                                                 unsigned long long *bar)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned base = smem_u32(sm);
+    // 32 image indices per lane in flight before the first copy is issued: two rounds for a tile of 2000 records
+    for (int k0 = lane; k0 < nh; k0 += 32 * 32) {
+        unsigned at[32];
+#pragma unroll
+        for (int u = 0; u < 32; ++u) at[u] = k0 + u * 32 < nh ? (unsigned)img[k0 + u * 32] : 0u;
+#pragma unroll
+        for (int u = 0; u < 32; ++u)
+            if (k0 + u * 32 < nh)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(base + (at[u] << 4)),
+                             "l"(src + halo_lo + k0 + u * 32) : "memory");
+    }
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// PASS 0: density (src = pos, out = xs); PASS 1: force (src = xs, out = force, sums, kick)
+struct PArgs {
+    const TileDesc *tiles;
+    const int *cell_start;
+    const float4 *src;
+    const uint2 *nl;
+    const int *nn;
+    float4 *xs;            // density: out
+    float4 *force;         // force: out
+    double *cta_sums;      // force: out
+    KickArgs kk;
+    int *ctrl;
+    int *claim;            // this pass's unit counter
+    int *claim_other;      // the other pass's, reset here (the two passes never run together)
+    ListSel ls;
+    int n_pad, s_cap, img_cap;
+    int nb;                // image buffers per CTA (2 .. kPMaxBuf)
+    PUnits U;
+    PairConst pc;
+};
+
+template <int PASS, bool VIRIAL, bool KICK>
+__global__ void __launch_bounds__(kPThreads, 2)
+k_gather_persist(const PArgs A)
+{
+    constexpr int NQ = VIRIAL ? 8 : 2;
+    extern __shared__ float4 smem_f4[];
+    __shared__ PShared sh;
+    const int NB = A.nb;
+    double *s_part = reinterpret_cast<double *>(smem_f4 + (size_t)NB * A.img_cap);    // force: [NB][NQ][max_chunks]
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int G = (int)gridDim.x;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *A.claim_other = 0;
+    // ---- prologue: units blockIdx.x and blockIdx.x + G, both images filled by everybody
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < NB; ++b) mbar_init(&sh.full[b], 33);
+        sh.ended = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __shared__ int s_pro[kPMaxBuf][2];       // prologue: halo_lo and records of the first NB units
+    if ((int)threadIdx.x < NB) {
+        const int b = threadIdx.x, u = (int)blockIdx.x + b * G;
+        PSlot S;
+        S.tile = -1; S.lo = S.hi = S.cb = S.ce = S.half = S.sums = S.pad = 0;
+        int tile = -1, hlo = 0, nh = 0;
+        if (u < A.U.n_units && !pslot_describe(S, A.U, u, A.tiles, A.cell_start, A.ls, A.s_cap, A.ctrl, tile, hlo, nh)) nh = 0;
+        sh.slot[b] = S;
+        sh.next[b] = S.cb;
+        sh.done[b] = 0;
+        s_pro[b][0] = hlo;
+        s_pro[b][1] = nh;
+    }
+    if ((int)threadIdx.x < NB) smem_f4[(size_t)threadIdx.x * A.img_cap] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
+    __syncthreads();
+#pragma unroll 1
+    for (int b = 0; b < NB; ++b) {
+        const int tile = sh.slot[b].tile, hlo = s_pro[b][0], nh = s_pro[b][1];
+        if (tile < 0 || nh <= 0) continue;
+        const unsigned short *__restrict__ img = A.ls.img + (size_t)tile * A.ls.img_stride;
+        float4 *sm = smem_f4 + (size_t)b * A.img_cap;
+        for (int k0 = threadIdx.x; k0 < nh; k0 += 4 * kPThreads) {
+            float4 rec[4];
+            unsigned short at[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int k = k0 + u * kPThreads;
+                if (k < nh) { at[u] = img[k]; rec[u] = A.src[hlo + k]; }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (k0 + u * kPThreads < nh) sm[at[u]] = rec[u];
+        }
+    }
+    __syncthreads();
+    // ---- the warps work through the units, each at its own pace
+    unsigned dead = 0u;          // bit b: buffer b has run out of units (for good)
+    bool bad = false;
+    int b = -1, round = 0;       // buffer of unit k = k % NB, round = k / NB
+#pragma unroll 1
+    for (;;) {
+        if (++b == NB) { b = 0; ++round; }
+        if (dead >> b & 1u) {
+            if (dead == (1u << NB) - 1u) break;
+            continue;
+        }
+        if (round >= 1) mbar_wait(&sh.full[b], (unsigned)((round - 1) & 1));
+        const PSlot S = sh.slot[b];
+        if (S.tile < 0) { dead |= 1u << b; continue; }
+        const float4 *sm = smem_f4 + (size_t)b * A.img_cap;
+        const uint2 *__restrict__ nl = A.nl + (size_t)S.half * A.ls.nl_stride;
+        const int *__restrict__ nn = A.nn + (size_t)S.half * A.ls.n_stride;
+        double *part = s_part + (size_t)b * NQ * A.U.max_chunks;
+        for (int ch = next_chunk(&sh.next[b]); ch < S.ce; ch = next_chunk(&sh.next[b])) {
+            const int i = S.lo + (ch << 5) + lane;
+            if (PASS == 0) {
+                if (i >= S.hi) continue;
+                // own record, count and the first three rows in ONE round trip: the rows are read whatever the count is (they
+                // exist: kg >= 3) and dropped afterwards if the list is shorter
+                const uint2 *row = nl + tbsma_lrow(i, A.ls.kg);
+                uint2 q0 = __ldcs(row), q1 = __ldcs(row + TBSMA_LROW), q2 = __ldcs(row + 2 * TBSMA_LROW);
+                const float4 pi = A.src[i];
+                const int ng = ((nn[i] & 0xffff) + 3) >> 2;
+                if (ng < 3) { q2 = make_uint2(0u, 0u); if (ng < 2) q1 = q2; if (ng < 1) q0 = q2; }
+                f32x2 rho2 = pk(0.f, 0.f);
+                auto group = [&](const uint2 jj) {
+                    const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
+                    const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
+                    rho2 = rho_term2(pi, p0, p1, A.pc, rho2);
+                    rho2 = rho_term2(pi, p2, p3, A.pc, rho2);
+                };
+                // three rows in flight; a row register is reloaded right AFTER its use (loaded before, the new value needs a
+                // second register while the old one is live, and the move back at the loop's end waits for the load)
+                int g = 0;
+                for (; g + 3 <= ng; g += 3) {
+                    group(q0); q0 = ld_row(row, g + 3, ng, A.n_pad);
+                    group(q1); q1 = ld_row(row, g + 4, ng, A.n_pad);
+                    group(q2); q2 = ld_row(row, g + 5, ng, A.n_pad);
+                }
+                if (g < ng) {
+                    group(q0);
+                    if (g + 1 < ng) group(q1);
+                }
+                float rho0, rho1;
+                unpk(rho2, rho0, rho1);
+                const float rho = rho0 + rho1;
+                const float s = rho > 0.f ? 1.0f / sqrtf(rho) : 0.f;     // once per atom, IEEE (D:A5 for rho = 0)
+                A.xs[i] = make_float4(pi.x, pi.y, pi.z, s);
+            } else {
+                double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+                if (i < S.hi) {
+                    const uint2 *row = nl + tbsma_lrow(i, A.ls.kg);
+                    uint2 q0 = __ldcs(row), q1 = __ldcs(row + TBSMA_LROW), q2 = __ldcs(row + 2 * TBSMA_LROW);
+                    const float4 pi = A.src[i];
+                    const int nni = nn[i];
+                    if (KICK) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.kk.vel + i));   // read at the end of the chunk
+                    const int ng = ((nni & 0xffff) + 3) >> 2;
+                    if (ng < 3) { q2 = make_uint2(0u, 0u); if (ng < 2) q1 = q2; if (ng < 1) q0 = q2; }
+                    const f32x2 z2 = pk(0.f, 0.f);
+                    AccT a = {z2, z2, z2, z2, z2, z2, z2, z2, z2, z2};
+                    auto group = [&](const uint2 jj) {
+                        const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
+                        const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
+                        force_term2<VIRIAL>(pi, p0, p1, A.pc, a);
+                        force_term2<VIRIAL>(pi, p2, p3, A.pc, a);
+                    };
+                    int g = 0;
+                    for (; g + 3 <= ng; g += 3) {
+                        group(q0); q0 = ld_row(row, g + 3, ng, A.n_pad);
+                        group(q1); q1 = ld_row(row, g + 4, ng, A.n_pad);
+                        group(q2); q2 = ld_row(row, g + 5, ng, A.n_pad);
+                    }
+                    if (g < ng) {
+                        group(q0);
+                        if (g + 1 < ng) group(q1);
+                    }
+                    const float fx = sum2(a.fx), fy = sum2(a.fy), fz = sum2(a.fz);
+                    const float sqrt_rho = pi.w > 0.f ? 1.0f / pi.w : 0.f;
+                    const float ei = __fmaf_rn(sum2(a.er), A.pc.e_rep_scale, -sqrt_rho);   // Eq.1-3: E_R^i + E_B^i
+                    A.force[i] = make_float4(fx, fy, fz, ei);
+                    bad = bad || !isfinite(fx + fy + fz + ei);
+                    se = (double)ei;
+                    if (KICK && (nni >> 16) == 0) {       // final B of the step, dynamic atoms only
+                        float4 v = A.kk.vel[i];
+                        v.x = __fmaf_rn(A.kk.kick, fx, v.x);
+                        v.y = __fmaf_rn(A.kk.kick, fy, v.y);
+                        v.z = __fmaf_rn(A.kk.kick, fz, v.z);
+                        A.kk.vel[i] = v;
+                        sk = (double)(A.kk.ke_scale * (v.x * v.x + v.y * v.y + v.z * v.z));
+                    }
+                    if (VIRIAL) {
+                        sw[0] = 0.5 * (double)sum2(a.wxx); sw[1] = 0.5 * (double)sum2(a.wyy); sw[2] = 0.5 * (double)sum2(a.wzz);
+                        sw[3] = 0.5 * (double)sum2(a.wxy); sw[4] = 0.5 * (double)sum2(a.wxz); sw[5] = 0.5 * (double)sum2(a.wyz);
+                    }
+                }
+                __syncwarp();
+                se = warp_sum_d(se);
+                if (KICK) sk = warp_sum_d(sk);
+                if (VIRIAL) {
+#pragma unroll
+                    for (int q = 0; q < 6; ++q) sw[q] = warp_sum_d(sw[q]);
+                }
+                if (lane == 0) {
+                    const int c = ch - S.cb;
+                    part[c] = se;
+                    part[A.U.max_chunks + c] = sk;
+                    if (VIRIAL) {
+#pragma unroll
+                        for (int q = 0; q < 6; ++q) part[(size_t)((2 + q) % NQ) * A.U.max_chunks + c] = sw[q];
+                    }
+                }
+            }
+        }
+        // ---- out of unit k.  The last warp out adds up the unit and refills the buffer with unit k + 2.
+        __syncwarp();
+        int last = 0;
+        if (lane == 0) {
+            __threadfence_block();
+            last = atomicAdd(&sh.done[b], 1) == kPWarps - 1 ? 1 : 0;
+        }
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (!last) continue;
+        __threadfence_block();
+        if (PASS == 1) {      // the unit's sums: chunks in chunk order (lane l takes chunks l, l + 32, ...; then a fixed tree)
+            double *my_sums = A.cta_sums + 8 * (size_t)S.sums;
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                double v = 0.0;
+                for (int c = lane; c < S.ce - S.cb; c += 32) v += part[(size_t)q * A.U.max_chunks + c];
+                v = warp_sum_d(v);
+                if (lane == 0) my_sums[q] = v;
+            }
+        }
+        int u = -1;
+        if (lane == 0 && !sh.ended) {
+            u = atomicAdd(A.claim, 1) + NB * G;
+            if (u >= A.U.n_units) { u = -1; sh.ended = 1; }
+        }
+        u = __shfl_sync(0xffffffffu, u, 0);
+        int tile = -1, hlo = 0, nh = 0;
+        if (lane == 0) {
+            PSlot N;
+            N.tile = -1; N.lo = N.hi = N.cb = N.ce = N.half = N.sums = N.pad = 0;
+            if (u >= 0 && !pslot_describe(N, A.U, u, A.tiles, A.cell_start, A.ls, A.s_cap, A.ctrl, tile, hlo, nh)) nh = 0;
+            sh.slot[b] = N;
+            sh.next[b] = N.cb;
+            sh.done[b] = 0;
+        }
+        tile = __shfl_sync(0xffffffffu, tile, 0);
+        hlo = __shfl_sync(0xffffffffu, hlo, 0);
+        nh = __shfl_sync(0xffffffffu, nh, 0);
+        if (tile < 0) nh = 0;
+        fill_image_async(smem_f4 + (size_t)b * A.img_cap, A.src, A.ls.img + (size_t)(tile < 0 ? 0 : tile) * A.ls.img_stride, hlo, nh, &sh.full[b]);
+        if (lane == 0) mbar_arrive(&sh.full[b]);       // releases the slot description written above
+    }
+    if (PASS == 1 && bad) atomicOr(A.ctrl + 1, (int)TBSMA_FLAG_NONFINITE);
+    // (density pass) launched as a programmatic dependent of the filter kernel: see k_density_tile
+    if (PASS == 0) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // per-replica sums of the CTA sums, in tile order (tbsma_compute; inside an MD step k_finish_step does it)
@@ -1020,9 +1366,9 @@ k_reduce_replicas(TileSums ts, int R)
 }
 
 // ---- inspection (parity tests, bench statistics) ----------------------------------------------
-__device__ __forceinline__ unsigned entry_of(const uint2 *__restrict__ nl, int n_pad, int i, int k)
+__device__ __forceinline__ unsigned entry_of(const uint2 *__restrict__ nl, int kg, int i, int k)
 {
-    const uint2 w = nl[(size_t)(k >> 2) * n_pad + i];
+    const uint2 w = nl[tbsma_lrow(i, kg) + (size_t)(k >> 2) * TBSMA_LROW];
     const unsigned h = (k & 2) ? w.y : w.x;
     return (k & 1) ? (h >> 16) : (h & 0xffffu);
 }
@@ -1043,7 +1389,7 @@ __global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *_
         counts[t] = cnt;
         for (int k = 0; k < cnt; ++k)
             list[(size_t)t * kmax + k] =
-                tag[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, n_pad, i, k) >> 4)]];
+                tag[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, kmax >> 2, i, k) >> 4)]];
     }
 }
 
@@ -1051,7 +1397,7 @@ __global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *
                                    const int *__restrict__ nn0, const int *__restrict__ hbase,
                                    const int *__restrict__ tileof, const unsigned short *__restrict__ inv,
                                    int inv_stride, const int *__restrict__ atom_rep, const int *__restrict__ cur,
-                                   size_t nl_stride, unsigned long long *__restrict__ out, int n, int n_pad, float rc2)
+                                   size_t nl_stride, unsigned long long *__restrict__ out, int n, int n_pad, float rc2, int kg)
 {
     unsigned long long entries = 0, inside = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
@@ -1062,7 +1408,7 @@ __global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *
         const int cnt = nn[i] & 0xffff;
         entries += cnt;
         for (int k = 0; k < cnt; ++k) {
-            const float4 pj = pos[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, n_pad, i, k) >> 4)]];
+            const float4 pj = pos[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, kg, i, k) >> 4)]];
             const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
             inside += d2 < rc2;
@@ -1098,6 +1444,11 @@ size_t finish_smem(const tbsma_ctx *c)
     return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax_o * finish_threads(c) * 2;
 }
 size_t gather_smem(const tbsma_ctx *c) { return (size_t)c->img_cap * 16; }
+size_t persist_smem(const tbsma_ctx *c, int pass, bool virial)
+{
+    return (size_t)c->p_nb * c->img_cap * 16 +
+           (pass == 1 ? (size_t)c->p_nb * (virial ? 8 : 2) * c->p_max_chunks * sizeof(double) : 0);
+}
 size_t inner_smem(const tbsma_ctx *c) { return gather_smem(c) + (size_t)kInnerThreads * (c->kmax + 1) * 2; }
 InnerArgs inner_args(const tbsma_ctx *c)
 {
@@ -1116,6 +1467,7 @@ InnerArgs inner_args(const tbsma_ctx *c)
     ia.pos_outer = c->d_pos_outer;
     ia.want_outer = c->d_want_outer;
     ia.kmax = c->kmax;
+    ia.kg_o = c->kmax_o / 4;
     ia.rl2 = c->pc.rl2;
     // candidates are valid while no atom moved more than S/2 since their build (viol2).  New ones are asked
     // for one rebuild early: by the NEXT rebuild an atom moves at most skin/2 (+ one step) further.
@@ -1232,7 +1584,34 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         if (c->tile_split_req > 0) nsplit = c->tile_split_req;
         if (nsplit < 1) nsplit = 1;
     }
-    if (e == cudaSuccess) e = ensure((void **)&c->d_cta_sums, &c->have_sums, sizeof(double) * 8 * nt1 * (size_t)nsplit);
+    // Units of the persistent gather kernels (k_gather_persist): whole tiles, except that the LAST tiles of the pass are
+    // cut into S parts so that the CTAs run out of work together, and that batches with few tiles are cut throughout.
+    int pS = 1, p_plain = (int)n_tiles;
+    {
+        const int G = 2 * c->n_sm;
+        int est_chunks = (own_cap * 4 / 5 + 31) / 32;
+        if (est_chunks < 1) est_chunks = 1;
+        if (c->tile_split_req > 0) { pS = c->tile_split_req; p_plain = 0; }
+        else if (n_tiles < 4 * (int64_t)G) {
+            pS = n_tiles > 0 ? (int)((4 * (int64_t)G + n_tiles - 1) / n_tiles) : 1;
+            if (pS > est_chunks) pS = est_chunks;
+            p_plain = 0;
+        } else {
+            // many tiles per CTA: whole tiles (a split tile is filled once per part, and the parts are too short to hide it)
+            pS = c->p_tail_split > 0 ? c->p_tail_split : 1;
+            if (pS > est_chunks) pS = est_chunks;
+            p_plain = (int)n_tiles - G;
+        }
+        if (pS < 1) pS = 1;
+        if (pS == 1) p_plain = (int)n_tiles;
+    }
+    c->p_S = pS;
+    c->p_plain = p_plain;
+    c->p_units = p_plain + ((int)n_tiles - p_plain) * pS;
+    c->p_max_chunks = (own_cap + 31) / 32 + 2;
+    const size_t sums_slots = nt1 * (size_t)(nsplit > pS ? nsplit : pS);
+    if (e == cudaSuccess) e = ensure((void **)&c->d_cta_sums, &c->have_sums, sizeof(double) * 8 * sums_slots);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->d_cta_sums, 0, sizeof(double) * 8 * sums_slots, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d_work, 0, sizeof(int) * (size_t)(2 + 2 * n_tiles), st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tiles, h, sizeof(TileDesc) * (size_t)n_tiles, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_tile_first, first, sizeof(int) * (size_t)(R + 1), cudaMemcpyHostToDevice, st);
@@ -1260,6 +1639,19 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     TBSMA_ATTR((k_force_tile<false, false, true>)); TBSMA_ATTR((k_force_tile<false, true, true>));
     TBSMA_ATTR((k_force_tile<true, false, true>)); TBSMA_ATTR((k_force_tile<true, true, true>));
 #undef TBSMA_ATTR
+    {
+        // image buffers per CTA: as many (up to the requested depth) as let two CTAs share an SM
+        c->p_nb = c->p_nb_req > 0 ? c->p_nb_req : 2;     // (3 measured no faster than 2 on config 3)
+        if (c->p_nb > kPMaxBuf) c->p_nb = kPMaxBuf;
+        while (c->p_nb > 2 && persist_smem(c, 1, true) > 112 * 1024) c->p_nb--;
+        const int sm_p0 = (int)persist_smem(c, 0, false), sm_p1 = (int)persist_smem(c, 1, false), sm_p1v = (int)persist_smem(c, 1, true);
+#define TBSMA_ATTR(K, B) if (e == cudaSuccess) e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, B)
+        TBSMA_ATTR((k_gather_persist<0, false, false>), sm_p0);
+        TBSMA_ATTR((k_gather_persist<1, false, false>), sm_p1); TBSMA_ATTR((k_gather_persist<1, false, true>), sm_p1);
+        TBSMA_ATTR((k_gather_persist<1, true, false>), sm_p1v); TBSMA_ATTR((k_gather_persist<1, true, true>), sm_p1v);
+#undef TBSMA_ATTR
+        c->persist_ok = sm_p1v <= 112 * 1024 && c->kmax >= 12;     // two CTAs per SM; three rows per atom exist
+    }
     if (e != cudaSuccess) return TBSMA_ECUDA;
     c->active_variant = 2;
     return TBSMA_OK;
@@ -1280,7 +1672,7 @@ cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int3
     FinishArgs fa;
     fa.cell_start = c->d_cell_start; fa.nl_tmp = ol_tmp; fa.nn_tmp = c->d_nn_tmp; fa.newslot = c->d_newslot;
     fa.oldof = c->d_oldof; fa.nl = ol; fa.nn = c->d_nn_o; fa.hbase = c->d_hbase; fa.tileof = c->d_tileof;
-    fa.img = c->d_img; fa.img_stride = c->tile_cap; fa.n_pad = c->n_pad;
+    fa.img = c->d_img; fa.img_stride = c->tile_cap; fa.n_pad = c->n_pad; fa.kg_o = c->kmax_o / 4;
     fa.s_cap = c->tile_cap;
     PlaceArgs pa;
     pa.cell_start = c->d_cell_start; pa.oldof = c->d_oldof; pa.pos_sorted = c->d_tmp_pos; pa.geom = c->d_geom;
@@ -1343,7 +1735,36 @@ static ListSel list_sel(const tbsma_ctx *c, int sync_level)
     ls.img = c->d_img;
     ls.img_stride = c->tile_cap;
     ls.nsplit = c->tile_nsplit;
+    ls.kg = c->kmax / 4;
     return ls;
+}
+
+// persistent kernels for batches with at least two tiles per CTA (or when asked for by depth, tbsma_set_gather(2..4));
+// a handful of tiles (one small wire) is quicker with one short-lived CTA per part of a tile
+static bool use_persist(const tbsma_ctx *c)
+{
+    return c->gather_mode != 0 && c->persist_ok && (c->p_nb_req > 0 || c->n_tiles >= 4 * c->n_sm);
+}
+
+static PArgs persist_args(tbsma_ctx *c, int pass, const float4 *src, int sync_level)
+{
+    PArgs A;
+    A.tiles = c->d_tiles; A.cell_start = c->d_cell_start; A.src = src;
+    A.nl = reinterpret_cast<const uint2 *>(c->d_nlist); A.nn = c->d_nn;
+    A.xs = c->d_xs; A.force = nullptr; A.cta_sums = c->d_cta_sums;
+    A.kk.vel = nullptr; A.kk.kick = 0.f; A.kk.ke_scale = 0.f; A.kk.ekin = nullptr;
+    A.ctrl = c->d_ctrl; A.claim = c->d_ctrl + 4 + pass; A.claim_other = c->d_ctrl + 4 + (pass ^ 1);
+    A.ls = list_sel(c, sync_level);
+    A.n_pad = c->n_pad; A.s_cap = c->tile_cap; A.img_cap = c->img_cap;
+    A.nb = c->p_nb;
+    A.U.n_units = c->p_units; A.U.n_plain = c->p_plain; A.U.S = c->p_S; A.U.max_chunks = c->p_max_chunks;
+    A.pc = c->pc;
+    return A;
+}
+static int persist_grid(const tbsma_ctx *c)
+{
+    const int G = 2 * c->n_sm;
+    return c->p_units < G ? (c->p_units > 0 ? c->p_units : 1) : G;
 }
 
 // early: the launch may begin while the kernel before it on the stream (the filter pass of the replicas renewing
@@ -1360,6 +1781,15 @@ cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = early ? 1 : 0;
+    if (use_persist(c)) {
+        cfg.gridDim = dim3((unsigned)persist_grid(c));
+        cfg.blockDim = dim3(kPThreads);
+        cfg.dynamicSmemBytes = persist_smem(c, 0, false);
+        const PArgs A = persist_args(c, 0, pos, sync_level);
+        const cudaError_t ep = cudaLaunchKernelEx(&cfg, k_gather_persist<0, false, false>, A);
+        c->launches++;
+        return ep != cudaSuccess ? ep : cudaGetLastError();
+    }
     const cudaError_t e =
         c->tile_nsplit > 1
             ? cudaLaunchKernelEx(&cfg, k_density_tile<true>, (const TileDesc *)c->d_tiles, (const int *)c->d_cell_start, pos,
@@ -1375,6 +1805,22 @@ cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, bool virial, KickArgs kk, int sync_level,
                                     cudaStream_t st)
 {
+    if (use_persist(c)) {
+        PArgs A = persist_args(c, 1, c->d_xs, sync_level);
+        A.force = force;
+        A.kk = kk;
+        const int g = persist_grid(c);
+        const size_t sm = persist_smem(c, 1, virial);
+        if (virial) {
+            if (kk.vel) k_gather_persist<1, true, true><<<g, kPThreads, sm, st>>>(A);
+            else k_gather_persist<1, true, false><<<g, kPThreads, sm, st>>>(A);
+        } else {
+            if (kk.vel) k_gather_persist<1, false, true><<<g, kPThreads, sm, st>>>(A);
+            else k_gather_persist<1, false, false><<<g, kPThreads, sm, st>>>(A);
+        }
+        c->launches++;
+        return cudaGetLastError();
+    }
     const uint2 *nl = reinterpret_cast<const uint2 *>(c->d_nlist);
     const size_t sm = gather_smem(c);
     const int g = c->n_tiles * c->tile_nsplit, b = c->tile_threads;
@@ -1396,7 +1842,7 @@ TileSums tbsma_tile_sums(const tbsma_ctx *c, double *e_rep, double *ekin, double
     TileSums ts;
     ts.cta_sums = c->d_cta_sums;
     ts.tile_first = c->d_tile_first;
-    ts.nsplit = c->tile_nsplit;
+    ts.nsplit = use_persist(c) ? c->p_S : c->tile_nsplit;
     ts.e_rep = e_rep; ts.ekin = ekin; ts.w_rep = w_rep;
     return ts;
 }
@@ -1428,7 +1874,7 @@ cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsig
                                                                  c->d_nn, c->d_hbase, c->d_tileof, c->d_inv, c->img_cap,
                                                                  c->d_atom_rep, c->d_cur,
                                                                  (size_t)(c->kmax / 4) * c->n_pad, d_out2, (int)c->n, c->n_pad,
-                                                                 c->pc.rc2);
+                                                                 c->pc.rc2, c->kmax / 4);
     c->launches++;
     return cudaGetLastError();
 }
