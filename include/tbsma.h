@@ -275,6 +275,57 @@ int tbsma_get_thermostat(tbsma_ctx *ctx, double *h_xi, double *h_eta);
  * at the restart, i.e. continues with another fp32 summation order: same physics, not the same bits.) */
 int tbsma_set_thermostat_state(tbsma_ctx *ctx, const double *h_xi, const double *h_eta);
 
+/* The paper's elongation protocol, beyond the one pulled slab and the constant temperature of tbsma_md_step.
+ * All pointers are DEVICE memory owned by the caller and are read at every step until changed; NULL switches a part off.
+ *   d_slab1_disp0 / d_slab1_rate (n_replicas doubles each): the OTHER gripping slab (flag 1) moves as well, "the
+ *       gripping atoms on the left and right sides of the wire are ... displaced ... in the [-100] and [100] directions"
+ *       (P:71): its atoms are PLACED at zref + D1_r, D1_r = disp0_1[r] + rate_1[r] * k, exactly as the flag-2 slab is at
+ *       zref + disp0[r] + rate[r] * k (tbsma_md_run; k = steps of the run done, the current one included).  Under
+ *       tbsma_md_step k = 1 and rates are NULL, i.e. the caller supplies the total displacements.
+ *   stepwise_period P > 0: both slabs move in strokes, "periodically displaced by 0.05 A ... between 20 ps of MD"
+ *       (P:71): k is replaced by P * floor(k / P) (paper: P = 10 000 steps of 2 fs, rate * P = +-0.05 A).  0 = every step.
+ *   d_T_rate (n_replicas floats, K per step): the target temperature of replica r during step s of a run starting at
+ *       step0 is T[r] + T_rate[r] * (s - step0), clamped at 0 ("(2) 400 ps of MD, ramping the temperature from 0.01 K
+ *       to the target value"); applies to the Langevin noise and to the Nose-Hoover target alike.
+ * NULL protocol = all off (the default). */
+typedef struct {
+    const double *d_slab1_disp0;
+    const double *d_slab1_rate;
+    int64_t stepwise_period;
+    const float *d_T_rate;
+} tbsma_protocol;
+int tbsma_set_protocol(tbsma_ctx *ctx, const tbsma_protocol *protocol);
+
+/* Observables of the tensile test as a series recorded ON THE DEVICE inside tbsma_md_run: after
+ * every step s with (s + 1) % every == 0 one record of 4 doubles is appended for every replica r at
+ * d_series[(r * capacity + d_count[r]) * 4 ...]:
+ *     [0] s   [1] strain (Eq.4) = (D2_r - D1_r) / d_L0[r], the displacements of the two slabs at that step
+ *     [2] sigma_zz = -(W_zz + K_zz) / d_volume[r] in eV/A^3 (Eq.5 as read in D:A11; z is the wire axis, tension positive;
+ *         V is the caller's constant "hard-sphere" volume)
+ *     [3] the largest gap (A) between consecutive z coordinates of the replica's atoms (exact when wider than 1/2048 of
+ *         the replica's box along z)
+ * and d_count[r] is incremented (the caller zeroes it; recording stops silently at `capacity`).  d_rupture_step[r]
+ * (nullable; the caller sets -1) receives the first recorded s whose gap exceeds r_cut: no interaction crosses the gap
+ * any more, the wire has parted ("until rupture").  While a series is on, every step evaluates the virial.
+ * All pointers are device memory owned by the caller.  NULL series (or every = 0) switches recording off. */
+typedef struct {
+    int32_t every, capacity;
+    double *d_series;
+    int32_t *d_count;
+    int64_t *d_rupture_step;
+    const double *d_volume;
+    const double *d_L0;
+} tbsma_series;
+int tbsma_set_series(tbsma_ctx *ctx, const tbsma_series *series);
+
+/* Stress-strain heat map over all replicas (Fig.4): d_hist[iy * nx + ix] += number of records (k < d_count[r]) of
+ * the series whose column col_x (0..3) falls into cell ix of [x_lo, x_hi) cut into nx equal cells and column col_y into
+ * cell iy of [y_lo, y_hi) cut into ny; records outside are not counted.  d_hist: nx * ny uint64, accumulated into (the
+ * caller zeroes it).  Cell of a value v: floor((v - lo) / (hi - lo) * n) in double. */
+int tbsma_series_histogram(tbsma_ctx *ctx, const double *d_series, const int32_t *d_count, int32_t capacity,
+                           int32_t col_x, int32_t col_y, double x_lo, double x_hi, int32_t nx, double y_lo, double y_hi,
+                           int32_t ny, uint64_t *d_hist, void *stream);
+
 /* Replicas built together (all of them, by tbsma_build_neighbors) that share a temperature would all need their
  * next list at nearly the same step, and again one period later.  When enabled (default 1, more than one replica)
  * replica r rebuilds for the first time as soon as an atom has moved f_r skin/2, f_r = 0.3 + 0.7 frac(0.618 r), and

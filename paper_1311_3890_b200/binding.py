@@ -21,6 +21,7 @@ EXPORTS = [
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_kinetic_tensor", "tbsma_stress", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
     "tbsma_get_variant", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_thermostat_state", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin", "tbsma_set_tile_split", "tbsma_set_gather",
+    "tbsma_set_protocol", "tbsma_set_series", "tbsma_series_histogram",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
 
@@ -33,6 +34,16 @@ class Params(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_steps", C.c_uint64), ("n_replica_builds", C.c_uint64), ("n_build_passes", C.c_uint64),
                 ("max_neighbors_seen", C.c_int32), ("n_candidate_builds", C.c_int32)]
+
+
+class Protocol(C.Structure):
+    _fields_ = [("d_slab1_disp0", C.c_void_p), ("d_slab1_rate", C.c_void_p), ("stepwise_period", C.c_int64),
+                ("d_T_rate", C.c_void_p)]
+
+
+class Series(C.Structure):
+    _fields_ = [("every", C.c_int32), ("capacity", C.c_int32), ("d_series", C.c_void_p), ("d_count", C.c_void_p),
+                ("d_rupture_step", C.c_void_p), ("d_volume", C.c_void_p), ("d_L0", C.c_void_p)]
 
 
 def au_params():
@@ -88,6 +99,9 @@ def lib():
         L.tbsma_set_outer_skin.argtypes = [vp, dbl]
         L.tbsma_set_tile_split.argtypes = [vp, i32]
         L.tbsma_set_gather.argtypes = [vp, i32]
+        L.tbsma_set_protocol.argtypes = [vp, C.POINTER(Protocol)]
+        L.tbsma_set_series.argtypes = [vp, C.POINTER(Series)]
+        L.tbsma_series_histogram.argtypes = [vp, vp, vp, i32, i32, i32, dbl, dbl, i32, dbl, dbl, i32, vp, vp]
         L.tbsma_set_timing.argtypes = [vp, i32]
         L.tbsma_get_timing.argtypes = [vp, C.POINTER(dbl), C.POINTER(i64)]
         L.tbsma_launch_count.argtypes = [vp]
@@ -247,6 +261,28 @@ class Context:
 
     def set_gather(self, mode):
         _check(lib().tbsma_set_gather(self._h, int(mode)), "tbsma_set_gather")
+
+    def set_protocol(self, slab1_disp0=None, slab1_rate=None, stepwise_period=0, T_rate=None):
+        """tbsma_set_protocol; device tensors (kept alive by the caller) or None; all None / 0 switches it off"""
+        def ptr(t):
+            return None if t is None else t.data_ptr()
+        p = Protocol(ptr(slab1_disp0), ptr(slab1_rate), int(stepwise_period), ptr(T_rate))
+        _check(lib().tbsma_set_protocol(self._h, C.byref(p)), "tbsma_set_protocol")
+
+    def set_series(self, every=0, capacity=0, series=None, count=None, rupture_step=None, volume=None, L0=None):
+        """tbsma_set_series; device tensors (kept alive by the caller); every = 0 switches recording off"""
+        def ptr(t):
+            return None if t is None else t.data_ptr()
+        if not every:
+            _check(lib().tbsma_set_series(self._h, None), "tbsma_set_series")
+            return
+        s = Series(int(every), int(capacity), ptr(series), ptr(count), ptr(rupture_step), ptr(volume), ptr(L0))
+        _check(lib().tbsma_set_series(self._h, C.byref(s)), "tbsma_set_series")
+
+    def series_histogram(self, series, count, capacity, col_x, col_y, x_lo, x_hi, nx, y_lo, y_hi, ny, hist, stream=None):
+        _check(lib().tbsma_series_histogram(self._h, _dp(series), _dp(count), int(capacity), int(col_x), int(col_y),
+                                            float(x_lo), float(x_hi), int(nx), float(y_lo), float(y_hi), int(ny),
+                                            _dp(hist), _stream(stream)), "tbsma_series_histogram")
 
     def set_thermostat(self, kind, tau_fs=0.0):
         _check(lib().tbsma_set_thermostat(self._h, int(kind), float(tau_fs)), "tbsma_set_thermostat")

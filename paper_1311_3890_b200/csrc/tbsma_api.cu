@@ -44,6 +44,8 @@ void free_system(tbsma_ctx *c)
     cudaFree(c->d_tiles); cudaFree(c->d_maxpop); cudaFree(c->d_hbase); cudaFree(c->d_tileof); cudaFree(c->d_img); cudaFree(c->d_inv);
     c->d_tileof = nullptr; c->d_img = nullptr; c->d_inv = nullptr;
     cudaFree(c->d_cta_sums); c->d_cta_sums = nullptr; c->have_sums = 0;
+    cudaFree(c->d_series_w); c->d_series_w = nullptr;
+    memset(&c->series, 0, sizeof(c->series));
     cudaFree(c->d_newslot); cudaFree(c->d_oldof);
     cudaFree(c->d_nn_tmp); cudaFree(c->d_tmp_pos);
     cudaFree(c->d_tile_first); cudaFree(c->d_work);
@@ -201,6 +203,12 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
     a.T = T; a.seed = seed; a.disp0 = disp0; a.rate = rate;
     a.want_outer = c->active_variant == 2 ? c->d_want_outer : nullptr;
     a.stagger = c->d_stagger;
+    a.disp0_1 = c->proto.d_slab1_disp0; a.rate_1 = c->proto.d_slab1_rate;
+    a.period = (long long)c->proto.stepwise_period;
+    a.T_rate = c->proto.d_T_rate;
+    // a series of the tensile observables needs the virial of every step it records
+    const bool series = advance && c->series.every > 0 && c->series.d_series;
+    if (series && !w_rep) w_rep = c->d_series_w;
     a.e_rep = e_rep; a.w_rep = w_rep; a.ekin = ekin;
     KickArgs kk;
     kk.vel = vel; kk.kick = a.kick; kk.ke_scale = (float)(0.5 * c->prm.mass_amu / TBSMA_ACC); kk.ekin = ekin;
@@ -285,6 +293,7 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
         if (forked && !joined) CK(cudaStreamWaitEvent(st, c->ev_join, 0));
         CK(tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, st,
                                     tiles ? tbsma_tile_sums(c, e_rep, ekin, w_rep) : TileSums()));
+        if (series) CK(tbsma_launch_series_record(c, pos, vel, w_rep, a, st));
         if (ev) CK(cudaEventRecord(ev[5], st));
     }
     return TBSMA_OK;
@@ -490,6 +499,44 @@ int tbsma_set_thermostat_state(tbsma_ctx *c, const double *h_xi, const double *h
     const cudaError_t e = cudaMemcpy(c->d_nh, h, sizeof(double) * 2 * (size_t)c->R, cudaMemcpyHostToDevice);
     free(h);
     CK(e);
+    return TBSMA_OK;
+}
+
+int tbsma_set_protocol(tbsma_ctx *c, const tbsma_protocol *p)
+{
+    if (!c || (p && p->stepwise_period < 0)) return TBSMA_EINVAL;
+    c->epoch++;
+    if (p) c->proto = *p;
+    else memset(&c->proto, 0, sizeof(c->proto));
+    return TBSMA_OK;
+}
+
+int tbsma_set_series(tbsma_ctx *c, const tbsma_series *s)
+{
+    if (!c) return TBSMA_EINVAL;
+    if (s && s->every > 0 && (s->capacity < 1 || !s->d_series || !s->d_count || !s->d_volume || !s->d_L0)) return TBSMA_EINVAL;
+    if (s && s->every < 0) return TBSMA_EINVAL;
+    c->epoch++;
+    if (s && s->every > 0) {
+        if (!c->d_geom) return TBSMA_ESTATE;
+        if (!c->d_series_w) CK(dalloc(&c->d_series_w, (size_t)6 * c->R));
+        c->series = *s;
+    } else {
+        memset(&c->series, 0, sizeof(c->series));
+    }
+    return TBSMA_OK;
+}
+
+int tbsma_series_histogram(tbsma_ctx *c, const double *d_series, const int32_t *d_count, int32_t capacity, int32_t col_x,
+                           int32_t col_y, double x_lo, double x_hi, int32_t nx, double y_lo, double y_hi, int32_t ny,
+                           uint64_t *d_hist, void *stream)
+{
+    if (!c || !d_series || !d_count || !d_hist || capacity < 1 || col_x < 0 || col_x > 3 || col_y < 0 || col_y > 3 ||
+        nx < 1 || ny < 1 || !(x_hi > x_lo) || !(y_hi > y_lo))
+        return TBSMA_EINVAL;
+    if (!c->d_geom) return TBSMA_ESTATE;
+    CK(tbsma_launch_series_histogram(c, d_series, d_count, capacity, col_x, col_y, x_lo, x_hi, nx, y_lo, y_hi, ny,
+                                     (unsigned long long *)d_hist, (cudaStream_t)stream));
     return TBSMA_OK;
 }
 

@@ -70,15 +70,23 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
         } else if (a.thermostat) {
             const unsigned trel = (unsigned)(tag[i] - geom[r].atom_begin);
             const float3 g = gauss3(a.seed[r], trel, step);
-            const float sg = a.c2 * a.sigma_scale * sqrtf(a.T[r]);
+            const float Tr = a.T_rate ? (float)((double)a.T[r] + (double)a.T_rate[r] * (double)off) : a.T[r];
+            const float sg = a.c2 * a.sigma_scale * sqrtf(fmaxf(Tr, 0.f));
             v.x = __fmaf_rn(a.c1, v.x, sg * g.x); v.y = __fmaf_rn(a.c1, v.y, sg * g.y); v.z = __fmaf_rn(a.c1, v.z, sg * g.z);
         }
         p.x = __fmaf_rn(a.half_dt, v.x, p.x); p.y = __fmaf_rn(a.half_dt, v.y, p.y); p.z = __fmaf_rn(a.half_dt, v.z, p.z);
     } else {       // rigid grip atom (D:A12): v = 0; a pulled atom is placed, never incremented (D:A10)
         v.x = v.y = v.z = 0.f;
+        // steps of slab motion since the run began: every step, or in strokes of `period` steps
+        unsigned long long nst = off + 1ull;
+        if (a.period > 0) nst = nst / (unsigned long long)a.period * (unsigned long long)a.period;
         if (flag == 2) {
             double D = a.disp0 ? a.disp0[r] : 0.0;
-            if (a.rate) D += a.rate[r] * (double)(off + 1ull);
+            if (a.rate) D += a.rate[r] * (double)nst;
+            p.z = (float)((double)v.w + D);
+        } else if (a.disp0_1 || a.rate_1) {      // the other end (both ends move); without a schedule it stays fixed
+            double D = a.disp0_1 ? a.disp0_1[r] : 0.0;
+            if (a.rate_1) D += a.rate_1[r] * (double)nst;
             p.z = (float)((double)v.w + D);
         }
     }
@@ -192,6 +200,7 @@ k_nh_kinetic(const float4 *__restrict__ pos, const float4 *__restrict__ vel, con
 // shuffle tree), then lane 0 advances xi and eta
 __global__ void __launch_bounds__(256)
 k_nh_update(const double *__restrict__ kpart, const int *__restrict__ blk_first, const float *__restrict__ T,
+            const float *__restrict__ T_rate, const unsigned long long *__restrict__ counters,
             double *__restrict__ nh, float *__restrict__ scale, double dt, double tau, int R)
 {
     const int r = (int)blockIdx.x * 8 + (int)(threadIdx.x >> 5), lane = threadIdx.x & 31;
@@ -204,7 +213,9 @@ k_nh_update(const double *__restrict__ kpart, const int *__restrict__ blk_first,
     }
     if (lane != 0) return;
     const double g = 3.0 * nd;
-    const double gkt = g * TBSMA_KB * (double)T[r];
+    double Tr = (double)T[r];
+    if (T_rate) Tr = fmax(Tr + (double)T_rate[r] * (double)counters[0], 0.0);      // temperature ramp
+    const double gkt = g * TBSMA_KB * Tr;
     double s = 1.0;
     if (gkt > 0.0 && tau > 0.0) {
         const double Q = gkt * tau * tau;
@@ -264,7 +275,124 @@ __global__ void k_stress(const double *__restrict__ w_rep, const double *__restr
     sigma[q] = -(w_rep[q] + (k_rep ? k_rep[q] : 0.0)) / volume[q / 6];
 }
 
+// ---- the tensile test as a device-side series ------------------------------------
+// One CTA per replica, after the last kernel of a step of tbsma_md_run.  When a record is due (the number of the step
+// just done, plus one, is a multiple of `every`) it appends
+//   step | strain (Eq.4: (L - L0) / L0, L - L0 = D_2 - D_1 of the two slabs) | sigma_zz = -(W_zz + K_zz) / V (Eq.5 as read
+//   in D:A11, z = the wire axis) | largest gap between consecutive z coordinates of the replica's atoms
+// and notes the first step whose gap exceeds r_cut: the wire has parted ("until rupture").  K_zz is added in a fixed
+// order (thread-strided partial sums, then a tree).  The gap comes from 2048 bins along z holding the least and the
+// greatest z that fell into them: exact whenever it is wider than a bin.
+#define TBSMA_SERIES_BINS 2048
+__device__ __forceinline__ int ord_of(float f) { const int k = __float_as_int(f); return k >= 0 ? k : k ^ 0x7fffffff; }
+__device__ __forceinline__ float f_of(int k) { return __int_as_float(k >= 0 ? k : k ^ 0x7fffffff); }
+
+__global__ void __launch_bounds__(256)
+k_series_record(const float4 *__restrict__ pos, const float4 *__restrict__ vel, const RepGeom *__restrict__ geom,
+                const double *__restrict__ w_rep, const unsigned long long *__restrict__ counters, tbsma_series S,
+                StepArgs a, double m_over_c, float r_cut)
+{
+    __shared__ int s_mn[TBSMA_SERIES_BINS], s_mx[TBSMA_SERIES_BINS];
+    __shared__ double s_red[256];
+    __shared__ float s_gap[256];
+    const unsigned long long nst_done = counters[0];          // steps of this run done, this one included (>= 1)
+    const unsigned long long step = (a.step_on_device ? counters[7] : a.step_base) + nst_done - 1ull;
+    if ((step + 1ull) % (unsigned long long)S.every != 0ull) return;
+    const int r = blockIdx.x, tid = threadIdx.x;
+    const int idx = S.d_count[r];
+    if (idx >= S.capacity) return;
+    const RepGeom *g = geom + r;
+    for (int b = tid; b < TBSMA_SERIES_BINS; b += 256) { s_mn[b] = 0x7fffffff; s_mx[b] = (int)0x80000000; }
+    __syncthreads();
+    const float z0 = g->lo[2], inv_w = g->len[2] > 0.f ? (float)TBSMA_SERIES_BINS / g->len[2] : 0.f;
+    double k = 0.0;
+    for (int i = g->atom_begin + tid; i < g->atom_end; i += 256) {
+        const float4 p = pos[i];
+        if ((__float_as_int(p.w) & 3) == 0) {
+            const double vz = (double)vel[i].z;
+            k += m_over_c * vz * vz;
+        }
+        int b = __float2int_rd((p.z - z0) * inv_w);
+        b = min(max(b, 0), TBSMA_SERIES_BINS - 1);
+        const int o = ord_of(p.z);
+        atomicMin(&s_mn[b], o);
+        atomicMax(&s_mx[b], o);
+    }
+    s_red[tid] = k;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (tid < o) s_red[tid] += s_red[tid + o];
+        __syncthreads();
+    }
+    // largest gap between a bin's least z and the greatest z of the nearest occupied bin below it
+    float gap = 0.f;
+    for (int b = tid; b < TBSMA_SERIES_BINS; b += 256) {
+        if (s_mn[b] == 0x7fffffff) continue;
+        int q = b - 1;
+        while (q >= 0 && s_mn[q] == 0x7fffffff) --q;
+        if (q >= 0) gap = fmaxf(gap, f_of(s_mn[b]) - f_of(s_mx[q]));
+    }
+    s_gap[tid] = gap;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (tid < o) s_gap[tid] = fmaxf(s_gap[tid], s_gap[tid + o]);
+        __syncthreads();
+    }
+    if (tid == 0) {
+        unsigned long long nst = nst_done;
+        if (a.period > 0) nst = nst / (unsigned long long)a.period * (unsigned long long)a.period;
+        double D2 = a.disp0 ? a.disp0[r] : 0.0, D1 = a.disp0_1 ? a.disp0_1[r] : 0.0;
+        if (a.rate) D2 += a.rate[r] * (double)nst;
+        if (a.rate_1) D1 += a.rate_1[r] * (double)nst;
+        double *rec = S.d_series + 4 * ((size_t)r * S.capacity + idx);
+        rec[0] = (double)step;
+        rec[1] = (D2 - D1) / S.d_L0[r];
+        rec[2] = -(w_rep[6 * (size_t)r + 2] + s_red[0]) / S.d_volume[r];
+        rec[3] = (double)s_gap[0];
+        S.d_count[r] = idx + 1;
+        if (S.d_rupture_step && S.d_rupture_step[r] < 0 && s_gap[0] > r_cut) S.d_rupture_step[r] = (long long)step;
+    }
+}
+
+// stress-strain "heat map" over the records of all replicas (Fig.4): counts per cell of an nx x ny grid over
+// [x_lo, x_hi) x [y_lo, y_hi); records outside are not counted
+__global__ void k_series_histogram(const double *__restrict__ series, const int *__restrict__ count, int capacity, int R,
+                                   int col_x, int col_y, double x_lo, double x_hi, int nx, double y_lo, double y_hi, int ny,
+                                   unsigned long long *__restrict__ hist)
+{
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= (long long)R * capacity) return;
+    const int r = (int)(q / capacity), k = (int)(q % capacity);
+    if (k >= count[r]) return;
+    const double x = series[4 * q + col_x], y = series[4 * q + col_y];
+    if (!(x >= x_lo && x < x_hi && y >= y_lo && y < y_hi)) return;
+    int ix = (int)floor((x - x_lo) / (x_hi - x_lo) * (double)nx), iy = (int)floor((y - y_lo) / (y_hi - y_lo) * (double)ny);
+    ix = min(ix, nx - 1); iy = min(iy, ny - 1);
+    atomicAdd(hist + (size_t)iy * nx + ix, 1ull);
+}
+
 }  // namespace
+
+cudaError_t tbsma_launch_series_record(tbsma_ctx *c, const float4 *pos, const float4 *vel, const double *w_rep,
+                                       const StepArgs &a, cudaStream_t st)
+{
+    k_series_record<<<c->R, 256, 0, st>>>(pos, vel, c->d_geom, w_rep, c->d_counters, c->series, a,
+                                          c->prm.mass_amu / TBSMA_ACC, (float)c->r_cut);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t tbsma_launch_series_histogram(tbsma_ctx *c, const double *series, const int32_t *count, int capacity, int col_x,
+                                          int col_y, double x_lo, double x_hi, int nx, double y_lo, double y_hi, int ny,
+                                          unsigned long long *hist, cudaStream_t st)
+{
+    const long long total = (long long)c->R * capacity;
+    if (total <= 0) return cudaSuccess;
+    k_series_histogram<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(series, count, capacity, c->R, col_x, col_y, x_lo, x_hi,
+                                                                        nx, y_lo, y_hi, ny, hist);
+    c->launches++;
+    return cudaGetLastError();
+}
 
 cudaError_t tbsma_launch_nose_hoover(tbsma_ctx *c, const float4 *pos, const float4 *vel, const float4 *force,
                                      const StepArgs &a, double dt, cudaStream_t st)
@@ -272,7 +400,8 @@ cudaError_t tbsma_launch_nose_hoover(tbsma_ctx *c, const float4 *pos, const floa
     if (c->n_blk == 0) return cudaSuccess;
     k_nh_kinetic<<<c->n_blk, 256, 0, st>>>(pos, vel, force, c->d_blk_rep, c->d_blk_first, c->d_geom, c->d_kmid, a.kick,
                                            0.5 * c->prm.mass_amu / TBSMA_ACC);
-    k_nh_update<<<(c->R + 7) / 8, 256, 0, st>>>(c->d_kmid, c->d_blk_first, a.T, c->d_nh, c->d_nh_scale, dt, c->nh_tau, c->R);
+    k_nh_update<<<(c->R + 7) / 8, 256, 0, st>>>(c->d_kmid, c->d_blk_first, a.T, a.T_rate, c->d_counters, c->d_nh,
+                                                c->d_nh_scale, dt, c->nh_tau, c->R);
     c->launches += 2;
     return cudaGetLastError();
 }

@@ -194,6 +194,11 @@ struct tbsma_ctx {
     int32_t *d_blk_first;      // R + 1: first run of every replica
     int n_blk;
     float *d_nh_scale;         // R
+    // the paper's elongation protocol (tbsma_set_protocol) and its observables as a device-side series
+    // (tbsma_set_series)
+    tbsma_protocol proto;
+    tbsma_series series;       // every == 0: off
+    double *d_series_w;        // R x 6: virial of the step when the caller of tbsma_md_run passes none
     int cells_built, list_built;
     int epoch;                 // bumped by every call after which a captured step would hold stale arguments
     int64_t launches;
@@ -343,6 +348,10 @@ struct StepArgs {
     const int *want_outer;   // nullable (tile variant): replicas whose next rebuild redoes cells + candidates
     const float *stagger;    // per replica factor on skin_half2
     const float *nh_scale;   // nullable: Nose-Hoover velocity scale of this step per replica (replaces the O part)
+    const double *disp0_1;   // nullable: the flag-1 slab (both ends are displaced), as disp0 / rate for the flag-2 slab
+    const double *rate_1;    // nullable
+    long long period;        // > 0: the slabs advance every `period` steps by period x rate ("periodically displaced")
+    const float *T_rate;     // nullable: target temperature of replica r during step s is T[r] + T_rate[r] (s - step0)
     double *e_rep, *w_rep, *ekin;  // zeroed here for the force pass; nullable
 };
 cudaError_t tbsma_launch_integrate_pre(tbsma_ctx *c, float4 *pos, float4 *vel, const float4 *force,
@@ -352,6 +361,12 @@ cudaError_t tbsma_launch_set_stagger(tbsma_ctx *c, cudaStream_t st);
 cudaError_t tbsma_launch_set_step_base(tbsma_ctx *c, unsigned long long step0, cudaStream_t st);
 cudaError_t tbsma_launch_nose_hoover(tbsma_ctx *c, const float4 *pos, const float4 *vel, const float4 *force,
                                      const StepArgs &a, double dt, cudaStream_t st);
+// after the last kernel of a step of tbsma_md_run: appends a record to the series of every replica when one is due
+cudaError_t tbsma_launch_series_record(tbsma_ctx *c, const float4 *pos, const float4 *vel, const double *w_rep,
+                                       const StepArgs &a, cudaStream_t st);
+cudaError_t tbsma_launch_series_histogram(tbsma_ctx *c, const double *series, const int32_t *count, int capacity, int col_x,
+                                          int col_y, double x_lo, double x_hi, int nx, double y_lo, double y_hi, int ny,
+                                          unsigned long long *hist, cudaStream_t st);
 cudaError_t tbsma_launch_kinetic_tensor(tbsma_ctx *c, const float4 *pos, const float4 *vel, double *k_rep, cudaStream_t st);
 cudaError_t tbsma_launch_stress(tbsma_ctx *c, const double *w_rep, const double *k_rep, const double *volume,
                                 double *sigma, cudaStream_t st);

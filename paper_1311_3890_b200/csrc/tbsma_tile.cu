@@ -773,9 +773,15 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
     for (int ch = next_chunk(&s_next); ch < (SPLIT ? s_end : nchunk); ch = next_chunk(&s_next)) {
         const int i = r.lo + (ch << 5) + lane;
         if (i >= r.hi) continue;
+        // own record, count and the first three rows in one round trip (the rows exist whatever the count: kg >= 3 or the
+        // loads are skipped); a row register is reloaded right after its use
+        const uint2 *row = nl + tbsma_lrow(i, kg);
+        uint2 q0 = make_uint2(0u, 0u), q1 = q0, q2 = q0;
+        if (kg >= 3) { q0 = __ldcs(row); q1 = __ldcs(row + TBSMA_LROW); q2 = __ldcs(row + 2 * TBSMA_LROW); }
         const float4 pi = pos[i];
         const int ng = ((nn[i] & 0xffff) + 3) >> 2;
-        const uint2 *row = nl + tbsma_lrow(i, kg);
+        if (kg < 3) { q0 = ld_row(row, 0, ng, n_pad); q1 = ld_row(row, 1, ng, n_pad); q2 = ld_row(row, 2, ng, n_pad); }
+        if (ng < 3) { q2 = make_uint2(0u, 0u); if (ng < 2) q1 = q2; if (ng < 1) q0 = q2; }
         f32x2 rho2 = pk(0.f, 0.f);
         auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
@@ -783,13 +789,11 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
             rho2 = rho_term2(pi, p0, p1, pc, rho2);
             rho2 = rho_term2(pi, p2, p3, pc, rho2);
         };
-        // three rows in flight, rotated by unrolling (a register move would wait for the newest load)
-        uint2 q0 = ld_row(row, 0, ng, n_pad), q1 = ld_row(row, 1, ng, n_pad), q2 = ld_row(row, 2, ng, n_pad);
         int g = 0;
         for (; g + 3 <= ng; g += 3) {
-            uint2 jj = q0; q0 = ld_row(row, g + 3, ng, n_pad); group(jj);
-            jj = q1; q1 = ld_row(row, g + 4, ng, n_pad); group(jj);
-            jj = q2; q2 = ld_row(row, g + 5, ng, n_pad); group(jj);
+            group(q0); q0 = ld_row(row, g + 3, ng, n_pad);
+            group(q1); q1 = ld_row(row, g + 4, ng, n_pad);
+            group(q2); q2 = ld_row(row, g + 5, ng, n_pad);
         }
         if (g < ng) {
             group(q0);
@@ -926,10 +930,14 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
         const int i = r.lo + (ch << 5) + lane;
         double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         if (i < r.hi) {
+        const uint2 *row = nl + tbsma_lrow(i, kg);
+        uint2 q0 = make_uint2(0u, 0u), q1 = q0, q2 = q0;
+        if (kg >= 3) { q0 = __ldcs(row); q1 = __ldcs(row + TBSMA_LROW); q2 = __ldcs(row + 2 * TBSMA_LROW); }
         const float4 pi = xs[i];
         const int nni = nn[i];
         const int ng = ((nni & 0xffff) + 3) >> 2;
-        const uint2 *row = nl + tbsma_lrow(i, kg);
+        if (kg < 3) { q0 = ld_row(row, 0, ng, n_pad); q1 = ld_row(row, 1, ng, n_pad); q2 = ld_row(row, 2, ng, n_pad); }
+        if (ng < 3) { q2 = make_uint2(0u, 0u); if (ng < 2) q1 = q2; if (ng < 1) q0 = q2; }
         const f32x2 z2 = pk(0.f, 0.f);
         AccT a = {z2, z2, z2, z2, z2, z2, z2, z2, z2, z2};
         auto group = [&](const uint2 jj) {
@@ -938,12 +946,11 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
             force_term2<VIRIAL>(pi, p0, p1, pc, a);
             force_term2<VIRIAL>(pi, p2, p3, pc, a);
         };
-        uint2 q0 = ld_row(row, 0, ng, n_pad), q1 = ld_row(row, 1, ng, n_pad), q2 = ld_row(row, 2, ng, n_pad);
         int g = 0;
         for (; g + 3 <= ng; g += 3) {
-            uint2 jj = q0; q0 = ld_row(row, g + 3, ng, n_pad); group(jj);
-            jj = q1; q1 = ld_row(row, g + 4, ng, n_pad); group(jj);
-            jj = q2; q2 = ld_row(row, g + 5, ng, n_pad); group(jj);
+            group(q0); q0 = ld_row(row, g + 3, ng, n_pad);
+            group(q1); q1 = ld_row(row, g + 4, ng, n_pad);
+            group(q2); q2 = ld_row(row, g + 5, ng, n_pad);
         }
         if (g < ng) {
             group(q0);

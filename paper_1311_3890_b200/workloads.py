@@ -42,6 +42,27 @@ def fcc_wire(diameter, length, a=A_LATTICE):
     return pts
 
 
+def ring_notch(x, a=A_LATTICE, planes=3, per_plane=9):
+    """The paper's "small, ring-shaped notch ... in the center of the NW ... three atoms wide and two atoms deep" (P:71,
+    P:77), reading A18: from each of the `planes` (100) planes nearest the wire's centre the `per_plane` atoms farthest
+    from the axis are removed (ties by azimuth): with 9 that is the two outermost radial shells of a 3.1 nm wire and
+    27 atoms in all, the difference between 8 850 and the 8 823 atoms of Table 2's first row.  Returns the
+    remaining atoms, order kept."""
+    z = x[:, 2]
+    lev_of = np.round((z - z.min()) / (0.5 * a)).astype(np.int64)      # (100) planes are a / 2 apart
+    levels = np.unique(lev_of)
+    zc = 0.5 * (z.min() + z.max())
+    centre = levels[np.argsort(np.abs(z.min() + levels * 0.5 * a - zc), kind="stable")[:planes]]
+    r = np.hypot(x[:, 0], x[:, 1])
+    phi = np.arctan2(x[:, 1], x[:, 0])
+    keep = np.ones(len(x), bool)
+    for lv in centre:
+        idx = np.nonzero(lev_of == lv)[0]
+        order = idx[np.lexsort((phi[idx], -np.round(r[idx], 6)))]
+        keep[order[:per_plane]] = False
+    return x[keep]
+
+
 def fcc_bulk(ncell, a=A_LATTICE):
     """Periodic cubic FCC block of ncell^3 conventional cells in [0, ncell*a)^3, z-major order."""
     basis = np.array([[0, 0, 0], [0.5, 0.5, 0], [0.5, 0, 0.5], [0, 0.5, 0.5]])

@@ -981,3 +981,128 @@ def test_long_run_keeps_a_clean_status_word(B):
     n_dyn = np.array([(w.flags[w.offsets[r]:w.offsets[r + 1]] == 0).sum() for r in range(w.n_replicas)])
     T_kin = 2 * st.ekin.cpu().numpy() / (3 * n_dyn * 8.617333262e-5)
     assert np.all(np.abs(T_kin - 298.0) < 15.0)
+
+
+# ---- the paper's elongation protocol and the device-side series of its observables ----------------
+def _tensile_setup(B, variant, n_rep=3, every=6, n_steps=60, period=7, capacity=16, ramp=True):
+    """n_rep short 3 nm wires (config-3 shape: grips at both ends, 10 K and 298 K), BOTH slabs pulled in strokes of
+    `period` steps, the target temperature ramped, the series recorded every `every` steps"""
+    w = W.config3(n_rep, seed=41, length=60.0)
+    ctx, st = setup(B, w, variant=variant)
+    R = w.n_replicas
+    rate2 = torch.from_numpy(w.slab_rate.copy()).cuda()
+    rate1 = torch.from_numpy(-0.5 * w.slab_rate).cuda()
+    disp1 = torch.from_numpy(np.linspace(-0.01, -0.03, R)).cuda()
+    T_rate = torch.from_numpy(np.linspace(0.05, 0.2, R).astype(np.float32)).cuda() if ramp else None
+    L0 = np.array([w.pos4[w.offsets[r]:w.offsets[r + 1], 2].max() - w.pos4[w.offsets[r]:w.offsets[r + 1], 2].min()
+                   for r in range(R)], dtype=np.float64)
+    vol = np.diff(w.offsets).astype(np.float64) * 4.08 ** 3 / 4
+    dev = dict(series=torch.zeros(R * capacity * 4, dtype=torch.float64, device="cuda"),
+               count=torch.zeros(R, dtype=torch.int32, device="cuda"),
+               rupture=torch.full((R,), -1, dtype=torch.int64, device="cuda"),
+               volume=torch.from_numpy(vol).cuda(), L0=torch.from_numpy(L0).cuda(),
+               rate2=rate2, rate1=rate1, disp1=disp1, T_rate=T_rate)
+    ctx.set_protocol(slab1_disp0=disp1, slab1_rate=rate1, stepwise_period=period, T_rate=T_rate)
+    ctx.set_series(every, capacity, dev["series"], dev["count"], dev["rupture"], dev["volume"], dev["L0"])
+    return w, ctx, st, dev, L0, vol
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_two_sided_stroke_pulling_ramp_and_series_match_oracle(B, variant):
+    """tbsma_set_protocol + tbsma_set_series: trajectory, slab placement, and every record of the series
+    against oracle/protocol.py:TensileMD"""
+    from oracle.protocol import TensileMD
+    every, n_steps, period, cap = 6, 60, 7, 16
+    w, ctx, st, dev, L0, vol = _tensile_setup(B, variant, every=every, n_steps=n_steps, period=period, capacity=cap)
+    R = w.n_replicas
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, dev["rate2"], 0,
+                   st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    zref = w.vel4[:, 3].astype(np.float64)
+    md = oracle.MD(w.x64(), w.v64(), w.flags, w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, cells=True, zref=zref)
+    t = TensileMD(md, w.dt, w.T.astype(np.float64), w.gamma, w.seed, 0, 0.0, w.slab_rate, dev["disp1"].cpu().numpy(),
+                  -0.5 * w.slab_rate, period=period, T_rate=dev["T_rate"].cpu().numpy().astype(np.float64), every=every,
+                  volume=vol, L0=L0)
+    for _ in range(n_steps):
+        t.step()
+    xg = st.untag(st.pos)
+    assert traj_rms(xg[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+    for fl in (1, 2):            # both slabs placed to the bit (D:A10)
+        assert np.array_equal(xg[w.flags == fl, 2], md.x[w.flags == fl, 2].astype(np.float32))
+    assert np.abs(xg[w.flags == 1, 2].astype(np.float64) - zref[w.flags == 1]).max() > 0.009     # the flag-1 slab moved
+    count = dev["count"].cpu().numpy()
+    assert np.all(count == n_steps // every)
+    ser = dev["series"].cpu().numpy().reshape(R, cap, 4)
+    for r in range(R):
+        ref = np.array(t.series[r])
+        got = ser[r, :count[r]]
+        assert np.array_equal(got[:, 0], ref[:, 0])                                  # step numbers
+        assert np.allclose(got[:, 1], ref[:, 1], rtol=1e-12, atol=1e-15)              # strain (Eq.4)
+        assert np.allclose(got[:, 2], ref[:, 2], rtol=2e-4, atol=2e-5 * np.abs(ref[:, 2]).max())   # sigma_zz (Eq.5)
+        assert np.allclose(got[:, 3], ref[:, 3], atol=2e-5)                           # largest z gap
+    assert np.all(dev["rupture"].cpu().numpy() == -1)
+    # the heat map over all replicas (P:147): exact counts
+    from oracle.protocol import heat_map
+    hist = torch.zeros(8 * 6, dtype=torch.int64, device="cuda")
+    lo_y, hi_y = float(ser[..., 2].min()) - 1e-3, float(ser[..., 2].max()) + 1e-3
+    ctx.series_histogram(dev["series"], dev["count"], cap, 1, 2, -0.001, 0.002, 8, lo_y, hi_y, 6, hist)
+    torch.cuda.synchronize()
+    xs = np.concatenate([ser[r, :count[r], 1] for r in range(R)])
+    ys = np.concatenate([ser[r, :count[r], 2] for r in range(R)])
+    assert np.array_equal(hist.cpu().numpy().reshape(6, 8).astype(np.uint64), heat_map(xs, ys, -0.001, 0.002, 8, lo_y, hi_y, 6))
+    assert hist.sum().item() > 0
+    # switched off again: no further records, the flag-1 slab stays where it is
+    ctx.set_series(0)
+    ctx.set_protocol()
+    z1 = st.untag(st.pos)[w.flags == 1, 2].copy()
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, n_steps, 12, None, None, 0,
+                   st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert np.array_equal(dev["count"].cpu().numpy(), count)
+    assert np.array_equal(st.untag(st.pos)[w.flags == 1, 2], z1)
+
+
+def test_series_detects_a_parted_wire(B):
+    """rupture: a wire whose upper half has been moved 8 A up the axis has a gap wider than r_cut: the first
+    record reports it, and the recorded gap is the oracle's"""
+    from oracle.protocol import largest_gap
+    w = W.config3(2, seed=43, length=60.0)
+    z = w.pos4[:, 2]
+    cut = (z > 1.0) & (np.arange(w.n_atoms) >= w.offsets[1])          # second replica only
+    w.pos4[cut, 2] += 8.0
+    w.vel4[cut, 3] += 8.0
+    w.box_hi[1, 2] += 8.0
+    ctx, st = setup(B, w)
+    R, cap = 2, 4
+    dev = dict(series=torch.zeros(R * cap * 4, dtype=torch.float64, device="cuda"),
+               count=torch.zeros(R, dtype=torch.int32, device="cuda"),
+               rupture=torch.full((R,), -1, dtype=torch.int64, device="cuda"),
+               volume=torch.ones(R, dtype=torch.float64, device="cuda"), L0=torch.full((R,), 60.0, dtype=torch.float64, device="cuda"))
+    ctx.set_series(5, cap, dev["series"], dev["count"], dev["rupture"], dev["volume"], dev["L0"])
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 100, 20, None, st.slab_rate, 0,
+                   st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    assert np.array_equal(dev["count"].cpu().numpy(), [4, 4])
+    rup = dev["rupture"].cpu().numpy()
+    assert rup[0] == -1 and rup[1] == 104                               # first record of a run starting at step 100
+    ser = dev["series"].cpu().numpy().reshape(R, cap, 4)
+    assert np.array_equal(ser[0, :, 0], [104, 109, 114, 119])
+    x = st.untag(st.pos)
+    assert ser[1, :, 3].min() > w.r_cut and ser[0, :, 3].max() < 3.0
+    assert abs(ser[1, -1, 3] - largest_gap(x[w.offsets[1]:, 2])) < 1e-5      # the last record is that of the last step
+    with torch.cuda.stream(stream):                                          # capacity reached: recording stops
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 120, 10, None, st.slab_rate, 0,
+                   st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert np.array_equal(dev["count"].cpu().numpy(), [4, 4]) and ctx.status() == 0

@@ -536,3 +536,108 @@ def test_nose_hoover_conserved_quantity_reduction_to_verlet_and_temperature():
     for s in range(20):
         nh2.step(w.dt)
     assert np.abs(nh2.x - x).max() < 1e-9
+
+
+# ---- the paper's elongation protocol and the series of its observables (oracle/protocol.py) --------------------------
+def test_slab_schedule_matches_the_papers_numbers():
+    """0.05 A per side every 20 ps (10 000 steps of 2 fs): after 25 000 steps each side has made two strokes, and
+    the strain rate of a 20.4 nm wire is 0.1 A / 20 ps / 204 A = 2.45e7 /s"""
+    from oracle.protocol import slab_displacement
+    P, stroke = 10_000, 0.05
+    k = np.array([0, 1, 9_999, 10_000, 19_999, 20_000, 25_000])
+    D2 = slab_displacement(k, 0.0, +stroke / P, P)
+    D1 = slab_displacement(k, 0.0, -stroke / P, P)
+    assert np.allclose(D2, [0, 0, 0, 0.05, 0.05, 0.10, 0.10], atol=1e-15)
+    assert np.allclose(D1, -D2, atol=0)
+    rate = (D2[5] - D1[5]) / 204.0 / (20_000 * 2e-15)
+    assert abs(rate - 2.45e7) < 0.01e7
+    # every step: a straight line through disp0
+    assert np.allclose(slab_displacement(k, 0.3, 2e-5), 0.3 + 2e-5 * k, atol=1e-15)
+    # a stroke never runs ahead of the continuous schedule and lags it by less than one stroke
+    kk = np.arange(0, 35_000, 777)
+    lag = slab_displacement(kk, 0.0, stroke / P) - slab_displacement(kk, 0.0, stroke / P, P)
+    assert np.all(lag >= 0) and np.all(lag < stroke)
+
+
+def test_temperature_ramp_and_largest_gap():
+    from oracle.protocol import temperature, largest_gap
+    # P:73: 0.01 K -> 298 K over 400 ps = 200 000 steps
+    rate = (298.0 - 0.01) / 200_000
+    assert abs(temperature(0.01, rate, 200_000) - 298.0) < 1e-9 and temperature(0.01, rate, 0) == 0.01
+    assert temperature(1.0, -1.0, 5) == 0.0                      # clamped
+    # largest gap: brute force (for every value the nearest one above it) on shuffled data
+    rng = np.random.default_rng(3)
+    z = np.concatenate([rng.uniform(0, 10, 50), rng.uniform(17.5, 30, 70)])
+    rng.shuffle(z)
+    up = [min((b - a for b in z if b > a), default=0.0) for a in z]
+    assert abs(largest_gap(z) - max(up)) < 1e-15 and largest_gap(z) >= 7.5
+    assert largest_gap(np.arange(5.0)[::-1] * 2.04) == pytest.approx(2.04)
+
+
+def test_heat_map_against_numpy_histogram2d():
+    from oracle.protocol import heat_map
+    rng = np.random.default_rng(5)
+    x, y = rng.uniform(-0.02, 0.25, 4000), rng.normal(2.0, 2.0, 4000)
+    h = heat_map(x, y, 0.0, 0.2, 40, -1.0, 6.0, 35)
+    ref, _, _ = np.histogram2d(y, x, bins=[35, 40], range=[[-1.0, 6.0], [0.0, 0.2]])
+    inside = (x >= 0.0) & (x < 0.2) & (y >= -1.0) & (y < 6.0)
+    assert h.sum() == inside.sum()
+    assert np.abs(h.astype(np.int64) - ref.astype(np.int64)).sum() <= 2      # numpy closes the last cell, float edges
+    one = heat_map([0.1], [3.0], 0.0, 0.2, 4, 0.0, 4.0, 4)
+    assert one[3, 2] == 1 and one.sum() == 1
+
+
+def test_ring_notch_removes_the_papers_27_atoms():
+    """Table 2's first row has 8 823 atoms = 8 850 - 27; "three atoms wide and two atoms deep" (reading A18)"""
+    x = W.fcc_wire(31.0, 204.0)
+    y = W.ring_notch(x)
+    assert len(x) == 8850 and len(y) == 8823
+    gone = np.array(sorted(set(map(tuple, np.round(x, 6))) - set(map(tuple, np.round(y, 6)))))
+    zs, cnt = np.unique(gone[:, 2], return_counts=True)
+    assert len(zs) == 3 and np.all(cnt == 9) and np.all(np.abs(zs) < 1.6 * 2.04)        # three central planes, nine each
+    r_gone = np.hypot(gone[:, 0], gone[:, 1])
+    for zv in zs:                                   # nothing farther from the axis is left in those planes
+        left = y[np.abs(y[:, 2] - zv) < 1e-6]
+        assert np.hypot(left[:, 0], left[:, 1]).max() <= r_gone[np.abs(gone[:, 2] - zv) < 1e-6].min() + 1e-9
+    assert r_gone.min() > 14.0                      # the two outermost radial shells of the 3.1 nm wire
+
+
+def test_tensile_protocol_oracle_two_sided_pull_is_one_sided_pull_in_a_moving_frame():
+    """TensileMD, both ends pulled by -d and +d per step, without thermostat: velocity Verlet is Galilean invariant, so the
+    same wire pulled at ONE end by 2 d per step (the path pinned by the tests above), seen from a frame moving with the other
+    end (all dynamic velocities shifted by u = d / dt), is the same trajectory.  Also: the strain of the series is
+    (D2 - D1) / L0 and the recorded stress is the stress of the configuration it was recorded at."""
+    import oracle
+    from oracle.protocol import TensileMD
+    from oracle.observables import kinetic_tensor, stress
+    x = W.displace(W.fcc_wire(20.0, 32.0), 0.02, 9)
+    fl = W.grip_flags(x)
+    v0 = W.maxwell_velocities(len(x), 50.0, 4, fl == 0)
+    d, dt, n_steps = 0.004, 2.0, 20
+    L0 = float(x[:, 2].max() - x[:, 2].min())
+    vol = np.array([len(x) * 4.08 ** 3 / 4])
+    zref = x[:, 2].copy()
+    a = TensileMD(oracle.MD(x, v0, fl, 7.0, cells=True, zref=zref), dt, 0.0, 0.0, 1, 0, 0.0, +d, 0.0, -d, every=5,
+                  volume=vol, L0=L0)
+    vb = v0.copy()
+    vb[fl == 0, 2] += d / dt
+    b = TensileMD(oracle.MD(x, vb, fl, 7.0, cells=True, zref=zref), dt, 0.0, 0.0, 1, 0, 0.0, 2 * d, None, None)
+    for _ in range(n_steps):
+        a.step()
+        b.step()
+    shift = np.array([0.0, 0.0, d * n_steps])
+    assert np.abs(b.md.x - shift - a.md.x).max() < 1e-9
+    assert np.abs(a.md.x[fl == 1, 2] - (zref[fl == 1] - d * n_steps)).max() == 0      # placed (D:A10), both slabs
+    assert np.abs(a.md.x[fl == 2, 2] - (zref[fl == 2] + d * n_steps)).max() == 0
+    rec = np.array(a.series[0])
+    assert rec.shape == (4, 4) and np.allclose(rec[:, 0], [4, 9, 14, 19])
+    assert np.allclose(rec[:, 1], np.array([5, 10, 15, 20]) * 2 * d / L0, rtol=1e-12)
+    K = kinetic_tensor(a.md.v, fl, a.md.offsets, 196.96657)
+    assert rec[-1, 2] == pytest.approx(stress(a.md.w_rep, K, vol)[0, 2], rel=1e-12)
+    assert abs(rec[-1, 3] - 2.04) < 0.3 and a.rupture_step[0] == -1
+    # strokes: nothing moves until a period is complete
+    c = TensileMD(oracle.MD(x, v0, fl, 7.0, cells=True, zref=zref), dt, 0.0, 0.0, 1, 0, 0.0, +d, 0.0, -d, period=7)
+    for _ in range(13):
+        c.step()
+    assert np.abs(c.md.x[fl == 2, 2] - (zref[fl == 2] + 7 * d)).max() == 0
+    assert np.abs(c.md.x[fl == 1, 2] - (zref[fl == 1] - 7 * d)).max() == 0
