@@ -180,10 +180,11 @@ int tbsma_get_stats(tbsma_ctx *ctx, tbsma_stats *h_out); /* synchronises */
 /* Selects the neighbour-gather kernel variant (takes effect at the next tbsma_build_cells):
  *   1 = thread per atom over a k-major int32 list, neighbour records gathered from global memory
  *       through L1 (any system, periodic or not);
- *   2 = shared-memory tiles: one CTA per run of z-layers of cells of a NON-periodic replica stages
- *       the positions of its atoms and their halo in shared memory; 16-bit list entries, atoms
- *       ordered by list length inside a layer, lists ordered for conflict-free shared-memory gathers.
- *       tbsma_build_cells returns TBSMA_EINVAL if a replica is periodic or its layers do not fit;
+ *   2 = shared-memory tiles: a CTA stages the positions of a tile of cells (a run of z-layers of a thin wire, a box of
+ *       cells of a thick wire or of a periodic replica) and of the cells around it in shared memory; 16-bit list
+ *       entries, atoms ordered by list length inside a layer (or cell), lists ordered for conflict-free shared-memory
+ *       gathers.  tbsma_build_cells returns TBSMA_EINVAL if a replica does not fit (a periodic axis shorter than five
+ *       cells of r_cut + skin + S, a cell neighbourhood of more than 4095 atoms);
  *   0 = auto (default): 2 when it fits, else 1.
  * tbsma_get_variant returns the variant the current lists were built for. */
 int tbsma_set_variant(tbsma_ctx *ctx, int32_t variant);
@@ -208,6 +209,12 @@ int tbsma_set_tile(tbsma_ctx *ctx, int32_t layers_per_tile, int32_t threads);
  * per CTA.  Changes cost and the order of the per-replica sums, nothing else.  Takes effect at the next
  * tbsma_build_cells. */
 int tbsma_set_tile_split(tbsma_ctx *ctx, int32_t ctas_per_tile);
+
+/* Shared-memory variant: a replica whose z-layers of cells fit a tile image (the paper's thin wires) is cut into runs of
+ * whole layers; thicker wires and periodic replicas are cut into boxes of up to 3 x 3 x 3 cells with a one-cell halo,
+ * wrapped around on periodic axes.  force != 0 cuts EVERY replica into boxes (for tests; default 0).  Takes effect at the
+ * next tbsma_build_cells. */
+int tbsma_set_tile_box(tbsma_ctx *ctx, int32_t force);
 
 /* Shared-memory variant: how the two gather passes (P:59 stages 1 and 2) are launched.
  *   1 (default) = persistent kernels: two CTAs of 16 warps per SM work through the tiles of the batch, each holding the

@@ -145,10 +145,23 @@ int set_geometry(tbsma_ctx *c, double width)
     return TBSMA_OK;
 }
 
+// The shared-memory tile variant cuts a periodic replica into boxes of cells with a one-cell halo that must not wrap onto
+// itself: at least five cells (of the candidate radius) along every periodic axis.  Shorter periodic boxes use the global
+// variant with its own, narrower cells.
+bool tiles_possible(const tbsma_ctx *c)
+{
+    if (c->variant == 1) return false;
+    const double w_min = (c->r_cut + c->skin + c->outer_skin) * (1.0 + 1e-5) + 1e-4;
+    for (int r = 0; r < c->R; ++r)
+        for (int a = 0; a < 3; ++a)
+            if ((c->h_geom[r].periodic >> a & 1) && (int)floor((double)c->h_geom[r].len[a] / w_min) < 5) return false;
+    return true;
+}
+
 // Cell width and candidate-list storage for the variant the next build will try (called by tbsma_build_cells).
 int ensure_variant_resources(tbsma_ctx *c)
 {
-    const bool tiles = c->variant != 1 && !c->any_periodic;
+    const bool tiles = tiles_possible(c);
     const double r_list = c->r_cut + c->skin;
     const double width = tiles ? r_list + c->outer_skin : r_list;
     if (width != c->cell_w) {
@@ -418,6 +431,15 @@ int tbsma_set_tile_split(tbsma_ctx *c, int32_t ctas_per_tile)
     return TBSMA_OK;
 }
 
+int tbsma_set_tile_box(tbsma_ctx *c, int32_t force)
+{
+    if (!c) return TBSMA_EINVAL;
+    c->epoch++;
+    c->tile_force_box = force != 0;
+    c->cells_built = c->list_built = 0;
+    return TBSMA_OK;
+}
+
 int tbsma_set_gather(tbsma_ctx *c, int32_t mode)
 {
     if (!c || mode < 0 || mode > 4) return TBSMA_EINVAL;
@@ -648,7 +670,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     cudaError_t e = cudaSuccess;
 #define DA(ptr, cnt) if (e == cudaSuccess) e = dalloc(&(ptr), (cnt))
     DA(c->d_geom, (size_t)R); DA(c->d_atom_rep, n); DA(c->d_cell_of, n); DA(c->d_slot, n); DA(c->d_order, n);
-    c->list_bufs = c->any_periodic ? 1 : 2;   // the tile variant (non-periodic systems only) double-buffers its lists
+    c->list_bufs = 2;   // the tile variant double-buffers its lists (the global variant uses the first half)
     const size_t nb = (size_t)c->list_bufs;
     DA(c->d_pos_build, nb * c->n_pad); DA(c->d_tmp4, n); DA(c->d_tmp_tag, n);
     DA(c->d_nlist, nb * (size_t)c->kmax * (size_t)c->n_pad); DA(c->d_nn, nb * c->n_pad); DA(c->d_xs, n);
@@ -658,7 +680,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     DA(c->d_cur, (size_t)R); DA(c->d_nh, 2 * (size_t)R); DA(c->d_kmid, 2 * (size_t)n_blk); DA(c->d_nh_scale, (size_t)R);
     DA(c->d_blk_rep, (size_t)n_blk); DA(c->d_blk_first, (size_t)R + 1);
     DA(c->d_dirty, (size_t)R); DA(c->d_ctrl, 8); DA(c->d_counters, 8); DA(c->d_stagger, (size_t)R);
-    DA(c->d_maxpop, (size_t)R); DA(c->d_hbase, n); DA(c->d_tileof, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
+    DA(c->d_maxpop, 2 * (size_t)R); DA(c->d_hbase, n); DA(c->d_tileof, n); DA(c->d_newslot, n); DA(c->d_oldof, n); DA(c->d_nn_tmp, n);
     DA(c->d_tmp_pos, n);
 #undef DA
     if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
@@ -692,7 +714,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     if (e != cudaSuccess) { free_system(c); return map_cuda(e); }
     c->cell_w = 0.0;
     c->kmax_o = c->kmax;
-    const int rc = set_geometry(c, (c->variant != 1 && !c->any_periodic) ? r_list + c->outer_skin : r_list);
+    const int rc = set_geometry(c, tiles_possible(c) ? r_list + c->outer_skin : r_list);
     if (rc) { free_system(c); return rc; }
     return TBSMA_OK;
 }
@@ -710,7 +732,7 @@ int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, 
         const int rc0 = ensure_variant_resources(c);
         if (rc0) return rc0;
     }
-    c->active_variant = (c->variant != 1 && !c->any_periodic) ? 2 : 1;   // provisional: selects the dirty level
+    c->active_variant = tiles_possible(c) ? 2 : 1;   // provisional: selects the dirty level
     // every list is rebuilt from here on: all replicas start from half 0 of the list buffers again (the global variant
     // only ever uses half 0; after a run in the tile variant some replicas would otherwise still point at half 1)
     CK(cudaMemsetAsync(c->d_cur, 0, sizeof(int32_t) * (size_t)c->R, st));

@@ -35,20 +35,37 @@ struct RepGeom {
     int atom_begin, atom_end;
 };
 
-// One tile of the shared-memory ("wire") variant: a run of consecutive z-layers of cells of one
-// non-periodic replica.  Atoms are in cell order (z slowest), so the tile's own atoms and its halo
-// (one more layer on each side) are contiguous index ranges; both follow from cell_start at run time.
+// One tile of the shared-memory variant: the cells whose atoms one CTA works on ("own") and the cells within one cell of
+// them ("halo", own cells included), whose records the CTA stages in shared memory.
+//   kind 0: whole z-layers of cells of a thin non-periodic replica (the paper's wires): own layers plus one layer on
+//           either side.  Atoms are in cell order (z slowest), so own atoms and halo are CONTIGUOUS slot ranges.
+//   kind 1: a box of cells of any replica (thick wires, periodic bulk): the halo is the box grown by one cell per side,
+//           wrapped around on periodic axes; every cell is a contiguous run of slots.
+// A "run" is a layer (kind 0) or a halo cell (kind 1): the unit inside which atoms are reordered by neighbour count, so
+// cell_start stays valid at run boundaries between rebuilds of the cells.
 struct TileDesc {
     int rep;          // replica
+    int kind;
+    int first_of_rep; // the first tile of its replica
+    int cell_base;    // first cell of the replica
+    int nx, ny, nz;   // cells of the replica per axis
+    // kind 0
     int ch0;          // global cell index of the first cell of the first halo layer
     int nlay_h;       // halo layers = own layers + (0..2)
     int own_first;    // index, among the halo layers, of the first own layer (0 or 1)
     int own_n;        // own layers
     int layer_cells;  // nx * ny
-    int nx, ny, nz;
     int z_h0;         // z index of the first halo layer
-    int cell_base;    // first cell of the replica
-    int pad;
+    // kind 1
+    short h0[3];      // first halo cell per axis (-1 or nc on a periodic axis: wraps)
+    short hn[3];      // halo cells per axis
+    short o0[3];      // first own cell per axis, counted from the first halo cell (0 or 1)
+    short on[3];      // own cells per axis
+    // A tile whose halo wraps around periodic axis a sees a record from across the boundary at a raw coordinate
+    // difference beyond half the box: D:A6's `if (d > L/2) d -= L; else if (d < -L/2) d += L` is, for every pair of an own
+    // atom and a staged record of THIS tile, `if (|d| > hL[a]) d += Ls[a]` with Ls = -L for a tile at the upper end of the
+    // axis, +L at the lower end (a tile is never at both: tbsma_tile_setup wants 2 own + 3 cells per periodic axis)
+    float Ls[3], hL[3];   // 0 and +inf on an axis this tile does not wrap
 };
 // Layout of every neighbour list (int4 rows of the global variant, uint2 rows of the tile variant, candidates too):
 // "block-major".  A row is a group of four entries; the rows of the 32 atoms [32 b, 32 b + 32) are contiguous, row g of
@@ -62,6 +79,8 @@ __host__ __device__ __forceinline__ size_t tbsma_lrow(int i, int kg)
 }
 #endif
 #define TBSMA_LROW 32                // elements between consecutive rows of an atom
+#define TBSMA_TILE_MAX_RUNS 128      // halo cells of a box tile
+#define TBSMA_TILE_MAX_OWN_RUNS 32
 #define TBSMA_TILE_MAX_LAYERS 8      // own layers per tile
 #define TBSMA_TILE_MAX_RECORDS 4095  // halo records per tile: (records + sentinel) * 16 B <= 64 KB, u16 byte offsets
 
@@ -115,6 +134,8 @@ struct tbsma_ctx {
     int own_cap;           // own atoms a tile may hold (sizes the split of the inner build)
     int tile_nsplit;       // CTAs of the gather kernels per tile (> 1 when the tiles are too few to fill the GPU)
     int tile_split_req;    // requested by tbsma_set_tile_split (0 = automatic)
+    int tile_force_box;    // tbsma_set_tile_box: box tiles even for replicas whose layers would fit (tests)
+    int any_box;           // some replica is cut into box tiles (kind 1)
     double *d_cta_sums;    // n_tiles x tile_nsplit x 8: E, E_kin, W (xx yy zz xy xz yz) of every CTA of the force pass
     // persistent gather kernels: units = p_plain whole tiles, then the remaining tiles in p_S parts each
     int gather_mode;       // 1 (default): persistent kernels (k_gather_persist); 0: one CTA per tile (or part of a tile)
@@ -123,11 +144,11 @@ struct tbsma_ctx {
     int p_tail_split;      // parts the last 2 n_sm tiles of a large batch are cut into (0 = whole)
     int p_nb, p_nb_req;    // tile images per CTA (the next units' images are filled while the current one is worked on)
     size_t have_sums;
-    int32_t *d_maxpop;  // R: largest layer population of each replica (measured at build_cells)
+    int32_t *d_maxpop;  // 2 R: largest layer population and largest cell population of each replica (measured at build_cells)
     int32_t *d_hbase;   // n: first halo slot of the tile that owns slot i
     int32_t *d_tileof;  // n: the tile that owns slot i
     unsigned short *d_img;  // n_tiles x tile_cap: image index of every halo record of a tile (k_tile_place)
-    unsigned short *d_inv;  // n_tiles x img_cap: the inverse
+    int32_t *d_inv;         // n_tiles x img_cap: the slot of the record at every image index (inspection calls)
     int img_cap;        // records of a tile image, sentinel and spare room of the colour classes included
     size_t have_tiles, have_first, have_work, have_img, have_inv;   // bytes allocated for the five tile tables
     int balance;        // records placed by colour (default 1) or in slot order

@@ -62,6 +62,108 @@ __device__ __forceinline__ TileRange tile_range(const TileDesc &t, const int *__
     return r;
 }
 
+// Runs of a tile (layers or halo cells, see TileDesc) in shared memory: where every halo record and every own atom lives.
+// Halo-local index k = position among the tile's staged records, runs concatenated in order; own-local index o = position
+// among the tile's own atoms, own runs concatenated in order.  Lane o & 31 handles atom o in the list builds and in the
+// gather passes alike (the bank schedule of the lists depends on it).
+struct TileMap {
+    int n_runs, nh, n_own_runs, n_own;
+    int lstart[TBSMA_TILE_MAX_RUNS + 1];   // halo-local index of the first record of run r; lstart[n_runs] = nh
+    int gslot[TBSMA_TILE_MAX_RUNS];        // slot of that record
+    int ostart[TBSMA_TILE_MAX_OWN_RUNS + 1];   // own-local index of the first atom of own run q
+    short orun[TBSMA_TILE_MAX_OWN_RUNS];       // which run it is
+};
+__device__ __forceinline__ int wrap_cell(int c, int nc) { return c < 0 ? c + nc : (c >= nc ? c - nc : c); }
+
+// called by every thread of the CTA; ends with a barrier
+__device__ __forceinline__ void tile_map_build(const TileDesc &t, const int *__restrict__ cell_start, TileMap &M)
+{
+    const int n_runs = t.kind == 0 ? t.nlay_h : (int)t.hn[0] * t.hn[1] * t.hn[2];
+    for (int r = threadIdx.x; r < n_runs; r += blockDim.x) {
+        int c0, nc;
+        if (t.kind == 0) {
+            c0 = t.ch0 + r * t.layer_cells;
+            nc = t.layer_cells;
+        } else {
+            const int hx = r % t.hn[0], hy = (r / t.hn[0]) % t.hn[1], hz = r / (t.hn[0] * t.hn[1]);
+            const int cx = wrap_cell(t.h0[0] + hx, t.nx), cy = wrap_cell(t.h0[1] + hy, t.ny), cz = wrap_cell(t.h0[2] + hz, t.nz);
+            c0 = t.cell_base + (cz * t.ny + cy) * t.nx + cx;
+            nc = 1;
+        }
+        const int s = cell_start[c0];
+        M.gslot[r] = s;
+        M.lstart[r + 1] = cell_start[c0 + nc] - s;       // population, made a prefix sum below
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {          // inclusive scan of the populations by one warp, 32 runs per round
+        const int lane = threadIdx.x;
+        int carry = 0;
+        for (int r0 = 0; r0 < n_runs; r0 += 32) {
+            int v = r0 + lane < n_runs ? M.lstart[r0 + lane + 1] : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, v, o);
+                if (lane >= o) v += y;
+            }
+            if (r0 + lane < n_runs) M.lstart[r0 + lane + 1] = carry + v;
+            carry += __shfl_sync(0xffffffffu, v, 31);
+        }
+        if (lane == 0) { M.lstart[0] = 0; M.n_runs = n_runs; M.nh = carry; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int q = 0, o = 0;
+        if (t.kind == 0) {
+            for (int l = 0; l < t.own_n; ++l) {
+                const int r = t.own_first + l;
+                M.orun[q] = (short)r; M.ostart[q] = o; o += M.lstart[r + 1] - M.lstart[r]; ++q;
+            }
+        } else {
+            for (int z = 0; z < t.on[2]; ++z)
+                for (int y = 0; y < t.on[1]; ++y)
+                    for (int x = 0; x < t.on[0]; ++x) {
+                        const int r = ((t.o0[2] + z) * t.hn[1] + t.o0[1] + y) * t.hn[0] + t.o0[0] + x;
+                        M.orun[q] = (short)r; M.ostart[q] = o; o += M.lstart[r + 1] - M.lstart[r]; ++q;
+                    }
+        }
+        M.ostart[q] = o;
+        M.n_own_runs = q;
+        M.n_own = o;
+    }
+    __syncthreads();
+}
+// run that holds halo-local index k (< nh)
+__device__ __forceinline__ int map_run_of(const TileMap &M, int k)
+{
+    int lo = 0, hi = M.n_runs - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (M.lstart[mid] <= k) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+__device__ __forceinline__ int map_slot(const TileMap &M, int k)
+{
+    const int r = map_run_of(M, k);
+    return M.gslot[r] + k - M.lstart[r];
+}
+// own-local index o (< n_own) -> slot; also its own run q and its halo-local index
+__device__ __forceinline__ int map_own(const TileMap &M, int o, int &q, int &k)
+{
+    q = 0;
+    while (q + 1 < M.n_own_runs && M.ostart[q + 1] <= o) ++q;
+    const int r = M.orun[q], off = o - M.ostart[q];
+    k = M.lstart[r] + off;
+    return M.gslot[r] + off;
+}
+__device__ __forceinline__ int map_own(const TileMap &M, int o)
+{
+    int q, k;
+    return map_own(M, o, q, k);
+}
+// D:A6 for a pair of an own atom and a staged record of a tile that wraps around periodic axes (see TileDesc)
+__device__ __forceinline__ float wrap_d(float d, float hL, float Ls) { return fabsf(d) > hL ? d + Ls : d; }
+
 // largest layer population of every replica (sizes the tiles; host reads it back at build_cells)
 __global__ void k_layer_maxpop(const RepGeom *__restrict__ geom, const int *__restrict__ cell_start,
                                int *__restrict__ maxpop, int R)
@@ -74,6 +176,10 @@ __global__ void k_layer_maxpop(const RepGeom *__restrict__ geom, const int *__re
     for (int z = 0; z < g->nc[2]; ++z)
         m = max(m, cell_start[g->cell_base + (z + 1) * lc] - cell_start[g->cell_base + z * lc]);
     maxpop[r] = m;
+    int mc = 0;        // and the largest cell population (sizes box tiles)
+    const int ncell = lc * g->nc[2];
+    for (int c = 0; c < ncell; ++c) mc = max(mc, cell_start[g->cell_base + c + 1] - cell_start[g->cell_base + c]);
+    maxpop[R + r] = mc;
 }
 
 // ---- worklists.  Only a few per cent of the replicas rebuild in a given step, so the kernels that
@@ -150,7 +256,7 @@ __device__ __forceinline__ void scan_tile(const TileDesc &t, const ScanArgs &A)
     int *__restrict__ want_outer = A.want_outer;
     const int n_pad = A.n_pad, kmax = A.kmax, s_cap = A.s_cap, cell_cap = A.cell_cap;
     const float ro2 = A.ro2, rl2 = A.rl2;
-    if (threadIdx.x == 0 && t.z_h0 == 0 && t.own_first == 0) want_outer[t.rep] = 0;   // new candidates: request served
+    if (threadIdx.x == 0 && t.first_of_rep) want_outer[t.rep] = 0;   // new candidates: request served
     extern __shared__ float4 smem_f4[];
     float4 *sm = smem_f4;
     int *cs = reinterpret_cast<int *>(sm + s_cap);
@@ -225,6 +331,83 @@ __device__ __forceinline__ void scan_tile(const TileDesc &t, const ScanArgs &A)
     }
 }
 
+// K1 for a box tile (kind 1): the same scan over the 3 x 3 runs of x-adjacent halo cells, pair differences wrapped as
+// D:A6 prescribes where the tile's halo wraps around a periodic axis; ranks inside the own CELL.
+__device__ __forceinline__ void scan_box(const TileDesc &t, const ScanArgs &A)
+{
+    extern __shared__ float4 smem_f4[];
+    float4 *sm = smem_f4;
+    unsigned short *cnts = reinterpret_cast<unsigned short *>(sm + A.s_cap);
+    __shared__ TileMap M;
+    const int tid = threadIdx.x;
+    if (tid == 0 && t.first_of_rep) A.want_outer[t.rep] = 0;   // new candidates: request served
+    tile_map_build(t, A.cell_start, M);
+    if (M.n_own <= 0) return;
+    if (M.nh > A.s_cap) {
+        if (tid == 0) atomicOr(A.ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
+        return;
+    }
+    for (int k = tid; k < M.nh; k += blockDim.x) sm[k] = A.pos_sorted[map_slot(M, k)];
+    __syncthreads();
+    const int hn0 = t.hn[0], hn1 = t.hn[1], hn2 = t.hn[2];
+    const float hLx = t.hL[0], hLy = t.hL[1], hLz = t.hL[2], Lsx = t.Ls[0], Lsy = t.Ls[1], Lsz = t.Ls[2];
+    const int kmax = A.kmax;
+    for (int o = tid; o < M.n_own; o += blockDim.x) {
+        int q, al;
+        const int a = map_own(M, o, q, al);
+        const float4 pi = sm[al];
+        const int run = M.orun[q];
+        const int hx = run % hn0, hy = (run / hn0) % hn1, hz = run / (hn0 * hn1);
+        const int x0 = max(hx - 1, 0), x1 = min(hx + 1, hn0 - 1);
+        uint2 *row = A.nl_tmp + tbsma_lrow(a, kmax >> 2);
+        unsigned w0 = 0u, w1 = 0u;
+        int cnt = 0, cnt_in = 0;
+        for (int zz = max(hz - 1, 0); zz <= min(hz + 1, hn2 - 1); ++zz)
+            for (int yy = max(hy - 1, 0); yy <= min(hy + 1, hn1 - 1); ++yy) {
+                const int rb = (zz * hn1 + yy) * hn0;
+                const int sb = M.lstart[rb + x0], e = M.lstart[rb + x1 + 1];
+                for (int j = sb; j < e; ++j) {
+                    const float4 pj = sm[j];
+                    const float dx = wrap_d(pi.x - pj.x, hLx, Lsx), dy = wrap_d(pi.y - pj.y, hLy, Lsy);
+                    const float dz = wrap_d(pi.z - pj.z, hLz, Lsz);
+                    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
+                    if (d2 < A.ro2 && j != al) {
+                        if (cnt < kmax) {
+                            const unsigned v = (unsigned)j << ((cnt & 1) << 4);
+                            if (cnt & 2) w1 |= v; else w0 |= v;
+                            if ((cnt & 3) == 3) {
+                                row[(size_t)(cnt >> 2) * TBSMA_LROW] = make_uint2(w0, w1);
+                                w0 = w1 = 0u;
+                            }
+                        }
+                        ++cnt;
+                        cnt_in += d2 < A.rl2;
+                    }
+                }
+            }
+        if (cnt > kmax) atomicOr(A.ctrl + 1, (int)TBSMA_FLAG_NLIST_OVERFLOW);
+        cnt = min(cnt, kmax);
+        if (cnt & 3) row[(size_t)(cnt >> 2) * TBSMA_LROW] = make_uint2(w0, w1);
+        cnts[o] = (unsigned short)cnt_in;
+        A.nn_tmp[a] = cnt | ((__float_as_int(pi.w) & 3) << 16);
+    }
+    __syncthreads();
+    for (int o = tid; o < M.n_own; o += blockDim.x) {
+        int q, al;
+        const int a = map_own(M, o, q, al);
+        const int l0 = M.ostart[q], l1 = M.ostart[q + 1];
+        const int my = cnts[o];
+        int rank = 0;
+        for (int b = l0; b < l1; ++b) {
+            const int cb = cnts[b];
+            rank += (cb > my) || (cb == my && b < o);
+        }
+        const int ns = M.gslot[M.orun[q]] + rank;
+        A.newslot[a] = ns;
+        A.oldof[ns] = a;
+    }
+}
+
 // K1 over the tiles of the replicas whose candidates are rebuilt (work list 1)
 __global__ void __launch_bounds__(kScanThreads)
 k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ work, int n_tiles, ScanArgs A)
@@ -232,7 +415,9 @@ k_tile_scan(const TileDesc *__restrict__ tiles, const int *__restrict__ work, in
     const int nw = work[1];
     for (int w = blockIdx.x; w < nw; w += gridDim.x) {
         __syncthreads();       // the previous tile's shared-memory image is no longer read
-        scan_tile(tiles[work[2 + n_tiles + w]], A);
+        const TileDesc t = tiles[work[2 + n_tiles + w]];
+        if (t.kind == 0) scan_tile(t, A);
+        else scan_box(t, A);
     }
 }
 
@@ -250,7 +435,8 @@ struct PlaceArgs {
     const int *cell_start, *oldof;
     const float4 *pos_sorted;        // cell-ordered positions of this rebuild
     const RepGeom *geom;
-    unsigned short *img, *inv;       // per tile: halo-local final index -> image index, and back
+    unsigned short *img;             // per tile: halo-local index -> image index
+    int *inv;                        // per tile: image index -> slot (inspection calls)
     int img_stride, inv_stride;      // tile_cap, img_cap
     int img_cap;                     // records an image may hold (sentinel included)
     float inv_h;                     // 1 / h; 0 = slot order (colour = index mod 8)
@@ -262,15 +448,19 @@ k_tile_place(const TileDesc *__restrict__ tiles, const int *__restrict__ work, i
 {
     __shared__ unsigned char s_col[TBSMA_TILE_MAX_RECORDS + 1];
     __shared__ int s_fallback;
+    __shared__ TileMap M;
     const int nw = work[1];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     for (int w = blockIdx.x; w < nw; w += gridDim.x) {
         const int ti = work[2 + n_tiles + w];
         const TileDesc t = tiles[ti];
-        const TileRange r = tile_range(t, A.cell_start);
-        if (r.hi <= r.lo || r.nh > A.img_stride) continue;
+        __syncthreads();
+        tile_map_build(t, A.cell_start, M);
+        struct { int nh; } r = {M.nh};
+        if (M.n_own <= 0 || r.nh > A.img_stride) continue;
         const RepGeom *g = A.geom + t.rep;
-        unsigned short *img = A.img + (size_t)ti * A.img_stride, *inv = A.inv + (size_t)ti * A.inv_stride;
+        unsigned short *img = A.img + (size_t)ti * A.img_stride;
+        int *inv = A.inv + (size_t)ti * A.inv_stride;
         __syncthreads();
         if (tid == 0) s_fallback = 0;
         for (int pass = 0; pass < 2; ++pass) {
@@ -278,7 +468,7 @@ k_tile_place(const TileDesc *__restrict__ tiles, const int *__restrict__ work, i
             for (int k = tid; k < r.nh; k += blockDim.x) {
                 int col = k & 7;
                 if (pass == 0 && A.inv_h > 0.f) {
-                    const float4 p = A.pos_sorted[A.oldof[r.halo_lo + k]];
+                    const float4 p = A.pos_sorted[A.oldof[map_slot(M, k)]];
                     const int ix = __float2int_rd((p.x - g->lo[0]) * A.inv_h), iy = __float2int_rd((p.y - g->lo[1]) * A.inv_h);
                     const int iz = __float2int_rd((p.z - g->lo[2]) * A.inv_h);
                     col = (ix + 2 * iy + 3 * iz) & 7;
@@ -294,7 +484,7 @@ k_tile_place(const TileDesc *__restrict__ tiles, const int *__restrict__ work, i
                     const unsigned m = __ballot_sync(0xffffffffu, mine);
                     if (mine) {
                         const int idx = 8 * (run + __popc(m & ((1u << lane) - 1u))) + wid + 1;
-                        if (idx < A.img_cap) { img[k] = (unsigned short)idx; inv[idx] = (unsigned short)k; }
+                        if (idx < A.img_cap) { img[k] = (unsigned short)idx; inv[idx] = map_slot(M, k); }
                     }
                     run += __popc(m);
                 }
@@ -321,7 +511,7 @@ struct FinishArgs {
     const uint2 *nl_tmp;
     const int *nn_tmp, *newslot, *oldof;
     uint2 *nl;
-    int *nn, *hbase, *tileof;
+    int *nn, *tileof;
     const unsigned short *img;   // image placement of every tile (k_tile_place)
     int img_stride;
     int n_pad, s_cap;
@@ -334,25 +524,30 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
     const uint2 *__restrict__ nl_tmp = A.nl_tmp;
     const int *__restrict__ nn_tmp = A.nn_tmp, *__restrict__ newslot = A.newslot, *__restrict__ oldof = A.oldof;
     uint2 *__restrict__ nl = A.nl;
-    int *__restrict__ nn = A.nn, *__restrict__ hbase = A.hbase;
-    const int n_pad = A.n_pad, s_cap = A.s_cap;
+    int *__restrict__ nn = A.nn;
+    const int s_cap = A.s_cap;
     extern __shared__ float4 smem_f4[];
     unsigned short *map = reinterpret_cast<unsigned short *>(smem_f4);   // s_cap entries
     unsigned short *scr = map + ((s_cap + 7) & ~7);                      // kmax x blockDim.x
-    const TileRange r = tile_range(t, cell_start);
-    if (r.hi <= r.lo || r.nh > s_cap) return;
+    __shared__ TileMap M;
+    tile_map_build(t, cell_start, M);
+    if (M.n_own <= 0 || M.nh > s_cap) return;
     const int tid = threadIdx.x, nthr = blockDim.x;
     const unsigned short *__restrict__ img = A.img + (size_t)ti * A.img_stride;
-    for (int k = tid; k < r.nh; k += blockDim.x)
-        map[k] = (unsigned short)((unsigned)img[newslot[r.halo_lo + k] - r.halo_lo] << 4);
+    // cell-order halo-local index -> byte offset of the record in the image: the atom moves inside its run only
+    for (int k = tid; k < M.nh; k += blockDim.x) {
+        const int sc = map_slot(M, k);
+        map[k] = (unsigned short)((unsigned)img[k + (newslot[sc] - sc)] << 4);
+    }
     __syncthreads();
-    for (int ip = r.lo + tid; ip < r.hi; ip += blockDim.x) {
+    for (int o = tid; o < M.n_own; o += blockDim.x) {
+        const int ip = map_own(M, o);
         const int a = oldof[ip];
         const int nnv = nn_tmp[a];
         const int cnt = nnv & 0xffff;
         const uint2 *src = nl_tmp + tbsma_lrow(a, A.kg_o);
         const int ng = (cnt + 3) >> 2;
-        const unsigned lane = (unsigned)(ip - r.lo) & 31u;     // the lane the inner build and the gather passes give this atom
+        const unsigned lane = (unsigned)o & 31u;     // the lane the inner build and the gather passes give this atom
         // pass A: population of the 8 classes, counted from the lane's own (packed bytes; kmax <= 248)
         unsigned long long pop = 0ull;
         for (int g = 0; g < ng; ++g) {
@@ -392,7 +587,6 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
             dst[(size_t)g * TBSMA_LROW] = make_uint2(e[0] | (e[1] << 16), e[2] | (e[3] << 16));
         }
         nn[ip] = nnv;
-        hbase[ip] = r.halo_lo;
         A.tileof[ip] = ti;
     }
 }
@@ -450,8 +644,9 @@ __global__ void k_stage_copy(const float4 *__restrict__ pos, const float4 *__res
 // previous image.  (A contiguous image was one cp.async.bulk; spreading the records over the bank groups is worth
 // more than the copy engine: a fifth fewer shared-memory wavefronts in the gather passes, 62 % fewer bank conflicts.)
 __device__ __forceinline__ void fill_image(float4 *sm, const float4 *__restrict__ src,
-                                           const unsigned short *__restrict__ img, int halo_lo, int nh)
+                                           const unsigned short *__restrict__ img, const TileMap &M)
 {
+    const int nh = M.nh;
     if (threadIdx.x == 0) sm[0] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
     // eight records per thread and round, all sixteen loads in flight before the first store
     const int nthr = blockDim.x;
@@ -461,7 +656,7 @@ __device__ __forceinline__ void fill_image(float4 *sm, const float4 *__restrict_
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             const int k = k0 + u * nthr;
-            if (k < nh) { at[u] = img[k]; rec[u] = src[halo_lo + k]; }
+            if (k < nh) { at[u] = img[k]; rec[u] = src[map_slot(M, k)]; }
         }
 #pragma unroll
         for (int u = 0; u < 8; ++u)
@@ -511,12 +706,30 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
 struct Pair2 {
     f32x2 dx, dy, dz, rinv, t;
 };
-__device__ __forceinline__ Pair2 pair2(const float4 &pi, const float4 &pa, const float4 &pb, const PairConst &pc)
+// a tile whose halo wraps around periodic axes (TileDesc::Ls, hL): d += Ls where |d| > hL, which is D:A6's minimum image
+// for every pair of an own atom and a staged record of that tile.  As m * Ls + d with m = 1.0 or 0.0: the product is
+// exact, the sum rounds once, like the addition it stands for (and adding 0 changes nothing).
+struct WrapC { float hLx, hLy, hLz, Lsx, Lsy, Lsz; };
+__device__ __forceinline__ float set_gt_abs(float d, float h)
+{
+    float m;
+    asm("set.gt.f32.f32 %0, %1, %2;" : "=f"(m) : "f"(fabsf(d)), "f"(h));
+    return m;
+}
+template <bool WRAP>
+__device__ __forceinline__ Pair2 pair2(const float4 &pi, const float4 &pa, const float4 &pb, const PairConst &pc,
+                                       const WrapC &wc)
 {
     Pair2 P;
     P.dx = pk(pi.x - pa.x, pi.x - pb.x);
     P.dy = pk(pi.y - pa.y, pi.y - pb.y);
     P.dz = pk(pi.z - pa.z, pi.z - pb.z);
+    if (WRAP) {
+        float a, b;
+        unpk(P.dx, a, b); P.dx = fma2(pk(set_gt_abs(a, wc.hLx), set_gt_abs(b, wc.hLx)), pk(wc.Lsx, wc.Lsx), P.dx);
+        unpk(P.dy, a, b); P.dy = fma2(pk(set_gt_abs(a, wc.hLy), set_gt_abs(b, wc.hLy)), pk(wc.Lsy, wc.Lsy), P.dy);
+        unpk(P.dz, a, b); P.dz = fma2(pk(set_gt_abs(a, wc.hLz), set_gt_abs(b, wc.hLz)), pk(wc.Lsz, wc.Lsz), P.dz);
+    }
     const f32x2 d2 = fma2(P.dz, P.dz, fma2(P.dy, P.dy, mul2(P.dx, P.dx)));
     float d2a, d2b;
     unpk(d2, d2a, d2b);
@@ -529,10 +742,11 @@ __device__ __forceinline__ Pair2 pair2(const float4 &pi, const float4 &pa, const
 }
 
 // xi^2 e^{-2q x} of two neighbours added to the two running sums in rho2
+template <bool WRAP = false>
 __device__ __forceinline__ f32x2 rho_term2(const float4 &pi, const float4 &pa, const float4 &pb, const PairConst &pc,
-                                           f32x2 rho2)
+                                           f32x2 rho2, const WrapC &wc = WrapC())
 {
-    const Pair2 P = pair2(pi, pa, pb, pc);
+    const Pair2 P = pair2<WRAP>(pi, pa, pb, pc, wc);
     const f32x2 arg = fma2(pk(pc.aq, pc.aq), P.t, pk(pc.b_rho, pc.b_rho));
     float a0, a1;
     unpk(arg, a0, a1);
@@ -576,11 +790,12 @@ struct InnerArgs {
 constexpr int kInnerThreads = 256;   // one atom per thread, kmax u16 of shared-memory scratch each
 
 // tmp: element k of thread t at [k * nthr + t], kmax + 1 rows (row kmax takes what does not fit)
-__device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRange &r, int i_begin, int i_end,
+template <bool WRAP>
+__device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileMap &M, int o_begin, int o_end,
                                                  const float4 *sm, const float4 *__restrict__ pos, unsigned short *tmp,
-                                                 const InnerArgs &ia, int *__restrict__ ctrl, int n_pad)
+                                                 const InnerArgs &ia, int *__restrict__ ctrl)
 {
-    // i_begin - r.lo is a multiple of 32, so tid & 31 is the lane the gather kernels give the atom
+    // o_begin is a multiple of 32, so tid & 31 is the lane the gather kernels give the atom
     const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31;
     int maxc = 0;
     bool want = false, viol = false, over = false;
@@ -589,7 +804,8 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
     int *nn_out = ia.nn + (size_t)ob * ia.n_stride;
     float4 *pb_out = ia.pos_build + (size_t)ob * ia.n_stride;
     unsigned short *col = tmp + tid;
-    for (int i = i_begin + tid; i < i_end; i += nthr) {
+    for (int o = o_begin + tid; o < o_end; o += nthr) {
+        const int i = map_own(M, o);
         const float4 pi = pos[i];
         const int nno = ia.nn_o[i];
         const int ng = ((nno & 0xffff) + 3) >> 2;
@@ -603,7 +819,8 @@ __device__ __forceinline__ void tile_inner_build(const TileDesc &t, const TileRa
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const float4 pj = lds_rec(sm, e[q]);
-                const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                if (WRAP) { dx = wrap_d(dx, t.hL[0], t.Ls[0]); dy = wrap_d(dy, t.hL[1], t.Ls[1]); dz = wrap_d(dz, t.hL[2], t.Ls[2]); }
                 d2[q] = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));   // D:A6
             }
 #pragma unroll
@@ -699,6 +916,7 @@ k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, c
              int which, int n_tiles)
 {
     extern __shared__ float4 smem_f4[];
+    __shared__ TileMap M;
     // the density pass may be launched as a programmatic dependent of this kernel (it reads the half of the list
     // buffers this kernel does not write): let it start at once
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -709,18 +927,19 @@ k_tile_inner(const TileDesc *__restrict__ tiles, const int *__restrict__ work, c
     for (int u = blockIdx.x; u < nu; u += gridDim.x) {
         const int ti = wl[u / nsplit];
         const TileDesc t = tiles[ti];
-        const TileRange r = tile_range(t, cell_start);
-        const int i_begin = r.lo + (u % nsplit) * blockDim.x;
-        if (i_begin >= r.hi) continue;
-        if (r.nh > s_cap) {
+        __syncthreads();       // nobody still reads the previous map or image
+        tile_map_build(t, cell_start, M);
+        const int o_begin = (u % nsplit) * blockDim.x;
+        if (o_begin >= M.n_own) continue;
+        if (M.nh > s_cap) {
             if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
             continue;
         }
-        __syncthreads();
-        fill_image(smem_f4, pos, ia.img + (size_t)ti * ia.img_stride, r.halo_lo, r.nh);
+        fill_image(smem_f4, pos, ia.img + (size_t)ti * ia.img_stride, M);
         // the last piece also takes whatever a tile holds beyond the headroom it was sized with
-        const int i_end = (u % nsplit) == nsplit - 1 ? r.hi : min(i_begin + (int)blockDim.x, r.hi);
-        tile_inner_build(t, r, i_begin, i_end, smem_f4, pos, tmp, ia, ctrl, n_pad);
+        const int o_end = (u % nsplit) == nsplit - 1 ? M.n_own : min(o_begin + (int)blockDim.x, M.n_own);
+        if (t.Ls[0] != 0.f || t.Ls[1] != 0.f || t.Ls[2] != 0.f) tile_inner_build<true>(t, M, o_begin, o_end, smem_f4, pos, tmp, ia, ctrl);
+        else tile_inner_build<false>(t, M, o_begin, o_end, smem_f4, pos, tmp, ia, ctrl);
     }
 }
 
@@ -743,19 +962,20 @@ __device__ __forceinline__ uint2 ld_row(const uint2 *row, int g, int ng, int n_p
 
 // stage 1 (Eq.1): rho_i over the list, s_i = rho_i^(-1/2) packed with the position.
 // SPLIT: the CTA takes part `part` of `nsplit` of the tile's chunks (small batches); otherwise all of them
-template <bool SPLIT>
-__device__ __forceinline__ void density_tile(const TileDesc &t, const int *__restrict__ cell_start,
+template <bool SPLIT, bool WRAP>
+__device__ __forceinline__ void density_tile(const TileDesc &t, const TileMap &M,
                                              const float4 *__restrict__ pos, const uint2 *__restrict__ nl,
                                              const int *__restrict__ nn, float4 *__restrict__ xs,
                                              int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
                                              const unsigned short *__restrict__ img, int part, int nsplit, int kg)
 {
-    const TileRange r = tile_range(t, cell_start);
+    struct { int lo, hi, nh; } r = {0, M.n_own, M.nh};      // own-local range
     if (r.hi <= r.lo) return;
     if (r.nh > s_cap) {
         if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
         return;
     }
+    const WrapC wc = {t.hL[0], t.hL[1], t.hL[2], t.Ls[0], t.Ls[1], t.Ls[2]};
     // this CTA's share of the tile's 32-atom chunks (all of them unless the batch is too small to fill the GPU)
     // (the range lives in shared memory: the loops below have no register to spare)
     extern __shared__ float4 smem_f4[];
@@ -767,12 +987,13 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
         if (threadIdx.x == 0) { s_next = cb; s_end = ce; }
     }
     const float4 *sm = smem_f4;
-    fill_image(smem_f4, pos, img, r.halo_lo, r.nh);
+    fill_image(smem_f4, pos, img, M);
     const int lane = threadIdx.x & 31;
     const int nchunk = (r.hi - r.lo + 31) >> 5;
     for (int ch = next_chunk(&s_next); ch < (SPLIT ? s_end : nchunk); ch = next_chunk(&s_next)) {
-        const int i = r.lo + (ch << 5) + lane;
-        if (i >= r.hi) continue;
+        const int o = (ch << 5) + lane;
+        if (o >= r.hi) continue;
+        const int i = map_own(M, o);
         // own record, count and the first three rows in one round trip (the rows exist whatever the count: kg >= 3 or the
         // loads are skipped); a row register is reloaded right after its use
         const uint2 *row = nl + tbsma_lrow(i, kg);
@@ -786,8 +1007,8 @@ __device__ __forceinline__ void density_tile(const TileDesc &t, const int *__res
         auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
             const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
-            rho2 = rho_term2(pi, p0, p1, pc, rho2);
-            rho2 = rho_term2(pi, p2, p3, pc, rho2);
+            rho2 = rho_term2<WRAP>(pi, p0, p1, pc, rho2, wc);
+            rho2 = rho_term2<WRAP>(pi, p2, p3, pc, rho2, wc);
         };
         int g = 0;
         for (; g + 3 <= ng; g += 3) {
@@ -835,8 +1056,14 @@ k_density_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_
     const int ti = SPLIT ? (int)blockIdx.x / ls.nsplit : (int)blockIdx.x, part = SPLIT ? (int)blockIdx.x % ls.nsplit : 0;
     const TileDesc t = tiles[ti];
     const int h = list_half(ls, t.rep);
-    density_tile<SPLIT>(t, cell_start, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad, s_cap,
-                 pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit, ls.kg);
+    __shared__ TileMap M;
+    tile_map_build(t, cell_start, M);
+    if (t.Ls[0] != 0.f || t.Ls[1] != 0.f || t.Ls[2] != 0.f)
+        density_tile<SPLIT, true>(t, M, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad,
+                                  s_cap, pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit, ls.kg);
+    else
+        density_tile<SPLIT, false>(t, M, pos, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, xs, ctrl, n_pad,
+                                   s_cap, pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit, ls.kg);
     // Launched as a programmatic dependent of the filter kernel this pass starts early and reads nothing of it; but the
     // kernels after it (force pass, then the swap of the list halves) are ordered after THIS kernel only, so it must
     // not complete before the filter kernel has (a no-op for an ordinary launch).
@@ -852,11 +1079,11 @@ struct AccT {
 // Two neighbours of atom i (pi.w = s_i, pa.w / pb.w = s_j):
 //   F_i += [ (2Ap/r0) e^{-p x} - (q xi^2/r0) e^{-2q x} (s_i + s_j) ] d_ij / r_ij   (derivative of Eq.1-3)
 // and the repulsive sum of Eq.2.  Outside the cutoff t = TBSMA_T_OUT makes both exponentials exactly 0.
-template <bool VIRIAL>
+template <bool VIRIAL, bool WRAP = false>
 __device__ __forceinline__ void force_term2(const float4 &pi, const float4 &pa, const float4 &pb, const PairConst &pc,
-                                            AccT &a)
+                                            AccT &a, const WrapC &wc = WrapC())
 {
-    const Pair2 P = pair2(pi, pa, pb, pc);
+    const Pair2 P = pair2<WRAP>(pi, pa, pb, pc, wc);
     const f32x2 ar = fma2(pk(pc.ap, pc.ap), P.t, pk(pc.b_rep, pc.b_rep));
     const f32x2 ab = fma2(pk(pc.aq, pc.aq), P.t, pk(pc.b_band, pc.b_band));
     float ar0, ar1, ab0, ab1;
@@ -896,8 +1123,8 @@ __device__ __forceinline__ double warp_sum_d(double v)
 constexpr int kMaxChunks = (TBSMA_TILE_MAX_RECORDS + 31) / 32 + 1;
 
 // stage 2 (Eq.1-3, Eq.5): forces, per-atom energy, virial, closing half kick, E_kin
-template <bool VIRIAL, bool KICK, bool SPLIT>
-__device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restrict__ cell_start,
+template <bool VIRIAL, bool KICK, bool SPLIT, bool WRAP>
+__device__ __forceinline__ void force_tile(const TileDesc &t, const TileMap &M,
                                            const float4 *__restrict__ xs, const uint2 *__restrict__ nl,
                                            const int *__restrict__ nn, float4 *__restrict__ force, const KickArgs &kk,
                                            int *__restrict__ ctrl, int n_pad, int s_cap, const PairConst &pc,
@@ -909,7 +1136,8 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
     const int lane = threadIdx.x & 31;
     // every CTA leaves its sums (E, E_kin, W): zero if it has nothing to do
     if (threadIdx.x < NQ) my_sums[threadIdx.x] = 0.0;
-    const TileRange r = tile_range(t, cell_start);
+    struct { int lo, hi, nh; } r = {0, M.n_own, M.nh};      // own-local range
+    const WrapC wc = {t.hL[0], t.hL[1], t.hL[2], t.Ls[0], t.Ls[1], t.Ls[2]};
     if (r.hi <= r.lo) return;
     if (r.nh > s_cap) {
         if (threadIdx.x == 0) atomicOr(ctrl + 1, (int)TBSMA_FLAG_TILE_OVERFLOW);
@@ -924,12 +1152,13 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
         if (threadIdx.x == 0) { s_next = cb; s_end = ce; s_begin = cb; }
     }
     const float4 *sm = smem_f4;
-    fill_image(smem_f4, xs, img, r.halo_lo, r.nh);
+    fill_image(smem_f4, xs, img, M);
     bool bad = false;
     for (int ch = next_chunk(&s_next); ch < s_end; ch = next_chunk(&s_next)) {
-        const int i = r.lo + (ch << 5) + lane;
+        const int o = (ch << 5) + lane;
         double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-        if (i < r.hi) {
+        if (o < r.hi) {
+        const int i = map_own(M, o);
         const uint2 *row = nl + tbsma_lrow(i, kg);
         uint2 q0 = make_uint2(0u, 0u), q1 = q0, q2 = q0;
         if (kg >= 3) { q0 = __ldcs(row); q1 = __ldcs(row + TBSMA_LROW); q2 = __ldcs(row + 2 * TBSMA_LROW); }
@@ -943,8 +1172,8 @@ __device__ __forceinline__ void force_tile(const TileDesc &t, const int *__restr
         auto group = [&](const uint2 jj) {
             const float4 p0 = lds_rec(sm, jj.x & 0xffffu), p1 = lds_rec(sm, jj.x >> 16);
             const float4 p2 = lds_rec(sm, jj.y & 0xffffu), p3 = lds_rec(sm, jj.y >> 16);
-            force_term2<VIRIAL>(pi, p0, p1, pc, a);
-            force_term2<VIRIAL>(pi, p2, p3, pc, a);
+            force_term2<VIRIAL, WRAP>(pi, p0, p1, pc, a, wc);
+            force_term2<VIRIAL, WRAP>(pi, p2, p3, pc, a, wc);
         };
         int g = 0;
         for (; g + 3 <= ng; g += 3) {
@@ -1017,9 +1246,16 @@ k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
     const int ti = SPLIT ? (int)blockIdx.x / ls.nsplit : (int)blockIdx.x, part = SPLIT ? (int)blockIdx.x % ls.nsplit : 0;
     const TileDesc t = tiles[ti];
     const int h = list_half(ls, t.rep);
-    force_tile<VIRIAL, KICK, SPLIT>(t, cell_start, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force, kk,
-                             ctrl, n_pad, s_cap, pc, ls.img + (size_t)ti * ls.img_stride, part, ls.nsplit,
-                             cta_sums + 8 * (size_t)blockIdx.x, ls.kg);
+    __shared__ TileMap M;
+    tile_map_build(t, cell_start, M);
+    if (t.Ls[0] != 0.f || t.Ls[1] != 0.f || t.Ls[2] != 0.f)
+        force_tile<VIRIAL, KICK, SPLIT, true>(t, M, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force,
+                                              kk, ctrl, n_pad, s_cap, pc, ls.img + (size_t)ti * ls.img_stride, part,
+                                              ls.nsplit, cta_sums + 8 * (size_t)blockIdx.x, ls.kg);
+    else
+        force_tile<VIRIAL, KICK, SPLIT, false>(t, M, xs, nl + (size_t)h * ls.nl_stride, nn + (size_t)h * ls.n_stride, force,
+                                               kk, ctrl, n_pad, s_cap, pc, ls.img + (size_t)ti * ls.img_stride, part,
+                                               ls.nsplit, cta_sums + 8 * (size_t)blockIdx.x, ls.kg);
 }
 
 // ---- persistent gather kernels ----------------------------------------------------------------------
@@ -1381,8 +1617,8 @@ __device__ __forceinline__ unsigned entry_of(const uint2 *__restrict__ nl, int k
 }
 
 __global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *__restrict__ nl0,
-                                     const int *__restrict__ nn0, const int *__restrict__ hbase,
-                                     const int *__restrict__ tileof, const unsigned short *__restrict__ inv,
+                                     const int *__restrict__ nn0,
+                                     const int *__restrict__ tileof, const int *__restrict__ inv,
                                      int inv_stride, const int *__restrict__ atom_rep, const int *__restrict__ cur,
                                      size_t nl_stride, int *__restrict__ counts, int *__restrict__ list, int n,
                                      int n_pad, int kmax)
@@ -1396,15 +1632,16 @@ __global__ void k_get_neighbors_tile(const int *__restrict__ tag, const uint2 *_
         counts[t] = cnt;
         for (int k = 0; k < cnt; ++k)
             list[(size_t)t * kmax + k] =
-                tag[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, kmax >> 2, i, k) >> 4)]];
+                tag[inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, kmax >> 2, i, k) >> 4)]];
     }
 }
 
 __global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *__restrict__ nl0,
-                                   const int *__restrict__ nn0, const int *__restrict__ hbase,
-                                   const int *__restrict__ tileof, const unsigned short *__restrict__ inv,
+                                   const int *__restrict__ nn0,
+                                   const int *__restrict__ tileof, const int *__restrict__ inv,
                                    int inv_stride, const int *__restrict__ atom_rep, const int *__restrict__ cur,
-                                   size_t nl_stride, unsigned long long *__restrict__ out, int n, int n_pad, float rc2, int kg)
+                                   size_t nl_stride, unsigned long long *__restrict__ out, int n, int n_pad, float rc2, int kg,
+                                   const RepGeom *__restrict__ geom)
 {
     unsigned long long entries = 0, inside = 0;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
@@ -1415,8 +1652,14 @@ __global__ void k_count_pairs_tile(const float4 *__restrict__ pos, const uint2 *
         const int cnt = nn[i] & 0xffff;
         entries += cnt;
         for (int k = 0; k < cnt; ++k) {
-            const float4 pj = pos[hbase[i] + (int)inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, kg, i, k) >> 4)]];
-            const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+            const float4 pj = pos[inv[(size_t)tileof[i] * inv_stride + (entry_of(nl, kg, i, k) >> 4)]];
+            float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+            {   // minimum image as D:A6 (a tile on a periodic boundary lists records from across it)
+                const RepGeom *g = geom + atom_rep[i];
+                if (g->periodic & 1) { const float hl = 0.5f * g->len[0]; if (dx > hl) dx -= g->len[0]; else if (dx < -hl) dx += g->len[0]; }
+                if (g->periodic & 2) { const float hl = 0.5f * g->len[1]; if (dy > hl) dy -= g->len[1]; else if (dy < -hl) dy += g->len[1]; }
+                if (g->periodic & 4) { const float hl = 0.5f * g->len[2]; if (dz > hl) dz -= g->len[2]; else if (dz < -hl) dz += g->len[2]; }
+            }
             const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
             inside += d2 < rc2;
         }
@@ -1486,22 +1729,96 @@ InnerArgs inner_args(const tbsma_ctx *c)
 
 }  // namespace
 
-// Sizes the tiles of every replica from the cells just binned: replica r gets L_r own layers per
-// tile, the largest L <= tile_layers whose halo (L + 2 layers of the replica's most populated
-// layer, + 25 %) fits the shared-memory image.  L_r depends on replica r alone, so a replica is
-// tiled (and therefore summed) identically whatever batch it is part of.  Returns TBSMA_OK and
-// sets active_variant = 2, or leaves active_variant = 1 when a replica does not fit.
+// box shapes tried for a replica whose layers do not fit an image (or that is periodic), best own / halo ratio first
+static const int kBoxCand[][3] = {{3, 3, 3}, {3, 3, 2}, {3, 2, 2}, {2, 2, 2}, {3, 3, 1}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
+constexpr int kNBoxCand = sizeof(kBoxCand) / sizeof(kBoxCand[0]);
+
+// own box b (clipped to the grid) of candidate cand for replica geometry g; false if a periodic axis is too short for it
+// (a tile must not see a cell twice, and must wrap at one end of an axis only: nc >= 2 b + 3)
+static bool box_dims(const RepGeom &g, int cand, int b[3])
+{
+    for (int a = 0; a < 3; ++a) {
+        b[a] = kBoxCand[cand][a] < g.nc[a] ? kBoxCand[cand][a] : g.nc[a];
+        if ((g.periodic >> a & 1) && g.nc[a] < 2 * b[a] + 3) return false;
+    }
+    return true;
+}
+
+namespace {
+// largest halo and own population over the box tiles of replica r for every candidate shape: out[(r * ncand + c) * 2 + {0, 1}]
+__global__ void __launch_bounds__(128)
+k_box_measure(const RepGeom *__restrict__ geom, const int *__restrict__ cell_start, int *__restrict__ out, int ncand)
+{
+    __shared__ int s_max[2];
+    const int r = blockIdx.x, cnd = blockIdx.y;
+    const RepGeom *g = geom + r;
+    if (threadIdx.x < 2) s_max[threadIdx.x] = 0;
+    __syncthreads();
+    const int cand[8][3] = {{3, 3, 3}, {3, 3, 2}, {3, 2, 2}, {2, 2, 2}, {3, 3, 1}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
+    int b[3], nt[3];
+    bool ok = true;
+    for (int a = 0; a < 3; ++a) {
+        b[a] = min(cand[cnd][a], g->nc[a]);
+        if ((g->periodic >> a & 1) && g->nc[a] < 2 * b[a] + 3) ok = false;
+        nt[a] = (g->nc[a] + b[a] - 1) / b[a];
+    }
+    int mh = 0, mo = 0;
+    if (ok) {
+        const int ntile = nt[0] * nt[1] * nt[2];
+        for (int ti = threadIdx.x; ti < ntile; ti += blockDim.x) {
+            const int t3[3] = {ti % nt[0], (ti / nt[0]) % nt[1], ti / (nt[0] * nt[1])};
+            int h0[3], hn[3], o0[3], on[3];
+            for (int a = 0; a < 3; ++a) {
+                o0[a] = t3[a] * b[a];
+                on[a] = min(b[a], g->nc[a] - o0[a]);
+                if (g->periodic >> a & 1) { h0[a] = o0[a] - 1; hn[a] = on[a] + 2; }
+                else { h0[a] = max(o0[a] - 1, 0); hn[a] = min(o0[a] + on[a] + 1, g->nc[a]) - h0[a]; }
+            }
+            int nh = 0, no = 0;
+            for (int z = 0; z < hn[2]; ++z)
+                for (int y = 0; y < hn[1]; ++y)
+                    for (int x = 0; x < hn[0]; ++x) {
+                        const int cx = wrap_cell(h0[0] + x, g->nc[0]), cy = wrap_cell(h0[1] + y, g->nc[1]);
+                        const int cz = wrap_cell(h0[2] + z, g->nc[2]);
+                        const int cc = g->cell_base + (cz * g->nc[1] + cy) * g->nc[0] + cx;
+                        const int pop = cell_start[cc + 1] - cell_start[cc];
+                        nh += pop;
+                        const int ax = h0[0] + x, ay = h0[1] + y, az = h0[2] + z;
+                        if (ax >= o0[0] && ax < o0[0] + on[0] && ay >= o0[1] && ay < o0[1] + on[1] && az >= o0[2] &&
+                            az < o0[2] + on[2])
+                            no += pop;
+                    }
+            mh = max(mh, nh);
+            mo = max(mo, no);
+        }
+    } else {
+        mh = 0x7fffffff;
+    }
+    atomicMax(&s_max[0], mh);
+    atomicMax(&s_max[1], mo);
+    __syncthreads();
+    if (threadIdx.x < 2) out[((size_t)r * ncand + cnd) * 2 + threadIdx.x] = s_max[threadIdx.x];
+}
+}  // namespace
+
+// Sizes the tiles of every replica from the cells just binned.  A thin non-periodic replica (the paper's wires) is cut
+// into runs of whole z-layers (kind 0): L_r own layers per tile, the largest L <= tile_layers whose halo (L + 2 layers of
+// the replica's most populated layer, + 25 %) fits the shared-memory image.  Any other replica (thick wires, periodic
+// bulk) is cut into boxes of cells (kind 1), the shape with the best own / halo ratio whose fullest halo, measured on the
+// cells as they are, fits with 4 % to spare.  The choice depends on replica r alone, so a replica is tiled (and therefore
+// summed) identically whatever batch it is part of.  Returns TBSMA_OK and sets active_variant = 2, or leaves
+// active_variant = 1 when a replica does not fit either way.
 int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
 {
     c->active_variant = 1;
     if (c->variant == 1 || c->n == 0) return TBSMA_OK;
-    if (c->any_periodic || c->kmax_o > 248) return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;
+    if (c->kmax_o > 248 || !c->d_olist) return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;
     const int R = c->R;
     k_layer_maxpop<<<(R + 127) / 128, 128, 0, st>>>(c->d_geom, c->d_cell_start, c->d_maxpop, R);
     c->launches++;
-    int *maxpop = (int *)malloc(sizeof(int) * R);
+    int *maxpop = (int *)malloc(sizeof(int) * 2 * R);
     if (!maxpop) return TBSMA_ENOMEM;
-    cudaError_t e = cudaMemcpyAsync(maxpop, c->d_maxpop, sizeof(int) * R, cudaMemcpyDeviceToHost, st);
+    cudaError_t e = cudaMemcpyAsync(maxpop, c->d_maxpop, sizeof(int) * 2 * R, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { free(maxpop); return TBSMA_ECUDA; }
     const int cap = TBSMA_TILE_MAX_RECORDS;
@@ -1510,17 +1827,16 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     if (lmax > TBSMA_TILE_MAX_LAYERS) lmax = TBSMA_TILE_MAX_LAYERS;
     int64_t n_tiles = 0;
     int cell_cap = 0, rec_cap = 0, own_cap = 0;
-    bool fits = true;
-    int *Lr = (int *)malloc(sizeof(int) * R);
+    bool fits = true, any_box = false;
+    int *Lr = (int *)malloc(sizeof(int) * R);      // > 0: own layers per tile (kind 0); <= 0: -(box candidate) (kind 1)
     if (!Lr) { free(maxpop); return TBSMA_ENOMEM; }
-    for (int r = 0; r < R && fits; ++r) {
+    for (int r = 0; r < R; ++r) {
         const RepGeom &g = c->h_geom[r];
         const int64_t pop = ((int64_t)maxpop[r] * 5 + 3) / 4 + 1;    // + 25 % for later rebuilds
         int L = (int)(cap / pop) - 2;
         if (L > lmax) L = lmax;
-        if (L < 1) { fits = false; break; }
         const int lc = g.nc[0] * g.nc[1];
-        if ((int64_t)(L + 2) * lc + 1 > 8192) { fits = false; break; }
+        if (g.periodic || c->tile_force_box || L < 1 || (int64_t)(L + 2) * lc + 1 > 8192) { Lr[r] = 0; any_box = true; continue; }
         if ((L + 2) * lc + 1 > cell_cap) cell_cap = (L + 2) * lc + 1;
         if ((int)((L + 2) * pop) > rec_cap) rec_cap = (int)((L + 2) * pop);
         if ((int)(L * pop) > own_cap) own_cap = (int)(L * pop);
@@ -1528,11 +1844,52 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         n_tiles += (g.nc[2] + L - 1) / L;
     }
     free(maxpop);
+    if (any_box) {
+        // measure every candidate shape on the cells as they are, take the best that fits
+        int *d_meas = nullptr;
+        const size_t nm = (size_t)R * kNBoxCand * 2;
+        int *meas = (int *)malloc(sizeof(int) * nm);
+        if (!meas) { free(Lr); return TBSMA_ENOMEM; }
+        e = cudaMalloc((void **)&d_meas, sizeof(int) * nm);
+        if (e == cudaSuccess) {
+            k_box_measure<<<dim3(R, kNBoxCand), 128, 0, st>>>(c->d_geom, c->d_cell_start, d_meas, kNBoxCand);
+            c->launches++;
+            e = cudaMemcpyAsync(meas, d_meas, sizeof(int) * nm, cudaMemcpyDeviceToHost, st);
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cudaFree(d_meas);
+        if (e != cudaSuccess) { free(meas); free(Lr); return TBSMA_ECUDA; }
+        for (int r = 0; r < R && fits; ++r) {
+            if (Lr[r] > 0) continue;
+            const RepGeom &g = c->h_geom[r];
+            int pick = -1;
+            for (int cnd = 0; cnd < kNBoxCand && pick < 0; ++cnd) {
+                int b[3];
+                if (!box_dims(g, cnd, b)) continue;
+                int hc = 1;
+                for (int a = 0; a < 3; ++a) hc *= (g.periodic >> a & 1) ? b[a] + 2 : (b[a] + 2 < g.nc[a] ? b[a] + 2 : g.nc[a]);
+                if (hc > TBSMA_TILE_MAX_RUNS || b[0] * b[1] * b[2] > TBSMA_TILE_MAX_OWN_RUNS) continue;
+                const int64_t mh = meas[((size_t)r * kNBoxCand + cnd) * 2];
+                if (mh + mh / 25 + 16 > cap) continue;
+                pick = cnd;
+            }
+            if (pick < 0) { fits = false; break; }
+            Lr[r] = -pick;
+            int b[3];
+            box_dims(g, pick, b);
+            const int mh = meas[((size_t)r * kNBoxCand + pick) * 2], mo = meas[((size_t)r * kNBoxCand + pick) * 2 + 1];
+            if (mh + mh / 25 + 16 > rec_cap) rec_cap = mh + mh / 25 + 16;
+            if (mo + mo / 25 + 16 > own_cap) own_cap = mo + mo / 25 + 16;
+            n_tiles += (int64_t)((g.nc[0] + b[0] - 1) / b[0]) * ((g.nc[1] + b[1] - 1) / b[1]) * ((g.nc[2] + b[2] - 1) / b[2]);
+        }
+        free(meas);
+    }
     if (!fits || n_tiles > 0x7fffffff) {
         free(Lr);
         return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;   // forced tile variant that does not fit
     }
-    TileDesc *h = (TileDesc *)malloc(sizeof(TileDesc) * (size_t)(n_tiles ? n_tiles : 1));
+    c->any_box = any_box ? 1 : 0;
+    TileDesc *h = (TileDesc *)calloc((size_t)(n_tiles ? n_tiles : 1), sizeof(TileDesc));
     int *first = (int *)malloc(sizeof(int) * (size_t)(R + 1));
     if (!h || !first) { free(Lr); free(h); free(first); return TBSMA_ENOMEM; }
     int64_t k = 0;
@@ -1540,21 +1897,56 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         first[r] = (int)k;
         const RepGeom &g = c->h_geom[r];
         const int lc = g.nc[0] * g.nc[1], nz = g.nc[2], L = Lr[r];
-        for (int z0 = 0; z0 < nz; z0 += L) {
-            const int z1 = z0 + L < nz ? z0 + L : nz;
-            const int zh0 = z0 > 0 ? z0 - 1 : 0, zh1 = z1 < nz ? z1 + 1 : nz;
-            TileDesc &t = h[k++];
-            t.rep = r;
-            t.ch0 = g.cell_base + zh0 * lc;
-            t.nlay_h = zh1 - zh0;
-            t.own_first = z0 - zh0;
-            t.own_n = z1 - z0;
-            t.layer_cells = lc;
-            t.nx = g.nc[0]; t.ny = g.nc[1]; t.nz = nz;
-            t.z_h0 = zh0;
-            t.cell_base = g.cell_base;
-            t.pad = 0;
+        if (L > 0) {
+            for (int z0 = 0; z0 < nz; z0 += L) {
+                const int z1 = z0 + L < nz ? z0 + L : nz;
+                const int zh0 = z0 > 0 ? z0 - 1 : 0, zh1 = z1 < nz ? z1 + 1 : nz;
+                TileDesc &t = h[k++];
+                t.rep = r;
+                t.kind = 0;
+                t.first_of_rep = z0 == 0;
+                t.ch0 = g.cell_base + zh0 * lc;
+                t.nlay_h = zh1 - zh0;
+                t.own_first = z0 - zh0;
+                t.own_n = z1 - z0;
+                t.layer_cells = lc;
+                t.nx = g.nc[0]; t.ny = g.nc[1]; t.nz = nz;
+                t.z_h0 = zh0;
+                t.cell_base = g.cell_base;
+                for (int a = 0; a < 3; ++a) { t.Ls[a] = 0.f; t.hL[a] = INFINITY; }
+            }
+            continue;
         }
+        int b[3];
+        box_dims(g, -L, b);
+        const int64_t k0 = k;
+        for (int oz = 0; oz < g.nc[2]; oz += b[2])
+            for (int oy = 0; oy < g.nc[1]; oy += b[1])
+                for (int ox = 0; ox < g.nc[0]; ox += b[0]) {
+                    TileDesc &t = h[k++];
+                    t.rep = r;
+                    t.kind = 1;
+                    t.first_of_rep = k - 1 == k0;
+                    t.cell_base = g.cell_base;
+                    t.nx = g.nc[0]; t.ny = g.nc[1]; t.nz = g.nc[2];
+                    const int o[3] = {ox, oy, oz};
+                    for (int a = 0; a < 3; ++a) {
+                        const int on = b[a] < g.nc[a] - o[a] ? b[a] : g.nc[a] - o[a];
+                        int h0, hn;
+                        t.Ls[a] = 0.f;
+                        t.hL[a] = INFINITY;
+                        if (g.periodic >> a & 1) {
+                            h0 = o[a] - 1;
+                            hn = on + 2;
+                            if (h0 < 0) { t.Ls[a] = g.len[a]; t.hL[a] = 0.5f * g.len[a]; }                    // lower end
+                            else if (h0 + hn > g.nc[a]) { t.Ls[a] = -g.len[a]; t.hL[a] = 0.5f * g.len[a]; }   // upper end
+                        } else {
+                            h0 = o[a] > 0 ? o[a] - 1 : 0;
+                            hn = (o[a] + on + 1 < g.nc[a] ? o[a] + on + 1 : g.nc[a]) - h0;
+                        }
+                        t.h0[a] = (short)h0; t.hn[a] = (short)hn; t.o0[a] = (short)(o[a] - h0); t.on[a] = (short)on;
+                    }
+                }
     }
     first[R] = (int)k;
     free(Lr);
@@ -1578,7 +1970,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     if (e == cudaSuccess) e = ensure((void **)&c->d_tile_first, &c->have_first, sizeof(int) * (size_t)(R + 1));
     if (e == cudaSuccess) e = ensure((void **)&c->d_work, &c->have_work, sizeof(int) * (size_t)(2 + 2 * n_tiles));
     if (e == cudaSuccess) e = ensure((void **)&c->d_img, &c->have_img, sizeof(unsigned short) * nt1 * new_tile_cap);
-    if (e == cudaSuccess) e = ensure((void **)&c->d_inv, &c->have_inv, sizeof(unsigned short) * nt1 * new_img_cap);
+    if (e == cudaSuccess) e = ensure((void **)&c->d_inv, &c->have_inv, sizeof(int) * nt1 * new_img_cap);
     // Few tiles (one or a few small wires): several CTAs share a tile, each filling the image and taking a share of the
     // 32-atom chunks, until the CTAs fill the GPU about twice (or every CTA is down to one chunk).
     int nsplit = 1;
@@ -1678,7 +2070,7 @@ cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int3
     sa.s_cap = c->tile_cap; sa.cell_cap = c->tile_cell_cap;
     FinishArgs fa;
     fa.cell_start = c->d_cell_start; fa.nl_tmp = ol_tmp; fa.nn_tmp = c->d_nn_tmp; fa.newslot = c->d_newslot;
-    fa.oldof = c->d_oldof; fa.nl = ol; fa.nn = c->d_nn_o; fa.hbase = c->d_hbase; fa.tileof = c->d_tileof;
+    fa.oldof = c->d_oldof; fa.nl = ol; fa.nn = c->d_nn_o; fa.tileof = c->d_tileof;
     fa.img = c->d_img; fa.img_stride = c->tile_cap; fa.n_pad = c->n_pad; fa.kg_o = c->kmax_o / 4;
     fa.s_cap = c->tile_cap;
     PlaceArgs pa;
@@ -1750,7 +2142,7 @@ static ListSel list_sel(const tbsma_ctx *c, int sync_level)
 // a handful of tiles (one small wire) is quicker with one short-lived CTA per part of a tile
 static bool use_persist(const tbsma_ctx *c)
 {
-    return c->gather_mode != 0 && c->persist_ok && (c->p_nb_req > 0 || c->n_tiles >= 4 * c->n_sm);
+    return c->gather_mode != 0 && c->persist_ok && !c->any_box && (c->p_nb_req > 0 || c->n_tiles >= 4 * c->n_sm);
 }
 
 static PArgs persist_args(tbsma_ctx *c, int pass, const float4 *src, int sync_level)
@@ -1866,7 +2258,7 @@ cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, in
                                             cudaStream_t st)
 {
     k_get_neighbors_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(tag, reinterpret_cast<const uint2 *>(c->d_nlist),
-                                                                   c->d_nn, c->d_hbase, c->d_tileof, c->d_inv, c->img_cap,
+                                                                   c->d_nn, c->d_tileof, c->d_inv, c->img_cap,
                                                                    c->d_atom_rep, c->d_cur,
                                                                    (size_t)(c->kmax / 4) * c->n_pad, counts, list, (int)c->n,
                                                                    c->n_pad, c->kmax);
@@ -1878,10 +2270,10 @@ cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsig
                                           cudaStream_t st)
 {
     k_count_pairs_tile<<<grid_for(c, c->n, 256, 8), 256, 0, st>>>(pos, reinterpret_cast<const uint2 *>(c->d_nlist),
-                                                                 c->d_nn, c->d_hbase, c->d_tileof, c->d_inv, c->img_cap,
+                                                                 c->d_nn, c->d_tileof, c->d_inv, c->img_cap,
                                                                  c->d_atom_rep, c->d_cur,
                                                                  (size_t)(c->kmax / 4) * c->n_pad, d_out2, (int)c->n, c->n_pad,
-                                                                 c->pc.rc2, c->kmax / 4);
+                                                                 c->pc.rc2, c->kmax / 4, c->d_geom);
     c->launches++;
     return cudaGetLastError();
 }
