@@ -180,6 +180,8 @@ def main():
                          "the timed region should see the steady rebuild cadence, not that transient")
     ap.add_argument("--outer-skin", type=float, default=None,
                     help="buffer radius S of the candidate lists of the tile variant (tbsma_set_outer_skin; library default if omitted)")
+    ap.add_argument("--variant", type=int, default=None,
+                    help="tbsma_set_variant: 0 = automatic (library default), 1 = global gather, 2 = shared-memory tiles")
     ap.add_argument("--gather", type=int, default=None,
                     help="tbsma_set_gather: 1 = persistent gather kernels (library default), 0 = one CTA per tile")
     ap.add_argument("--plain-graph", action="store_true",
@@ -242,6 +244,8 @@ def main():
         ctx.set_outer_skin(args.outer_skin)
     if args.gather is not None:
         ctx.set_gather(args.gather)
+    if args.variant is not None:
+        ctx.set_variant(args.variant)
     st = B.DeviceState(w, dev)
     stream = torch.cuda.Stream(device=dev)
     K, Wm, P0 = args.steps, args.warmup, max(args.preroll, 0)

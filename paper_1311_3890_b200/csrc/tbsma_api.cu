@@ -150,7 +150,7 @@ int set_geometry(tbsma_ctx *c, double width)
 // variant with its own, narrower cells.
 bool tiles_possible(const tbsma_ctx *c)
 {
-    if (c->variant == 1) return false;
+    if (c->variant == 1 || (c->variant == 0 && c->tiles_rejected)) return false;
     const double w_min = (c->r_cut + c->skin + c->outer_skin) * (1.0 + 1e-5) + 1e-4;
     for (int r = 0; r < c->R; ++r)
         for (int a = 0; a < 3; ++a)
@@ -403,6 +403,7 @@ int tbsma_set_variant(tbsma_ctx *c, int32_t variant)
 {
     if (!c || variant < 0 || variant > 2) return TBSMA_EINVAL;
     c->epoch++;
+    c->tiles_rejected = 0;
     c->variant = variant;
     c->cells_built = c->list_built = 0;   // lists must be rebuilt for the new variant
     return TBSMA_OK;
@@ -416,6 +417,7 @@ int tbsma_set_tile(tbsma_ctx *c, int32_t layers_per_tile, int32_t threads)
         (threads & 31))
         return TBSMA_EINVAL;
     c->epoch++;
+    c->tiles_rejected = 0;
     c->tile_layers = layers_per_tile;
     c->tile_threads = threads;
     c->cells_built = c->list_built = 0;
@@ -426,6 +428,7 @@ int tbsma_set_tile_split(tbsma_ctx *c, int32_t ctas_per_tile)
 {
     if (!c || ctas_per_tile < 0 || ctas_per_tile > 128) return TBSMA_EINVAL;
     c->epoch++;
+    c->tiles_rejected = 0;
     c->tile_split_req = ctas_per_tile;
     c->cells_built = c->list_built = 0;
     return TBSMA_OK;
@@ -435,6 +438,7 @@ int tbsma_set_tile_box(tbsma_ctx *c, int32_t force)
 {
     if (!c) return TBSMA_EINVAL;
     c->epoch++;
+    c->tiles_rejected = 0;
     c->tile_force_box = force != 0;
     c->cells_built = c->list_built = 0;
     return TBSMA_OK;
@@ -454,6 +458,7 @@ int tbsma_set_outer_skin(tbsma_ctx *c, double outer_skin)
 {
     if (!c || !(outer_skin >= 0.0) || !(outer_skin <= 16.0)) return TBSMA_EINVAL;
     c->epoch++;
+    c->tiles_rejected = 0;
     if (c->d_olist) {
         cudaDeviceSynchronize();
         cudaFree(c->d_tile_first); cudaFree(c->d_work);
@@ -630,6 +635,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
         max_neighbors < 1 || max_neighbors > 4096)
         return TBSMA_EINVAL;
     c->epoch++;
+    c->tiles_rejected = 0;
     if (h_off[0] != 0 || h_off[n_replicas] != n_atoms) return TBSMA_EINVAL;
     for (int r = 0; r < n_replicas; ++r)
         if (h_off[r + 1] < h_off[r]) return TBSMA_EINVAL;
@@ -740,6 +746,16 @@ int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, 
     CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, true, false, st));
     const int rc = tbsma_tile_setup(c, st);   // picks the gather variant for these cells (synchronises)
     if (rc) return rc;
+    if (c->active_variant == 1 && c->cell_w != c->r_cut + c->skin) {
+        // the tiles were tried and not taken: the global variant wants its own, narrower cells (fewer candidates per atom
+        // in its list build), so bin once more
+        c->tiles_rejected = 1;      // (remembered until the system or a tile setting changes: later builds bin once)
+        CK(cudaStreamSynchronize(st));
+        const int rg = set_geometry(c, c->r_cut + c->skin);
+        if (rg) return rg;
+        CK(tbsma_launch_mark_all_dirty(c, st));
+        CK(tbsma_launch_rebuild(c, (float4 *)d_pos, (float4 *)d_vel, d_tag, true, false, st));
+    }
     c->cells_built = 1;
     return TBSMA_OK;
 }

@@ -136,6 +136,7 @@ struct tbsma_ctx {
     int tile_split_req;    // requested by tbsma_set_tile_split (0 = automatic)
     int tile_force_box;    // tbsma_set_tile_box: box tiles even for replicas whose layers would fit (tests)
     int any_box;           // some replica is cut into box tiles (kind 1)
+    int tiles_rejected;    // variant 0: the tiles were tried for this system and the global variant taken instead
     double *d_cta_sums;    // n_tiles x tile_nsplit x 8: E, E_kin, W (xx yy zz xy xz yz) of every CTA of the force pass
     // persistent gather kernels: units = p_plain whole tiles, then the remaining tiles in p_S parts each
     int gather_mode;       // 1 (default): persistent kernels (k_gather_persist); 0: one CTA per tile (or part of a tile)

@@ -1888,6 +1888,11 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         free(Lr);
         return c->variant == 2 ? TBSMA_EINVAL : TBSMA_OK;   // forced tile variant that does not fit
     }
+    // A box tile stages eight halo records per own atom (a wire's layer tile: two and a half) and holds few chunks of
+    // work; measured, box tiles beat the global gather on the 10^6-atom periodic block (2 197 tiles: 1.92 against 1.74 G
+    // atom-steps/s) and lose to it on the 165 000-atom thick wire (882 tiles: 1.18 against 1.77 G).  Left to itself
+    // (variant 0) the library takes them for large batches only.
+    if (c->variant == 0 && any_box && n_tiles < 8 * (int64_t)c->n_sm) { free(Lr); return TBSMA_OK; }
     c->any_box = any_box ? 1 : 0;
     TileDesc *h = (TileDesc *)calloc((size_t)(n_tiles ? n_tiles : 1), sizeof(TileDesc));
     int *first = (int *)malloc(sizeof(int) * (size_t)(R + 1));
@@ -1978,7 +1983,8 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         const int slots = 8 * c->n_sm;
         int est_chunks = (own_cap * 4 / 5 + 31) / 32;     // own_cap carries 25 % headroom
         if (est_chunks < 1) est_chunks = 1;
-        if (n_tiles > 0 && n_tiles < slots) nsplit = (int)((slots + n_tiles - 1) / n_tiles);
+        // (box tiles hold few chunks and cost a large image each: they are split only when there are very few of them)
+        if (n_tiles > 0 && n_tiles < (any_box ? slots / 4 : slots)) nsplit = (int)((slots + n_tiles - 1) / n_tiles);
         if (nsplit > est_chunks) nsplit = est_chunks;
         if (c->tile_split_req > 0) nsplit = c->tile_split_req;
         if (nsplit < 1) nsplit = 1;
