@@ -349,8 +349,8 @@ def main():
         except Exception:
             pass
     roofline["note"] = ("HBM is the designated roofline (BASELINE.json); with 16-bit lists the gather passes move less than "
-                        "the algorithmic bytes and are bound by the shared-memory data pipe and the MUFU pipe "
-                        "(profiles/r1e_ncu_full_summary.md)")
+                        "the algorithmic bytes and are bound on chip: MUFU, shared-memory data pipe and issue slots at "
+                        "55-75 % each (profiles/r2_ncu_full_summary.md)")
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -361,7 +361,7 @@ def main():
         hf = torch.zeros_like(hp).pin_memory()
         ht = torch.arange(w.n_atoms, dtype=torch.int32).pin_memory()
         he, hk = np.zeros(w.n_replicas), np.zeros(w.n_replicas)
-        k2 = max(10, K // 3)
+        k2 = max(10, K)              # one call of the end-to-end entry point integrates as many steps as the timed region
         # warm-up call (allocates the staging buffers, instantiates the graph)
         ctx2.md_run_host(hp.numpy(), hv.numpy(), hf.numpy(), ht.numpy(), w.dt, w.T, w.gamma, w.seed, 0, 8, None,
                          w.slab_rate, w.rebuild_every, he, None, hk)
@@ -408,6 +408,7 @@ def main():
                        "mean_list_length": n_l, "mean_steps_between_rebuilds": k_eff,
                        "l2": "inputs larger than L2 (index list %.0f MB per pass)" % (entries * 4 / 1e6),
                        "variant": {1: "global gather (int32 list)", 2: "shared-memory tiles (u16 lists)"}.get(ctx.get_variant()),
+                       "gather_kernels": ctx.describe_gather(),
                        "list_renewal": "asynchronous, margin 0.03 A, beside the gather passes (density pass = programmatic dependent of the filter kernel)" if ctx.get_variant() == 2 and not w.rebuild_every else "ahead of the gather passes",
                        "graph": "plain" if args.plain_graph else "conditional node around the cells+candidates chain",
                        "preroll_steps": P0,

@@ -189,6 +189,10 @@ int tbsma_get_stats(tbsma_ctx *ctx, tbsma_stats *h_out); /* synchronises */
  * tbsma_get_variant returns the variant the current lists were built for. */
 int tbsma_set_variant(tbsma_ctx *ctx, int32_t variant);
 int tbsma_get_variant(const tbsma_ctx *ctx);
+/* What the current lists were built for (each pointer may be NULL): number of tiles (0 under the global variant), whether
+ * some replica is cut into boxes of cells rather than layers (tbsma_set_tile_box), whether the gather passes run as
+ * persistent kernels (tbsma_set_gather). */
+int tbsma_get_tiling(const tbsma_ctx *ctx, int32_t *n_tiles, int32_t *box_tiles, int32_t *persistent);
 
 /* Shared-memory variant: buffer radius S of the CANDIDATE list (default 2.5 A).  The cell scan collects every
  * pair within r_cut + skin + S, once; while no atom has moved more than S/2 since then, the replica's list

@@ -1280,6 +1280,11 @@ struct PShared {
     unsigned long long full[kPMaxBuf];   // mbarriers: image + slot description of the buffer are in place
     PSlot slot[kPMaxBuf];
     int next[kPMaxBuf], done[kPMaxBuf];
+    // the unit that comes to a buffer next, claimed and described by the FIRST warp that leaves the current one (the chain
+    // claim -> tile -> cell_start -> list half is three dependent round trips to memory, off the filling warp's path)
+    PSlot pend[kPMaxBuf];
+    int pend_tile[kPMaxBuf], pend_hlo[kPMaxBuf], pend_nh[kPMaxBuf];
+    volatile int pend_ok[kPMaxBuf];
     int ended;
 };
 constexpr int kPThreads = 512;
@@ -1310,8 +1315,9 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity
     const unsigned a = smem_u32(b);
     unsigned ok;
     do {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        // (may suspend the thread for up to the hinted time instead of spinning through the issue slots)
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(a), "r"(parity), "r"(2000u) : "memory");
     } while (!ok);
 }
 
@@ -1397,7 +1403,7 @@ k_gather_persist(const PArgs A)
     if (blockIdx.x == 0 && threadIdx.x == 0) *A.claim_other = 0;
     // ---- prologue: units blockIdx.x and blockIdx.x + G, both images filled by everybody
     if (threadIdx.x == 0) {
-        for (int b = 0; b < NB; ++b) mbar_init(&sh.full[b], 33);
+        for (int b = 0; b < NB; ++b) { mbar_init(&sh.full[b], 33); sh.pend_ok[b] = 0; }
         sh.ended = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -1448,14 +1454,15 @@ k_gather_persist(const PArgs A)
             continue;
         }
         if (round >= 1) mbar_wait(&sh.full[b], (unsigned)((round - 1) & 1));
-        const PSlot S = sh.slot[b];
+        // (the unit's description stays in shared memory: the chunk loops have no register to spare)
+        const volatile PSlot &S = sh.slot[b];
         if (S.tile < 0) { dead |= 1u << b; continue; }
         const float4 *sm = smem_f4 + (size_t)b * A.img_cap;
-        const uint2 *__restrict__ nl = A.nl + (size_t)S.half * A.ls.nl_stride;
-        const int *__restrict__ nn = A.nn + (size_t)S.half * A.ls.n_stride;
-        double *part = s_part + (size_t)b * NQ * A.U.max_chunks;
         for (int ch = next_chunk(&sh.next[b]); ch < S.ce; ch = next_chunk(&sh.next[b])) {
             const int i = S.lo + (ch << 5) + lane;
+            const uint2 *__restrict__ nl = A.nl + (size_t)S.half * A.ls.nl_stride;
+            const int *__restrict__ nn = A.nn + (size_t)S.half * A.ls.n_stride;
+            double *part = s_part + (size_t)b * NQ * A.U.max_chunks;
             if (PASS == 0) {
                 if (i >= S.hi) continue;
                 // own record, count and the first three rows in ONE round trip: the rows are read whatever the count is (they
@@ -1493,12 +1500,15 @@ k_gather_persist(const PArgs A)
                 double se = 0.0, sk = 0.0, sw[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
                 if (i < S.hi) {
                     const uint2 *row = nl + tbsma_lrow(i, A.ls.kg);
+                    // FOUR rows in flight here (the density pass: three): the returning rows queue behind the shared-memory
+                    // gathers on the load / store data path, and the force pass has the longer queue
                     uint2 q0 = __ldcs(row), q1 = __ldcs(row + TBSMA_LROW), q2 = __ldcs(row + 2 * TBSMA_LROW);
+                    uint2 q3 = __ldcs(row + 3 * TBSMA_LROW);
                     const float4 pi = A.src[i];
                     const int nni = nn[i];
                     if (KICK) asm volatile("prefetch.global.L2 [%0];" ::"l"(A.kk.vel + i));   // read at the end of the chunk
                     const int ng = ((nni & 0xffff) + 3) >> 2;
-                    if (ng < 3) { q2 = make_uint2(0u, 0u); if (ng < 2) q1 = q2; if (ng < 1) q0 = q2; }
+                    if (ng < 4) { q3 = make_uint2(0u, 0u); if (ng < 3) q2 = q3; if (ng < 2) q1 = q3; if (ng < 1) q0 = q3; }
                     const f32x2 z2 = pk(0.f, 0.f);
                     AccT a = {z2, z2, z2, z2, z2, z2, z2, z2, z2, z2};
                     auto group = [&](const uint2 jj) {
@@ -1508,14 +1518,16 @@ k_gather_persist(const PArgs A)
                         force_term2<VIRIAL>(pi, p2, p3, A.pc, a);
                     };
                     int g = 0;
-                    for (; g + 3 <= ng; g += 3) {
-                        group(q0); q0 = ld_row(row, g + 3, ng, A.n_pad);
-                        group(q1); q1 = ld_row(row, g + 4, ng, A.n_pad);
-                        group(q2); q2 = ld_row(row, g + 5, ng, A.n_pad);
+                    for (; g + 4 <= ng; g += 4) {
+                        group(q0); q0 = ld_row(row, g + 4, ng, A.n_pad);
+                        group(q1); q1 = ld_row(row, g + 5, ng, A.n_pad);
+                        group(q2); q2 = ld_row(row, g + 6, ng, A.n_pad);
+                        group(q3); q3 = ld_row(row, g + 7, ng, A.n_pad);
                     }
                     if (g < ng) {
                         group(q0);
                         if (g + 1 < ng) group(q1);
+                        if (g + 2 < ng) group(q2);
                     }
                     const float fx = sum2(a.fx), fy = sum2(a.fy), fz = sum2(a.fz);
                     const float sqrt_rho = pi.w > 0.f ? 1.0f / pi.w : 0.f;
@@ -1559,13 +1571,30 @@ k_gather_persist(const PArgs A)
         int last = 0;
         if (lane == 0) {
             __threadfence_block();
-            last = atomicAdd(&sh.done[b], 1) == kPWarps - 1 ? 1 : 0;
+            const int cnt = atomicAdd(&sh.done[b], 1);
+            last = cnt == kPWarps - 1 ? 1 : 0;
+            if (cnt == 0) {      // first out: claim and describe the unit that comes to this buffer next
+                int u = -1;
+                if (!sh.ended) {
+                    u = atomicAdd(A.claim, 1) + NB * G;
+                    if (u >= A.U.n_units) { u = -1; sh.ended = 1; }
+                }
+                PSlot N;
+                N.tile = -1; N.lo = N.hi = N.cb = N.ce = N.half = N.sums = N.pad = 0;
+                int tile = -1, hlo = 0, nh = 0;
+                if (u >= 0 && !pslot_describe(N, A.U, u, A.tiles, A.cell_start, A.ls, A.s_cap, A.ctrl, tile, hlo, nh)) nh = 0;
+                sh.pend[b] = N;
+                sh.pend_tile[b] = tile; sh.pend_hlo[b] = hlo; sh.pend_nh[b] = tile < 0 ? 0 : nh;
+                __threadfence_block();
+                sh.pend_ok[b] = 1;
+            }
         }
         last = __shfl_sync(0xffffffffu, last, 0);
         if (!last) continue;
         __threadfence_block();
         if (PASS == 1) {      // the unit's sums: chunks in chunk order (lane l takes chunks l, l + 32, ...; then a fixed tree)
             double *my_sums = A.cta_sums + 8 * (size_t)S.sums;
+            double *part = s_part + (size_t)b * NQ * A.U.max_chunks;
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
                 double v = 0.0;
@@ -1574,17 +1603,13 @@ k_gather_persist(const PArgs A)
                 if (lane == 0) my_sums[q] = v;
             }
         }
-        int u = -1;
-        if (lane == 0 && !sh.ended) {
-            u = atomicAdd(A.claim, 1) + NB * G;
-            if (u >= A.U.n_units) { u = -1; sh.ended = 1; }
-        }
-        u = __shfl_sync(0xffffffffu, u, 0);
         int tile = -1, hlo = 0, nh = 0;
         if (lane == 0) {
-            PSlot N;
-            N.tile = -1; N.lo = N.hi = N.cb = N.ce = N.half = N.sums = N.pad = 0;
-            if (u >= 0 && !pslot_describe(N, A.U, u, A.tiles, A.cell_start, A.ls, A.s_cap, A.ctrl, tile, hlo, nh)) nh = 0;
+            while (!sh.pend_ok[b]) { }       // (the first warp out left long ago)
+            __threadfence_block();
+            const PSlot N = sh.pend[b];
+            tile = sh.pend_tile[b]; hlo = sh.pend_hlo[b]; nh = sh.pend_nh[b];
+            sh.pend_ok[b] = 0;
             sh.slot[b] = N;
             sh.next[b] = N.cb;
             sh.done[b] = 0;
@@ -1592,7 +1617,6 @@ k_gather_persist(const PArgs A)
         tile = __shfl_sync(0xffffffffu, tile, 0);
         hlo = __shfl_sync(0xffffffffu, hlo, 0);
         nh = __shfl_sync(0xffffffffu, nh, 0);
-        if (tile < 0) nh = 0;
         fill_image_async(smem_f4 + (size_t)b * A.img_cap, A.src, A.ls.img + (size_t)(tile < 0 ? 0 : tile) * A.ls.img_stride, hlo, nh, &sh.full[b]);
         if (lane == 0) mbar_arrive(&sh.full[b]);       // releases the slot description written above
     }
@@ -2055,7 +2079,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         TBSMA_ATTR((k_gather_persist<1, false, false>), sm_p1); TBSMA_ATTR((k_gather_persist<1, false, true>), sm_p1);
         TBSMA_ATTR((k_gather_persist<1, true, false>), sm_p1v); TBSMA_ATTR((k_gather_persist<1, true, true>), sm_p1v);
 #undef TBSMA_ATTR
-        c->persist_ok = sm_p1v <= 112 * 1024 && c->kmax >= 12;     // two CTAs per SM; three rows per atom exist
+        c->persist_ok = sm_p1v <= 112 * 1024 && c->kmax >= 16;     // two CTAs per SM; four rows per atom exist
     }
     if (e != cudaSuccess) return TBSMA_ECUDA;
     c->active_variant = 2;
@@ -2282,4 +2306,15 @@ cudaError_t tbsma_launch_count_pairs_tile(tbsma_ctx *c, const float4 *pos, unsig
                                                                  c->pc.rc2, c->kmax / 4, c->d_geom);
     c->launches++;
     return cudaGetLastError();
+}
+
+// what the current lists were built for (bench.py and the tests report it)
+extern "C" int tbsma_get_tiling(const tbsma_ctx *c, int32_t *n_tiles, int32_t *box_tiles, int32_t *persistent)
+{
+    if (!c) return TBSMA_EINVAL;
+    const bool tiles = c->active_variant == 2;
+    if (n_tiles) *n_tiles = tiles ? c->n_tiles : 0;
+    if (box_tiles) *box_tiles = tiles ? c->any_box : 0;
+    if (persistent) *persistent = tiles && use_persist(c) ? 1 : 0;
+    return TBSMA_OK;
 }
