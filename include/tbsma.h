@@ -220,6 +220,14 @@ int tbsma_set_tile_split(tbsma_ctx *ctx, int32_t ctas_per_tile);
  * next tbsma_build_cells. */
 int tbsma_set_tile_box(tbsma_ctx *ctx, int32_t force);
 
+/* Small batches of the shared-memory variant (every tile, or part of a tile, resident on the GPU at once: one wire, a few
+ * wires): inside tbsma_md_run's captured step the WHOLE step -- integration, density pass, force pass with the closing
+ * kick, per-replica sums, bookkeeping -- is one cooperative kernel with three grid-wide barriers in place of five kernel
+ * boundaries (the paper's "+35 % run time due to thread synchronization" between its two stages, is this cost).
+ * A step in which a replica needs a new list runs the separate kernels instead (decided on the device).  enable = 0:
+ * always the separate kernels.  Default 1.  Changes cost, never results (same operations in the same order). */
+int tbsma_set_fused_step(tbsma_ctx *ctx, int32_t enable);
+
 /* Shared-memory variant: how the two gather passes (P:59 stages 1 and 2) are launched.
  *   1 (default) = persistent kernels: two CTAs of 16 warps per SM work through the tiles of the batch, each holding the
  *       image of its NEXT tile while it works on the current one; warps move on to the next tile without a CTA-wide

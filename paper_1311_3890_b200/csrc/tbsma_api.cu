@@ -242,6 +242,39 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
                 use_cond = cudaGraphConditionalHandleCreate(&cond, cg, 0, cudaGraphCondAssignDefault) == cudaSuccess;
         }
         if (nose_hoover) CK(tbsma_launch_nose_hoover(c, pos, vel, force, a, dt, st));
+        if (tiles && use_cond && !ev && tbsma_step_small_ok(c)) {
+            // Small batch: the whole step is ONE cooperative kernel (k_step_small).  Only when the displacement check in it
+            // finds a replica that needs a new list is the rest of the step run by the ordinary kernels, the body of an IF.
+            const int sync_level_f = async ? 2 : 1;
+            CK(tbsma_launch_step_small(c, pos, vel, force, tag, a, kk, w_rep != nullptr, (advance ? 1 : 0) | 2,
+                                       tbsma_tile_sums(c, e_rep, ekin, w_rep), (unsigned long long)cond, st));
+            CK(cudaStreamGetCaptureInfo(st, &cap, nullptr, &cg, &deps, &n_deps));
+            cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+            np.type = cudaGraphNodeTypeConditional;
+            np.conditional.handle = cond;
+            np.conditional.type = cudaGraphCondTypeIf;
+            np.conditional.size = 1;
+            cudaGraphNode_t cnode;
+            CK(cudaGraphAddNode(&cnode, cg, deps, n_deps, &np));
+            cudaGraph_t body = np.conditional.phGraph_out[0];
+            cudaStream_t bs = c->body_stream;
+            CK(cudaStreamBeginCaptureToGraph(bs, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+            const int64_t before = c->launches;
+            cudaError_t eb = tbsma_launch_tile_worklist(c, bs, 0ull, 0);
+            if (eb == cudaSuccess) eb = tbsma_launch_rebuild(c, pos, vel, tag, true, true, bs);
+            if (eb == cudaSuccess) eb = tbsma_launch_tile_inner(c, pos, 1, bs);
+            if (eb == cudaSuccess) eb = tbsma_launch_tile_inner(c, pos, 0, bs);
+            if (eb == cudaSuccess) eb = tbsma_launch_density_tile(c, pos, sync_level_f, bs, false);
+            if (eb == cudaSuccess) eb = tbsma_launch_force_tile(c, force, w_rep != nullptr, kk, sync_level_f, bs);
+            if (eb == cudaSuccess) eb = tbsma_launch_finish_step(c, (advance ? 1 : 0) | 2, bs, tbsma_tile_sums(c, e_rep, ekin, w_rep));
+            c->launches = before;      // (the body runs in the few steps that renew a list)
+            cudaGraph_t body_out = nullptr;
+            CK(cudaStreamEndCapture(bs, &body_out));
+            CK(eb);
+            CK(cudaStreamUpdateCaptureDependencies(st, &cnode, 1, cudaStreamSetCaptureDependencies));
+            if (series) CK(tbsma_launch_series_record(c, pos, vel, w_rep, a, st));
+            continue;
+        }
         CK(tbsma_launch_integrate_pre(c, pos, vel, force, tag, a, st));
         if (ev) CK(cudaEventRecord(ev[1], st));
         bool forked = false, early = false, joined = false;
@@ -351,6 +384,7 @@ int tbsma_create(const tbsma_params *params, double r_cut, double skin, tbsma_ct
     c->tile_layers = 2;
     c->tile_threads = 256;
     c->gather_mode = 1;
+    c->fused_step = 1;
     c->use_graph = 1;
     c->overlap = 2;
     c->stagger = 1;
@@ -384,6 +418,7 @@ int tbsma_destroy(tbsma_ctx *c)
 {
     if (!c) return TBSMA_EINVAL;
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->graph_exec_multi) cudaGraphExecDestroy(c->graph_exec_multi);
     free_system(c);
     free_staging(c);
     if (c->own_stream) cudaStreamDestroy(c->own_stream);
@@ -444,6 +479,16 @@ int tbsma_set_tile_box(tbsma_ctx *c, int32_t force)
     return TBSMA_OK;
 }
 
+int tbsma_set_fused_step(tbsma_ctx *c, int32_t enable)
+{
+    if (!c) return TBSMA_EINVAL;
+    c->epoch++;
+    c->fused_step = enable != 0;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph_exec_multi) { cudaGraphExecDestroy(c->graph_exec_multi); c->graph_exec_multi = nullptr; }
+    return TBSMA_OK;
+}
+
 int tbsma_set_gather(tbsma_ctx *c, int32_t mode)
 {
     if (!c || mode < 0 || mode > 4) return TBSMA_EINVAL;
@@ -479,6 +524,7 @@ int tbsma_set_graph(tbsma_ctx *c, int32_t enable)
     c->use_graph = enable != 0;
     c->use_cond = enable != 1;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph_exec_multi) { cudaGraphExecDestroy(c->graph_exec_multi); c->graph_exec_multi = nullptr; }
     return TBSMA_OK;
 }
 
@@ -582,6 +628,7 @@ int tbsma_set_async(tbsma_ctx *c, int32_t enable, double margin)
     c->async_inner = enable != 0;
     c->async_margin = margin;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph_exec_multi) { cudaGraphExecDestroy(c->graph_exec_multi); c->graph_exec_multi = nullptr; }
     return TBSMA_OK;
 }
 
@@ -591,6 +638,7 @@ int tbsma_set_overlap(tbsma_ctx *c, int32_t enable)
     c->epoch++;
     c->overlap = enable;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph_exec_multi) { cudaGraphExecDestroy(c->graph_exec_multi); c->graph_exec_multi = nullptr; }
     return TBSMA_OK;
 }
 
@@ -640,6 +688,7 @@ int tbsma_set_system(tbsma_ctx *c, int64_t n_atoms, int32_t n_replicas, const in
     for (int r = 0; r < n_replicas; ++r)
         if (h_off[r + 1] < h_off[r]) return TBSMA_EINVAL;
     if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph_exec_multi) { cudaGraphExecDestroy(c->graph_exec_multi); c->graph_exec_multi = nullptr; }
     free_system(c);
     const int R = n_replicas;
     c->n = n_atoms;
@@ -733,7 +782,8 @@ int tbsma_build_cells(tbsma_ctx *c, float *d_pos, float *d_vel, int32_t *d_tag, 
     if (c->n == 0) { c->cells_built = 1; return TBSMA_OK; }
     cudaStream_t st = (cudaStream_t)stream;
     c->list_built = 0;
-    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }   // tiles may change
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph_exec_multi) { cudaGraphExecDestroy(c->graph_exec_multi); c->graph_exec_multi = nullptr; }   // tiles may change
     {
         const int rc0 = ensure_variant_resources(c);
         if (rc0) return rc0;
@@ -845,24 +895,37 @@ int tbsma_md_run(tbsma_ctx *c, float *d_pos, float *d_vel, float *d_force_energy
         key.epoch = c->epoch;
         if (!c->graph_exec || memcmp(&key, &c->graph_key, sizeof(key)) != 0) {
             if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
-            cudaGraph_t g = nullptr;
-            CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
-            const int64_t before = c->launches;
-            int rc = run_steps(c, pos, vel, force, d_tag, dt_fs, d_T, gamma_per_fs, seed, 0, 1, d_disp0, d_rate,
-                               rebuild_every, d_e, d_w, d_k, true, st, true);
-            cudaError_t e = cudaStreamEndCapture(st, &g);
-            c->graph_launches_per_step = c->launches - before;
-            c->launches = before;
-            if (rc) { if (g) cudaGraphDestroy(g); return rc; }
-            if (e != cudaSuccess) return map_cuda(e);
-            e = cudaGraphInstantiate(&c->graph_exec, g, 0);
-            cudaGraphDestroy(g);
-            if (e != cudaSuccess) { c->graph_exec = nullptr; return map_cuda(e); }
+            if (c->graph_exec_multi) { cudaGraphExecDestroy(c->graph_exec_multi); c->graph_exec_multi = nullptr; }
+            // A small batch (the fused step, a few tens of microseconds) pays as much for the launch of a graph as for a
+            // kernel: eight steps are captured into a second graph, replayed n / 8 times; the one-step graph takes the rest.
+            const int multi = c->active_variant == 2 && tbsma_step_small_ok(c) ? 8 : 1;
+            for (int which = 0; which < (multi > 1 ? 2 : 1); ++which) {
+                cudaGraph_t g = nullptr;
+                CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+                const int64_t before = c->launches;
+                int rc = run_steps(c, pos, vel, force, d_tag, dt_fs, d_T, gamma_per_fs, seed, 0, which ? multi : 1, d_disp0,
+                                   d_rate, rebuild_every, d_e, d_w, d_k, true, st, true);
+                cudaError_t e = cudaStreamEndCapture(st, &g);
+                if (!which) c->graph_launches_per_step = c->launches - before;
+                c->launches = before;
+                if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+                if (e != cudaSuccess) return map_cuda(e);
+                e = cudaGraphInstantiate(which ? &c->graph_exec_multi : &c->graph_exec, g, 0);
+                cudaGraphDestroy(g);
+                if (e != cudaSuccess) {
+                    if (which) c->graph_exec_multi = nullptr; else c->graph_exec = nullptr;
+                    return map_cuda(e);
+                }
+            }
+            c->graph_multi_steps = multi;
             c->graph_key = key;
         }
         // the captured step reads the number of the run's first step from the device: one graph serves every step0
         CK(tbsma_launch_set_step_base(c, step0, st));
-        for (int64_t s = 0; s < n_steps; ++s) CK(cudaGraphLaunch(c->graph_exec, st));
+        int64_t s = 0;
+        if (c->graph_exec_multi)
+            for (; s + c->graph_multi_steps <= n_steps; s += c->graph_multi_steps) CK(cudaGraphLaunch(c->graph_exec_multi, st));
+        for (; s < n_steps; ++s) CK(cudaGraphLaunch(c->graph_exec, st));
         c->launches += c->graph_launches_per_step * n_steps;
     }
     CK(cudaMemsetAsync(c->d_counters, 0, sizeof(unsigned long long), st));

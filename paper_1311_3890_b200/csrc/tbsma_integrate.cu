@@ -7,39 +7,9 @@
 //   B: v += (dt/2)(c/m) F    A: x += (dt/2) v    O: v <- c1 v + c2 sigma_v g    A: x += (dt/2) v
 // (forces and the closing B run in tbsma_force.cu).  The same kernel measures every atom's
 // displacement since the last list build and raises its replica's dirty flag (D:A14).
-#include "tbsma_internal.cuh"
+#include "tbsma_integrate.cuh"
 
 namespace {
-
-// Philox4x32-10 (Salmon et al., SC'11), written out; D:A9 fixes key/counter layout:
-// key = (seed_lo, seed_hi), counter = (tag inside replica, step_lo, step_hi, 0).
-__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k)
-{
-    const unsigned M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
-#pragma unroll
-    for (int round = 0; round < 10; ++round) {
-        const unsigned hi0 = __umulhi(M0, c.x), lo0 = M0 * c.x;
-        const unsigned hi1 = __umulhi(M1, c.z), lo1 = M1 * c.z;
-        c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
-        k.x += W0; k.y += W1;
-    }
-    return c;
-}
-
-// u = ((x >> 8) + 0.5) 2^-24 in (0,1); Box-Muller as in D:A9.
-__device__ __forceinline__ float3 gauss3(unsigned long long seed, unsigned tag, unsigned long long step)
-{
-    const uint4 x = philox4x32_10(make_uint4(tag, (unsigned)step, (unsigned)(step >> 32), 0u),
-                                  make_uint2((unsigned)seed, (unsigned)(seed >> 32)));
-    const float s = 1.0f / 16777216.0f, h = 0.5f / 16777216.0f;
-    const float u0 = __fmaf_rn((float)(x.x >> 8), s, h), u1 = __fmaf_rn((float)(x.y >> 8), s, h);
-    const float u2 = __fmaf_rn((float)(x.z >> 8), s, h), u3 = __fmaf_rn((float)(x.w >> 8), s, h);
-    const float ra = sqrtf(-2.0f * logf(u0)), rb = sqrtf(-2.0f * logf(u2));
-    float sn, cs, cs2;
-    sincospif(2.0f * u1, &sn, &cs);
-    cs2 = cospif(2.0f * u3);
-    return make_float3(ra * cs, ra * sn, rb * cs2);
-}
 
 __global__ void __launch_bounds__(256)
 k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ force,
@@ -48,67 +18,8 @@ k_integrate_pre(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4
                 const unsigned long long *__restrict__ counters, int *__restrict__ dirty,
                 int *__restrict__ ctrl, int n, int R)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < R) {   // zero the per-replica accumulators of the force pass that follows
-        if (a.e_rep) a.e_rep[i] = 0.0;
-        if (a.ekin) a.ekin[i] = 0.0;
-        if (a.w_rep) for (int k = 0; k < 6; ++k) a.w_rep[6 * i + k] = 0.0;
-    }
-    if (i < n) {
-    const unsigned long long off = counters[0];
-    const unsigned long long step = (a.step_on_device ? counters[7] : a.step_base) + off;
-    const int r = atom_rep[i];
-    float4 p = pos[i], v = vel[i];
-    const int flag = __float_as_int(p.w) & 3;
-    if (flag == 0) {
-        const float4 f = force[i];
-        v.x = __fmaf_rn(a.kick, f.x, v.x); v.y = __fmaf_rn(a.kick, f.y, v.y); v.z = __fmaf_rn(a.kick, f.z, v.z);
-        p.x = __fmaf_rn(a.half_dt, v.x, p.x); p.y = __fmaf_rn(a.half_dt, v.y, p.y); p.z = __fmaf_rn(a.half_dt, v.z, p.z);
-        if (a.nh_scale) {              // N of B A N A B (Nose-Hoover, k_nh_update): v *= exp(-xi dt)
-            const float sc = a.nh_scale[r];
-            v.x *= sc; v.y *= sc; v.z *= sc;
-        } else if (a.thermostat) {
-            const unsigned trel = (unsigned)(tag[i] - geom[r].atom_begin);
-            const float3 g = gauss3(a.seed[r], trel, step);
-            const float Tr = a.T_rate ? (float)((double)a.T[r] + (double)a.T_rate[r] * (double)off) : a.T[r];
-            const float sg = a.c2 * a.sigma_scale * sqrtf(fmaxf(Tr, 0.f));
-            v.x = __fmaf_rn(a.c1, v.x, sg * g.x); v.y = __fmaf_rn(a.c1, v.y, sg * g.y); v.z = __fmaf_rn(a.c1, v.z, sg * g.z);
-        }
-        p.x = __fmaf_rn(a.half_dt, v.x, p.x); p.y = __fmaf_rn(a.half_dt, v.y, p.y); p.z = __fmaf_rn(a.half_dt, v.z, p.z);
-    } else {       // rigid grip atom (D:A12): v = 0; a pulled atom is placed, never incremented (D:A10)
-        v.x = v.y = v.z = 0.f;
-        // steps of slab motion since the run began: every step, or in strokes of `period` steps
-        unsigned long long nst = off + 1ull;
-        if (a.period > 0) nst = nst / (unsigned long long)a.period * (unsigned long long)a.period;
-        if (flag == 2) {
-            double D = a.disp0 ? a.disp0[r] : 0.0;
-            if (a.rate) D += a.rate[r] * (double)nst;
-            p.z = (float)((double)v.w + D);
-        } else if (a.disp0_1 || a.rate_1) {      // the other end (both ends move); without a schedule it stays fixed
-            double D = a.disp0_1 ? a.disp0_1[r] : 0.0;
-            if (a.rate_1) D += a.rate_1[r] * (double)nst;
-            p.z = (float)((double)v.w + D);
-        }
-    }
-    pos[i] = p;
-    vel[i] = v;
-    const float4 pb = pos_build[(size_t)a.cur[r] * a.pb_stride + i];
-    const float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
-    const float d2 = dx * dx + dy * dy + dz * dz;
-    const bool cadence = a.rebuild_every > 0 && (step % (unsigned long long)a.rebuild_every) == 0ull;
-    if (d2 > a.skin_half2 && a.trigger2 < a.skin_half2) atomicOr(ctrl + 1, (int)TBSMA_FLAG_SKIN_VIOLATED);
-    // (the staggered first rebuild is for displacement-triggered lists only: with a fixed cadence an early trigger
-    // would be reported as a violated skin)
-    const float trig2 = a.rebuild_every > 0 ? a.trigger2 : a.trigger2 * a.stagger[r];
-    if (d2 > trig2 || cadence) {
-        // level 2 = cells + candidate list too (tile variant, decided at the replica's previous rebuild)
-        const int level = (a.want_outer && a.want_outer[r]) ? 2 : 1;
-        dirty[r] = level;
-        ctrl[0] = 1;
-        if (level == 2) ctrl[3] = 1;
-        if (a.rebuild_every > 0 && !cadence) atomicOr(ctrl + 1, (int)TBSMA_FLAG_SKIN_VIOLATED);
-    }
-    }
+    tbsma_integrate_one(blockIdx.x * blockDim.x + threadIdx.x, pos, vel, force, pos_build, atom_rep, geom, tag, a, counters,
+                        dirty, ctrl, n, R);
 }
 
 // end of step: statistics, clear the dirty flags, advance the in-run step offset
@@ -117,30 +28,9 @@ k_finish_step(int *__restrict__ dirty, int *__restrict__ ctrl, int *__restrict__
               float *__restrict__ stagger, int *__restrict__ cur, int swap,
               unsigned long long *__restrict__ counters, int R, int advance, int count_step, TileSums ts)
 {
-    __shared__ int s_cnt, s_cnt2;
     tbsma_reduce_replicas(ts, R);      // a6 of the tile variant: per-replica E, E_kin, W in a fixed order (all CTAs)
     if (blockIdx.x != 0) return;       // the bookkeeping below is CTA 0's
-    if (threadIdx.x == 0) { s_cnt = 0; s_cnt2 = 0; }
-    __syncthreads();
-    if (ctrl[0]) {
-        int mine = 0, mine2 = 0;
-        for (int r = threadIdx.x; r < R; r += blockDim.x) {
-            const int d = dirty[r];
-            if (d) { ++mine; dirty[r] = 0; stagger[r] = 1.0f; if (swap) cur[r] ^= 1; }
-            if (d == 2) ++mine2;
-        }
-        if (mine) atomicAdd(&s_cnt, mine);
-        if (mine2) atomicAdd(&s_cnt2, mine2);
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        if (ctrl[0]) {
-            counters[1] += (unsigned long long)s_cnt; counters[2] += 1ull; counters[6] += (unsigned long long)s_cnt2;
-            ctrl[0] = 0; ctrl[3] = 0;
-        }
-        if (count_step) counters[3] += 1ull;
-        if (advance) counters[0] += 1ull;
-    }
+    tbsma_finish_bookkeeping(dirty, ctrl, stagger, cur, swap, counters, R, advance, count_step);
 }
 
 // Replicas that are built together (all of them, at the start of a run) and share a temperature would all ask

@@ -136,6 +136,8 @@ struct tbsma_ctx {
     int tile_split_req;    // requested by tbsma_set_tile_split (0 = automatic)
     int tile_force_box;    // tbsma_set_tile_box: box tiles even for replicas whose layers would fit (tests)
     int any_box;           // some replica is cut into box tiles (kind 1)
+    int fused_step;        // tbsma_set_fused_step (default 1): small batches run a step as one cooperative kernel
+    int fused_max_ctas;    // CTAs of that kernel the GPU holds at once
     int tiles_rejected;    // variant 0: the tiles were tried for this system and the global variant taken instead
     double *d_cta_sums;    // n_tiles x tile_nsplit x 8: E, E_kin, W (xx yy zz xy xz yz) of every CTA of the force pass
     // persistent gather kernels: units = p_plain whole tiles, then the remaining tiles in p_S parts each
@@ -227,6 +229,8 @@ struct tbsma_ctx {
     // md_run: one step captured as a CUDA graph and replayed
     int use_graph;
     cudaGraphExec_t graph_exec;
+    cudaGraphExec_t graph_exec_multi;   // graph_multi_steps steps in one graph (small batches)
+    int graph_multi_steps;
     GraphKey graph_key;
     int64_t graph_launches_per_step;
     cudaStream_t own_stream;   // used by the *_host entry point
@@ -317,6 +321,38 @@ __device__ inline void tbsma_reduce_replicas(const TileSums &ts, int R)
 }
 #endif
 
+#ifdef __CUDACC__
+// end of a step, by all threads of ONE CTA: statistics, clear the dirty flags, swap the list halves of the replicas that
+// were rebuilt, advance the in-run step offset (k_finish_step; the fused step kernel of small batches)
+__device__ inline void tbsma_finish_bookkeeping(int *__restrict__ dirty, int *__restrict__ ctrl, float *__restrict__ stagger,
+                                                int *__restrict__ cur, int swap, unsigned long long *__restrict__ counters,
+                                                int R, int advance, int count_step)
+{
+    __shared__ int s_cnt, s_cnt2;
+    if (threadIdx.x == 0) { s_cnt = 0; s_cnt2 = 0; }
+    __syncthreads();
+    if (ctrl[0]) {
+        int mine = 0, mine2 = 0;
+        for (int r = threadIdx.x; r < R; r += blockDim.x) {
+            const int d = dirty[r];
+            if (d) { ++mine; dirty[r] = 0; stagger[r] = 1.0f; if (swap) cur[r] ^= 1; }
+            if (d == 2) ++mine2;
+        }
+        if (mine) atomicAdd(&s_cnt, mine);
+        if (mine2) atomicAdd(&s_cnt2, mine2);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (ctrl[0]) {
+            counters[1] += (unsigned long long)s_cnt; counters[2] += 1ull; counters[6] += (unsigned long long)s_cnt2;
+            ctrl[0] = 0; ctrl[3] = 0;
+        }
+        if (count_step) counters[3] += 1ull;
+        if (advance) counters[0] += 1ull;
+    }
+}
+#endif
+
 // forces (tbsma_force.cu)
 struct KickArgs {
     float4 *vel;          // nullptr = no fused half kick
@@ -347,6 +383,11 @@ cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_
 cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, bool virial, KickArgs kick, int sync_level,
                                     cudaStream_t st);
 TileSums tbsma_tile_sums(const tbsma_ctx *c, double *e_rep, double *ekin, double *w_rep);
+struct StepArgs;
+bool tbsma_step_small_ok(const tbsma_ctx *c);
+cudaError_t tbsma_launch_step_small(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, const int32_t *tag,
+                                    const StepArgs &a, KickArgs kick, bool virial, int advance_offset, TileSums ts,
+                                    unsigned long long cond, cudaStream_t st);
 cudaError_t tbsma_launch_reduce_replicas(tbsma_ctx *c, double *e_rep, double *ekin, double *w_rep, cudaStream_t st);
 cudaError_t tbsma_launch_get_neighbors_tile(tbsma_ctx *c, const int32_t *tag, int32_t *counts, int32_t *list,
                                             cudaStream_t st);

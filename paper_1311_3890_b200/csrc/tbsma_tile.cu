@@ -29,7 +29,9 @@
 // checks that (status flag) and asks for new candidates one rebuild earlier (want_outer).  Slots (and
 // so the u16 offsets) only change when candidates are rebuilt.  The list, its counts and its build
 // positions exist twice (ListSel): a renewal writes the half not in use, the step's last kernel swaps.
-#include "tbsma_internal.cuh"
+#include <cooperative_groups.h>
+
+#include "tbsma_integrate.cuh"
 
 namespace {
 
@@ -68,6 +70,8 @@ __device__ __forceinline__ TileRange tile_range(const TileDesc &t, const int *__
 // gather passes alike (the bank schedule of the lists depends on it).
 struct TileMap {
     int n_runs, nh, n_own_runs, n_own;
+    int contig;                            // layer tiles: halo and own atoms are contiguous slot ranges (no search)
+    int own_slot0;                         // slot of own-local index 0
     int lstart[TBSMA_TILE_MAX_RUNS + 1];   // halo-local index of the first record of run r; lstart[n_runs] = nh
     int gslot[TBSMA_TILE_MAX_RUNS];        // slot of that record
     int ostart[TBSMA_TILE_MAX_OWN_RUNS + 1];   // own-local index of the first atom of own run q
@@ -78,6 +82,32 @@ __device__ __forceinline__ int wrap_cell(int c, int nc) { return c < 0 ? c + nc 
 // called by every thread of the CTA; ends with a barrier
 __device__ __forceinline__ void tile_map_build(const TileDesc &t, const int *__restrict__ cell_start, TileMap &M)
 {
+    if (t.kind == 0) {       // a handful of layers: one thread, one barrier
+        if (threadIdx.x == 0) {
+            const int base = cell_start[t.ch0];
+            M.lstart[0] = 0;
+            for (int r = 0; r < t.nlay_h; ++r) {
+                const int s = r == 0 ? base : M.gslot[r - 1] + (M.lstart[r] - M.lstart[r - 1]);
+                const int e = cell_start[t.ch0 + (r + 1) * t.layer_cells];
+                M.gslot[r] = s;
+                M.lstart[r + 1] = e - base;
+            }
+            M.n_runs = t.nlay_h;
+            M.nh = M.lstart[t.nlay_h];
+            int o = 0;
+            for (int l = 0; l < t.own_n; ++l) {
+                const int r = t.own_first + l;
+                M.orun[l] = (short)r; M.ostart[l] = o; o += M.lstart[r + 1] - M.lstart[r];
+            }
+            M.ostart[t.own_n] = o;
+            M.n_own_runs = t.own_n;
+            M.n_own = o;
+            M.contig = 1;
+            M.own_slot0 = M.gslot[t.own_first];
+        }
+        __syncthreads();
+        return;
+    }
     const int n_runs = t.kind == 0 ? t.nlay_h : (int)t.hn[0] * t.hn[1] * t.hn[2];
     for (int r = threadIdx.x; r < n_runs; r += blockDim.x) {
         int c0, nc;
@@ -129,6 +159,8 @@ __device__ __forceinline__ void tile_map_build(const TileDesc &t, const int *__r
         M.ostart[q] = o;
         M.n_own_runs = q;
         M.n_own = o;
+        M.contig = 0;
+        M.own_slot0 = 0;
     }
     __syncthreads();
 }
@@ -144,6 +176,7 @@ __device__ __forceinline__ int map_run_of(const TileMap &M, int k)
 }
 __device__ __forceinline__ int map_slot(const TileMap &M, int k)
 {
+    if (M.contig) return M.gslot[0] + k;
     const int r = map_run_of(M, k);
     return M.gslot[r] + k - M.lstart[r];
 }
@@ -158,6 +191,7 @@ __device__ __forceinline__ int map_own(const TileMap &M, int o, int &q, int &k)
 }
 __device__ __forceinline__ int map_own(const TileMap &M, int o)
 {
+    if (M.contig) return M.own_slot0 + o;
     int q, k;
     return map_own(M, o, q, k);
 }
@@ -1258,6 +1292,84 @@ k_force_tile(const TileDesc *__restrict__ tiles, const int *__restrict__ cell_st
                                                ls.nsplit, cta_sums + 8 * (size_t)blockIdx.x, ls.kg);
 }
 
+// ---- the whole step of a small batch in ONE kernel ---------------------------------------
+// The paper pays "+35 % run time due to thread synchronization" between its two stages; a single wire per GPU is its
+// unit of work.  For a batch whose tiles (or parts of tiles) all fit the GPU at once the step is one cooperative
+// launch: every CTA integrates its share of the atoms (B A O A, grips, displacement check), the grid synchronises, the CTA
+// works its tile's chunks through the density pass, the grid synchronises, the force pass with the closing kick, the grid
+// synchronises, and the first CTAs add up the replicas and do the step's bookkeeping.  Three grid barriers of about a
+// microsecond in place of five kernel boundaries.  If the displacement check finds a replica that needs a new list the
+// kernel stops after the integration and sets the graph conditional: the rest of that step (list renewal, density,
+// force, bookkeeping) is run by the ordinary kernels in the body of an IF node.  Same device functions as the separate
+// kernels, same order of operations: bit-identical results.
+struct FusedArgs {
+    // integration
+    float4 *pos, *vel;
+    float4 *force;
+    const float4 *pos_build;
+    const int *atom_rep;
+    const RepGeom *geom;
+    const int *tag;
+    StepArgs a;
+    unsigned long long *counters;
+    int *dirty, *ctrl;
+    int n, R;
+    // gather passes
+    const TileDesc *tiles;
+    const int *cell_start;
+    const uint2 *nl;
+    const int *nn;
+    float4 *xs;
+    double *cta_sums;
+    KickArgs kk;
+    ListSel ls;
+    int n_pad, s_cap;
+    PairConst pc;
+    // bookkeeping
+    float *stagger;
+    int *cur;
+    int swap, advance, count_step;
+    TileSums ts;
+    cudaGraphConditionalHandle cond;
+};
+
+template <bool VIRIAL, bool SPLIT>
+__global__ void __launch_bounds__(256, 4)
+k_step_small(const FusedArgs F)
+{
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    const int nthr = (int)(gridDim.x * blockDim.x);
+    const int work = F.n > F.R ? F.n : F.R;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < work; i += nthr)
+        tbsma_integrate_one(i, F.pos, F.vel, F.force, F.pos_build, F.atom_rep, F.geom, F.tag, F.a, F.counters, F.dirty, F.ctrl,
+                            F.n, F.R);
+    grid.sync();
+    const int any_dirty = *(volatile int *)F.ctrl;
+    if (blockIdx.x == 0 && threadIdx.x == 0) cudaGraphSetConditional(F.cond, any_dirty ? 1u : 0u);
+    if (any_dirty) return;         // every CTA sees the same flag: nobody is left waiting at a barrier
+    const int ti = SPLIT ? (int)blockIdx.x / F.ls.nsplit : (int)blockIdx.x, part = SPLIT ? (int)blockIdx.x % F.ls.nsplit : 0;
+    const TileDesc t = F.tiles[ti];
+    const int h = F.ls.cur[t.rep];
+    const uint2 *nl = F.nl + (size_t)h * F.ls.nl_stride;
+    const int *nn = F.nn + (size_t)h * F.ls.n_stride;
+    const unsigned short *img = F.ls.img + (size_t)ti * F.ls.img_stride;
+    __shared__ TileMap M;
+    tile_map_build(t, F.cell_start, M);
+    const bool wrap = t.Ls[0] != 0.f || t.Ls[1] != 0.f || t.Ls[2] != 0.f;
+    if (wrap) density_tile<SPLIT, true>(t, M, F.pos, nl, nn, F.xs, F.ctrl, F.n_pad, F.s_cap, F.pc, img, part, F.ls.nsplit, F.ls.kg);
+    else density_tile<SPLIT, false>(t, M, F.pos, nl, nn, F.xs, F.ctrl, F.n_pad, F.s_cap, F.pc, img, part, F.ls.nsplit, F.ls.kg);
+    grid.sync();
+    double *my_sums = F.cta_sums + 8 * (size_t)blockIdx.x;
+    if (wrap) force_tile<VIRIAL, true, SPLIT, true>(t, M, F.xs, nl, nn, F.force, F.kk, F.ctrl, F.n_pad, F.s_cap, F.pc, img, part,
+                                                    F.ls.nsplit, my_sums, F.ls.kg);
+    else force_tile<VIRIAL, true, SPLIT, false>(t, M, F.xs, nl, nn, F.force, F.kk, F.ctrl, F.n_pad, F.s_cap, F.pc, img, part,
+                                                F.ls.nsplit, my_sums, F.ls.kg);
+    grid.sync();
+    tbsma_reduce_replicas(F.ts, F.R);
+    if (blockIdx.x == 0) tbsma_finish_bookkeeping(F.dirty, F.ctrl, F.stagger, F.cur, F.swap, F.counters, F.R, F.advance, F.count_step);
+}
+
 // ---- persistent gather kernels ----------------------------------------------------------------------
 // One CTA of 16 warps per half SM for the whole pass.  Work comes in UNITS (a tile, or 1 / S of a tile's 32-atom chunks for
 // the last tiles of the pass and for batches with few tiles), claimed from a global counter.  A CTA holds TWO tile images:
@@ -2081,6 +2193,20 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
 #undef TBSMA_ATTR
         c->persist_ok = sm_p1v <= 112 * 1024 && c->kmax >= 16;     // two CTAs per SM; four rows per atom exist
     }
+    {   // the fused step of small batches: every CTA of the grid must be resident at once (cooperative launch)
+        int occ = 0, min_occ = 1 << 30;
+#define TBSMA_FUSED(V, S)                                                                                                     \
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_step_small<V, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm_g);   \
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_step_small<V, S>, 256, (size_t)sm_g);     \
+        if (occ < min_occ) min_occ = occ;
+        TBSMA_FUSED(false, false) TBSMA_FUSED(false, true) TBSMA_FUSED(true, false) TBSMA_FUSED(true, true)
+#undef TBSMA_FUSED
+        c->fused_max_ctas = e == cudaSuccess ? min_occ * c->n_sm : 0;
+        // a batch that would fit the fused step with fewer parts per tile gets fewer parts
+        if (c->fused_step && c->tile_split_req <= 0 && c->n_tiles <= c->fused_max_ctas &&
+            (int64_t)c->n_tiles * c->tile_nsplit > c->fused_max_ctas)
+            c->tile_nsplit = c->fused_max_ctas / c->n_tiles;
+    }
     if (e != cudaSuccess) return TBSMA_ECUDA;
     c->active_variant = 2;
     return TBSMA_OK;
@@ -2264,6 +2390,35 @@ cudaError_t tbsma_launch_force_tile(tbsma_ctx *c, float4 *force, bool virial, Ki
 #undef TBSMA_FT
     c->launches++;
     return cudaGetLastError();
+}
+
+// the whole step in one cooperative launch (k_step_small): small batches of the tile variant
+bool tbsma_step_small_ok(const tbsma_ctx *c)
+{
+    return c->active_variant == 2 && c->fused_step && !use_persist(c) && c->tile_threads == 256 &&
+           (int64_t)c->n_tiles * c->tile_nsplit <= c->fused_max_ctas && c->n_tiles > 0;
+}
+
+cudaError_t tbsma_launch_step_small(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, const int32_t *tag,
+                                    const StepArgs &a, KickArgs kk, bool virial, int advance_offset, TileSums ts,
+                                    unsigned long long cond, cudaStream_t st)
+{
+    FusedArgs F;
+    F.pos = pos; F.vel = vel; F.force = force; F.pos_build = c->d_pos_build; F.atom_rep = c->d_atom_rep; F.geom = c->d_geom;
+    F.tag = tag; F.a = a; F.counters = c->d_counters; F.dirty = c->d_dirty; F.ctrl = c->d_ctrl; F.n = (int)c->n; F.R = c->R;
+    F.tiles = c->d_tiles; F.cell_start = c->d_cell_start; F.nl = reinterpret_cast<const uint2 *>(c->d_nlist); F.nn = c->d_nn;
+    F.xs = c->d_xs; F.cta_sums = c->d_cta_sums; F.kk = kk; F.ls = list_sel(c, 2); F.n_pad = c->n_pad; F.s_cap = c->tile_cap;
+    F.pc = c->pc; F.stagger = c->d_stagger; F.cur = c->d_cur; F.swap = c->list_bufs == 2;
+    F.advance = advance_offset & 1; F.count_step = (advance_offset >> 1) & 1; F.ts = ts;
+    F.cond = (cudaGraphConditionalHandle)cond;
+    void *args[] = {&F};
+    const dim3 grid((unsigned)(c->n_tiles * c->tile_nsplit)), block(256);
+    const size_t sm = gather_smem(c);
+    const void *fn = virial ? (c->tile_nsplit > 1 ? (const void *)k_step_small<true, true> : (const void *)k_step_small<true, false>)
+                            : (c->tile_nsplit > 1 ? (const void *)k_step_small<false, true> : (const void *)k_step_small<false, false>);
+    const cudaError_t e = cudaLaunchCooperativeKernel(fn, grid, block, args, sm, st);
+    c->launches++;
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 TileSums tbsma_tile_sums(const tbsma_ctx *c, double *e_rep, double *ekin, double *w_rep)

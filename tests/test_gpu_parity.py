@@ -1222,3 +1222,37 @@ def test_box_tiles_trajectory_100_steps(B, name):
     xf = st.untag(st.pos)
     co, lo = oracle.neighbors(xf, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
     assert_same_sets(cg, lg, co, lo)
+
+
+@pytest.mark.parametrize("name", ["config1", "config2", "config3_small", "config4_ragged"])
+def test_fused_step_of_small_batches_is_bitwise_identical(B, name):
+    """tbsma_set_fused_step: the whole step of a small batch as one cooperative kernel, the steps
+    that renew a list falling back to the separate kernels, gives the bits of the separate kernels throughout: positions,
+    velocities, forces, per-replica energies, kinetic energies and virials, rebuild statistics"""
+    w = WORKLOADS[name]()
+    n_steps = 150
+
+    def run(fused):
+        ctx, st = setup(B, w, variant=2)
+        ctx.set_fused_step(fused)
+        ctx.set_overlap(0)
+        ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
+        stream = torch.cuda.Stream()
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate, 0,
+                       st.e_rep, st.w_rep, st.ekin)
+        torch.cuda.synchronize()
+        assert ctx.status() == 0
+        return ctx, st
+
+    ca, a = run(True)
+    cb, b = run(False)
+    assert ca.get_stats() == cb.get_stats() and ca.get_stats()["n_replica_builds"] > w.n_replicas
+    for nm in ("pos", "vel", "force"):
+        assert np.array_equal(a.untag(getattr(a, nm)), b.untag(getattr(b, nm))), nm
+    for nm in ("e_rep", "ekin", "w_rep"):
+        assert np.array_equal(getattr(a, nm).cpu().numpy(), getattr(b, nm).cpu().numpy()), nm
+    assert ca.launch_count() < 0.45 * cb.launch_count()          # one kernel per ordinary step instead of six
+    md = run_oracle_md(w, n_steps)
+    assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
