@@ -682,6 +682,24 @@ __device__ __forceinline__ void fill_image(float4 *sm, const float4 *__restrict_
 {
     const int nh = M.nh;
     if (threadIdx.x == 0) sm[0] = make_float4(TBSMA_SENTINEL, TBSMA_SENTINEL, TBSMA_SENTINEL, 0.f);
+    if (!M.contig) {
+        // box tile: run by run (a halo cell of ~60 records each), a warp per run, no search for the slot of a record
+        const int lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+        for (int r = threadIdx.x >> 5; r < M.n_runs; r += nw) {
+            const int s0 = M.lstart[r], e0 = M.lstart[r + 1], g0 = M.gslot[r] - s0;
+            for (int k = s0 + lane; k < e0; k += 64) {
+                const bool two = k + 32 < e0;
+                const unsigned short a0 = img[k], a1 = two ? img[k + 32] : (unsigned short)0;
+                const float4 r0 = src[g0 + k];
+                float4 r1 = r0;
+                if (two) r1 = src[g0 + k + 32];
+                sm[a0] = r0;
+                if (two) sm[a1] = r1;
+            }
+        }
+        __syncthreads();
+        return;
+    }
     // eight records per thread and round, all sixteen loads in flight before the first store
     const int nthr = blockDim.x;
     for (int k0 = threadIdx.x; k0 < nh; k0 += 8 * nthr) {
@@ -1941,7 +1959,7 @@ k_box_measure(const RepGeom *__restrict__ geom, const int *__restrict__ cell_sta
 // into runs of whole z-layers (kind 0): L_r own layers per tile, the largest L <= tile_layers whose halo (L + 2 layers of
 // the replica's most populated layer, + 25 %) fits the shared-memory image.  Any other replica (thick wires, periodic
 // bulk) is cut into boxes of cells (kind 1), the shape with the best own / halo ratio whose fullest halo, measured on the
-// cells as they are, fits with 4 % to spare.  The choice depends on replica r alone, so a replica is tiled (and therefore
+// cells as they are, fits with 2.5 % to spare.  The choice depends on replica r alone, so a replica is tiled (and therefore
 // summed) identically whatever batch it is part of.  Returns TBSMA_OK and sets active_variant = 2, or leaves
 // active_variant = 1 when a replica does not fit either way.
 int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
@@ -2006,7 +2024,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
                 for (int a = 0; a < 3; ++a) hc *= (g.periodic >> a & 1) ? b[a] + 2 : (b[a] + 2 < g.nc[a] ? b[a] + 2 : g.nc[a]);
                 if (hc > TBSMA_TILE_MAX_RUNS || b[0] * b[1] * b[2] > TBSMA_TILE_MAX_OWN_RUNS) continue;
                 const int64_t mh = meas[((size_t)r * kNBoxCand + cnd) * 2];
-                if (mh + mh / 25 + 16 > cap) continue;
+                if (mh + mh / 40 + 8 > cap) continue;
                 pick = cnd;
             }
             if (pick < 0) { fits = false; break; }
@@ -2014,8 +2032,8 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
             int b[3];
             box_dims(g, pick, b);
             const int mh = meas[((size_t)r * kNBoxCand + pick) * 2], mo = meas[((size_t)r * kNBoxCand + pick) * 2 + 1];
-            if (mh + mh / 25 + 16 > rec_cap) rec_cap = mh + mh / 25 + 16;
-            if (mo + mo / 25 + 16 > own_cap) own_cap = mo + mo / 25 + 16;
+            if (mh + mh / 40 + 8 > rec_cap) rec_cap = mh + mh / 40 + 8;
+            if (mo + mo / 20 + 16 > own_cap) own_cap = mo + mo / 20 + 16;
             n_tiles += (int64_t)((g.nc[0] + b[0] - 1) / b[0]) * ((g.nc[1] + b[1] - 1) / b[1]) * ((g.nc[2] + b[2] - 1) / b[2]);
         }
         free(meas);
