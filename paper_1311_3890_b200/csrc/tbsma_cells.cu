@@ -133,6 +133,26 @@ k_cell_sort(const RepGeom *__restrict__ geom, DirtyView dv, const int *__restric
             for (int k = 0; k < m; ++k) rank += __shfl_sync(0xffffffffu, key, k) < key;
             __syncwarp();
             if (lane < m) order[s + rank] = o;
+        } else if (m <= 128) {       // up to four atoms per lane (the 9.8 A cells of the tile variant hold ~55)
+            int o[4], key[4], rank[4] = {0, 0, 0, 0};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int k = q * 32 + lane;
+                o[q] = k < m ? order[s + k] : 0;
+                key[q] = k < m ? tag[o[q]] : 0x7fffffff;
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                for (int k = 0; k < 32; ++k) {
+                    if (q * 32 + k >= m) break;
+                    const int other = __shfl_sync(0xffffffffu, key[q], k);
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) rank[p] += other < key[p];
+                }
+            __syncwarp();
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (q * 32 + lane < m) order[s + rank[q]] = o[q];
         } else if (lane == 0) {      // crowded cell: insertion sort by one lane
             for (int a = s + 1; a < s + m; ++a) {
                 const int oa = order[a];

@@ -37,7 +37,7 @@ namespace {
 
 constexpr int kScanThreads = 1024;  // k_tile_scan: one round for tiles of <= 1024 own atoms (the rebuild chain is
                                     // latency bound: only the dirty replicas' tiles do any work)
-constexpr int kFinishMaxThreads = 768;   // k_tile_finish: bounded by its kmax x threads x 2 B shared-memory scratch
+constexpr int kFinishMaxThreads = 1024;
 
 __device__ __forceinline__ float ex2_approx(float x)
 {
@@ -556,17 +556,16 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
 {
     const int *__restrict__ cell_start = A.cell_start;
     const uint2 *__restrict__ nl_tmp = A.nl_tmp;
-    const int *__restrict__ nn_tmp = A.nn_tmp, *__restrict__ newslot = A.newslot, *__restrict__ oldof = A.oldof;
+    const int *__restrict__ nn_tmp = A.nn_tmp, *__restrict__ newslot = A.newslot;
     uint2 *__restrict__ nl = A.nl;
     int *__restrict__ nn = A.nn;
     const int s_cap = A.s_cap;
     extern __shared__ float4 smem_f4[];
     unsigned short *map = reinterpret_cast<unsigned short *>(smem_f4);   // s_cap entries
-    unsigned short *scr = map + ((s_cap + 7) & ~7);                      // kmax x blockDim.x
     __shared__ TileMap M;
     tile_map_build(t, cell_start, M);
     if (M.n_own <= 0 || M.nh > s_cap) return;
-    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int tid = threadIdx.x;
     const unsigned short *__restrict__ img = A.img + (size_t)ti * A.img_stride;
     // cell-order halo-local index -> byte offset of the record in the image: the atom moves inside its run only
     for (int k = tid; k < M.nh; k += blockDim.x) {
@@ -574,9 +573,13 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
         map[k] = (unsigned short)((unsigned)img[k + (newslot[sc] - sc)] << 4);
     }
     __syncthreads();
-    for (int o = tid; o < M.n_own; o += blockDim.x) {
-        const int ip = map_own(M, o);
-        const int a = oldof[ip];
+    // (thread per atom in CELL order, so that the reads of the temporary rows are coalesced; the atom's final slot ip, in
+    // the same run, and with it its own-local index o there, follow from newslot)
+    for (int oc = tid; oc < M.n_own; oc += blockDim.x) {
+        int q, kh;
+        const int a = map_own(M, oc, q, kh);
+        const int ip = newslot[a];
+        const int o = M.ostart[q] + (ip - M.gslot[M.orun[q]]);
         const int nnv = nn_tmp[a];
         const int cnt = nnv & 0xffff;
         const uint2 *src = nl_tmp + tbsma_lrow(a, A.kg_o);
@@ -597,7 +600,9 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
 #pragma unroll
             for (int c = 0; c < 8; ++c) { off |= (unsigned long long)run << (c << 3); run += byte_of(pop, c); }
         }
-        // pass B: class-sorted copy in shared memory (column tid: conflict-free for any row)
+        // pass B: every entry straight to its class-sorted place in the atom's rows (two-byte stores that the L2 merges: a
+        // shared-memory staging column per thread capped the CTA at 384 threads, one CTA per SM)
+        unsigned short *dst16 = reinterpret_cast<unsigned short *>(nl + tbsma_lrow(ip, A.kg_o));
         unsigned long long cur = 0ull;
         for (int g = 0; g < ng; ++g) {
             const uint2 w = src[(size_t)g * TBSMA_LROW];
@@ -609,17 +614,11 @@ __device__ __forceinline__ void finish_tile(const TileDesc &t, int ti, const Fin
                     const int c = ((m >> 4) - lane) & 7;
                     const unsigned idx = byte_of(off, c) + byte_of(cur, c);
                     cur += 1ull << (c << 3);
-                    scr[idx * nthr + tid] = (unsigned short)m;
+                    dst16[(size_t)(idx >> 2) * (TBSMA_LROW * 4) + (idx & 3u)] = (unsigned short)m;
                 }
         }
-        // rows of four entries, unused entries = 0 = the sentinel
-        uint2 *dst = nl + tbsma_lrow(ip, A.kg_o);
-        for (int g = 0; g < ng; ++g) {
-            unsigned e[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) e[q] = 4 * g + q < cnt ? (unsigned)scr[(4 * g + q) * nthr + tid] : 0u;
-            dst[(size_t)g * TBSMA_LROW] = make_uint2(e[0] | (e[1] << 16), e[2] | (e[3] << 16));
-        }
+        for (int k = cnt; k < 4 * ng; ++k)       // unused entries of the last row = 0 = the sentinel
+            dst16[(size_t)(k >> 2) * (TBSMA_LROW * 4) + (k & 3)] = (unsigned short)0;
         nn[ip] = nnv;
         A.tileof[ip] = ti;
     }
@@ -1835,18 +1834,8 @@ size_t scan_smem(const tbsma_ctx *c)
 {
     return (size_t)c->tile_cap * 16 + (size_t)c->tile_cell_cap * 4 + (size_t)c->tile_cap * 2;
 }
-int finish_threads(const tbsma_ctx *c)
-{
-    const size_t budget = 200 * 1024 - (size_t)((c->tile_cap + 7) & ~7) * 2;
-    int t = (int)(budget / ((size_t)c->kmax_o * 2)) & ~31;
-    if (t > kFinishMaxThreads) t = kFinishMaxThreads;
-    if (t < 32) t = 32;
-    return t;
-}
-size_t finish_smem(const tbsma_ctx *c)
-{
-    return (size_t)((c->tile_cap + 7) & ~7) * 2 + (size_t)c->kmax_o * finish_threads(c) * 2;
-}
+int finish_threads(const tbsma_ctx *) { return kFinishMaxThreads; }
+size_t finish_smem(const tbsma_ctx *c) { return (size_t)((c->tile_cap + 7) & ~7) * 2; }
 size_t gather_smem(const tbsma_ctx *c) { return (size_t)c->img_cap * 16; }
 size_t persist_smem(const tbsma_ctx *c, int pass, bool virial)
 {
