@@ -227,6 +227,8 @@ int tbsma_set_tile_box(tbsma_ctx *ctx, int32_t force);
  * A step in which a replica needs a new list runs the separate kernels instead (decided on the device).  enable = 0:
  * always the separate kernels.  Default 1.  Changes cost, never results (same operations in the same order). */
 int tbsma_set_fused_step(tbsma_ctx *ctx, int32_t enable);
+/* 1 if the captured step of tbsma_md_run is that single kernel for the batch as it is now built, else 0. */
+int tbsma_get_fused_step(const tbsma_ctx *ctx);
 
 /* Shared-memory variant: how the two gather passes (P:59 stages 1 and 2) are launched.
  *   1 (default) = persistent kernels: two CTAs of 16 warps per SM work through the tiles of the batch, each holding the

@@ -20,7 +20,7 @@ EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
     "tbsma_count_pairs", "tbsma_kinetic_tensor", "tbsma_stress", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
-    "tbsma_get_variant", "tbsma_get_tiling", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_thermostat_state", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin", "tbsma_set_tile_split", "tbsma_set_gather", "tbsma_set_tile_box", "tbsma_set_fused_step",
+    "tbsma_get_variant", "tbsma_get_tiling", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_thermostat_state", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin", "tbsma_set_tile_split", "tbsma_set_gather", "tbsma_set_tile_box", "tbsma_set_fused_step", "tbsma_get_fused_step",
     "tbsma_set_protocol", "tbsma_set_series", "tbsma_series_histogram",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
 ]
@@ -100,6 +100,7 @@ def lib():
         L.tbsma_set_tile_split.argtypes = [vp, i32]
         L.tbsma_set_gather.argtypes = [vp, i32]
         L.tbsma_set_fused_step.argtypes = [vp, i32]
+        L.tbsma_get_fused_step.argtypes = [vp]
         L.tbsma_get_tiling.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
         L.tbsma_set_tile_box.argtypes = [vp, i32]
         L.tbsma_set_protocol.argtypes = [vp, C.POINTER(Protocol)]
@@ -259,8 +260,9 @@ class Context:
         n_tiles, box, persistent = self.get_tiling()
         if not n_tiles:
             return "thread per atom, records gathered through L1"
-        return ("%d %s tiles, %s" % (n_tiles, "box" if box else "layer",
-                                     "persistent kernels (two CTAs of 16 warps per SM)" if persistent else "one CTA per tile"))
+        how = ("persistent kernels (two CTAs of 16 warps per SM)" if persistent else
+               "whole step in one cooperative kernel" if lib().tbsma_get_fused_step(self._h) == 1 else "one CTA per tile")
+        return "%d %s tiles, %s" % (n_tiles, "box" if box else "layer", how)
 
     def set_tile(self, layers_per_tile, threads):
         _check(lib().tbsma_set_tile(self._h, int(layers_per_tile), int(threads)), "tbsma_set_tile")

@@ -2480,3 +2480,10 @@ extern "C" int tbsma_get_tiling(const tbsma_ctx *c, int32_t *n_tiles, int32_t *b
     if (persistent) *persistent = tiles && use_persist(c) ? 1 : 0;
     return TBSMA_OK;
 }
+
+// 1 if tbsma_md_run's captured step of the current batch is the single cooperative kernel (tbsma_set_fused_step)
+extern "C" int tbsma_get_fused_step(const tbsma_ctx *c)
+{
+    if (!c) return TBSMA_EINVAL;
+    return tbsma_step_small_ok(c) && c->use_graph && c->use_cond ? 1 : 0;
+}
