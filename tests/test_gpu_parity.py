@@ -1256,3 +1256,46 @@ def test_fused_step_of_small_batches_is_bitwise_identical(B, name):
     assert ca.launch_count() < 0.45 * cb.launch_count()          # one kernel per ordinary step instead of six
     md = run_oracle_md(w, n_steps)
     assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+
+
+@pytest.mark.parametrize("depth", [2, 3])
+def test_persistent_gather_kernels_on_a_small_batch_match_one_cta_per_tile(B, depth):
+    """tbsma_set_gather(2 | 3): the persistent kernels forced onto a batch of a few tiles (every tile cut into parts, the
+    units claimed from the global counter, two or three images per CTA), with virial and closing kick: positions,
+    velocities and forces bit-identical to one CTA per tile, per-replica sums equal up to their fp64 summation order,
+    and the trajectory is the oracle's"""
+    w = W.config3(4, seed=51, length=60.0)
+    n_steps = 120
+
+    def run(mode):
+        ctx = B.make_context(w)
+        ctx.set_variant(2)
+        ctx.set_gather(mode)
+        ctx.set_fused_step(False)
+        st = B.DeviceState(w)
+        ctx.build_cells(st.pos, st.vel, st.tag)
+        ctx.build_neighbors(st.pos, st.vel, st.tag)
+        assert ctx.get_tiling()[2] == (mode != 0)
+        ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
+        torch.cuda.synchronize()
+        e0, w0 = st.e_rep.cpu().numpy().copy(), st.w_rep.cpu().numpy().copy()
+        stream = torch.cuda.Stream()
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate, 0,
+                       st.e_rep, st.w_rep, st.ekin)
+        torch.cuda.synchronize()
+        assert ctx.status() == 0
+        return ctx, st, e0, w0
+
+    ca, a, ea, wa = run(depth)
+    cb, b, eb, wb = run(0)
+    assert ca.get_stats() == cb.get_stats()
+    for nm in ("pos", "vel", "force"):
+        assert np.array_equal(a.untag(getattr(a, nm)), b.untag(getattr(b, nm))), nm
+    assert np.allclose(ea, eb, rtol=1e-12) and np.allclose(wa, wb, rtol=1e-11, atol=1e-9)
+    for nm in ("e_rep", "ekin", "w_rep"):
+        assert np.allclose(getattr(a, nm).cpu().numpy(), getattr(b, nm).cpu().numpy(), rtol=1e-11, atol=1e-9), nm
+    md = run_oracle_md(w, n_steps)
+    assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+    assert np.all(np.abs(a.e_rep.cpu().numpy() - md.e_rep) <= 10 * E_REL * np.abs(md.e_rep))
