@@ -1,5 +1,7 @@
-// tbsma_tile.cu -- the shared-memory ("wire") variant of the neighbour machinery and of the two
-// neighbour-gather passes for NON-PERIODIC replicas.
+// tbsma_tile.cu -- the shared-memory variant of the neighbour machinery and of the two neighbour-gather passes (SURVEY
+// rows a2, a3, a4, a6): layer tiles for thin wires (below), box tiles for thick wires and periodic replicas (TileDesc,
+// TileMap), persistent gather kernels for large batches (k_gather_persist), the whole step as one cooperative kernel
+// for small ones (k_step_small).
 //
 // The paper's systems are thin [100] wires and its best performance came with the
 // atoms ordered along the wire axis.  With cells numbered z-slowest, a run of z-layers of
