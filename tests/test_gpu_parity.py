@@ -1299,3 +1299,42 @@ def test_persistent_gather_kernels_on_a_small_batch_match_one_cta_per_tile(B, de
     md = run_oracle_md(w, n_steps)
     assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
     assert np.all(np.abs(a.e_rep.cpu().numpy() - md.e_rep) <= 10 * E_REL * np.abs(md.e_rep))
+
+
+def test_mixed_batch_of_layer_and_box_tiles(B):
+    """one batch holding a thin wire (cut into layer tiles), a 6 nm wire (its layers do not fit an image: box tiles) and a
+    second thin wire: lists bit for bit, forces and energies against the oracle, and a 60-step Langevin trajectory with the
+    lists renewed on the way; each replica's trajectory is the one it has alone (tiles are chosen per replica)"""
+    thin = W.displace(W.fcc_wire(30.0, 60.0), 0.05, 61)
+    thick = W.displace(W.fcc_wire(60.0, 70.0), 0.05, 62)
+    thin2 = W.displace(W.fcc_wire(30.0, 80.0), 0.05, 63)
+    wires = [thin, thick, thin2]
+    flags = [np.zeros(len(x), np.int32) for x in wires]
+    vels = [W.maxwell_velocities(len(x), 200.0, 70 + k, f == 0) for k, (x, f) in enumerate(zip(wires, flags))]
+    w = W._assemble("mixed_thin_thick_thin", wires, flags, vels, [200.0] * 3, [5, 6, 7], [0.0] * 3, 1e-3)
+    ctx, st = setup(B, w, variant=2, stagger=False)
+    n_tiles, box, persistent = ctx.get_tiling()
+    assert box and not persistent and n_tiles > 6
+    cg, lg = gpu_neighbors(B, ctx, st)
+    co, lo = oracle.neighbors(w.pos4, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=96)
+    assert_same_sets(cg, lg, co, lo)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    torch.cuda.synchronize()
+    o = oracle.compute(w.x64(), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi)
+    assert_forces(st.untag(st.force)[:, :3].astype(np.float64), o["f"])
+    assert np.all(np.abs(st.e_rep.cpu().numpy() - o["e_rep"]) <= E_REL * np.abs(o["e_rep"]))
+    n_steps = 60
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate, 0,
+                   st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0 and ctx.get_stats()["n_replica_builds"] > 3
+    md = run_oracle_md(w, n_steps)
+    xg = st.untag(st.pos)
+    assert traj_rms(xg[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+    # the thin wire alone is cut into the same tiles: same bits
+    single = w.take(0, 1)
+    _, ss = run_gpu_md(B, single, n_steps, variant=2, stagger=False)
+    assert np.array_equal(xg[:w.offsets[1]], ss.untag(ss.pos))
