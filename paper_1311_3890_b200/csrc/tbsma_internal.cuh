@@ -284,9 +284,13 @@ __device__ inline void tbsma_reduce_replicas(const TileSums &ts, int R)
         if (r >= R) return;
         double acc[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         const int j0 = ts.tile_first[r] * ts.nsplit, j1 = ts.tile_first[r + 1] * ts.nsplit;
-        for (int j = j0 + lane; j < j1; j += 32)
-            for (int q = 0; q < nq; ++q) acc[q] += ts.cta_sums[8 * (size_t)j + q];
-        for (int q = 0; q < nq; ++q)
+        for (int j = j0 + lane; j < j1; j += 32) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+                if (q < nq) acc[q] += ts.cta_sums[8 * (size_t)j + q];
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
             for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
         if (lane == 0) {
             if (ts.e_rep) ts.e_rep[r] = acc[0];
@@ -301,14 +305,22 @@ __device__ inline void tbsma_reduce_replicas(const TileSums &ts, int R)
     for (int r = 0; r < R; ++r) {
         double acc[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         const int j0 = ts.tile_first[r] * ts.nsplit, j1 = ts.tile_first[r + 1] * ts.nsplit;
-        for (int j = j0 + (int)threadIdx.x; j < j1; j += 256)
-            for (int q = 0; q < nq; ++q) acc[q] += ts.cta_sums[8 * (size_t)j + q];
+        // (unrolled over the eight quantities with a guard: a run-time index would put acc[] into local memory)
+        for (int j = j0 + (int)threadIdx.x; j < j1; j += 256) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+                if (q < nq) acc[q] += ts.cta_sums[8 * (size_t)j + q];
+        }
         __syncthreads();
-        for (int q = 0; q < nq; ++q) red[q][threadIdx.x] = acc[q];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) red[q][threadIdx.x] = acc[q];
         __syncthreads();
         for (int o = 128; o > 0; o >>= 1) {
-            if ((int)threadIdx.x < o)
-                for (int q = 0; q < nq; ++q) red[q][threadIdx.x] += red[q][threadIdx.x + o];
+            if ((int)threadIdx.x < o) {
+#pragma unroll
+                for (int q = 0; q < 8; ++q)
+                    if (q < nq) red[q][threadIdx.x] += red[q][threadIdx.x + o];
+            }
             __syncthreads();
         }
         if (threadIdx.x == 0) {
