@@ -313,14 +313,14 @@ int run_steps(tbsma_ctx *c, float4 *pos, float4 *vel, float4 *force, int32_t *ta
             // (after the chain: idle, its kernels take 1.5 us each on an empty GPU, but each would wait for room on every SM
             // behind a filter kernel already running)
             if (async && c->overlap == 2 && !c->timing && st) {
-                CK(tbsma_launch_tile_inner(c, pos, 0, st));
+                CK(tbsma_launch_tile_inner(c, pos, 0, st, true));
                 early = true;
                 forked = true;       // (nothing to join: same stream)
                 joined = true;
             } else if (async && c->overlap && !c->timing && c->aux_stream) {
                 CK(cudaEventRecord(c->ev_fork, st));
                 CK(cudaStreamWaitEvent(c->aux_stream, c->ev_fork, 0));
-                CK(tbsma_launch_tile_inner(c, pos, 0, c->aux_stream));
+                CK(tbsma_launch_tile_inner(c, pos, 0, c->aux_stream, true));
                 CK(cudaEventRecord(c->ev_join, c->aux_stream));
                 forked = true;
             }

@@ -383,7 +383,7 @@ cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int3
 // tiles of the dirty replicas, from the flags; use_cond: also sets the graph conditional `cond` (any replica with dirty == 2)
 cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st, unsigned long long cond = 0ull, int use_cond = 0);
 // inner lists of the replicas on work list `which` (0: dirty == 1, 1: dirty == 2), written to the buffer not in use
-cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, int which, cudaStream_t st);
+cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, int which, cudaStream_t st, bool beside = false);
 cudaError_t tbsma_launch_stage_copy(tbsma_ctx *c, const float4 *pos, const float4 *vel, const int32_t *tag,
                                     cudaStream_t st);
 // sync_level: the gather passes read the freshly written half of the list buffers for replicas with

@@ -2261,15 +2261,17 @@ cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st, unsigned l
     return cudaGetLastError();
 }
 
-cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, int which, cudaStream_t st)
+cudaError_t tbsma_launch_tile_inner(tbsma_ctx *c, const float4 *pos, int which, cudaStream_t st, bool beside)
 {
     int nsplit = (c->own_cap + kInnerThreads - 1) / kInnerThreads;
     if (nsplit < 1) nsplit = 1;
     const int64_t units = (int64_t)c->n_tiles * nsplit;
     const size_t sm = inner_smem(c);
-    // list 0 is worked on beside the gather passes of the step (second stream): two CTAs per SM leave most of the
-    // shared memory and registers to them; list 1 (and the first build of everything) runs alone
-    int per_sm = which == 0 ? 2 : (int)((200 * 1024) / (sm + 1024));
+    // Beside the gather passes of the step (their kernels fill the register file: a filter CTA on an SM keeps a gather CTA
+    // off it) the pass gets ONE CTA per SM; measured against two: config 4 1.0081 -> 0.9941 ms, config 3 0.5208 -> 0.5186 ms
+    // per step.  Run on its own (first build, fixed cadence, new candidates) it takes what fits.
+    int per_sm = 1;
+    if (!beside && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_tile_inner, kInnerThreads, sm) != cudaSuccess) per_sm = 1;
     if (per_sm > 4) per_sm = 4;
     if (per_sm < 1) per_sm = 1;
     const int64_t cap = (int64_t)per_sm * c->n_sm;
