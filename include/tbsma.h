@@ -183,7 +183,7 @@ int tbsma_get_stats(tbsma_ctx *ctx, tbsma_stats *h_out); /* synchronises */
  *   2 = shared-memory tiles: a CTA stages the positions of a tile of cells (a run of z-layers of a thin wire, a box of
  *       cells of a thick wire or of a periodic replica) and of the cells around it in shared memory; 16-bit list
  *       entries, atoms ordered by list length inside a layer (or cell), lists ordered for conflict-free shared-memory
- *       gathers.  tbsma_build_cells returns TBSMA_EINVAL if a replica does not fit (a periodic axis shorter than five
+ *       gathers.  tbsma_build_cells returns TBSMA_EINVAL if a replica does not fit (a periodic axis shorter than three
  *       cells of r_cut + skin + S, a cell neighbourhood of more than 4095 atoms);
  *   0 = auto (default): 2 when it fits, else 1.
  * tbsma_get_variant returns the variant the current lists were built for. */

@@ -146,7 +146,7 @@ int set_geometry(tbsma_ctx *c, double width)
 }
 
 // The shared-memory tile variant cuts a periodic replica into boxes of cells with a one-cell halo that must not wrap onto
-// itself: at least five cells (of the candidate radius) along every periodic axis.  Shorter periodic boxes use the global
+// itself: at least three cells (of the candidate radius) along every periodic axis.  Shorter periodic boxes use the global
 // variant with its own, narrower cells.
 bool tiles_possible(const tbsma_ctx *c)
 {
@@ -154,7 +154,7 @@ bool tiles_possible(const tbsma_ctx *c)
     const double w_min = (c->r_cut + c->skin + c->outer_skin) * (1.0 + 1e-5) + 1e-4;
     for (int r = 0; r < c->R; ++r)
         for (int a = 0; a < 3; ++a)
-            if ((c->h_geom[r].periodic >> a & 1) && (int)floor((double)c->h_geom[r].len[a] / w_min) < 5) return false;
+            if ((c->h_geom[r].periodic >> a & 1) && (int)floor((double)c->h_geom[r].len[a] / w_min) < 3) return false;
     return true;
 }
 

@@ -64,7 +64,11 @@ struct TileDesc {
     // A tile whose halo wraps around periodic axis a sees a record from across the boundary at a raw coordinate
     // difference beyond half the box: D:A6's `if (d > L/2) d -= L; else if (d < -L/2) d += L` is, for every pair of an own
     // atom and a staged record of THIS tile, `if (|d| > hL[a]) d += Ls[a]` with Ls = -L for a tile at the upper end of the
-    // axis, +L at the lower end (a tile is never at both: tbsma_tile_setup wants 2 own + 3 cells per periodic axis)
+    // axis, +L at the lower end.  A tile is never at both ends and sees no cell twice because a periodic axis holds at
+    // least b + 2 cells for a box of b (tbsma_tile_setup).  With so few cells the two forms can differ in VALUE for pairs
+    // more than a cell width w apart (an unwrapped record beyond L/2, which D:A6 would fold back to L - |d| > w), never in
+    // the decision: both values exceed w >= r_cut + skin + S.  Every pair that is a member has |d| < w <= L/3 on the near
+    // side or L - |d| < w on the far side, where both forms do the same operation.
     float Ls[3], hL[3];   // 0 and +inf on an axis this tile does not wrap
 };
 // Layout of every neighbour list (int4 rows of the global variant, uint2 rows of the tile variant, candidates too):

@@ -1879,12 +1879,12 @@ static const int kBoxCand[][3] = {{3, 3, 3}, {3, 3, 2}, {3, 2, 2}, {2, 2, 2}, {3
 constexpr int kNBoxCand = sizeof(kBoxCand) / sizeof(kBoxCand[0]);
 
 // own box b (clipped to the grid) of candidate cand for replica geometry g; false if a periodic axis is too short for it
-// (a tile must not see a cell twice, and must wrap at one end of an axis only: nc >= 2 b + 3)
+// (a tile must not see a cell twice and must wrap at one end of an axis only: nc >= b + 2, see TileDesc)
 static bool box_dims(const RepGeom &g, int cand, int b[3])
 {
     for (int a = 0; a < 3; ++a) {
         b[a] = kBoxCand[cand][a] < g.nc[a] ? kBoxCand[cand][a] : g.nc[a];
-        if ((g.periodic >> a & 1) && g.nc[a] < 2 * b[a] + 3) return false;
+        if ((g.periodic >> a & 1) && g.nc[a] < b[a] + 2) return false;
     }
     return true;
 }
@@ -1904,7 +1904,7 @@ k_box_measure(const RepGeom *__restrict__ geom, const int *__restrict__ cell_sta
     bool ok = true;
     for (int a = 0; a < 3; ++a) {
         b[a] = min(cand[cnd][a], g->nc[a]);
-        if ((g->periodic >> a & 1) && g->nc[a] < 2 * b[a] + 3) ok = false;
+        if ((g->periodic >> a & 1) && g->nc[a] < b[a] + 2) ok = false;
         nt[a] = (g->nc[a] + b[a] - 1) / b[a];
     }
     int mh = 0, mo = 0;

@@ -29,8 +29,8 @@ VARIANTS = [1, 2]     # 1 = global-gather lists, 2 = shared-memory tiles (non-pe
 
 
 def setup(B, w, max_nb=96, variant=0, tile=None, stagger=True, box=False):
-    if variant == 2 and np.any(w.periodic) and float((w.box_hi - w.box_lo)[w.periodic != 0].min()) < 5 * 9.81:
-        pytest.skip("the shared-memory tile variant needs five cells of r_cut + skin + S along a periodic axis")
+    if variant == 2 and np.any(w.periodic) and float((w.box_hi - w.box_lo)[w.periodic != 0].min()) < 3 * 9.81:
+        pytest.skip("the shared-memory tile variant needs three cells of r_cut + skin + S along a periodic axis")
     ctx = B.make_context(w, max_nb)
     ctx.set_variant(variant)
     if tile:
@@ -1168,7 +1168,7 @@ def test_youngs_modulus_of_the_papers_smallest_wire(B):
 
 
 # ---- box tiles (thick wires, periodic bulk; tbsma_set_tile_box forces them on thin wires) -------------------------------
-BOX_WORKLOADS = ["config1", "config2", "config4_ragged", "bulk_13", "bulk_18", "thick_wire"]
+BOX_WORKLOADS = ["config1", "config2", "config4_ragged", "bulk_9", "bulk_13", "bulk_18", "thick_wire"]
 
 
 @pytest.mark.parametrize("name", BOX_WORKLOADS)
@@ -1195,7 +1195,7 @@ def test_box_tiles_lists_forces_energy(B, name):
     assert n_list == int(co.sum()) and 0 < n_cut <= n_list
 
 
-@pytest.mark.parametrize("name", ["config2", "bulk_13", "thick_wire"])
+@pytest.mark.parametrize("name", ["config2", "bulk_9", "bulk_13", "thick_wire"])
 def test_box_tiles_trajectory_100_steps(B, name):
     """100 steps on box tiles against the oracle: a pulled Langevin wire (lists renewed from their candidates as atoms
     move), periodic bulk and a thick wire with the fixed cadence of BASELINE config 5"""
