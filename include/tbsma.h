@@ -53,7 +53,8 @@ enum {
     TBSMA_EINVAL = -1, /* bad argument (NULL, negative size, box shorter than 2 (r_cut+skin) on a periodic axis) */
     TBSMA_ENOMEM = -2, /* device or host allocation failed */
     TBSMA_ECUDA = -3,  /* a CUDA runtime call failed (or no device) */
-    TBSMA_ESTATE = -4  /* call order violated (e.g. compute before build_neighbors) */
+    TBSMA_ESTATE = -4, /* call order violated (e.g. compute before build_neighbors) */
+    TBSMA_ELIMIT = -5  /* a size exceeds the fixed capacity of a no-allocation entry point (tbsma_kinetic_tensor_noalloc) */
 };
 
 /* bits of the status word returned by tbsma_status */
@@ -163,6 +164,48 @@ int tbsma_md_run_host(tbsma_ctx *ctx, float *h_pos, float *h_vel, float *h_force
 int tbsma_kinetic_tensor(tbsma_ctx *ctx, const float *d_pos, const float *d_vel, double *d_replica_kinetic, void *stream);
 int tbsma_stress(tbsma_ctx *ctx, const double *d_replica_virial, const double *d_replica_kinetic,
                  const double *d_volume, double *d_sigma, void *stream);
+
+/* tbsma_kinetic_tensor for callers that cannot allocate device memory.
+ *
+ * Everything else in this header needs a tbsma_ctx, and a context gets its tables from cudaMalloc (tbsma_set_system,
+ * tbsma_build_cells).  That rules the library out for a caller whose process has already handed the GPU's memory to a pool
+ * of its own (an MD engine or a training framework this code is plugged into: a cudaMalloc there fails, or takes memory the
+ * pool's owner counts as its own), for a hook that runs between the steps of a loop that must not stall (cudaMalloc and
+ * cudaFree synchronise the whole device), and for a job that was given a fixed memory budget.  This one call needs no
+ * context and calls no cudaMalloc, cudaFree or other allocating routine, on its first call or any later one.
+ *
+ * It computes what tbsma_kinetic_tensor computes, K_ab = sum_i m v_i,a v_i,b over the dynamic atoms (flag 0 in pos.w) of
+ * every replica, in eV, order xx yy zz xy xz yz (Eq.5 as read in D:A11), from
+ *   d_pos, d_vel          n_atoms x 4 floats each, DEVICE, the layouts of the top of this file (only pos.w and vel.xyz
+ *                         are read)
+ *   d_replica_offsets     n_replicas + 1 int32, DEVICE (not host, unlike tbsma_set_system): atoms of replica r are
+ *                         [off[r], off[r+1]); an empty replica gets K = 0
+ *   mass_amu              atomic mass (tbsma_params.mass_amu)
+ *   d_replica_kinetic     out, n_replicas x 6 doubles, DEVICE; overwritten, need not be cleared
+ * asynchronously on `stream`.  All buffers stay the caller's.  The sums are added in a fixed order (which depends on
+ * n_atoms, n_replicas and the offsets only), so the result is bitwise repeatable; it agrees with tbsma_kinetic_tensor,
+ * which adds with atomics, to fp64 rounding.
+ *
+ * The working memory of the kernel (per-slice partial sums and one counter per replica) is a fixed array of
+ * TBSMA_NOALLOC_SCRATCH_BYTES (784 KiB) inside the library's device code.  Consequences a caller must know:
+ *   - Limits: n_replicas <= TBSMA_NOALLOC_MAX_REPLICAS (4096) and n_atoms <= TBSMA_NOALLOC_MAX_ATOMS (int32 offsets).
+ *     Beyond them the call does nothing and returns TBSMA_ELIMIT; split the batch into several calls.
+ *   - Every GPU on which the CUDA runtime loads this library holds those 784 KiB until the process exits, used or not.
+ *   - There is one array per GPU, shared by all callers, threads and streams of the process.  Calls that can execute on
+ *     the same GPU at the same time (different streams with no dependency between them) overwrite each other's partial
+ *     sums and counters: wrong results, no error.  Put the calls on one stream or order them with events.  Calls that run
+ *     one after the other need no care: the array keeps the previous call's contents, and every call first clears the
+ *     counters it will use (on `stream`) and writes every partial sum before reading it.
+ *   - The first call on a GPU (with that GPU current) looks up the array's device address and caches it; the runtime may
+ *     load the library's device code at that point.  Make that first call before you begin any stream capture.
+ * Errors: TBSMA_EINVAL (NULL pointer, negative size, mass <= 0), TBSMA_ELIMIT, TBSMA_ECUDA (no device, launch failed). */
+#define TBSMA_NOALLOC_MAX_REPLICAS 4096
+#define TBSMA_NOALLOC_MAX_SLOTS 16384 /* (replica, slice) partial sums; slices per replica = min(256, 16384 / n_replicas, ...) */
+#define TBSMA_NOALLOC_MAX_ATOMS 2147483647
+#define TBSMA_NOALLOC_SCRATCH_BYTES 802816 /* 4096 x 4 + 16384 x 6 x 8 */
+int tbsma_kinetic_tensor_noalloc(const float *d_pos, const float *d_vel, const int32_t *d_replica_offsets,
+                                 int64_t n_atoms, int32_t n_replicas, double mass_amu, double *d_replica_kinetic,
+                                 void *stream);
 
 /* Neighbour lists in TAG space for parity checks: d_counts[t] and d_list[t*max_neighbors + k]
  * (k < count, unsorted) for the atom whose tag is t.  d_tag as left by tbsma_build_cells. */

@@ -13,13 +13,14 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtbsma.so")
 
-OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ELIMIT = 0, -1, -2, -3, -4, -5
+NOALLOC_MAX_REPLICAS = 4096          # TBSMA_NOALLOC_MAX_REPLICAS of tbsma.h
 FLAG_NLIST_OVERFLOW, FLAG_OUT_OF_BOX, FLAG_NONFINITE, FLAG_SKIN_VIOLATED, FLAG_TILE_OVERFLOW = 1, 2, 4, 8, 16
 
 EXPORTS = [
     "tbsma_create", "tbsma_destroy", "tbsma_set_system", "tbsma_build_cells", "tbsma_build_neighbors",
     "tbsma_compute", "tbsma_md_step", "tbsma_md_run", "tbsma_md_run_host", "tbsma_get_neighbors",
-    "tbsma_count_pairs", "tbsma_kinetic_tensor", "tbsma_stress", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
+    "tbsma_count_pairs", "tbsma_kinetic_tensor", "tbsma_kinetic_tensor_noalloc", "tbsma_stress", "tbsma_status", "tbsma_clear_status", "tbsma_get_stats", "tbsma_set_variant",
     "tbsma_get_variant", "tbsma_get_tiling", "tbsma_set_tile", "tbsma_set_overlap", "tbsma_set_stagger", "tbsma_set_thermostat", "tbsma_get_thermostat", "tbsma_set_thermostat_state", "tbsma_set_async", "tbsma_set_balance", "tbsma_set_outer_skin", "tbsma_set_tile_split", "tbsma_set_gather", "tbsma_set_tile_box", "tbsma_set_fused_step", "tbsma_get_fused_step",
     "tbsma_set_protocol", "tbsma_set_series", "tbsma_series_histogram",
     "tbsma_set_graph", "tbsma_set_timing", "tbsma_get_timing", "tbsma_launch_count", "tbsma_strerror", "tbsma_version",
@@ -80,6 +81,7 @@ def lib():
         L.tbsma_md_run_host.argtypes = [vp, vp, vp, vp, vp, dbl, vp, dbl, vp, C.c_uint64, i64, vp, vp, i32, vp, vp, vp]
         L.tbsma_get_neighbors.argtypes = [vp, vp, vp, vp, vp]
         L.tbsma_kinetic_tensor.argtypes = [vp, vp, vp, vp, vp]
+        L.tbsma_kinetic_tensor_noalloc.argtypes = [vp, vp, vp, i64, i32, dbl, vp, vp]
         L.tbsma_stress.argtypes = [vp, vp, vp, vp, vp, vp]
         L.tbsma_count_pairs.argtypes = [vp, vp, C.POINTER(i64), C.POINTER(i64), vp]
         L.tbsma_status.argtypes = [vp, C.POINTER(C.c_uint32)]
@@ -146,6 +148,21 @@ def _stream(stream):
 def _check(rc, what):
     if rc != 0:
         raise TbsmaError(rc, what)
+
+
+def kinetic_tensor_noalloc(pos, vel, replica_offsets, k_rep, mass_amu=None, stream=None):
+    """tbsma_kinetic_tensor_noalloc: the kinetic tensor of every replica without a Context and without any device
+    allocation by the library -- for a caller that lives inside somebody else's memory pool, or between the steps of a loop
+    that cannot take the device-wide stall of a cudaMalloc.  All four tensors are the caller's CUDA tensors:
+    pos, vel (n x 4 float32), replica_offsets (R + 1 int32, ON THE DEVICE), k_rep (R x 6 float64, overwritten).  The
+    library's working memory is one fixed array per GPU shared by every call: at most NOALLOC_MAX_REPLICAS replicas
+    (TbsmaError with code ELIMIT beyond), and calls must not overlap on the GPU (same stream, or ordered by events).
+    Make the first call on a GPU outside any stream capture."""
+    assert replica_offsets.dtype == torch.int32 and k_rep.dtype == torch.float64
+    n, R = int(pos.shape[0]), int(replica_offsets.numel()) - 1
+    m = au_params().mass_amu if mass_amu is None else float(mass_amu)
+    _check(lib().tbsma_kinetic_tensor_noalloc(_dp(pos), _dp(vel), _dp(replica_offsets), n, R, m, _dp(k_rep),
+                                              _stream(stream)), "tbsma_kinetic_tensor_noalloc")
 
 
 class Context:

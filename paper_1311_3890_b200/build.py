@@ -11,7 +11,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtbsma.so")
-SOURCES = ["tbsma_api.cu", "tbsma_cells.cu", "tbsma_force.cu", "tbsma_integrate.cu", "tbsma_tile.cu"]
+SOURCES = ["tbsma_api.cu", "tbsma_cells.cu", "tbsma_force.cu", "tbsma_integrate.cu", "tbsma_tile.cu",
+           "tbsma_noalloc.cu"]
 
 
 def _stale():

@@ -359,6 +359,7 @@ const char *tbsma_strerror(int code)
         case TBSMA_ENOMEM: return "out of memory";
         case TBSMA_ECUDA: return "CUDA runtime error (or no CUDA device)";
         case TBSMA_ESTATE: return "call order violated";
+        case TBSMA_ELIMIT: return "size exceeds the fixed capacity of a no-allocation entry point";
         default: return "unknown error";
     }
 }
