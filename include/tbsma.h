@@ -64,7 +64,9 @@ enum {
     TBSMA_FLAG_NONFINITE = 4u,      /* a non-finite force was produced */
     TBSMA_FLAG_SKIN_VIOLATED = 8u,  /* with a fixed rebuild cadence an atom moved more than skin/2 between rebuilds */
     TBSMA_FLAG_TILE_OVERFLOW = 16u  /* shared-memory variant: a tile's halo outgrew its shared-memory image (sized at
-                                       tbsma_build_cells with 25 % headroom); that tile was skipped, results invalid */
+                                       tbsma_build_cells from the populations found then, with 25 % headroom for layer
+                                       tiles and 2.5 - 10 % for box tiles, as much as costs no residency); that tile was
+                                       skipped, results invalid: call tbsma_build_cells again, or use variant 1 */
 };
 
 typedef struct {
@@ -268,7 +270,9 @@ int tbsma_set_tile_box(tbsma_ctx *ctx, int32_t force);
  * kick, per-replica sums, bookkeeping -- is one cooperative kernel with three grid-wide barriers in place of five kernel
  * boundaries (the paper's "+35 % run time due to thread synchronization" between its two stages, is this cost).
  * A step in which a replica needs a new list runs the separate kernels instead (decided on the device).  enable = 0:
- * always the separate kernels.  Default 1.  Changes cost, never results (same operations in the same order). */
+ * always the separate kernels.  Default 1.  Changes cost, never results (same operations in the same order), and may be
+ * called before or after tbsma_build_cells: how a small batch's tiles are cut into parts (which fixes the grouping of the
+ * per-replica sums) does not depend on it. */
 int tbsma_set_fused_step(tbsma_ctx *ctx, int32_t enable);
 /* 1 if the captured step of tbsma_md_run is that single kernel for the batch as it is now built, else 0. */
 int tbsma_get_fused_step(const tbsma_ctx *ctx);
@@ -367,7 +371,8 @@ int tbsma_set_protocol(tbsma_ctx *ctx, const tbsma_protocol *protocol);
  *     [2] sigma_zz = -(W_zz + K_zz) / d_volume[r] in eV/A^3 (Eq.5 as read in D:A11; z is the wire axis, tension positive;
  *         V is the caller's constant "hard-sphere" volume)
  *     [3] the largest gap (A) between consecutive z coordinates of the replica's atoms (exact when wider than 1/2048 of
- *         the replica's box along z)
+ *         the z range the replica's atoms occupy at that step, wherever they are: atoms pulled beyond the box given to
+ *         tbsma_set_system count like all others; on a periodic z axis the gap across the boundary is not looked at)
  * and d_count[r] is incremented (the caller zeroes it; recording stops silently at `capacity`).  d_rupture_step[r]
  * (nullable; the caller sets -1) receives the first recorded s whose gap exceeds r_cut: no interaction crosses the gap
  * any more, the wire has parted ("until rupture").  While a series is on, every step evaluates the virial.

@@ -172,7 +172,9 @@ __global__ void k_stress(const double *__restrict__ w_rep, const double *__restr
 //   in D:A11, z = the wire axis) | largest gap between consecutive z coordinates of the replica's atoms
 // and notes the first step whose gap exceeds r_cut: the wire has parted ("until rupture").  K_zz is added in a fixed
 // order (thread-strided partial sums, then a tree).  The gap comes from 2048 bins along z holding the least and the
-// greatest z that fell into them: exact whenever it is wider than a bin.
+// greatest z that fell into them: exact whenever it is wider than a bin.  The bins span the z range the replica's atoms
+// occupy AT THIS STEP (a first pass finds it), not the box given to tbsma_set_system: a slab pulled beyond the box, and a
+// gap that opens out there, are seen like any other.  (A periodic z axis: the gap across the boundary is not looked at.)
 #define TBSMA_SERIES_BINS 2048
 __device__ __forceinline__ int ord_of(float f) { const int k = __float_as_int(f); return k >= 0 ? k : k ^ 0x7fffffff; }
 __device__ __forceinline__ float f_of(int k) { return __int_as_float(k >= 0 ? k : k ^ 0x7fffffff); }
@@ -192,9 +194,24 @@ k_series_record(const float4 *__restrict__ pos, const float4 *__restrict__ vel, 
     const int idx = S.d_count[r];
     if (idx >= S.capacity) return;
     const RepGeom *g = geom + r;
+    __shared__ int s_zlo, s_zhi;
     for (int b = tid; b < TBSMA_SERIES_BINS; b += 256) { s_mn[b] = 0x7fffffff; s_mx[b] = (int)0x80000000; }
+    if (tid == 0) { s_zlo = 0x7fffffff; s_zhi = (int)0x80000000; }
     __syncthreads();
-    const float z0 = g->lo[2], inv_w = g->len[2] > 0.f ? (float)TBSMA_SERIES_BINS / g->len[2] : 0.f;
+    {
+        int zlo = 0x7fffffff, zhi = (int)0x80000000;
+        for (int i = g->atom_begin + tid; i < g->atom_end; i += 256) {
+            const int o = ord_of(pos[i].z);
+            zlo = min(zlo, o);
+            zhi = max(zhi, o);
+        }
+        zlo = __reduce_min_sync(0xffffffffu, zlo);
+        zhi = __reduce_max_sync(0xffffffffu, zhi);
+        if ((tid & 31) == 0) { atomicMin(&s_zlo, zlo); atomicMax(&s_zhi, zhi); }
+    }
+    __syncthreads();
+    const float z0 = f_of(s_zlo), span = g->atom_end > g->atom_begin ? f_of(s_zhi) - z0 : 0.f;
+    const float inv_w = span > 0.f ? (float)TBSMA_SERIES_BINS / span : 0.f;
     double k = 0.0;
     for (int i = g->atom_begin + tid; i < g->atom_end; i += 256) {
         const float4 p = pos[i];

@@ -199,7 +199,9 @@ struct tbsma_ctx {
     float *d_stagger;       // R: factor on (skin/2)^2 until the replica's first rebuild (spreads the rebuilds of
                             // replicas that start together over the steps); 1 afterwards
     int stagger;            // enabled (default 1)
-    int32_t *d_ctrl;        // [0] any replica dirty, [1] status flags, [2] max neighbours seen, [3] any dirty == 2
+    int32_t *d_ctrl;        // [0] any replica dirty, [1] status flags, [2] max neighbours seen, [3] any dirty == 2,
+                            // [4] / [5] next unit of the persistent density / force pass (k_gather_persist; zeroed ahead of
+                            // every density pass by k_tile_worklist or a memset, and by the opposite pass), [6..7] unused
     unsigned long long *d_counters; // [0] step offset inside md_run, [1] replica builds, [2] build passes, [3] steps,
                                     // [4..5] count_pairs scratch, [6] replica builds that redid cells + candidates,
                                     // [7] step number of the first step of the md_run in flight (captured steps read it)

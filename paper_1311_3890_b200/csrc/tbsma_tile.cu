@@ -224,10 +224,12 @@ __global__ void k_layer_maxpop(const RepGeom *__restrict__ geom, const int *__re
 // (new cells and candidates first), then the two tile lists.
 __global__ void __launch_bounds__(256)
 k_tile_worklist(const int *__restrict__ dirty, const int *__restrict__ tile_first, int *__restrict__ work, int R,
-                int n_tiles, cudaGraphConditionalHandle cond, int use_cond)
+                int n_tiles, cudaGraphConditionalHandle cond, int use_cond, int *__restrict__ claims)
 {
     __shared__ int s_base[2], s_warp[2][8];
-    if (threadIdx.x < 2) s_base[threadIdx.x] = 0;
+    // unit counters of the persistent gather passes of this step (ctrl[4..5]): they start every step at zero whatever the
+    // step before left behind (a pass that was launched without its partner, a launch that failed)
+    if (threadIdx.x < 2) { s_base[threadIdx.x] = 0; claims[threadIdx.x] = 0; }
     __syncthreads();
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     for (int r0 = 0; r0 < R; r0 += 256) {
@@ -1512,7 +1514,8 @@ struct PArgs {
     KickArgs kk;
     int *ctrl;
     int *claim;            // this pass's unit counter
-    int *claim_other;      // the other pass's, reset here (the two passes never run together)
+    int *claim_other;      // the other pass's, reset here (the two passes never run together); both are also zeroed ahead
+                           // of the density pass: by k_tile_worklist inside a step, by a memset node otherwise
     ListSel ls;
     int n_pad, s_cap, img_cap;
     int nb;                // image buffers per CTA (2 .. kPMaxBuf)
@@ -1971,7 +1974,7 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
     if (lmax < 1) lmax = 1;
     if (lmax > TBSMA_TILE_MAX_LAYERS) lmax = TBSMA_TILE_MAX_LAYERS;
     int64_t n_tiles = 0;
-    int cell_cap = 0, rec_cap = 0, own_cap = 0;
+    int cell_cap = 0, rec_cap = 0, own_cap = 0, box_min = 0, box_want = 0;
     bool fits = true, any_box = false;
     int *Lr = (int *)malloc(sizeof(int) * R);      // > 0: own layers per tile (kind 0); <= 0: -(box candidate) (kind 1)
     if (!Lr) { free(maxpop); return TBSMA_ENOMEM; }
@@ -2023,11 +2026,45 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
             int b[3];
             box_dims(g, pick, b);
             const int mh = meas[((size_t)r * kNBoxCand + pick) * 2], mo = meas[((size_t)r * kNBoxCand + pick) * 2 + 1];
-            if (mh + mh / 40 + 8 > rec_cap) rec_cap = mh + mh / 40 + 8;
+            // A candidate is taken when its halo fits with 2.5 % to spare; the image is then sized with up to 10 %
+            // (below): later rebuilds of the cells inside tbsma_md_run (a thick wire strained or compressed, atoms
+            // diffusing between cells) cannot resize it.
+            if (mh + mh / 40 + 8 > box_min) box_min = mh + mh / 40 + 8;
+            int want = mh + mh / 10 + 8;
+            if (want > cap) want = cap;
+            if (want > box_want) box_want = want;
             if (mo + mo / 20 + 16 > own_cap) own_cap = mo + mo / 20 + 16;
             n_tiles += (int64_t)((g.nc[0] + b[0] - 1) / b[0]) * ((g.nc[1] + b[1] - 1) / b[1]) * ((g.nc[2] + b[2] - 1) / b[2]);
         }
         free(meas);
+        if (fits && box_min > 0) {
+            // Image size of the box tiles: between what the 2.5 % rule needs and 10 % headroom, the largest that costs
+            // no CTA per SM in the kernels whose residency the image decides (the list filter, whose shared memory is the
+            // image plus a column per thread, and the gather passes).  Measured on the 64^3 block: 10 % regardless took
+            // the filter kernel from two CTAs per SM to one and the list renewal from 0.153 to 0.219 ms per step.
+            int per_sm = 0, dev = 0;
+            cudaFuncAttributes fa_inner = {}, fa_gather = {};
+            e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+            if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa_inner, k_tile_inner);
+            if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa_gather, k_force_tile<false, true, false>);
+            if (e != cudaSuccess) { free(Lr); return TBSMA_ECUDA; }
+            auto img_of = [](int rec) {
+                int img = rec + rec / 8 + 64 + 1;
+                if (img > TBSMA_TILE_MAX_RECORDS + 1) img = TBSMA_TILE_MAX_RECORDS + 1;
+                return img < rec + 1 ? rec + 1 : img;
+            };
+            auto resident = [&](int rec, int which) {
+                const size_t dyn = (size_t)img_of(rec) * 16 + (which == 0 ? (size_t)kInnerThreads * (c->kmax + 1) * 2 : 0);
+                const size_t stat = which == 0 ? fa_inner.sharedSizeBytes : fa_gather.sharedSizeBytes;
+                return (int)((size_t)per_sm / (dyn + stat + 1024));
+            };
+            const int lo = rec_cap > box_min ? rec_cap : box_min, hi = box_want > lo ? box_want : lo;
+            int pick = lo;
+            for (int rcand = hi; rcand > lo; rcand -= 8)
+                if (resident(rcand, 0) == resident(lo, 0) && resident(rcand, 1) == resident(lo, 1)) { pick = rcand; break; }
+            rec_cap = pick;
+        }
     }
     if (!fits || n_tiles > 0x7fffffff) {
         free(Lr);
@@ -2211,8 +2248,10 @@ int tbsma_tile_setup(tbsma_ctx *c, cudaStream_t st)
         TBSMA_FUSED(false, false) TBSMA_FUSED(false, true) TBSMA_FUSED(true, false) TBSMA_FUSED(true, true)
 #undef TBSMA_FUSED
         c->fused_max_ctas = e == cudaSuccess ? min_occ * c->n_sm : 0;
-        // a batch that would fit the fused step with fewer parts per tile gets fewer parts
-        if (c->fused_step && c->tile_split_req <= 0 && c->n_tiles <= c->fused_max_ctas &&
+        // a batch that would fit the fused step with fewer parts per tile gets fewer parts -- whether or not the fused step
+        // is switched on: the parts fix the grouping of the per-replica fp64 sums, and tbsma_set_fused_step promises to
+        // change cost only, whenever it is called
+        if (c->tile_split_req <= 0 && c->n_tiles <= c->fused_max_ctas &&
             (int64_t)c->n_tiles * c->tile_nsplit > c->fused_max_ctas)
             c->tile_nsplit = c->fused_max_ctas / c->n_tiles;
     }
@@ -2256,7 +2295,7 @@ cudaError_t tbsma_launch_tile_lists(tbsma_ctx *c, float4 *pos, float4 *vel, int3
 cudaError_t tbsma_launch_tile_worklist(tbsma_ctx *c, cudaStream_t st, unsigned long long cond, int use_cond)
 {
     k_tile_worklist<<<1, 256, 0, st>>>(c->d_dirty, c->d_tile_first, c->d_work, c->R, c->n_tiles,
-                                       (cudaGraphConditionalHandle)cond, use_cond);
+                                       (cudaGraphConditionalHandle)cond, use_cond, c->d_ctrl + 4);
     c->launches++;
     return cudaGetLastError();
 }
@@ -2348,6 +2387,13 @@ cudaError_t tbsma_launch_density_tile(tbsma_ctx *c, const float4 *pos, int sync_
     cfg.attrs = attr;
     cfg.numAttrs = early ? 1 : 0;
     if (use_persist(c)) {
+        // Both passes' unit counters start at zero without relying on the previous pair of passes having run to its end.
+        // An early launch is a programmatic dependent of the filter kernel (nothing may sit between the two); it is only
+        // used inside a step, whose k_tile_worklist has cleared the counters already.
+        if (!early) {
+            const cudaError_t em = cudaMemsetAsync(c->d_ctrl + 4, 0, 2 * sizeof(int), st);
+            if (em != cudaSuccess) return em;
+        }
         cfg.gridDim = dim3((unsigned)persist_grid(c));
         cfg.blockDim = dim3(kPThreads);
         cfg.dynamicSmemBytes = persist_smem(c, 0, false);

@@ -25,7 +25,7 @@ def B():
     return binding
 
 
-VARIANTS = [1, 2]     # 1 = global-gather lists, 2 = shared-memory tiles (non-periodic replicas only)
+VARIANTS = [1, 2]     # 1 = global-gather lists, 2 = shared-memory tiles (layer tiles of thin wires, box tiles otherwise)
 
 
 def setup(B, w, max_nb=96, variant=0, tile=None, stagger=True, box=False):
@@ -203,8 +203,8 @@ def test_call_order_and_arguments(B):
 
 
 def run_gpu_md(B, w, n_steps, use_run=True, graph=True, virial=False, variant=0, tile=None, overlap=2,
-               stagger=True, async_inner=True, conditional=True):
-    ctx, st = setup(B, w, variant=variant, tile=tile, stagger=stagger)
+               stagger=True, async_inner=True, conditional=True, max_nb=96):
+    ctx, st = setup(B, w, max_nb=max_nb, variant=variant, tile=tile, stagger=stagger)
     ctx.set_graph(graph, conditional=conditional)
     ctx.set_overlap(overlap)
     ctx.set_async(async_inner)
@@ -614,7 +614,7 @@ def test_auto_variant_and_tile_shapes(B):
     bad = B.make_context(small_bulk(4))
     bad.set_variant(2)
     stb = B.DeviceState(small_bulk(4))
-    with pytest.raises(B.TbsmaError) as e:       # periodic replicas cannot use the tile variant
+    with pytest.raises(B.TbsmaError) as e:       # a periodic axis shorter than three tile cells cannot use the tile variant
         bad.build_cells(stb.pos, stb.vel, stb.tag)
     assert e.value.code == B.EINVAL
 
@@ -1113,6 +1113,117 @@ def test_series_detects_a_parted_wire(B):
     assert np.array_equal(dev["count"].cpu().numpy(), [4, 4]) and ctx.status() == 0
 
 
+def test_series_sees_a_gap_that_opens_beyond_the_box(B):
+    """the z bins of the series cover the range the atoms occupy at the step of the record, not the box handed to
+    tbsma_set_system: a wire whose box ends at z = 20 A, cut at z = 24 A with the top moved 8 A up (everything above the
+    box, where fixed bins would put both sides of the gap into the last bin) is reported parted, with the oracle's gap.
+    Atoms outside a non-periodic box are legal (edge cells grow, OUT_OF_BOX says so)."""
+    from oracle.protocol import largest_gap
+    w = W.config3(2, seed=47, length=60.0)
+    second = np.arange(w.n_atoms) >= w.offsets[1]
+    cut = (w.pos4[:, 2] > 24.0) & second
+    w.pos4[cut, 2] += 8.0
+    w.vel4[cut, 3] += 8.0
+    w.box_hi[1, 2] = 20.0
+    ctx, st = setup(B, w, variant=1)
+    R, cap = 2, 2
+    dev = dict(series=torch.zeros(R * cap * 4, dtype=torch.float64, device="cuda"),
+               count=torch.zeros(R, dtype=torch.int32, device="cuda"),
+               rupture=torch.full((R,), -1, dtype=torch.int64, device="cuda"),
+               volume=torch.ones(R, dtype=torch.float64, device="cuda"), L0=torch.full((R,), 60.0, dtype=torch.float64, device="cuda"))
+    ctx.set_series(5, cap, dev["series"], dev["count"], dev["rupture"], dev["volume"], dev["L0"])
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, 10, None, st.slab_rate, 0,
+                   st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == B.FLAG_OUT_OF_BOX
+    rup = dev["rupture"].cpu().numpy()
+    assert rup[0] == -1 and rup[1] == 4
+    ser = dev["series"].cpu().numpy().reshape(R, cap, 4)
+    x = st.untag(st.pos)
+    assert ser[1, :, 3].min() > w.r_cut and ser[0, :, 3].max() < 3.0
+    for r in range(R):
+        assert abs(ser[r, -1, 3] - largest_gap(x[w.offsets[r]:w.offsets[r + 1], 2])) < 1e-5
+
+
+def test_box_tiles_keep_up_with_a_compressed_thick_wire(B):
+    """the images of box tiles are sized at tbsma_build_cells and cannot grow inside tbsma_md_run, whose cell rebuilds
+    re-bin the atoms: a 6 nm x 8 nm wire between grips, compressed by 3 % in 1500 Langevin steps at 298 K (more atoms
+    per cell than at the build), must finish with a clean status word and the oracle's forces for its final positions"""
+    w = W._replica_batch("thick_wire_6x8nm_gripped", 1, 60.0, 80.0, [298.0], 71)
+    L0 = float(w.pos4[:, 2].max() - w.pos4[:, 2].min())
+    n_steps = 1500
+    w.slab_rate[:] = -0.03 * L0 / n_steps
+    ctx, st = run_gpu_md(B, w, n_steps, variant=2, max_nb=136)    # the seventh fcc shell (7.63 A) comes within r_cut + skin
+    n_tiles, box, _ = ctx.get_tiling()
+    assert box and n_tiles > 1
+    assert ctx.status() == 0
+    assert ctx.get_stats()["n_candidate_builds"] >= 1          # cells were re-binned on the way
+    xf = st.untag(st.pos)
+    assert xf[:, 2].max() < w.pos4[:, 2].max() - 0.02 * L0      # it really was compressed
+    o = oracle.compute(xf[:, :3].astype(np.float64), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi,
+                       periodic=w.periodic)
+    assert_forces(st.untag(st.force)[:, :3].astype(np.float64), o["f"])
+
+
+def z_periodic_wire(ncell=13, radius=15.0, seed=61):
+    """a [100] wire periodic along its axis only: ncell cubic cells long (13: 53.04 A = five tile cells of 9.8 A)"""
+    a = W.A_LATTICE
+    x = W.fcc_bulk(ncell)
+    c = 0.5 * ncell * a + 0.25 * a
+    x = W.displace(x[(x[:, 0] - c) ** 2 + (x[:, 1] - c) ** 2 < radius ** 2], 0.05, seed)
+    x32 = x.astype(np.float32)
+    Lf = np.float32(ncell * a)
+    x32[:, 2] = np.where(x32[:, 2] < 0, x32[:, 2] + Lf, x32[:, 2])
+    x32[:, 2] = np.where(x32[:, 2] >= Lf, x32[:, 2] - Lf, x32[:, 2])
+    n = len(x32)
+    pos4 = W.pack_pos4(x32, np.zeros(n, np.int32))
+    vel4 = W.pack_vel4(np.zeros((n, 3)), pos4)
+    lo = np.array([[x32[:, 0].min() - 2, x32[:, 1].min() - 2, 0.0]], np.float32)
+    hi = np.array([[x32[:, 0].max() + 2, x32[:, 1].max() + 2, ncell * a]], np.float32)
+    return W.Workload(f"z_periodic_wire_{ncell}", pos4, vel4, np.array([0, n], np.int32), lo, hi,
+                      np.array([[0, 0, 1]], np.uint8), np.zeros(1, np.float32), np.array([seed], np.uint64), np.zeros(1), 0.0)
+
+
+@pytest.mark.parametrize("name", ["bulk_10_b2_nc4", "zwire_13_b3_nc5"])
+def test_box_tiles_on_a_periodic_axis_of_exactly_b_plus_2_cells_after_drift(B, name):
+    """the shortest periodic axis a box of b cells may sit on holds b + 2 cells (TileDesc): the halo of a
+    tile is then the whole axis, wrapped at one end.  b = 2 on the four cells of a 40.8 A cube (boxes of 2 x 2 x 1), b = 3
+    on the five cells of a 53 A z-periodic wire (boxes of 3 x 3 x 3).  Hot atoms (900 K, NVE) drift across the boundary
+    while the cells and candidates of step 0 stay in use (positions are wrapped only when cells are rebuilt), the lists
+    being re-filtered in every step: after 120 steps they must be the oracle's sets for the final, unwrapped positions"""
+    if name.startswith("bulk"):
+        w, tiles = W.config5a(10, seed=67), 16
+    else:
+        w, tiles = z_periodic_wire(), 2
+    w.vel4[:, :3] = W.maxwell_velocities(w.n_atoms, 900.0, 69)
+    ctx, st = setup(B, w, max_nb=128, variant=2)      # hot: the seventh fcc shell (7.63 A) reaches into r_cut + skin
+    assert ctx.get_tiling()[:2] == (tiles, True)
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    n_steps = 120
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, 0.0, st.seed, 0, n_steps, None, None, 1, st.e_rep, None,
+                   st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    assert ctx.get_stats()["n_candidate_builds"] == 1           # the cells of step 0 throughout
+    final = st.untag(st.pos)
+    per = np.nonzero(w.periodic[0])[0]
+    out = (final[:, per] < w.box_lo[0, per]) | (final[:, per] >= w.box_hi[0, per])
+    assert out.sum() >= 10                                       # atoms beyond the boundary, not wrapped back
+    cg, lg = gpu_neighbors(B, ctx, st)
+    co, lo = oracle.neighbors(final, w.r_cut + w.skin, w.offsets, w.box_lo, w.box_hi, w.periodic, max_nb=128)
+    assert_same_sets(cg, lg, co, lo)
+    o = oracle.compute(final[:, :3].astype(np.float64), w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi,
+                       periodic=w.periodic)
+    assert_forces(st.untag(st.force)[:, :3].astype(np.float64), o["f"])
+
+
 def test_youngs_modulus_of_the_papers_smallest_wire(B):
     """Table 3: E = 69.6 GPa at 10 K for D0 = 3.1 nm, L0 = 20.4 nm.  Eight such wires (r_cut = 5.8 A, buffer
     0.29 A, Nose-Hoover, both ends pulled, sigma_zz from the device-side series with the hard-sphere volume N 4/3 pi (r0/2)^3,
@@ -1256,6 +1367,43 @@ def test_fused_step_of_small_batches_is_bitwise_identical(B, name):
     assert ca.launch_count() < 0.45 * cb.launch_count()          # one kernel per ordinary step instead of six
     md = run_oracle_md(w, n_steps)
     assert traj_rms(a.untag(a.pos)[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+
+
+def test_fused_step_flag_before_the_build_changes_no_bits(B):
+    """tbsma_set_fused_step called BEFORE tbsma_build_cells (the other test toggles it afterwards): a batch of 90 tiles
+    that fits the fused step only with fewer parts per tile than the automatic split would give is cut the same way
+    whether the fused step is on or off, so the per-replica fp64 sums have the same grouping and the same bits"""
+    w = W.config4(30, seed=77)
+    n_steps = 40
+
+    def run(fused):
+        ctx = B.make_context(w)
+        ctx.set_variant(2)
+        ctx.set_fused_step(fused)
+        ctx.set_overlap(0)
+        st = B.DeviceState(w)
+        ctx.build_cells(st.pos, st.vel, st.tag)
+        ctx.build_neighbors(st.pos, st.vel, st.tag)
+        ctx.compute(st.pos, st.force, st.e_rep, st.w_rep)
+        torch.cuda.synchronize()
+        first = (st.e_rep.cpu().numpy().copy(), st.w_rep.cpu().numpy().copy())
+        stream = torch.cuda.Stream()
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, st.slab_rate, 0,
+                       st.e_rep, st.w_rep, st.ekin)
+        torch.cuda.synchronize()
+        assert ctx.status() == 0
+        return ctx, st, first
+
+    ca, a, fa = run(True)
+    cb, b, fb = run(False)
+    assert B.lib().tbsma_get_fused_step(ca._h) == 1 and B.lib().tbsma_get_fused_step(cb._h) == 0
+    assert np.array_equal(fa[0], fb[0]) and np.array_equal(fa[1], fb[1])
+    for nm in ("pos", "vel", "force"):
+        assert np.array_equal(a.untag(getattr(a, nm)), b.untag(getattr(b, nm))), nm
+    for nm in ("e_rep", "ekin", "w_rep"):
+        assert np.array_equal(getattr(a, nm).cpu().numpy(), getattr(b, nm).cpu().numpy()), nm
 
 
 @pytest.mark.parametrize("depth", [2, 3])
