@@ -60,6 +60,83 @@ def make_workload(cfg, rank=0, replicas=None):
     raise SystemExit(f"unknown --config {cfg}")
 
 
+def force_kernel_name(ctx):
+    """the kernel the force pass of this batch is launched as (what roofline.kernel names)"""
+    n_tiles, box, persistent = ctx.get_tiling()
+    if not n_tiles:
+        return "k_force (thread per atom, int32 list)"
+    if persistent:
+        return "k_gather_persist<1,...> (persistent force/energy pass + closing half kick)"
+    if "cooperative" in ctx.describe_gather():
+        return "k_step_small (whole step in one cooperative kernel; force pass = its third phase)"
+    return "k_force_tile (one CTA per %s tile)" % ("box" if box else "layer")
+
+
+def measure_workload(cfg, args, B, torch, dev, local_rank, peak):
+    """One of the other BASELINE workloads, measured like the headline (same --steps / --warmup / --preroll, CUDA events on
+    the launching stream, per-kernel pass, clocks sampled during the timed region): a compact record for the `workloads`
+    block of the JSON line."""
+    w = make_workload(cfg, 0, None)
+    ctx = B.make_context(w)
+    st = B.DeviceState(w, dev)
+    stream = torch.cuda.Stream(device=dev)
+    K, Wm, P0 = args.steps, args.warmup, max(args.preroll, 0)
+
+    def run(step0, n):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, step0, n, st.slab_rate * float(step0),
+                   st.slab_rate, w.rebuild_every, st.e_rep, None, st.ekin)
+
+    with torch.cuda.stream(stream):
+        ctx.build_cells(st.pos, st.vel, st.tag)
+        ctx.build_neighbors(st.pos, st.vel, st.tag)
+        ctx.compute(st.pos, st.force, st.e_rep, None)
+        if P0:
+            run(0, P0)
+        run(P0, Wm)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    torch.cuda.synchronize()
+    stats0 = ctx.get_stats()
+    launches0 = ctx.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        run(P0 + Wm, K)
+        ev1.record(stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    sampler.stop_flag = True
+    ms = ev0.elapsed_time(ev1)
+    launches = ctx.launch_count() - launches0
+    stats1 = ctx.get_stats()
+    entries, pairs = ctx.count_pairs(st.pos, stream)
+    n_l = entries / w.n_atoms
+    k_eff = K * w.n_replicas / max(stats1["n_replica_builds"] - stats0["n_replica_builds"], 1)
+    ctx.set_timing(True)
+    with torch.cuda.stream(stream):
+        run(P0 + Wm + K, min(args.kernel_steps, 512))
+    tms, tsteps = ctx.get_timing()
+    ctx.set_timing(False)
+    pk = {k: v / max(tsteps, 1) for k, v in tms.items()}
+    status = ctx.status()
+    step_bytes = (8.0 * n_l + 160.0 + (4.0 * n_l + 120.0) / k_eff) * w.n_atoms
+    out = {"workload": w.name, "atoms": w.n_atoms, "replicas": w.n_replicas, "value": w.n_atoms * K / (ms * 1e-3),
+           "unit": UNIT, "ms_per_step": ms / K, "pair_interactions_per_s": 0.5 * pairs * K / (ms * 1e-3),
+           "variant": {1: "global gather (int32 list)", 2: "shared-memory tiles (u16 lists)"}.get(ctx.get_variant()),
+           "gather_kernels": ctx.describe_gather(), "force_kernel": force_kernel_name(ctx),
+           "mean_list_length": n_l, "mean_steps_between_rebuilds": k_eff,
+           "whole_step_frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
+           "force_frac": ((4.0 * n_l + 40.0) * w.n_atoms / (pk["force"] * 1e-3) / 1e9 / peak) if pk["force"] > 0 else None,
+           "density_frac": ((4.0 * n_l + 24.0) * w.n_atoms / (pk["density"] * 1e-3) / 1e9 / peak) if pk["density"] > 0 else None,
+           "per_kernel_ms": pk, "gpu_launches": int(launches), "status_flags": status,
+           "clocks": sampler.summary(t0, t1)}
+    ctx.destroy()
+    del st
+    torch.cuda.empty_cache()
+    return out
+
+
 class ClockSampler(threading.Thread):
     """SM clock / throttle reasons sampled with NVML while the timed region runs."""
 
@@ -174,6 +251,9 @@ def main():
     ap.add_argument("--impl", default="tbsma", choices=["tbsma", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--workloads", default=None,
+                    help="comma-separated configs measured after the headline and reported under `workloads` in the same "
+                         "JSON line (default with --config 3 on one GPU: 4,5a,5b,1,2; 'none' to skip)")
     ap.add_argument("--kernel-steps", type=int, default=60, help="steps of the per-kernel CUDA-event timing pass")
     ap.add_argument("--preroll", type=int, default=300,
                     help="declared, untimed steps before the warm-up: replicas built together rebuild together at first; "
@@ -314,7 +394,7 @@ def main():
     ach_force = force_bytes / (per_kernel_ms["force"] * 1e-3) / 1e9 if per_kernel_ms["force"] > 0 else 0.0
     ach_dens = dens_bytes / (per_kernel_ms["density"] * 1e-3) / 1e9 if per_kernel_ms["density"] > 0 else 0.0
     ach_step = step_bytes / (ms / K * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_force (force/energy pass + closing half kick)",
+    roofline = {"bound": "hbm", "kernel": force_kernel_name(ctx),
                 "achieved": ach_force, "peak": peak, "unit": "GB/s", "frac": ach_force / peak, "traffic": None,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": force_bytes,
                 "avg_launch_ms": per_kernel_ms["force"],
@@ -338,12 +418,13 @@ def main():
     # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu capture
     # (a number from a committed capture, NOT measured in this run: it names the capture it comes from and is refreshed
     # with every change of the kernel; null for workloads that have no capture)
-    traffic_file = os.path.join(ROOT, "profiles", "r2_force_kernel_traffic.csv")
+    traffic_file = next((f for f in (os.path.join(ROOT, "profiles", "r%d_force_kernel_traffic.csv" % r) for r in (3, 2))
+                         if os.path.exists(f)), "")
     if os.path.exists(traffic_file):
         try:
             import csv
             for row in csv.DictReader(open(traffic_file)):
-                if row["workload"] == w.name and row["kernel"].startswith("k_force"):
+                if row["workload"] == w.name and row["kernel"].startswith(("k_force", "k_gather_persist<1")):
                     roofline["traffic"] = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
                     roofline["traffic_from"] = "committed ncu capture: " + row["source"]
         except Exception:
@@ -379,6 +460,18 @@ def main():
                "call": "tbsma_md_run_host (H2D pos/vel/tag, cell+list build, initial forces, steps, D2H pos/vel/force/tag)"}
         ctx2.destroy()
 
+    # the other workloads of BASELINE.json, same binary, same call, same --steps / --warmup (one GPU, headline config only)
+    others = None
+    variant_ran, gather_desc = ctx.get_variant(), ctx.describe_gather()
+    wl = args.workloads if args.workloads is not None else ("4,5a,5b,1,2" if args.config == "3" and world == 1 else "none")
+    if rank == 0 and world == 1 and wl != "none":
+        ctx.destroy()
+        del st
+        torch.cuda.empty_cache()
+        others = {}
+        for cfg in wl.split(","):
+            others[cfg] = measure_workload(cfg, args, B, torch, dev, local_rank, peak)
+
     cpu = cpu_bf = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         # bounded samples (about 10-20 s of CPU work together): the linked-cell oracle is the CPU baseline, the brute-force
@@ -407,9 +500,9 @@ def main():
                        "rebuild": "displacement > skin/2 per replica" if not w.rebuild_every else f"every {w.rebuild_every} steps",
                        "mean_list_length": n_l, "mean_steps_between_rebuilds": k_eff,
                        "l2": "inputs larger than L2 (index list %.0f MB per pass)" % (entries * 4 / 1e6),
-                       "variant": {1: "global gather (int32 list)", 2: "shared-memory tiles (u16 lists)"}.get(ctx.get_variant()),
-                       "gather_kernels": ctx.describe_gather(),
-                       "list_renewal": "asynchronous, margin 0.03 A, beside the gather passes (density pass = programmatic dependent of the filter kernel)" if ctx.get_variant() == 2 and not w.rebuild_every else "ahead of the gather passes",
+                       "variant": {1: "global gather (int32 list)", 2: "shared-memory tiles (u16 lists)"}.get(variant_ran),
+                       "gather_kernels": gather_desc,
+                       "list_renewal": "asynchronous, margin 0.03 A, beside the gather passes (density pass = programmatic dependent of the filter kernel)" if variant_ran == 2 and not w.rebuild_every else "ahead of the gather passes",
                        "graph": "plain" if args.plain_graph else "conditional node around the cells+candidates chain",
                        "preroll_steps": P0,
                        "parallelism": "replicas only" if world > 1 else "1 gpu"},
@@ -419,6 +512,7 @@ def main():
             "clocks": sampler.summary(t_host0, t_host1),
             "e2e": e2e, "gpu_launches": int(launches), "status_flags": status,
             "roofline": roofline, "cpu_baseline": cpu, "cpu_baseline_cl": cpu, "cpu_baseline_bf": cpu_bf,
+            "workloads": others,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

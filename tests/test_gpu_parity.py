@@ -756,6 +756,50 @@ def test_full_size_trajectory_in_bench_configuration(B):
         assert abs(ekin[r] - md.ekin_rep[0]) <= 2e-3 * md.ekin_rep[0]
 
 
+def test_full_size_trajectory_config4_in_bench_configuration(B):
+    """config 4 at full size (2048 ragged replicas, 5.4 M atoms, all at 298 K: the persistent gather kernels on a ragged
+    tile list with every replica renewing its list), every default of bench.py: 100 steps, then five replicas covering
+    the three layer counts are compared with the oracle's run of that replica ALONE"""
+    w = W.config4()
+    n_steps = 100
+    ctx, st = run_gpu_md(B, w, n_steps)
+    assert ctx.status() == 0 and ctx.get_variant() == 2
+    n_tiles, box, persistent = ctx.get_tiling()
+    assert persistent and not box and n_tiles >= 3 * w.n_replicas
+    assert ctx.get_stats()["n_replica_builds"] >= 2 * w.n_replicas
+    sizes = np.diff(w.offsets)
+    assert len(set(sizes)) == 3
+    picks = [int(np.nonzero(sizes == n)[0][k]) for n, k in zip(sorted(set(sizes)), (0, -1, 7))] + [1000, w.n_replicas - 1]
+    x = st.untag(st.pos)[:, :3].astype(np.float64)
+    v = st.untag(st.vel)[:, :3].astype(np.float64)
+    e_rep, ekin = st.e_rep.cpu().numpy(), st.ekin.cpu().numpy()
+    for r in picks:
+        md = run_oracle_md(w.take(r, r + 1), n_steps)
+        sl = slice(w.offsets[r], w.offsets[r + 1])
+        assert traj_rms(x[sl], md.x) <= TRAJ_RMS
+        assert np.abs(v[sl] - md.v).max() < 2e-5
+        assert abs(e_rep[r] - md.e_rep[0]) <= 10 * E_REL * abs(md.e_rep[0])
+        assert abs(ekin[r] - md.ekin_rep[0]) <= 2e-3 * md.ekin_rep[0]
+
+
+@pytest.mark.parametrize("name", ["5a", "5b"])
+def test_full_size_trajectory_config5_in_bench_configuration(B, name):
+    """config 5 at full size with the library's own choices, as bench.py runs it: the 64^3 periodic block (1 048 576 atoms,
+    4 394 box tiles) and the 6 nm x 100 nm wire (164 885 atoms, global gather), NVE, lists rebuilt every 10 steps, 100
+    steps against the linked-cell oracle: positions, velocities, energy"""
+    w = W.config5a() if name == "5a" else W.config5b()
+    n_steps = 100
+    ctx, st = run_gpu_md(B, w, n_steps)
+    assert ctx.status() == 0
+    n_tiles, box, _ = ctx.get_tiling()
+    assert (ctx.get_variant(), n_tiles, box) == ((2, 4394, True) if name == "5a" else (1, 0, False))
+    md = run_oracle_md(w, n_steps)
+    L = float(w.box_hi[0, 0] - w.box_lo[0, 0]) if name == "5a" else None
+    assert traj_rms(st.untag(st.pos)[:, :3].astype(np.float64), md.x, L) <= TRAJ_RMS
+    assert np.abs(st.untag(st.vel)[:, :3].astype(np.float64) - md.v).max() < 2e-5
+    assert abs(st.e_rep.item() - md.e_rep[0]) <= 10 * E_REL * abs(md.e_rep[0])
+
+
 def test_trajectory_ragged_config4_batch_100_steps(B):
     """BASELINE config 4 in small: six replicas of the jittered 3 nm x 6 nm wire (three different layer counts), 298 K
     Langevin + pulling, every bench default on; 100 steps, EVERY replica against the oracle's run of the whole batch
@@ -1071,6 +1115,67 @@ def test_two_sided_stroke_pulling_ramp_and_series_match_oracle(B, variant):
     torch.cuda.synchronize()
     assert np.array_equal(dev["count"].cpu().numpy(), count)
     assert np.array_equal(st.untag(st.pos)[w.flags == 1, 2], z1)
+
+
+def test_notched_paper_wire_under_the_stroke_schedule_matches_oracle(B):
+    """the paper's specimen and loading: the 3.1 nm x 20.4 nm wire with its ring notch (8 850 - 27 =
+    8 823 atoms), r_cut 5.8 A, buffer 0.29 A, both gripping slabs displaced by +-0.05 A per stroke (here a stroke every 25
+    steps instead of every 10 000), 298 K; two wires with their own seeds, 100 steps = four strokes, against
+    oracle/protocol.py:TensileMD: trajectory, slabs placed to the bit, every record of the series"""
+    from oracle.protocol import TensileMD
+    x = W.ring_notch(W.fcc_wire(31.0, 204.0))
+    assert len(x) == 8823
+    fl = W.grip_flags(x)
+    R, every, n_steps, period, cap = 2, 10, 100, 25, 16
+    seeds = [83, 89]
+    vels = [W.maxwell_velocities(len(x), 298.0, sd, fl == 0) for sd in seeds]
+    w = W._assemble("paper_notched_wire_3.1x20.4nm", [x] * R, [fl] * R, vels, [298.0] * R, seeds, [0.05 / period] * R, 1e-3,
+                    stretch=1.0)
+    w.r_cut, w.skin = 5.8, 0.29
+    ctx, st = setup(B, w)
+    assert ctx.get_variant() == 2
+    rate2 = torch.from_numpy(w.slab_rate.copy()).cuda()
+    rate1 = torch.from_numpy(-w.slab_rate).cuda()
+    disp1 = torch.zeros(R, dtype=torch.float64, device="cuda")
+    L0 = np.full(R, float(x[:, 2].max() - x[:, 2].min()))
+    vol = np.full(R, len(x) * 4.0 / 3.0 * math.pi * (2.884 / 2) ** 3)          # hard-sphere volume (P:87)
+    dev = dict(series=torch.zeros(R * cap * 4, dtype=torch.float64, device="cuda"),
+               count=torch.zeros(R, dtype=torch.int32, device="cuda"),
+               rupture=torch.full((R,), -1, dtype=torch.int64, device="cuda"),
+               volume=torch.from_numpy(vol).cuda(), L0=torch.from_numpy(L0).cuda())
+    ctx.set_protocol(slab1_disp0=disp1, slab1_rate=rate1, stepwise_period=period, T_rate=None)
+    ctx.set_series(every, cap, dev["series"], dev["count"], dev["rupture"], dev["volume"], dev["L0"])
+    ctx.compute(st.pos, st.force, st.e_rep, None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.md_run(st.pos, st.vel, st.force, st.tag, w.dt, st.T, w.gamma, st.seed, 0, n_steps, None, rate2, 0,
+                   st.e_rep, None, st.ekin)
+    torch.cuda.synchronize()
+    assert ctx.status() == 0
+    zref = w.vel4[:, 3].astype(np.float64)
+    md = oracle.MD(w.x64(), w.v64(), w.flags, w.r_cut, offsets=w.offsets, lo=w.box_lo, hi=w.box_hi, cells=True, zref=zref)
+    t = TensileMD(md, w.dt, w.T.astype(np.float64), w.gamma, w.seed, 0, 0.0, w.slab_rate, np.zeros(R), -w.slab_rate,
+                  period=period, T_rate=None, every=every, volume=vol, L0=L0)
+    for _ in range(n_steps):
+        t.step()
+    xg = st.untag(st.pos)
+    assert traj_rms(xg[:, :3].astype(np.float64), md.x) <= TRAJ_RMS
+    for f in (1, 2):
+        assert np.array_equal(xg[w.flags == f, 2], md.x[w.flags == f, 2].astype(np.float32))
+    moved = xg[w.flags == 2, 2].astype(np.float64) - zref[w.flags == 2]
+    assert np.allclose(moved, 0.2, atol=1e-5)                     # four strokes of 0.05 A
+    count = dev["count"].cpu().numpy()
+    assert np.all(count == n_steps // every)
+    ser = dev["series"].cpu().numpy().reshape(R, cap, 4)
+    for r in range(R):
+        ref = np.array(t.series[r])
+        got = ser[r, :count[r]]
+        assert np.array_equal(got[:, 0], ref[:, 0])
+        assert np.allclose(got[:, 1], ref[:, 1], rtol=1e-12, atol=1e-15)
+        assert np.allclose(got[:, 2], ref[:, 2], rtol=2e-4, atol=2e-5 * np.abs(ref[:, 2]).max())
+        assert np.allclose(got[:, 3], ref[:, 3], atol=2e-5)
+    assert np.all(dev["rupture"].cpu().numpy() == -1)
 
 
 def test_series_detects_a_parted_wire(B):
